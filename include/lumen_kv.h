@@ -1,0 +1,183 @@
+/*
+ * lumen_kv.h -- C ABI of the B200-native KV checkpoint pack / restore unpack.
+ *
+ * The operation is the data-parallel hot path of LUMEN's load-aware KV
+ * checkpointing and recovery:
+ *   - pack   = step (3) of the incremental checkpoint pipeline: "workers track
+ *     checkpoint progress and transmit only newly generated KV pages after each
+ *     prefill or decode batch. A background thread copies these pages from GPU
+ *     memory to the local pinned buffer" (section 4.2);
+ *   - unpack = KV-reuse recovery: the checkpoint holder locates "the longest
+ *     contiguous checkpointed prefix ... subsequently loading the matching KV
+ *     pages into GPU memory" (section 4.3).
+ *   A "KV page" is "a fixed-size block of cached keys and values for contiguous
+ *   token positions" (section 2.1).
+ *
+ * Data model (BASELINE.json north_star)
+ *   Pool: 2L "planes" -- for every layer l one K plane and one V plane, each a
+ *   dense device array [num_pages][page_size][kv_heads][head_dim] of opaque
+ *   elem_bytes-wide words (bf16 in the paper's models; never interpreted).
+ *   row = kv_heads*head_dim*elem_bytes is one token in one plane; it must be a
+ *   multiple of 16 bytes and every plane / buffer base must be 16-byte aligned.
+ *   A request owns a page table (logical page i -> physical page) shared by all
+ *   2L planes, and a token range [t_begin, t_end).
+ *   Checkpoint buffer: dense, no padding, laid out
+ *       [request][layer][K|V][token][head][dim]
+ *   requests in plan order; request r starts at lumen_kv_plan_req_offset(r).
+ *   With n_r = t_end - t_begin, plane = 2*layer + (0 for K, 1 for V):
+ *       B[off_r + (plane*n_r + j)*row + b]  <->
+ *       planes[plane][(PT_r[(t_begin+j)/S]*S + (t_begin+j)%S)*row + b]
+ *   pack copies right to left, unpack left to right; unpack leaves every other
+ *   pool byte untouched.
+ *
+ * Conventions
+ *   - All functions return LUMEN_KV_OK (0) or a negative lumen_kv_status.
+ *   - All validation happens in lumen_kv_plan_build on the host, before any
+ *     launch; pack/unpack never read or write out of bounds for a plan that built.
+ *   - pack/unpack are asynchronous on the caller's cudaStream_t (passed as
+ *     void*), perform no synchronisation and no allocation.  Results are
+ *     complete (and, for host destinations, host-visible) once an event recorded
+ *     on that stream after the call has fired (nothing is promised
+ *     earlier).
+ *   - A plan is immutable and direction-agnostic: the same plan drives pack and
+ *     unpack.  The caller owns pools, buffers, streams and page tables (page
+ *     tables are copied at build time).  Plans may be used concurrently from
+ *     different streams; one plan must not be used from two host threads at once.
+ *   - There is no CPU fallback: without a CUDA device every call except the
+ *     host-only plan build and the accessors fails with LUMEN_KV_ECUDA.
+ */
+#ifndef LUMEN_KV_H
+#define LUMEN_KV_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define LUMEN_KV_VERSION 1
+
+#if defined(__GNUC__)
+#define LUMEN_KV_API __attribute__((visibility("default")))
+#else
+#define LUMEN_KV_API
+#endif
+
+typedef enum {
+    LUMEN_KV_OK       =  0,
+    LUMEN_KV_EINVAL   = -1,  /* null pointer, bad geometry, misaligned base, bad kind/flag   */
+    LUMEN_KV_ERANGE   = -2,  /* page index outside [0, num_pages) or range outside the table */
+    LUMEN_KV_EOVERLAP = -3,  /* VALIDATE_UNIQUE_DST: a physical page is addressed twice      */
+    LUMEN_KV_ESIZE    = -4,  /* buffer smaller than lumen_kv_plan_bytes()                    */
+    LUMEN_KV_ENOMEM   = -5,  /* host or device allocation of the descriptors failed          */
+    LUMEN_KV_ECUDA    = -6   /* CUDA runtime error; see lumen_kv_last_cuda_error()           */
+} lumen_kv_status;
+
+/* Geometry of the caller's paged pool (host struct, read during plan_build only). */
+typedef struct {
+    int32_t num_layers;        /* L >= 1                                              */
+    int32_t kv_heads;          /* H >= 1                                              */
+    int32_t head_dim;          /* D >= 1                                              */
+    int32_t page_size;         /* S >= 1 tokens per page                              */
+    int32_t elem_bytes;        /* bytes per element; H*D*elem_bytes must be % 16 == 0 */
+    int32_t reserved;          /* must be 0                                           */
+    int64_t num_pages;         /* N, 1 <= N < 2^31                                    */
+    int64_t page_stride_bytes; /* 0 => dense: S*H*D*elem_bytes; else >= that, % 16    */
+} lumen_kv_geom;
+
+/* One request's contribution to a plan (host struct; page_table is a HOST pointer
+ * and is copied).  Entries outside [t_begin/S, (t_end-1)/S] are ignored (A6).     */
+typedef struct {
+    const int32_t* page_table;
+    int64_t        page_table_len;
+    int64_t        t_begin, t_end;   /* 0 <= t_begin <= t_end <= page_table_len*S  */
+} lumen_kv_req;
+
+typedef struct lumen_kv_plan lumen_kv_plan;  /* opaque; library owns its descriptors */
+
+/* plan_build flags */
+#define LUMEN_KV_VALIDATE_UNIQUE_DST 0x1u /* reject plans that address a physical page twice  */
+#define LUMEN_KV_MERGE_ADJACENT      0x2u /* merge runs whose physical pages are adjacent     */
+#define LUMEN_KV_HOST_ONLY           0x4u /* build descriptors on the host only (no CUDA call);
+                                             such a plan can be inspected but not executed   */
+/* kernel selection (default 0 = library heuristic); for benchmarking / evidence   */
+#define LUMEN_KV_KERNEL_SHIFT        8
+#define LUMEN_KV_KERNEL_MASK         0xF00u
+#define LUMEN_KV_KERNEL_AUTO         0x000u
+#define LUMEN_KV_KERNEL_WARP         0x100u /* SIMT: warp per (run, plane), 16 B ld/st        */
+#define LUMEN_KV_KERNEL_BULK         0x200u /* TMA 1-D bulk copies through a shared-memory ring */
+
+/* where the checkpoint buffer lives */
+#define LUMEN_KV_MEM_DEVICE      0  /* device pointer (HBM)                                   */
+#define LUMEN_KV_MEM_HOST_MAPPED 1  /* pinned host memory (cudaHostAlloc / cudaHostRegister);
+                                       pass the HOST pointer, the kernel writes/reads it
+                                       directly over the host link                           */
+
+/*
+ * lumen_kv_plan_build -- step a2: flatten the requests'
+ * ranges into token-run descriptors and upload them.
+ *   geom, reqs : host pointers, read only during the call.  num_reqs >= 0.
+ *   stream     : cudaStream_t on which the descriptor upload is enqueued; the plan
+ *                may be used on that stream immediately, on other streams after the
+ *                caller orders them behind it.  Ignored with LUMEN_KV_HOST_ONLY.
+ *   out        : receives the plan; release with lumen_kv_plan_free.
+ * Zero-length ranges and num_reqs == 0 are legal (A4) and yield 0 bytes.
+ * Errors: EINVAL, ERANGE, EOVERLAP (with VALIDATE_UNIQUE_DST), ENOMEM, ECUDA.
+ */
+LUMEN_KV_API int lumen_kv_plan_build(const lumen_kv_geom* geom, const lumen_kv_req* reqs,
+                        int32_t num_reqs, uint32_t flags, void* stream,
+                        lumen_kv_plan** out);
+
+/* total checkpoint-buffer bytes = sum_r n_r * 2L * row */
+LUMEN_KV_API int64_t lumen_kv_plan_bytes(const lumen_kv_plan* plan);
+/* byte offset of request r in the buffer (exclusive prefix sum); r == num_reqs gives the total */
+LUMEN_KV_API int64_t lumen_kv_plan_req_offset(const lumen_kv_plan* plan, int32_t r);
+/* number of token-run descriptors in the plan */
+LUMEN_KV_API int64_t lumen_kv_plan_num_runs(const lumen_kv_plan* plan);
+
+/* One run, for inspection (tests of the plan logic; not needed to use the library). */
+typedef struct {
+    int64_t src_slot;   /* page*S + first slot, in tokens                    */
+    int64_t dst_token;  /* request-relative first token j                    */
+    int32_t req;        /* request index                                     */
+    int32_t count;      /* tokens in the run                                 */
+} lumen_kv_run_info;
+LUMEN_KV_API int lumen_kv_plan_get_run(const lumen_kv_plan* plan, int64_t i, lumen_kv_run_info* out);
+
+/*
+ * lumen_kv_checkpoint_pack -- steps a3/a4: gather the plan's token ranges from the
+ * planes into the contiguous checkpoint buffer dst.
+ *   k_planes, v_planes : HOST arrays of num_layers DEVICE pointers (one per layer);
+ *                        read during the call, not retained.
+ *   dst, dst_bytes     : buffer and its capacity; dst_kind says where it lives.
+ * Errors: EINVAL (null / misaligned / host-only plan), ESIZE, ECUDA.
+ */
+LUMEN_KV_API int lumen_kv_checkpoint_pack(const lumen_kv_plan* plan,
+                             const void* const* k_planes, const void* const* v_planes,
+                             void* dst, int64_t dst_bytes, int dst_kind, void* stream);
+
+/*
+ * lumen_kv_restore_unpack -- step a7: scatter the checkpoint buffer src into the
+ * planes under the plan's page tables.  Destinations must be disjoint (use
+ * LUMEN_KV_VALIDATE_UNIQUE_DST at build time; otherwise undefined for overlaps).
+ */
+LUMEN_KV_API int lumen_kv_restore_unpack(const lumen_kv_plan* plan,
+                            void* const* k_planes, void* const* v_planes,
+                            const void* src, int64_t src_bytes, int src_kind, void* stream);
+
+/* Release a plan.  Safe to call while work using the plan is still in flight on a
+ * stream: the descriptors are recycled only after that work has completed.       */
+LUMEN_KV_API void lumen_kv_plan_free(lumen_kv_plan* plan);
+
+/* Release cached descriptor memory held by the library (synchronises the device). */
+LUMEN_KV_API void lumen_kv_trim(void);
+
+LUMEN_KV_API const char* lumen_kv_strerror(int status);
+/* last cudaError_t seen by the calling thread inside the library (0 if none) */
+LUMEN_KV_API int lumen_kv_last_cuda_error(void);
+LUMEN_KV_API int lumen_kv_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LUMEN_KV_H */

@@ -1,0 +1,17 @@
+"""paper_2606_17787_b200 -- B200-native KV checkpoint pack / restore unpack.
+
+The data-parallel hot path of LUMEN's load-aware KV checkpointing and recovery
+(arxiv/paper_2606_17787; section 4.2 step 3, PAPER.md:157-163
+section 4.3): hand-written sm_100a kernels behind the C ABI of
+include/lumen_kv.h, plus this thin ctypes binding with the same names.
+Build the library with `python -m paper_2606_17787_b200.build`.
+"""
+from .binding import (  # noqa: F401
+    EXPORTS, LumenKVError, Plan, library_path, lumen_kv_checkpoint_pack, lumen_kv_geom,
+    lumen_kv_plan_build, lumen_kv_plan_free, lumen_kv_req, lumen_kv_restore_unpack,
+    lumen_kv_run_info, lumen_kv_strerror, lumen_kv_trim, lumen_kv_version, make_geom, plane_ptrs,
+    LUMEN_KV_OK, LUMEN_KV_EINVAL, LUMEN_KV_ERANGE, LUMEN_KV_EOVERLAP, LUMEN_KV_ESIZE,
+    LUMEN_KV_ENOMEM, LUMEN_KV_ECUDA, LUMEN_KV_VALIDATE_UNIQUE_DST, LUMEN_KV_MERGE_ADJACENT,
+    LUMEN_KV_HOST_ONLY, LUMEN_KV_KERNEL_AUTO, LUMEN_KV_KERNEL_WARP, LUMEN_KV_KERNEL_BULK,
+    LUMEN_KV_MEM_DEVICE, LUMEN_KV_MEM_HOST_MAPPED,
+)

@@ -1,0 +1,244 @@
+"""ctypes binding of include/lumen_kv.h -- argument marshalling only.
+
+Every step of the path (plan flattening, pack, unpack) runs inside
+liblumen_kv.so; this module converts Python objects to the C structs and raises
+LumenKVError on a negative status.  There is no fallback of any kind: if the
+shared library is missing the import fails.
+
+torch is *not* imported here.  Callers pass raw integers: device pointers
+(`tensor.data_ptr()`), host pointers of pinned memory, and the `cudaStream_t`
+handle (`torch.cuda.Stream.cuda_stream`).  Page tables are numpy int32 arrays.
+"""
+from __future__ import annotations
+
+import ctypes
+from pathlib import Path
+from typing import Iterable, Sequence, Tuple
+
+import numpy as np
+
+_SO = Path(__file__).resolve().parent / "liblumen_kv.so"
+
+# ---- constants mirrored from include/lumen_kv.h -----------------------------------
+LUMEN_KV_OK, LUMEN_KV_EINVAL, LUMEN_KV_ERANGE = 0, -1, -2
+LUMEN_KV_EOVERLAP, LUMEN_KV_ESIZE, LUMEN_KV_ENOMEM, LUMEN_KV_ECUDA = -3, -4, -5, -6
+LUMEN_KV_VALIDATE_UNIQUE_DST = 0x1
+LUMEN_KV_MERGE_ADJACENT = 0x2
+LUMEN_KV_HOST_ONLY = 0x4
+LUMEN_KV_KERNEL_AUTO, LUMEN_KV_KERNEL_WARP, LUMEN_KV_KERNEL_BULK = 0x000, 0x100, 0x200
+LUMEN_KV_MEM_DEVICE, LUMEN_KV_MEM_HOST_MAPPED = 0, 1
+
+EXPORTS = (
+    "lumen_kv_plan_build", "lumen_kv_plan_bytes", "lumen_kv_plan_req_offset",
+    "lumen_kv_plan_num_runs", "lumen_kv_plan_get_run", "lumen_kv_checkpoint_pack",
+    "lumen_kv_restore_unpack", "lumen_kv_plan_free", "lumen_kv_trim",
+    "lumen_kv_strerror", "lumen_kv_last_cuda_error", "lumen_kv_version",
+)
+
+
+class lumen_kv_geom(ctypes.Structure):
+    _fields_ = [("num_layers", ctypes.c_int32), ("kv_heads", ctypes.c_int32),
+                ("head_dim", ctypes.c_int32), ("page_size", ctypes.c_int32),
+                ("elem_bytes", ctypes.c_int32), ("reserved", ctypes.c_int32),
+                ("num_pages", ctypes.c_int64), ("page_stride_bytes", ctypes.c_int64)]
+
+
+class lumen_kv_req(ctypes.Structure):
+    _fields_ = [("page_table", ctypes.c_void_p), ("page_table_len", ctypes.c_int64),
+                ("t_begin", ctypes.c_int64), ("t_end", ctypes.c_int64)]
+
+
+class lumen_kv_run_info(ctypes.Structure):
+    _fields_ = [("src_slot", ctypes.c_int64), ("dst_token", ctypes.c_int64),
+                ("req", ctypes.c_int32), ("count", ctypes.c_int32)]
+
+
+class LumenKVError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        msg = _lib().lumen_kv_strerror(status).decode()
+        cuda = _lib().lumen_kv_last_cuda_error() if status == LUMEN_KV_ECUDA else 0
+        super().__init__(f"{where}: {msg} (status {status}" +
+                         (f", cudaError {cuda})" if cuda else ")"))
+        self.status = status
+        self.cuda_error = cuda
+
+
+_handle = None
+
+
+def _lib() -> ctypes.CDLL:
+    global _handle
+    if _handle is not None:
+        return _handle
+    if not _SO.exists():
+        raise ImportError(
+            f"{_SO} is missing: run `python -m paper_2606_17787_b200.build` "
+            "(nvcc, sm_100a).  There is no fallback path.")
+    L = ctypes.CDLL(str(_SO))
+    vp, i32, i64, u32 = ctypes.c_void_p, ctypes.c_int32, ctypes.c_int64, ctypes.c_uint32
+    L.lumen_kv_plan_build.restype = ctypes.c_int
+    L.lumen_kv_plan_build.argtypes = [ctypes.POINTER(lumen_kv_geom), ctypes.POINTER(lumen_kv_req),
+                                      i32, u32, vp, ctypes.POINTER(vp)]
+    L.lumen_kv_plan_bytes.restype = i64
+    L.lumen_kv_plan_bytes.argtypes = [vp]
+    L.lumen_kv_plan_req_offset.restype = i64
+    L.lumen_kv_plan_req_offset.argtypes = [vp, i32]
+    L.lumen_kv_plan_num_runs.restype = i64
+    L.lumen_kv_plan_num_runs.argtypes = [vp]
+    L.lumen_kv_plan_get_run.restype = ctypes.c_int
+    L.lumen_kv_plan_get_run.argtypes = [vp, i64, ctypes.POINTER(lumen_kv_run_info)]
+    for name in ("lumen_kv_checkpoint_pack", "lumen_kv_restore_unpack"):
+        f = getattr(L, name)
+        f.restype = ctypes.c_int
+        f.argtypes = [vp, ctypes.POINTER(vp), ctypes.POINTER(vp), vp, i64, ctypes.c_int, vp]
+    L.lumen_kv_plan_free.restype = None
+    L.lumen_kv_plan_free.argtypes = [vp]
+    L.lumen_kv_trim.restype = None
+    L.lumen_kv_trim.argtypes = []
+    L.lumen_kv_strerror.restype = ctypes.c_char_p
+    L.lumen_kv_strerror.argtypes = [ctypes.c_int]
+    L.lumen_kv_last_cuda_error.restype = ctypes.c_int
+    L.lumen_kv_version.restype = ctypes.c_int
+    _handle = L
+    return L
+
+
+def library_path() -> Path:
+    return _SO
+
+
+def make_geom(num_layers, kv_heads, head_dim, page_size, num_pages, *, elem_bytes=2,
+              page_stride_bytes=0) -> lumen_kv_geom:
+    return lumen_kv_geom(int(num_layers), int(kv_heads), int(head_dim), int(page_size),
+                         int(elem_bytes), 0, int(num_pages), int(page_stride_bytes))
+
+
+Req = Tuple[np.ndarray, int, int]
+
+
+class Plan:
+    """Owner of a `lumen_kv_plan*`; freed on close() / garbage collection."""
+
+    def __init__(self, handle: int, geom: lumen_kv_geom, num_reqs: int):
+        self._h = ctypes.c_void_p(handle)
+        self.geom = geom
+        self.num_reqs = num_reqs
+
+    @property
+    def handle(self) -> ctypes.c_void_p:
+        if not self._h:
+            raise ValueError("plan already freed")
+        return self._h
+
+    @property
+    def nbytes(self) -> int:
+        return int(_lib().lumen_kv_plan_bytes(self.handle))
+
+    @property
+    def num_runs(self) -> int:
+        return int(_lib().lumen_kv_plan_num_runs(self.handle))
+
+    def req_offset(self, r: int) -> int:
+        v = int(_lib().lumen_kv_plan_req_offset(self.handle, int(r)))
+        if v < 0:
+            raise LumenKVError(v, "lumen_kv_plan_req_offset")
+        return v
+
+    def run(self, i: int) -> lumen_kv_run_info:
+        info = lumen_kv_run_info()
+        rc = _lib().lumen_kv_plan_get_run(self.handle, int(i), ctypes.byref(info))
+        if rc:
+            raise LumenKVError(rc, "lumen_kv_plan_get_run")
+        return info
+
+    def close(self) -> None:
+        if self._h:
+            _lib().lumen_kv_plan_free(self._h)
+            self._h = ctypes.c_void_p(None)
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+
+def lumen_kv_plan_build(geom: lumen_kv_geom, reqs: Sequence[Req], flags: int = 0,
+                        stream: int = 0) -> Plan:
+    """reqs: sequence of (page_table int32 ndarray, t_begin, t_end)."""
+    n = len(reqs)
+    arr = (lumen_kv_req * max(n, 1))()
+    keep = []
+    for i, (pt, tb, te) in enumerate(reqs):
+        pt = np.ascontiguousarray(pt, dtype=np.int32)
+        keep.append(pt)
+        arr[i].page_table = pt.ctypes.data if pt.size else None
+        arr[i].page_table_len = pt.size
+        arr[i].t_begin, arr[i].t_end = int(tb), int(te)
+    out = ctypes.c_void_p()
+    rc = _lib().lumen_kv_plan_build(ctypes.byref(geom), arr, n, int(flags),
+                                    ctypes.c_void_p(int(stream)), ctypes.byref(out))
+    del keep
+    if rc:
+        raise LumenKVError(rc, "lumen_kv_plan_build")
+    return Plan(out.value, geom, n)
+
+
+def _ptr_array(ptrs: Iterable[int], L: int):
+    ptrs = list(ptrs)
+    if len(ptrs) != L:
+        raise ValueError(f"need {L} plane pointers, got {len(ptrs)}")
+    return (ctypes.c_void_p * L)(*[int(p) for p in ptrs])
+
+
+def plane_ptrs(ptrs: Iterable[int], L: int):
+    """Pre-marshal a list of device pointers once (reuse it across calls)."""
+    return _ptr_array(ptrs, L)
+
+
+def _as_ptr_array(x, L):
+    return x if isinstance(x, ctypes.Array) else _ptr_array(x, L)
+
+
+def lumen_kv_checkpoint_pack(plan: Plan, k_planes, v_planes, dst: int, dst_bytes: int,
+                             dst_kind: int = LUMEN_KV_MEM_DEVICE, stream: int = 0) -> None:
+    L = plan.geom.num_layers
+    rc = _lib().lumen_kv_checkpoint_pack(plan.handle, _as_ptr_array(k_planes, L),
+                                         _as_ptr_array(v_planes, L), ctypes.c_void_p(int(dst)),
+                                         int(dst_bytes), int(dst_kind),
+                                         ctypes.c_void_p(int(stream)))
+    if rc:
+        raise LumenKVError(rc, "lumen_kv_checkpoint_pack")
+
+
+def lumen_kv_restore_unpack(plan: Plan, k_planes, v_planes, src: int, src_bytes: int,
+                            src_kind: int = LUMEN_KV_MEM_DEVICE, stream: int = 0) -> None:
+    L = plan.geom.num_layers
+    rc = _lib().lumen_kv_restore_unpack(plan.handle, _as_ptr_array(k_planes, L),
+                                        _as_ptr_array(v_planes, L), ctypes.c_void_p(int(src)),
+                                        int(src_bytes), int(src_kind),
+                                        ctypes.c_void_p(int(stream)))
+    if rc:
+        raise LumenKVError(rc, "lumen_kv_restore_unpack")
+
+
+def lumen_kv_plan_free(plan: Plan) -> None:
+    plan.close()
+
+
+def lumen_kv_trim() -> None:
+    _lib().lumen_kv_trim()
+
+
+def lumen_kv_strerror(status: int) -> str:
+    return _lib().lumen_kv_strerror(int(status)).decode()
+
+
+def lumen_kv_version() -> int:
+    return int(_lib().lumen_kv_version())

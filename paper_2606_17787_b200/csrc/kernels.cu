@@ -1,0 +1,335 @@
+// sm_100a kernels for the KV checkpoint pack (gather) and restore unpack (scatter).
+//
+// Both directions are the same byte permutation (PAPER.md:145 step 3 and
+// PAPER.md:157-163; index map in include/lumen_kv.h): a work item is one
+// (token-run, plane) pair, `count*row` contiguous bytes on the pool side and on the
+// buffer side.  Pure data movement: no tensor cores, no arithmetic on the payload,
+// the 16-bit words are never interpreted (they include NaN encodings).
+//
+// Two kernels, chosen per launch:
+//   kv_copy_warp : SIMT.  One warp per item, 16-byte ld/st per lane, UNROLL
+//                  independent loads in flight per lane before the first store.
+//   kv_copy_bulk : TMA.   Persistent single-warp CTAs; one elected lane moves
+//                  whole items global -> shared ring -> global with 1-D
+//                  cp.async.bulk (UBLKCP), completion tracked by mbarriers (loads)
+//                  and bulk groups (stores).  The other lanes only prefetch and
+//                  decode descriptors.
+#include "kernels.hpp"
+
+namespace lumen {
+namespace {
+
+struct PlaneTable {
+    const void* p[kMaxPlanesPerLaunch];
+};
+
+// ---------------------------------------------------------------------------------
+// small PTX helpers
+// ---------------------------------------------------------------------------------
+__device__ __forceinline__ uint4 ld_stream16(const void* p) {
+    uint4 v;
+    asm volatile("ld.global.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];"
+                 : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w)
+                 : "l"(p)
+                 : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_stream16(void* p, const uint4& v) {
+    asm volatile("st.global.L1::no_allocate.v4.u32 [%0], {%1,%2,%3,%4};" ::"l"(p), "r"(v.x),
+                 "r"(v.y), "r"(v.z), "r"(v.w)
+                 : "memory");
+}
+
+// Decode one item into (pool pointer, buffer pointer, bytes).
+struct Item {
+    char* pool;
+    char* buf;
+    uint32_t bytes;
+};
+
+__device__ __forceinline__ Item decode_item(const RunDesc* __restrict__ runs,
+                                            const ReqDesc* __restrict__ reqs, int64_t run,
+                                            const void* plane_base, int32_t plane, char* buf,
+                                            uint32_t row_bytes) {
+    const uint4 d = __ldg(reinterpret_cast<const uint4*>(runs + run));
+    // d.x = src_lo, d.y = dst_tok, d.z = req, d.w = count | src_hi << 16
+    const uint32_t count = d.w & 0xFFFFu;
+    const uint64_t off16 = (static_cast<uint64_t>(d.w >> 16) << 32) | d.x;
+    const longlong2 q = __ldg(reinterpret_cast<const longlong2*>(reqs + d.z));
+    // q.x = row_base, q.y = n
+    const int64_t row = q.x + static_cast<int64_t>(plane) * q.y + d.y;
+    Item it;
+    it.pool = const_cast<char*>(static_cast<const char*>(plane_base)) + (off16 << 4);
+    it.buf = buf + row * static_cast<int64_t>(row_bytes);
+    it.bytes = count * row_bytes;
+    return it;
+}
+
+// ---------------------------------------------------------------------------------
+// SIMT kernel: warp per (run, plane)
+// ---------------------------------------------------------------------------------
+constexpr int kWarpsPerCta = 8;
+
+template <int UNROLL>
+__global__ void __launch_bounds__(kWarpsPerCta * 32)
+kv_copy_warp(const PlaneTable planes, const RunDesc* __restrict__ runs,
+             const ReqDesc* __restrict__ reqs, int64_t n_runs, char* buf, uint32_t row_bytes,
+             int32_t plane0, int pack) {
+    const int lane = threadIdx.x & 31;
+    const int64_t run = static_cast<int64_t>(blockIdx.x) * kWarpsPerCta + (threadIdx.x >> 5);
+    if (run >= n_runs) return;
+    const Item it = decode_item(runs, reqs, run, planes.p[blockIdx.y], plane0 + blockIdx.y, buf,
+                                row_bytes);
+    const char* src = pack ? it.pool : it.buf;
+    char* dst = pack ? it.buf : it.pool;
+    const uint32_t nvec = it.bytes >> 4;
+
+    uint32_t i = lane;
+    // full batches: UNROLL independent 16-byte loads per lane, then the stores
+    for (; i + (UNROLL - 1) * 32 < nvec; i += UNROLL * 32) {
+        uint4 v[UNROLL];
+#pragma unroll
+        for (int u = 0; u < UNROLL; ++u) v[u] = ld_stream16(src + (static_cast<size_t>(i + u * 32) << 4));
+#pragma unroll
+        for (int u = 0; u < UNROLL; ++u) st_stream16(dst + (static_cast<size_t>(i + u * 32) << 4), v[u]);
+    }
+    // ragged tail (< UNROLL*32 vectors), still loads-before-stores
+    {
+        uint4 v[UNROLL];
+#pragma unroll
+        for (int u = 0; u < UNROLL; ++u)
+            if (i + u * 32 < nvec) v[u] = ld_stream16(src + (static_cast<size_t>(i + u * 32) << 4));
+#pragma unroll
+        for (int u = 0; u < UNROLL; ++u)
+            if (i + u * 32 < nvec) st_stream16(dst + (static_cast<size_t>(i + u * 32) << 4), v[u]);
+    }
+}
+
+// ---------------------------------------------------------------------------------
+// TMA kernel: persistent single-warp CTAs, 1-D bulk copies through a shared ring
+// ---------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) {
+    return static_cast<uint32_t>(__cvta_generic_to_shared(p));
+}
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes)
+                 : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(bar),
+        "r"(parity)
+        : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(uint32_t dst_smem, const void* src, uint32_t bytes,
+                                         uint32_t bar) {
+    asm volatile(
+        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::
+            "r"(dst_smem),
+        "l"(src), "r"(bytes), "r"(bar)
+        : "memory");
+}
+__device__ __forceinline__ void bulk_s2g(void* dst, uint32_t src_smem, uint32_t bytes) {
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst),
+                 "r"(src_smem), "r"(bytes)
+                 : "memory");
+}
+__device__ __forceinline__ void bulk_commit() {
+    asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+}
+template <int N>
+__device__ __forceinline__ void bulk_wait_read() {
+    asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(N) : "memory");
+}
+__device__ __forceinline__ void bulk_wait_all() {
+    asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
+}
+
+struct StageMeta {
+    char* dst;
+    uint32_t bytes;
+    uint32_t pad;
+};
+
+// STAGES ring slots of stage_bytes each; the store of item i is issued LAG
+// iterations after its load so that LAG loads are in flight per CTA.
+template <int STAGES>
+__global__ void __launch_bounds__(32)
+kv_copy_bulk(const PlaneTable planes, const RunDesc* __restrict__ runs,
+             const ReqDesc* __restrict__ reqs, int64_t n_runs, int32_t n_planes, char* buf,
+             uint32_t row_bytes, uint32_t stage_bytes, int32_t plane0, int pack) {
+    constexpr int LAG = (STAGES + 1) / 2;
+    extern __shared__ __align__(128) unsigned char smem[];
+    __shared__ __align__(8) uint64_t full_bar[STAGES];
+    __shared__ StageMeta meta[STAGES];
+
+    const int lane = threadIdx.x;
+    if (lane == 0) {
+        for (int s = 0; s < STAGES; ++s) mbar_init(smem_u32(&full_bar[s]), 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncwarp();
+
+    const int64_t total = n_runs * n_planes;     // item = plane * n_runs + run (plane-major)
+    const int64_t G = gridDim.x;
+    const uint32_t ring = smem_u32(smem);
+    int64_t it = 0;                               // items issued by this CTA so far
+
+    for (int64_t base = blockIdx.x; base < total; base += 32 * G) {
+        // every lane decodes one of the next 32 items of this CTA
+        const int64_t mine = base + static_cast<int64_t>(lane) * G;
+        Item my{nullptr, nullptr, 0};
+        if (mine < total) {
+            const int32_t pl = static_cast<int32_t>(mine / n_runs);
+            const int64_t run = mine - static_cast<int64_t>(pl) * n_runs;
+            my = decode_item(runs, reqs, run, planes.p[pl], plane0 + pl, buf, row_bytes);
+        }
+        const char* my_src = pack ? my.pool : my.buf;
+        char* my_dst = pack ? my.buf : my.pool;
+        const int64_t left = (total - base + G - 1) / G;   // items of this CTA from base on
+        const int nb = left < 32 ? static_cast<int>(left) : 32;
+        for (int k = 0; k < nb; ++k, ++it) {
+            const char* src = reinterpret_cast<const char*>(
+                __shfl_sync(0xffffffffu, reinterpret_cast<unsigned long long>(my_src), k));
+            char* dst = reinterpret_cast<char*>(
+                __shfl_sync(0xffffffffu, reinterpret_cast<unsigned long long>(my_dst), k));
+            const uint32_t bytes = __shfl_sync(0xffffffffu, my.bytes, k);
+            if (lane == 0) {
+                const int st = static_cast<int>(it % STAGES);
+                // slot st was last read by the store of item it-STAGES: all but the
+                // newest STAGES-1-LAG store groups must have finished reading smem
+                bulk_wait_read<STAGES - 1 - LAG>();
+                const uint32_t bar = smem_u32(&full_bar[st]);
+                meta[st].dst = dst;
+                meta[st].bytes = bytes;
+                mbar_expect_tx(bar, bytes);
+                bulk_g2s(ring + st * stage_bytes, src, bytes, bar);
+                if (it >= LAG) {
+                    const int64_t j = it - LAG;
+                    const int sj = static_cast<int>(j % STAGES);
+                    mbar_wait(smem_u32(&full_bar[sj]), static_cast<uint32_t>((j / STAGES) & 1));
+                    bulk_s2g(meta[sj].dst, ring + sj * stage_bytes, meta[sj].bytes);
+                    bulk_commit();
+                }
+            }
+        }
+    }
+    if (lane == 0) {
+        // drain: stores of the last min(it, LAG) items
+        for (int64_t j = (it > LAG ? it - LAG : 0); j < it; ++j) {
+            const int sj = static_cast<int>(j % STAGES);
+            mbar_wait(smem_u32(&full_bar[sj]), static_cast<uint32_t>((j / STAGES) & 1));
+            bulk_s2g(meta[sj].dst, ring + sj * stage_bytes, meta[sj].bytes);
+            bulk_commit();
+        }
+        bulk_wait_all();
+    }
+}
+
+struct BulkCfg {
+    int stages;
+    uint32_t stage_bytes;
+    size_t smem;
+    int ctas_per_sm;
+};
+
+BulkCfg bulk_config(int64_t item_bytes_max) {
+    // round the slot to 128 B; total ring per SM ~192 KiB, more CTAs for small items
+    const uint32_t sb = static_cast<uint32_t>((item_bytes_max + 127) & ~int64_t{127});
+    BulkCfg c{};
+    c.stage_bytes = sb;
+    if (sb > 16384)      { c.stages = 3;  c.ctas_per_sm = 2; }
+    else if (sb > 8192)  { c.stages = 4;  c.ctas_per_sm = 3; }
+    else if (sb > 4096)  { c.stages = 6;  c.ctas_per_sm = 4; }
+    else if (sb > 2048)  { c.stages = 8;  c.ctas_per_sm = 6; }
+    else                 { c.stages = 16; c.ctas_per_sm = 6; }
+    c.smem = static_cast<size_t>(c.stages) * sb;
+    return c;
+}
+
+int g_num_sms = 0;
+
+template <int STAGES>
+cudaError_t launch_bulk(const PlaneTable& pt, const CopyArgs& a, int32_t plane0, int32_t np,
+                        const BulkCfg& c) {
+    auto kern = kv_copy_bulk<STAGES>;
+    static bool attr_set = false;
+    if (!attr_set) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             200 * 1024);
+        if (e != cudaSuccess) return e;
+        attr_set = true;
+    }
+    const int64_t total = a.n_runs * np;
+    int64_t grid = static_cast<int64_t>(g_num_sms) * c.ctas_per_sm;
+    if (grid > total) grid = total;
+    kern<<<static_cast<unsigned>(grid), 32, c.smem, a.stream>>>(
+        pt, a.runs, a.reqs, a.n_runs, np, static_cast<char*>(a.buf),
+        static_cast<uint32_t>(a.row_bytes), c.stage_bytes, plane0, a.pack ? 1 : 0);
+    return cudaGetLastError();
+}
+
+}  // namespace
+
+int resolve_kernel(const CopyArgs& a) {
+    int k = a.kernel;
+    const int64_t item_max = static_cast<int64_t>(a.max_count) * a.row_bytes;
+    if (k == kKernelBulk && item_max > kChunkBytes) k = kKernelWarp;  // one row > ring slot
+    if (k == kKernelAuto) k = kKernelWarp;
+    return k;
+}
+
+cudaError_t launch_kv_copy(const CopyArgs& a) {
+    if (a.n_runs == 0 || a.n_planes == 0) return cudaSuccess;
+    if (g_num_sms == 0) {
+        int dev = 0;
+        cudaError_t e = cudaGetDevice(&dev);
+        if (e != cudaSuccess) return e;
+        e = cudaDeviceGetAttribute(&g_num_sms, cudaDevAttrMultiProcessorCount, dev);
+        if (e != cudaSuccess) return e;
+    }
+    const int kernel = resolve_kernel(a);
+    const int64_t item_max = static_cast<int64_t>(a.max_count) * a.row_bytes;
+
+    for (int32_t plane0 = 0; plane0 < a.n_planes; plane0 += kMaxPlanesPerLaunch) {
+        const int32_t np = (a.n_planes - plane0 < kMaxPlanesPerLaunch) ? a.n_planes - plane0
+                                                                        : kMaxPlanesPerLaunch;
+        PlaneTable pt;
+        for (int i = 0; i < np; ++i) pt.p[i] = a.planes[plane0 + i];
+        for (int i = np; i < kMaxPlanesPerLaunch; ++i) pt.p[i] = nullptr;
+
+        cudaError_t e = cudaSuccess;
+        if (kernel == kKernelBulk) {
+            const BulkCfg c = bulk_config(item_max);
+            switch (c.stages) {
+                case 3:  e = launch_bulk<3>(pt, a, plane0, np, c); break;
+                case 4:  e = launch_bulk<4>(pt, a, plane0, np, c); break;
+                case 6:  e = launch_bulk<6>(pt, a, plane0, np, c); break;
+                case 8:  e = launch_bulk<8>(pt, a, plane0, np, c); break;
+                default: e = launch_bulk<16>(pt, a, plane0, np, c); break;
+            }
+        } else {
+            const int64_t gx = (a.n_runs + kWarpsPerCta - 1) / kWarpsPerCta;
+            // gridDim.x is limited to 2^31-1 blocks; n_runs < 2^34 is far beyond any plan
+            dim3 grid(static_cast<unsigned>(gx), static_cast<unsigned>(np), 1);
+            kv_copy_warp<8><<<grid, kWarpsPerCta * 32, 0, a.stream>>>(
+                pt, a.runs, a.reqs, a.n_runs, static_cast<char*>(a.buf),
+                static_cast<uint32_t>(a.row_bytes), plane0, a.pack ? 1 : 0);
+            e = cudaGetLastError();
+        }
+        if (e != cudaSuccess) return e;
+    }
+    return cudaSuccess;
+}
+
+}  // namespace lumen

@@ -1,0 +1,36 @@
+// Launcher interface between the C entry points (lib.cu) and the kernels (kernels.cu).
+#pragma once
+#include <cuda_runtime.h>
+
+#include <cstdint>
+
+#include "plan.hpp"
+
+namespace lumen {
+
+constexpr int kMaxPlanesPerLaunch = 256;  // plane pointers travel as kernel parameters
+
+enum KernelKind : int { kKernelAuto = 0, kKernelWarp = 1, kKernelBulk = 2 };
+
+struct CopyArgs {
+    const RunDesc* runs = nullptr;   // device
+    const ReqDesc* reqs = nullptr;   // device
+    int64_t n_runs = 0;
+    int64_t row_bytes = 0;
+    int32_t max_count = 0;           // longest run in tokens
+    const void* const* planes = nullptr;  // HOST array of n_planes device pointers (K0,V0,K1,V1,..)
+    int32_t n_planes = 0;
+    void* buf = nullptr;             // device-accessible checkpoint buffer
+    bool buf_is_host = false;        // mapped pinned host memory
+    bool pack = true;                // true: planes -> buf, false: buf -> planes
+    int kernel = kKernelAuto;
+    cudaStream_t stream = nullptr;
+};
+
+// Enqueues the copy.  No synchronisation, no allocation.
+cudaError_t launch_kv_copy(const CopyArgs& a);
+
+// Which kernel AUTO resolves to for these arguments (exposed for tests / bench notes).
+int resolve_kernel(const CopyArgs& a);
+
+}  // namespace lumen

@@ -1,0 +1,343 @@
+// C entry points of include/lumen_kv.h: plan objects, the descriptor arena and the
+// marshalling into launch_kv_copy.  All CUDA runtime use outside the kernels is here.
+#include <cuda_runtime.h>
+
+#include <cstdlib>
+#include <cstring>
+#include <mutex>
+#include <new>
+#include <vector>
+
+#include "kernels.hpp"
+#include "lumen_kv.h"
+#include "plan.hpp"
+
+namespace lumen {
+namespace {
+
+thread_local int t_last_cuda_error = 0;
+
+inline int cuda_fail(cudaError_t e) {
+    t_last_cuda_error = static_cast<int>(e);
+    (void)cudaGetLastError();  // clear the sticky-free error state
+    return LUMEN_KV_ECUDA;
+}
+
+// A descriptor blob: pinned host staging + device copy + the events that say when
+// the device copy is no longer read by enqueued work.
+struct Blob {
+    void* host = nullptr;   // cudaHostAlloc (or malloc for HOST_ONLY)
+    void* dev = nullptr;    // cudaMalloc
+    size_t cap = 0;
+    bool host_only = false;
+    std::vector<std::pair<cudaStream_t, cudaEvent_t>> uses;  // last use per stream
+};
+
+// Recycles blobs so that a build -> pack -> free loop per decode iteration performs
+// no cudaMalloc / cudaHostAlloc in steady state (SURVEY.md section 7.3 hard part 2).
+class Arena {
+public:
+    int acquire(size_t bytes, Blob** out) {
+        size_t cap = 4096;
+        while (cap < bytes) cap <<= 1;
+        {
+            std::lock_guard<std::mutex> g(mu_);
+            for (size_t i = 0; i < free_.size(); ++i) {
+                Blob* b = free_[i];
+                if (b->cap != cap || !idle(b)) continue;
+                free_.erase(free_.begin() + static_cast<long>(i));
+                *out = b;
+                return LUMEN_KV_OK;
+            }
+        }
+        Blob* b = new (std::nothrow) Blob();
+        if (!b) return LUMEN_KV_ENOMEM;
+        b->cap = cap;
+        cudaError_t e = cudaHostAlloc(&b->host, cap, cudaHostAllocDefault);
+        if (e == cudaSuccess) e = cudaMalloc(&b->dev, cap);
+        if (e != cudaSuccess) {
+            if (b->host) cudaFreeHost(b->host);
+            delete b;
+            if (e == cudaErrorMemoryAllocation) {
+                (void)cudaGetLastError();
+                return LUMEN_KV_ENOMEM;
+            }
+            return cuda_fail(e);
+        }
+        *out = b;
+        return LUMEN_KV_OK;
+    }
+
+    void release(Blob* b) {
+        if (b->host_only) {
+            std::free(b->host);
+            delete b;
+            return;
+        }
+        std::lock_guard<std::mutex> g(mu_);
+        free_.push_back(b);
+        // bound the cache: drop the oldest idle blobs beyond 64 entries
+        while (free_.size() > 64) {
+            Blob* old = free_.front();
+            if (!idle(old)) break;
+            free_.erase(free_.begin());
+            destroy(old);
+        }
+    }
+
+    void trim() {
+        cudaDeviceSynchronize();
+        std::lock_guard<std::mutex> g(mu_);
+        for (Blob* b : free_) destroy(b);
+        free_.clear();
+    }
+
+private:
+    static bool idle(Blob* b) {
+        for (auto& u : b->uses)
+            if (cudaEventQuery(u.second) != cudaSuccess) {
+                (void)cudaGetLastError();
+                return false;
+            }
+        return true;
+    }
+    static void destroy(Blob* b) {
+        for (auto& u : b->uses) cudaEventDestroy(u.second);
+        if (b->host) cudaFreeHost(b->host);
+        if (b->dev) cudaFree(b->dev);
+        delete b;
+    }
+    std::mutex mu_;
+    std::vector<Blob*> free_;
+};
+
+Arena& arena() {
+    static Arena* a = new Arena();  // leaked on purpose: no CUDA calls at process exit
+    return *a;
+}
+
+}  // namespace
+}  // namespace lumen
+
+struct lumen_kv_plan {
+    lumen::HostPlan hp;        // runs/reqs vectors are released after upload unless host-only
+    lumen::Blob* blob = nullptr;
+    const lumen::RunDesc* h_runs = nullptr;   // inside blob->host
+    const lumen::ReqDesc* h_reqs = nullptr;
+    const lumen::RunDesc* d_runs = nullptr;   // inside blob->dev
+    const lumen::ReqDesc* d_reqs = nullptr;
+    int64_t n_runs = 0;
+    int32_t n_reqs = 0;
+    uint32_t flags = 0;
+};
+
+namespace lumen {
+namespace {
+
+// record "plan still in use on `stream`" so the arena does not recycle the blob early
+int note_use(lumen_kv_plan* p, cudaStream_t stream) {
+    Blob* b = p->blob;
+    for (auto& u : b->uses)
+        if (u.first == stream) {
+            cudaError_t e = cudaEventRecord(u.second, stream);
+            return e == cudaSuccess ? LUMEN_KV_OK : cuda_fail(e);
+        }
+    cudaEvent_t ev;
+    cudaError_t e = cudaEventCreateWithFlags(&ev, cudaEventDisableTiming);
+    if (e != cudaSuccess) return cuda_fail(e);
+    e = cudaEventRecord(ev, stream);
+    if (e != cudaSuccess) {
+        cudaEventDestroy(ev);
+        return cuda_fail(e);
+    }
+    b->uses.emplace_back(stream, ev);
+    return LUMEN_KV_OK;
+}
+
+int run_copy(const lumen_kv_plan* plan, const void* const* k_planes, const void* const* v_planes,
+             void* buf, int64_t buf_bytes, int kind, void* stream, bool pack) {
+    if (!plan) return LUMEN_KV_EINVAL;
+    if (plan->flags & LUMEN_KV_HOST_ONLY) return LUMEN_KV_EINVAL;
+    if (kind != LUMEN_KV_MEM_DEVICE && kind != LUMEN_KV_MEM_HOST_MAPPED) return LUMEN_KV_EINVAL;
+    if (buf_bytes < plan->hp.total_bytes) return LUMEN_KV_ESIZE;
+    if (plan->hp.total_bytes == 0) return LUMEN_KV_OK;  // A4: empty plan launches nothing
+    if (!k_planes || !v_planes || !buf) return LUMEN_KV_EINVAL;
+
+    const int32_t L = plan->hp.geom.num_layers;
+    std::vector<const void*> planes(static_cast<size_t>(2 * L));
+    for (int32_t l = 0; l < L; ++l) {
+        const void* k = k_planes[l];
+        const void* v = v_planes[l];
+        if (!k || !v) return LUMEN_KV_EINVAL;
+        if ((reinterpret_cast<uintptr_t>(k) | reinterpret_cast<uintptr_t>(v)) & 15)
+            return LUMEN_KV_EINVAL;
+        planes[2 * l] = k;
+        planes[2 * l + 1] = v;
+    }
+    void* dev_buf = buf;
+    if (kind == LUMEN_KV_MEM_HOST_MAPPED) {
+        cudaError_t e = cudaHostGetDevicePointer(&dev_buf, buf, 0);
+        if (e != cudaSuccess) {
+            t_last_cuda_error = static_cast<int>(e);
+            (void)cudaGetLastError();
+            return LUMEN_KV_EINVAL;  // not pinned / not mapped
+        }
+    }
+    if (reinterpret_cast<uintptr_t>(dev_buf) & 15) return LUMEN_KV_EINVAL;
+
+    CopyArgs a;
+    a.runs = plan->d_runs;
+    a.reqs = plan->d_reqs;
+    a.n_runs = plan->n_runs;
+    a.row_bytes = plan->hp.row_bytes;
+    a.max_count = plan->hp.max_count;
+    a.planes = planes.data();
+    a.n_planes = 2 * L;
+    a.buf = dev_buf;
+    a.buf_is_host = (kind == LUMEN_KV_MEM_HOST_MAPPED);
+    a.pack = pack;
+    a.kernel = static_cast<int>((plan->flags & LUMEN_KV_KERNEL_MASK) >> LUMEN_KV_KERNEL_SHIFT);
+    a.stream = static_cast<cudaStream_t>(stream);
+    cudaError_t e = launch_kv_copy(a);
+    if (e != cudaSuccess) return cuda_fail(e);
+    return note_use(const_cast<lumen_kv_plan*>(plan), a.stream);
+}
+
+}  // namespace
+}  // namespace lumen
+
+extern "C" {
+
+int lumen_kv_plan_build(const lumen_kv_geom* geom, const lumen_kv_req* reqs, int32_t num_reqs,
+                        uint32_t flags, void* stream, lumen_kv_plan** out) {
+    using namespace lumen;
+    if (!out) return LUMEN_KV_EINVAL;
+    *out = nullptr;
+    const uint32_t ksel = flags & LUMEN_KV_KERNEL_MASK;
+    if (ksel != LUMEN_KV_KERNEL_AUTO && ksel != LUMEN_KV_KERNEL_WARP && ksel != LUMEN_KV_KERNEL_BULK)
+        return LUMEN_KV_EINVAL;
+    lumen_kv_plan* p = new (std::nothrow) lumen_kv_plan();
+    if (!p) return LUMEN_KV_ENOMEM;
+    int rc;
+    try {
+        rc = build_host_plan(geom, reqs, num_reqs, flags, &p->hp);
+    } catch (const std::bad_alloc&) {
+        rc = LUMEN_KV_ENOMEM;
+    }
+    if (rc != LUMEN_KV_OK) {
+        delete p;
+        return rc;
+    }
+    p->flags = flags;
+    p->n_runs = static_cast<int64_t>(p->hp.runs.size());
+    p->n_reqs = num_reqs;
+
+    const size_t run_bytes = p->hp.runs.size() * sizeof(RunDesc);
+    const size_t req_bytes = p->hp.reqs.size() * sizeof(ReqDesc);
+    const size_t total = run_bytes + req_bytes;
+
+    if (flags & LUMEN_KV_HOST_ONLY) {
+        Blob* b = new (std::nothrow) Blob();
+        if (!b) { delete p; return LUMEN_KV_ENOMEM; }
+        b->host_only = true;
+        b->cap = total ? total : 16;
+        b->host = std::malloc(b->cap);
+        if (!b->host) { delete b; delete p; return LUMEN_KV_ENOMEM; }
+        p->blob = b;
+    } else if (total > 0) {
+        rc = arena().acquire(total, &p->blob);
+        if (rc != LUMEN_KV_OK) { delete p; return rc; }
+    }
+    if (p->blob) {
+        char* h = static_cast<char*>(p->blob->host);
+        if (run_bytes) std::memcpy(h, p->hp.runs.data(), run_bytes);
+        if (req_bytes) std::memcpy(h + run_bytes, p->hp.reqs.data(), req_bytes);
+        p->h_runs = reinterpret_cast<const RunDesc*>(h);
+        p->h_reqs = reinterpret_cast<const ReqDesc*>(h + run_bytes);
+        if (!(flags & LUMEN_KV_HOST_ONLY)) {
+            char* d = static_cast<char*>(p->blob->dev);
+            p->d_runs = reinterpret_cast<const RunDesc*>(d);
+            p->d_reqs = reinterpret_cast<const ReqDesc*>(d + run_bytes);
+            cudaStream_t s = static_cast<cudaStream_t>(stream);
+            cudaError_t e = cudaMemcpyAsync(d, h, total, cudaMemcpyHostToDevice, s);
+            if (e != cudaSuccess) {
+                arena().release(p->blob);
+                delete p;
+                return cuda_fail(e);
+            }
+            rc = note_use(p, s);
+            if (rc != LUMEN_KV_OK) { arena().release(p->blob); delete p; return rc; }
+        }
+    }
+    // the vectors are no longer needed: descriptors live in the blob
+    std::vector<RunDesc>().swap(p->hp.runs);
+    std::vector<ReqDesc>().swap(p->hp.reqs);
+    *out = p;
+    return LUMEN_KV_OK;
+}
+
+int64_t lumen_kv_plan_bytes(const lumen_kv_plan* plan) {
+    return plan ? plan->hp.total_bytes : int64_t{LUMEN_KV_EINVAL};
+}
+
+int64_t lumen_kv_plan_req_offset(const lumen_kv_plan* plan, int32_t r) {
+    if (!plan || r < 0 || r > plan->n_reqs) return LUMEN_KV_EINVAL;
+    return plan->hp.req_offset[static_cast<size_t>(r)];
+}
+
+int64_t lumen_kv_plan_num_runs(const lumen_kv_plan* plan) {
+    return plan ? plan->n_runs : int64_t{LUMEN_KV_EINVAL};
+}
+
+int lumen_kv_plan_get_run(const lumen_kv_plan* plan, int64_t i, lumen_kv_run_info* out) {
+    if (!plan || !out || i < 0 || i >= plan->n_runs) return LUMEN_KV_EINVAL;
+    const lumen::RunDesc& d = plan->h_runs[i];
+    const int64_t off = ((static_cast<int64_t>(d.src_hi) << 32) | d.src_lo) << 4;
+    const int64_t page = off / plan->hp.page_stride;
+    const int64_t slot = (off % plan->hp.page_stride) / plan->hp.row_bytes;
+    out->src_slot = page * plan->hp.geom.page_size + slot;
+    out->dst_token = d.dst_tok;
+    out->req = static_cast<int32_t>(d.req);
+    out->count = d.count;
+    return LUMEN_KV_OK;
+}
+
+int lumen_kv_checkpoint_pack(const lumen_kv_plan* plan, const void* const* k_planes,
+                             const void* const* v_planes, void* dst, int64_t dst_bytes,
+                             int dst_kind, void* stream) {
+    return lumen::run_copy(plan, k_planes, v_planes, dst, dst_bytes, dst_kind, stream, true);
+}
+
+int lumen_kv_restore_unpack(const lumen_kv_plan* plan, void* const* k_planes,
+                            void* const* v_planes, const void* src, int64_t src_bytes,
+                            int src_kind, void* stream) {
+    return lumen::run_copy(plan, const_cast<const void* const*>(k_planes),
+                           const_cast<const void* const*>(v_planes), const_cast<void*>(src),
+                           src_bytes, src_kind, stream, false);
+}
+
+void lumen_kv_plan_free(lumen_kv_plan* plan) {
+    if (!plan) return;
+    if (plan->blob) lumen::arena().release(plan->blob);
+    delete plan;
+}
+
+void lumen_kv_trim(void) { lumen::arena().trim(); }
+
+const char* lumen_kv_strerror(int status) {
+    switch (status) {
+        case LUMEN_KV_OK: return "ok";
+        case LUMEN_KV_EINVAL: return "invalid argument (null, misaligned, bad geometry, kind or flag)";
+        case LUMEN_KV_ERANGE: return "page index or token range outside the page table / pool";
+        case LUMEN_KV_EOVERLAP: return "a physical page is addressed more than once";
+        case LUMEN_KV_ESIZE: return "buffer smaller than the plan's bytes";
+        case LUMEN_KV_ENOMEM: return "out of host or device memory for descriptors";
+        case LUMEN_KV_ECUDA: return "CUDA runtime error (see lumen_kv_last_cuda_error)";
+        default: return "unknown status";
+    }
+}
+
+int lumen_kv_last_cuda_error(void) { return lumen::t_last_cuda_error; }
+int lumen_kv_version(void) { return LUMEN_KV_VERSION; }
+
+}  // extern "C"

@@ -1,0 +1,163 @@
+// Host plan builder: step a2 of the hot path.
+// Splits each request's token range [t_begin, t_end) -- the KV produced since the
+// last checkpoint, PAPER.md:145 -- at page boundaries into token-runs, computes the
+// per-request buffer offsets (exclusive prefix sum of n_r * 2L * row), optionally
+// merges runs over physically adjacent pages, and validates everything so that the
+// kernels never need a bounds check.  Pure C++: no CUDA types or calls in here.
+#include "plan.hpp"
+
+#include <algorithm>
+#include <limits>
+
+namespace lumen {
+namespace {
+
+struct Extent {           // a pool-contiguous, buffer-contiguous stretch of tokens
+    int64_t src_off = 0;  // byte offset inside a plane
+    int64_t dst_tok = 0;  // request-relative first token
+    int64_t count = 0;    // tokens
+};
+
+inline void emit(HostPlan* hp, const Extent& x, int32_t req, int64_t chunk_tokens) {
+    int64_t done = 0;
+    while (done < x.count) {
+        const int64_t c = std::min(chunk_tokens, x.count - done);
+        const uint64_t off16 = static_cast<uint64_t>(x.src_off + done * hp->row_bytes) >> 4;
+        RunDesc d;
+        d.src_lo = static_cast<uint32_t>(off16 & 0xFFFFFFFFu);
+        d.src_hi = static_cast<uint16_t>(off16 >> 32);
+        d.dst_tok = static_cast<uint32_t>(x.dst_tok + done);
+        d.req = static_cast<uint32_t>(req);
+        d.count = static_cast<uint16_t>(c);
+        hp->runs.push_back(d);
+        hp->max_count = std::max<int32_t>(hp->max_count, static_cast<int32_t>(c));
+        done += c;
+    }
+}
+
+}  // namespace
+
+int build_host_plan(const lumen_kv_geom* g, const lumen_kv_req* reqs, int32_t num_reqs,
+                    uint32_t flags, HostPlan* hp) {
+    if (!g || !hp) return LUMEN_KV_EINVAL;
+    if (num_reqs < 0 || (num_reqs > 0 && !reqs)) return LUMEN_KV_EINVAL;
+    const uint32_t known = LUMEN_KV_VALIDATE_UNIQUE_DST | LUMEN_KV_MERGE_ADJACENT |
+                           LUMEN_KV_HOST_ONLY | LUMEN_KV_KERNEL_MASK;
+    if (flags & ~known) return LUMEN_KV_EINVAL;
+    if (g->num_layers < 1 || g->kv_heads < 1 || g->head_dim < 1 || g->page_size < 1 ||
+        g->elem_bytes < 1 || g->reserved != 0)
+        return LUMEN_KV_EINVAL;
+    if (g->num_pages < 1 || g->num_pages >= (int64_t{1} << 31)) return LUMEN_KV_EINVAL;
+    if (g->num_layers > 32767) return LUMEN_KV_EINVAL;
+
+    const int64_t S = g->page_size;
+    const int64_t row = int64_t{g->kv_heads} * g->head_dim * g->elem_bytes;
+    if (row % 16 != 0 || row > (int64_t{1} << 30)) return LUMEN_KV_EINVAL;
+    if (S > (int64_t{1} << 20)) return LUMEN_KV_EINVAL;
+    const int64_t dense = S * row;
+    int64_t stride = g->page_stride_bytes;
+    if (stride == 0) stride = dense;
+    if (stride < dense || stride % 16 != 0) return LUMEN_KV_EINVAL;
+    // pool byte offsets must fit 48 bits of 16-byte units
+    if (static_cast<long double>(stride) * static_cast<long double>(g->num_pages) >=
+        static_cast<long double>(int64_t{1} << 52))
+        return LUMEN_KV_EINVAL;
+
+    hp->geom = *g;
+    hp->row_bytes = row;
+    hp->page_stride = stride;
+    hp->runs.clear();
+    hp->reqs.assign(static_cast<size_t>(num_reqs), ReqDesc{0, 0});
+    hp->req_offset.assign(static_cast<size_t>(num_reqs) + 1, 0);
+    hp->max_count = 0;
+
+    const bool merge = (flags & LUMEN_KV_MERGE_ADJACENT) && stride == dense;
+    const bool unique = (flags & LUMEN_KV_VALIDATE_UNIQUE_DST) != 0;
+    const int64_t chunk_tokens =
+        std::min<int64_t>(65535, std::max<int64_t>(1, kChunkBytes / row));
+    const int64_t planes = 2 * int64_t{g->num_layers};
+
+    // pass 1: validate ranges, sizes and page indices; count touched pages
+    int64_t tokens = 0, touched = 0;
+    for (int32_t r = 0; r < num_reqs; ++r) {
+        const lumen_kv_req& q = reqs[r];
+        if (q.t_begin < 0 || q.t_end < q.t_begin || q.page_table_len < 0) return LUMEN_KV_EINVAL;
+        const int64_t n = q.t_end - q.t_begin;
+        if (n >= (int64_t{1} << 32)) return LUMEN_KV_EINVAL;
+        hp->reqs[r].row_base = tokens * planes;
+        hp->reqs[r].n = n;
+        hp->req_offset[r] = tokens * planes * row;
+        if (n == 0) continue;
+        const int64_t lp0 = q.t_begin / S, lp1 = (q.t_end - 1) / S;
+        if (!q.page_table || lp1 >= q.page_table_len) return LUMEN_KV_ERANGE;
+        for (int64_t lp = lp0; lp <= lp1; ++lp) {
+            const int32_t p = q.page_table[lp];
+            if (p < 0 || int64_t{p} >= g->num_pages) return LUMEN_KV_ERANGE;
+        }
+        touched += lp1 - lp0 + 1;
+        tokens += n;
+        if (tokens > (std::numeric_limits<int64_t>::max() / 4) / (planes * row))
+            return LUMEN_KV_EINVAL;
+    }
+    hp->total_tokens = tokens;
+    hp->total_bytes = tokens * planes * row;
+    hp->req_offset[num_reqs] = hp->total_bytes;
+
+    // optional: every physical page addressed at most once across the whole plan (A5)
+    if (unique && touched > 0) {
+        const int64_t N = g->num_pages;
+        if (N <= 64 * touched || N <= (int64_t{1} << 23)) {
+            std::vector<uint64_t> bits(static_cast<size_t>((N + 63) / 64), 0);
+            for (int32_t r = 0; r < num_reqs; ++r) {
+                const lumen_kv_req& q = reqs[r];
+                if (q.t_end == q.t_begin) continue;
+                for (int64_t lp = q.t_begin / S; lp <= (q.t_end - 1) / S; ++lp) {
+                    const uint32_t p = static_cast<uint32_t>(q.page_table[lp]);
+                    uint64_t& w = bits[p >> 6];
+                    const uint64_t m = uint64_t{1} << (p & 63);
+                    if (w & m) return LUMEN_KV_EOVERLAP;
+                    w |= m;
+                }
+            }
+        } else {
+            std::vector<int32_t> all;
+            all.reserve(static_cast<size_t>(touched));
+            for (int32_t r = 0; r < num_reqs; ++r) {
+                const lumen_kv_req& q = reqs[r];
+                if (q.t_end == q.t_begin) continue;
+                for (int64_t lp = q.t_begin / S; lp <= (q.t_end - 1) / S; ++lp)
+                    all.push_back(q.page_table[lp]);
+            }
+            std::sort(all.begin(), all.end());
+            if (std::adjacent_find(all.begin(), all.end()) != all.end())
+                return LUMEN_KV_EOVERLAP;
+        }
+    }
+
+    // pass 2: flatten into runs
+    hp->runs.reserve(static_cast<size_t>(touched * std::max<int64_t>(1, (dense + kChunkBytes - 1) / kChunkBytes)));
+    for (int32_t r = 0; r < num_reqs; ++r) {
+        const lumen_kv_req& q = reqs[r];
+        if (q.t_end == q.t_begin) continue;
+        Extent cur;
+        int64_t t = q.t_begin;
+        while (t < q.t_end) {
+            const int64_t lp = t / S, slot = t % S;
+            const int64_t cnt = std::min(S - slot, q.t_end - t);
+            const int64_t off = int64_t{q.page_table[lp]} * stride + slot * row;
+            if (cur.count > 0 && merge && cur.src_off + cur.count * row == off) {
+                cur.count += cnt;           // physically adjacent: extend
+            } else {
+                if (cur.count > 0) emit(hp, cur, r, chunk_tokens);
+                cur.src_off = off;
+                cur.dst_tok = t - q.t_begin;
+                cur.count = cnt;
+            }
+            t += cnt;
+        }
+        if (cur.count > 0) emit(hp, cur, r, chunk_tokens);
+    }
+    return LUMEN_KV_OK;
+}
+
+}  // namespace lumen

@@ -1,0 +1,232 @@
+"""GPU parity, small and mid sizes: CUDA path through the C ABI vs the CPU oracle,
+bit for bit, on the same seeded inputs (T2 of SURVEY.md section 4).
+
+Every case runs both kernels (SIMT warp / TMA bulk), both buffer kinds (HBM, mapped
+pinned host) and checks: the packed buffer equals oracle.pack element by element;
+after unpack the WHOLE destination pool equals the oracle's pool (so every non-target
+byte is untouched, including partial first/last pages); guard bands around the
+buffer are intact.
+"""
+import numpy as np
+import pytest
+
+import oracle
+from workloads import cfg0_tiny, cfg1_qwen14b, cfg2_qwen32b, cfg4_longctx, random_tiny, substream, MASTER_SEED
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def G():
+    import torch
+    assert torch.cuda.is_available()
+    from tests import gpu_util
+    gpu_util.build_all()
+    return gpu_util
+
+
+def run_case(G, w, kernel, where, *, merge=False, seed=MASTER_SEED):
+    import torch
+    lk = G.lk
+    flags = G.KERNELS[kernel] | (lk.LUMEN_KV_MERGE_ADJACENT if merge else 0)
+    # ---- oracle side -----------------------------------------------------------
+    K, V = G.host_planes(w.geom, seed)
+    B_ref = oracle.pack(w.geom, K, V, w.reqs)
+    K2, V2 = G.host_planes(w.geom, seed + 1)
+    oracle.unpack(w.geom, K2, V2, w.restore_reqs, B_ref, check_overlap=len(w.reqs) and w.tokens < 3000)
+    # ---- CUDA side -------------------------------------------------------------
+    pool_a = G.make_pool(w.geom, seed)
+    pool_b = G.make_pool(w.geom, seed + 1)
+    ck_a, ck_b = G.Checkpointer(pool_a, flags), G.Checkpointer(pool_b, flags)
+    plan = ck_a.plan(w.reqs)
+    assert plan.nbytes == B_ref.size * 2
+    whole, buf = G.alloc_buffer(plan.nbytes, where)
+    ck_a.pack(plan, buf)
+    torch.cuda.synchronize()
+    got = G.buf_to_np(buf, plan.nbytes)
+    assert np.array_equal(got, B_ref), f"pack mismatch kernel={kernel} where={where}"
+    assert G.guards_intact(whole, plan.nbytes)
+    # source pool unchanged by pack
+    for t, ref in zip(pool_a.planes(), [x for kv in zip(K, V) for x in kv]):
+        assert np.array_equal(G.plane_to_np(t), ref)
+    # ---- restore into pool B under the fresh page tables -----------------------
+    rplan = ck_b.plan(w.restore_reqs, unique_dst=True)
+    ck_b.unpack(rplan, buf)
+    torch.cuda.synchronize()
+    for t, ref in zip(pool_b.planes(), [x for kv in zip(K2, V2) for x in kv]):
+        assert np.array_equal(G.plane_to_np(t), ref), f"unpack mismatch kernel={kernel} where={where}"
+    # P3 on the GPU: packing the restored pool returns the identical buffer
+    whole2, buf2 = G.alloc_buffer(plan.nbytes, "device")
+    ck_b.pack(rplan, buf2)
+    torch.cuda.synchronize()
+    assert np.array_equal(G.buf_to_np(buf2, plan.nbytes), B_ref)
+    assert G.guards_intact(whole2, plan.nbytes)
+    plan.close(); rplan.close()
+
+
+@pytest.mark.parametrize("where", ["device", "host"])
+@pytest.mark.parametrize("kernel", ["warp", "bulk", "auto"])
+def test_cfg0_tiny(G, kernel, where):
+    run_case(G, cfg0_tiny(), kernel, where)
+    run_case(G, cfg0_tiny(full_prefix=True), kernel, where)
+
+
+@pytest.mark.parametrize("kernel", ["warp", "bulk"])
+def test_random_tiny_geometries(G, kernel):
+    rng = substream(2024, "gpu_tiny")
+    n = 0
+    while n < 40:
+        w = random_tiny(rng)
+        if (w.geom[1] * w.geom[2] * 2) % 16:
+            continue
+        run_case(G, w, kernel, "device" if n % 3 else "host", merge=bool(n % 2), seed=n)
+        n += 1
+
+
+@pytest.mark.parametrize("kernel", ["warp", "bulk"])
+def test_mid_cfg1_shape(G, kernel):
+    """Qwen3-14B row/page shape, fewer layers/pages: 32 KiB runs, ragged 16-token deltas."""
+    w = cfg1_qwen14b(L=3, N=1024, n_reqs=24, grow_iters=2, hi=512, lo=20)
+    run_case(G, w, kernel, "device")
+    run_case(G, w.advanced(16), kernel, "host")
+    run_case(G, cfg1_qwen14b(L=3, N=1024, n_reqs=24, grow_iters=2, hi=512, lo=20, aligned=True), kernel, "device")
+
+
+@pytest.mark.parametrize("kernel", ["warp", "bulk"])
+def test_mid_cfg2_shape_full_prefix(G, kernel):
+    w = cfg2_qwen32b(L=2, N=1200, n_reqs=5, prompt=1000)      # 1000 tokens: ragged last page
+    run_case(G, w, kernel, "device")
+
+
+@pytest.mark.parametrize("kernel", ["warp", "bulk"])
+def test_mid_cfg4_token_granular(G, kernel):
+    w = cfg4_longctx(L=2, tokens=3001, wave_reqs=2)          # S = 1: 6002 runs of one 2 KiB row
+    run_case(G, w, kernel, "device")
+    run_case(G, w, kernel, "host", merge=True)
+
+
+@pytest.mark.parametrize("kernel", ["warp", "bulk"])
+def test_tp_rank_shape_and_odd_rows(G, kernel):
+    # H = 4 (one TP2 rank of an 8-kv-head model); and a 48-byte row
+    run_case(G, cfg1_qwen14b(L=2, H=4, N=512, n_reqs=8, grow_iters=2, hi=256, lo=20), kernel, "device")
+    run_case(G, cfg1_qwen14b(L=2, H=1, D=24, N=512, n_reqs=8, grow_iters=2, hi=256, lo=20), kernel, "device")
+    # page larger than the 32 KiB chunk: S = 64 tokens of 2 KiB
+    run_case(G, cfg2_qwen32b(L=1, S=64, N=64, n_reqs=3, prompt=500), kernel, "device")
+
+
+def test_pack_allows_shared_pages(G):
+    import torch
+    rng = substream(5, "shared")
+    for i in range(10):
+        w = random_tiny(rng, allow_shared=True)
+        K, V = G.host_planes(w.geom, i)
+        ref = oracle.pack(w.geom, K, V, w.reqs)
+        pool = G.make_pool(w.geom, i)
+        ck = G.Checkpointer(pool)
+        plan = ck.plan(w.reqs)
+        whole, buf = G.alloc_buffer(plan.nbytes, "device")
+        ck.pack(plan, buf)
+        torch.cuda.synchronize()
+        assert np.array_equal(G.buf_to_np(buf, plan.nbytes), ref)
+
+
+def test_empty_plan_and_errors(G):
+    import torch
+    lk = G.lk
+    w = cfg0_tiny()
+    pool = G.make_pool(w.geom, 1)
+    ck = G.Checkpointer(pool)
+    empty = ck.plan([])
+    buf = torch.zeros(64, dtype=torch.uint8, device="cuda")
+    ck.pack(empty, buf); ck.unpack(empty, buf)            # A4: launches nothing, returns OK
+    zero = ck.plan([(w.reqs[0][0], 5, 5)])
+    ck.pack(zero, buf)
+    plan = ck.plan(w.reqs)
+    small = torch.zeros(plan.nbytes - 16, dtype=torch.uint8, device="cuda")
+    with pytest.raises(lk.LumenKVError) as e:
+        ck.pack(plan, small)
+    assert e.value.status == lk.LUMEN_KV_ESIZE
+    big = torch.zeros(plan.nbytes + 16, dtype=torch.uint8, device="cuda")
+    with pytest.raises(lk.LumenKVError) as e:
+        ck.pack(plan, big[8:])                               # misaligned base
+    assert e.value.status == lk.LUMEN_KV_EINVAL
+    pageable = torch.zeros(plan.nbytes, dtype=torch.uint8)
+    with pytest.raises(lk.LumenKVError) as e:                # pageable host memory is not mapped
+        lk.lumen_kv_checkpoint_pack(plan, pool.k_ptrs, pool.v_ptrs, pageable.data_ptr(), plan.nbytes,
+                                    lk.LUMEN_KV_MEM_HOST_MAPPED, 0)
+    assert e.value.status == lk.LUMEN_KV_EINVAL
+    torch.cuda.synchronize()
+
+
+def test_delta_concat_on_gpu(G):
+    """P4 form 2 on the CUDA path: unpack(delta_1); unpack(delta_2) == unpack(full)."""
+    import torch
+    w = cfg0_tiny(full_prefix=True)
+    pool_src = G.make_pool(w.geom, 3)
+    ck_src = G.Checkpointer(pool_src)
+    pool_full, pool_inc = G.make_pool(w.geom, 4), G.make_pool(w.geom, 4)
+    ck_full, ck_inc = G.Checkpointer(pool_full), G.Checkpointer(pool_inc)
+    full = ck_src.plan(w.reqs)
+    bfull = torch.empty(full.nbytes, dtype=torch.uint8, device="cuda")
+    ck_src.pack(full, bfull)
+    ck_full.unpack(ck_full.plan(w.restore_reqs), bfull)
+    cuts = [0, 7, 16, 33, 10**9]
+    for a, b in zip(cuts[:-1], cuts[1:]):
+        d_src = [(pt, min(a, te), min(b, te)) for pt, tb, te in w.reqs]
+        d_dst = [(pt, min(a, te), min(b, te)) for pt, tb, te in w.restore_reqs]
+        p = ck_src.plan(d_src)
+        bd = torch.empty(max(p.nbytes, 16), dtype=torch.uint8, device="cuda")
+        ck_src.pack(p, bd)
+        ck_inc.unpack(ck_inc.plan(d_dst), bd)
+    torch.cuda.synchronize()
+    for x, y in zip(pool_full.planes(), pool_inc.planes()):
+        assert torch.equal(x.view(torch.int16), y.view(torch.int16))
+
+
+def test_plan_reuse_and_free_while_in_flight(G):
+    """build -> pack -> free in a loop with no host sync: the arena must keep descriptors
+    alive until the enqueued work is done, and recycle them afterwards."""
+    import torch
+    w = cfg1_qwen14b(L=2, N=2048, n_reqs=32, grow_iters=40, hi=512, lo=20)
+    K, V = G.host_planes(w.geom, 9)
+    pool = G.make_pool(w.geom, 9)
+    ck = G.Checkpointer(pool)
+    bufs, refs, cur = [], [], w
+    for it in range(32):
+        plan = ck.plan(cur.reqs)
+        buf = torch.empty(plan.nbytes, dtype=torch.uint8, device="cuda")
+        ck.pack(plan, buf)
+        plan.close()                                         # freed while possibly in flight
+        bufs.append(buf); refs.append(oracle.pack(cur.geom, K, V, cur.reqs))
+        cur = cur.advanced(16)
+    torch.cuda.synchronize()
+    for buf, ref in zip(bufs, refs):
+        assert np.array_equal(G.buf_to_np(buf, buf.numel()), ref)
+    G.lk.lumen_kv_trim()
+
+
+def test_two_streams_concurrent(G):
+    """a8 in miniature: unpack on stream 1 while packs of other requests run on stream 2."""
+    import torch
+    w = cfg2_qwen32b(L=2, N=1200, n_reqs=6, prompt=900)
+    seed = 21
+    K, V = G.host_planes(w.geom, seed)
+    pool = G.make_pool(w.geom, seed)
+    ck = G.Checkpointer(pool)
+    # requests 0-2 are "running" (packed); requests 3-5's checkpoint is restored into fresh pages
+    run_reqs, ckpt_reqs, fresh = w.reqs[:3], w.reqs[3:], w.restore_reqs[3:]
+    B_ckpt = oracle.pack(w.geom, K, V, ckpt_reqs)
+    B_run = oracle.pack(w.geom, K, V, run_reqs)
+    oracle.unpack(w.geom, K, V, fresh, B_ckpt)
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    src = torch.from_numpy(B_ckpt.view(np.uint8)).pin_memory()
+    out = G.pinned_buffer(B_run.size * 2)
+    torch.cuda.synchronize()
+    p1 = ck.plan(fresh, unique_dst=True, stream=s1)
+    p2 = ck.plan(run_reqs, stream=s2)
+    ck.unpack(p1, src, stream=s1)
+    ck.pack(p2, out, stream=s2)
+    torch.cuda.synchronize()
+    assert np.array_equal(G.buf_to_np(out, out.numel()), B_run)
+    for t, ref in zip(pool.planes(), [x for kv in zip(K, V) for x in kv]):
+        assert np.array_equal(G.plane_to_np(t), ref)

@@ -1,0 +1,233 @@
+"""CPU tests of the C-ABI library's host logic (no GPU, no compute calls).
+
+T1 of SURVEY.md section 4: the plan builder's runs, expanded back to per-token
+(request, token) -> (pool slot, buffer row), must equal the oracle's index map
+(oracle.pool_index / oracle.buffer_index, i.e. definition C1).  Also: the library
+loads and exports every symbol include/lumen_kv.h declares, sizes and offsets
+match the closed forms, validation rules of section 8(b)/C6 return the documented
+status codes, and compute entry points fail loudly without a CUDA device.
+"""
+import re
+from pathlib import Path
+
+import numpy as np
+import pytest
+
+import oracle
+from oracle import oracle_np
+from workloads import cfg0_tiny, cfg1_qwen14b, cfg2_qwen32b, cfg4_longctx, random_tiny, substream
+
+ROOT = Path(__file__).resolve().parent.parent
+
+
+@pytest.fixture(scope="module")
+def lk():
+    from paper_2606_17787_b200 import build
+    build.build()
+    import paper_2606_17787_b200 as lk
+    return lk
+
+
+def geom_of(lk, w, **kw):
+    L, H, D, S, N = w.geom
+    return lk.make_geom(L, H, D, S, N, **kw)
+
+
+def expand(plan, geom, reqs):
+    """runs -> dict (req, j) -> (global pool slot, count bookkeeping)."""
+    L, H, D, S, N = geom
+    out = {}
+    for i in range(plan.num_runs):
+        r = plan.run(i)
+        assert r.count >= 1
+        for k in range(r.count):
+            key = (r.req, r.dst_token + k)
+            assert key not in out, "token covered twice"
+            out[key] = r.src_slot + k
+    return out
+
+
+def test_exports_match_header(lk):
+    import ctypes
+    text = (ROOT / "include" / "lumen_kv.h").read_text()
+    declared = set(re.findall(r"LUMEN_KV_API[^;(]*?\b(lumen_kv_\w+)\s*\(", text))
+    assert declared == set(lk.EXPORTS)
+    lib = ctypes.CDLL(str(lk.library_path()))
+    for name in declared:
+        assert hasattr(lib, name), name
+    assert lk.lumen_kv_version() == int(re.search(r"#define LUMEN_KV_VERSION (\d+)", text).group(1))
+
+
+def test_struct_layouts_match_header(lk):
+    import ctypes
+    assert ctypes.sizeof(lk.lumen_kv_geom) == 40
+    assert ctypes.sizeof(lk.lumen_kv_req) == 32
+    assert ctypes.sizeof(lk.lumen_kv_run_info) == 24
+
+
+@pytest.mark.parametrize("merge", [False, True])
+def test_t1_runs_equal_oracle_index_map(lk, merge):
+    rng = substream(77, "t1")
+    flags = lk.LUMEN_KV_HOST_ONLY | (lk.LUMEN_KV_MERGE_ADJACENT if merge else 0)
+    cases = [cfg0_tiny(), cfg0_tiny(full_prefix=True)] + [random_tiny(rng, allow_shared=True) for _ in range(150)]
+    for w in cases:
+        L, H, D, S, N = w.geom
+        E = H * D
+        plan = lk.lumen_kv_plan_build(geom_of(lk, w), w.reqs, flags)
+        assert plan.nbytes == 2 * oracle.total_elems(w.geom, w.reqs)
+        m = expand(plan, w.geom, w.reqs)
+        assert len(m) == w.tokens
+        for r, (pt, tb, te) in enumerate(w.reqs):
+            assert plan.req_offset(r) == 2 * oracle.req_offset_elems(w.geom, w.reqs, r)
+            for j in range(te - tb):
+                # oracle: word e=0 of token j lives at pool word slot*E
+                assert m[(r, j)] * E == oracle.pool_index(w.geom, w.reqs, r, j, 0)
+        assert plan.req_offset(len(w.reqs)) == plan.nbytes
+        plan.close()
+
+
+def test_runs_never_cross_pages_unless_merged_and_respect_chunk(lk):
+    w = cfg2_qwen32b(N=2048, n_reqs=4, prompt=1000)
+    L, H, D, S, N = w.geom
+    row = H * D * 2
+    plan = lk.lumen_kv_plan_build(geom_of(lk, w), w.reqs, lk.LUMEN_KV_HOST_ONLY)
+    assert plan.num_runs == sum((te - 1) // S - tb // S + 1 for _, tb, te in w.reqs)
+    for i in range(plan.num_runs):
+        r = plan.run(i)
+        assert r.src_slot // S == (r.src_slot + r.count - 1) // S
+        assert r.count * row <= 32768
+
+
+def test_p9_merge_adjacent_identity_table(lk):
+    # identity page table: every page adjacent -> merged runs are chunk-sized (32 KiB)
+    L, H, D, S, N = 1, 2, 8, 4, 4096          # row = 32 B, page = 128 B
+    g = lk.make_geom(L, H, D, S, N)
+    pt = np.arange(N, dtype=np.int32)
+    a = lk.lumen_kv_plan_build(g, [(pt, 3, 4 * N - 5)], lk.LUMEN_KV_HOST_ONLY)
+    b = lk.lumen_kv_plan_build(g, [(pt, 3, 4 * N - 5)], lk.LUMEN_KV_HOST_ONLY | lk.LUMEN_KV_MERGE_ADJACENT)
+    assert a.num_runs == N - 1                            # last token 4N-6 lies in page N-2
+    assert b.num_runs == -(-(4 * N - 8) // 1024)          # ceil(tokens / (32 KiB / 32 B))
+    assert expand(a, (L, H, D, S, N), None) == expand(b, (L, H, D, S, N), None)
+
+
+def test_page_stride(lk):
+    L, H, D, S, N = 1, 2, 8, 4, 16
+    row = H * D * 2
+    g = lk.make_geom(L, H, D, S, N, page_stride_bytes=S * row + 64)
+    pt = np.array([3, 4, 9], dtype=np.int32)
+    p = lk.lumen_kv_plan_build(g, [(pt, 1, 11)], lk.LUMEN_KV_HOST_ONLY | lk.LUMEN_KV_MERGE_ADJACENT)
+    # padded stride: adjacent pages are not byte-contiguous, so no merging
+    assert [(p.run(i).src_slot, p.run(i).count) for i in range(p.num_runs)] == [(13, 3), (16, 4), (36, 3)]
+
+
+def test_closed_form_sizes_big_configs(lk):
+    w1 = cfg1_qwen14b()
+    p1 = lk.lumen_kv_plan_build(geom_of(lk, w1), w1.reqs, lk.LUMEN_KV_HOST_ONLY)
+    assert p1.nbytes == 167_772_160
+    assert 64 <= p1.num_runs <= 128
+    w2 = cfg2_qwen32b()
+    p2 = lk.lumen_kv_plan_build(geom_of(lk, w2), w2.reqs,
+                                lk.LUMEN_KV_HOST_ONLY | lk.LUMEN_KV_VALIDATE_UNIQUE_DST)
+    assert p2.nbytes == 32 * 2**30 and p2.num_runs == 8192
+    w4 = cfg4_longctx(tokens=4096, wave_reqs=2)
+    p4 = lk.lumen_kv_plan_build(geom_of(lk, w4), w4.reqs,
+                                lk.LUMEN_KV_HOST_ONLY | lk.LUMEN_KV_VALIDATE_UNIQUE_DST)
+    assert p4.num_runs == 8192 and p4.nbytes == 8192 * 256 * 1024
+
+
+def test_oracle_np_layout_equals_plan_offsets(lk):
+    w = cfg1_qwen14b(N=4096, n_reqs=8, grow_iters=2, hi=2048)
+    plan = lk.lumen_kv_plan_build(geom_of(lk, w), w.reqs, lk.LUMEN_KV_HOST_ONLY)
+    lay, total = oracle_np.layout(w.geom, w.reqs)
+    assert plan.nbytes == 2 * total
+    assert [plan.req_offset(r) for r in range(len(w.reqs))] == [2 * o for o, _ in lay]
+
+
+def test_validation_status_codes(lk):
+    E = lk.LumenKVError
+    H = lk.LUMEN_KV_HOST_ONLY
+    g = lk.make_geom(2, 2, 8, 4, 16)
+    pt = np.array([1, 2, 3], dtype=np.int32)
+
+    def status(fn):
+        with pytest.raises(E) as e:
+            fn()
+        return e.value.status
+
+    # geometry
+    assert status(lambda: lk.lumen_kv_plan_build(lk.make_geom(0, 2, 8, 4, 16), [], H)) == lk.LUMEN_KV_EINVAL
+    assert status(lambda: lk.lumen_kv_plan_build(lk.make_geom(1, 1, 4, 4, 16), [], H)) == lk.LUMEN_KV_EINVAL  # row 8 B
+    assert status(lambda: lk.lumen_kv_plan_build(lk.make_geom(1, 2, 8, 4, 0), [], H)) == lk.LUMEN_KV_EINVAL
+    assert status(lambda: lk.lumen_kv_plan_build(lk.make_geom(1, 2, 8, 4, 2**31), [], H)) == lk.LUMEN_KV_EINVAL
+    assert status(lambda: lk.lumen_kv_plan_build(lk.make_geom(1, 2, 8, 4, 16, page_stride_bytes=100), [], H)) == lk.LUMEN_KV_EINVAL
+    # ranges
+    assert status(lambda: lk.lumen_kv_plan_build(g, [(pt, 5, 4)], H)) == lk.LUMEN_KV_EINVAL
+    assert status(lambda: lk.lumen_kv_plan_build(g, [(pt, -1, 4)], H)) == lk.LUMEN_KV_EINVAL
+    assert status(lambda: lk.lumen_kv_plan_build(g, [(pt, 0, 13)], H)) == lk.LUMEN_KV_ERANGE
+    assert status(lambda: lk.lumen_kv_plan_build(g, [(np.array([1, 16], np.int32), 0, 8)], H)) == lk.LUMEN_KV_ERANGE
+    assert status(lambda: lk.lumen_kv_plan_build(g, [(np.array([1, -1], np.int32), 0, 8)], H)) == lk.LUMEN_KV_ERANGE
+    # A6: entries outside the touched range are ignored
+    lk.lumen_kv_plan_build(g, [(np.array([99, 2, 99], np.int32), 4, 8)], H).close()
+    # unknown flag / kernel selector
+    assert status(lambda: lk.lumen_kv_plan_build(g, [], H | 0x80)) == lk.LUMEN_KV_EINVAL
+    assert status(lambda: lk.lumen_kv_plan_build(g, [], H | 0x300)) == lk.LUMEN_KV_EINVAL
+    # A5: duplicate destination page, across and within requests
+    U = H | lk.LUMEN_KV_VALIDATE_UNIQUE_DST
+    assert status(lambda: lk.lumen_kv_plan_build(g, [(pt, 0, 4), (pt, 0, 4)], U)) == lk.LUMEN_KV_EOVERLAP
+    assert status(lambda: lk.lumen_kv_plan_build(g, [(np.array([5, 5], np.int32), 0, 8)], U)) == lk.LUMEN_KV_EOVERLAP
+    lk.lumen_kv_plan_build(g, [(pt, 0, 4), (pt, 0, 4)], H).close()        # pack may share pages
+    lk.lumen_kv_plan_build(g, [(pt, 0, 4), (pt, 4, 12)], U).close()       # disjoint pages are fine
+    # sparse path of the uniqueness check (huge N, few pages)
+    big = lk.make_geom(1, 2, 8, 4, 2**31 - 1)
+    far = np.array([2**31 - 2, 7], dtype=np.int32)
+    assert status(lambda: lk.lumen_kv_plan_build(big, [(far, 0, 8), (far, 4, 8)], U)) == lk.LUMEN_KV_EOVERLAP
+    lk.lumen_kv_plan_build(big, [(far, 0, 8)], U).close()
+
+
+def test_empty_plans(lk):
+    g = lk.make_geom(2, 2, 8, 4, 16)
+    p = lk.lumen_kv_plan_build(g, [], lk.LUMEN_KV_HOST_ONLY)
+    assert p.nbytes == 0 and p.num_runs == 0 and p.req_offset(0) == 0
+    pt = np.array([1], dtype=np.int32)
+    p = lk.lumen_kv_plan_build(g, [(pt, 2, 2), (np.zeros(0, np.int32), 0, 0)], lk.LUMEN_KV_HOST_ONLY)
+    assert p.nbytes == 0 and p.num_runs == 0 and p.req_offset(2) == 0
+
+
+def test_no_cpu_fallback(lk):
+    """Without a CUDA device the executable plan build must fail loudly (ECUDA)."""
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("GPU present")
+    g = lk.make_geom(2, 2, 8, 4, 16)
+    pt = np.array([1], dtype=np.int32)
+    with pytest.raises(lk.LumenKVError) as e:
+        lk.lumen_kv_plan_build(g, [(pt, 0, 2)], 0)
+    assert e.value.status == lk.LUMEN_KV_ECUDA
+    # a host-only plan cannot be executed
+    p = lk.lumen_kv_plan_build(g, [(pt, 0, 2)], lk.LUMEN_KV_HOST_ONLY)
+    with pytest.raises(lk.LumenKVError) as e:
+        lk.lumen_kv_checkpoint_pack(p, [16, 16], [16, 16], 16, 1 << 20)
+    assert e.value.status == lk.LUMEN_KV_EINVAL
+
+
+def test_product_does_not_import_oracle():
+    for p in (ROOT / "paper_2606_17787_b200").rglob("*"):
+        if p.suffix in {".py", ".cu", ".cpp", ".hpp", ".h"}:
+            s = p.read_text()
+            assert "oracle" not in s.lower(), p
+    for p in (ROOT / "oracle").rglob("*"):
+        if p.suffix in {".py", ".c"}:
+            s = p.read_text()
+            assert "import paper_2606_17787_b200" not in s and "lumen_kv.h\"" not in s, p
+
+
+def test_plan_build_speed_host(lk):
+    """a2 must be microsecond-scale for per-decode-step deltas (SURVEY 7.3 hard part 2)."""
+    import time
+    w = cfg1_qwen14b()
+    g = geom_of(lk, w)
+    t0 = time.perf_counter()
+    for _ in range(200):
+        lk.lumen_kv_plan_build(g, w.reqs, lk.LUMEN_KV_HOST_ONLY).close()
+    dt = (time.perf_counter() - t0) / 200
+    assert dt < 2e-3, dt      # includes the ctypes marshalling of 64 requests

@@ -1,0 +1,55 @@
+"""Device-side helpers for tests and bench: build/load workloads/libkvfill.so and fill
+torch CUDA tensors with the pattern g of workloads/content.py.  Test tooling only."""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+from pathlib import Path
+
+_HERE = Path(__file__).resolve().parent
+_SRC = _HERE / "csrc" / "kvfill.cu"
+_SO = _HERE / "libkvfill.so"
+_lib = None
+
+
+def build(force: bool = False) -> Path:
+    if force or not _SO.exists() or _SO.stat().st_mtime < _SRC.stat().st_mtime:
+        nvcc = os.environ.get("NVCC") or "/usr/local/cuda/bin/nvcc"
+        tmp = _SO.with_suffix(f".so.tmp{os.getpid()}")
+        subprocess.check_call([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3",
+                               "-Xcompiler", "-fPIC,-fvisibility=hidden", "-shared", "-cudart", "static",
+                               "-o", str(tmp), str(_SRC)])
+        os.replace(tmp, _SO)
+    return _SO
+
+
+def lib() -> ctypes.CDLL:
+    global _lib
+    if _lib is None:
+        if not _SO.exists():
+            raise ImportError(f"{_SO} missing: run workloads.device.build()")
+        _lib = ctypes.CDLL(str(_SO))
+        vp, i64, u64 = ctypes.c_void_p, ctypes.c_int64, ctypes.c_uint64
+        _lib.kvfill_fill.restype = ctypes.c_int
+        _lib.kvfill_fill.argtypes = [vp, i64, i64, u64, u64, vp]
+        _lib.kvfill_page_checksums.restype = ctypes.c_int
+        _lib.kvfill_page_checksums.argtypes = [vp, i64, i64, vp, vp]
+    return _lib
+
+
+def fill_plane(t, seed: int, plane: int, stream: int = 0) -> None:
+    """t: contiguous torch CUDA tensor viewed as 16-bit words; fills words [0, numel)."""
+    n_words = t.numel() * t.element_size() // 2
+    rc = lib().kvfill_fill(t.data_ptr(), 0, n_words, seed & 0xFFFFFFFFFFFFFFFF, plane, stream)
+    if rc:
+        raise RuntimeError(f"kvfill_fill failed ({rc})")
+
+
+def page_checksums(t, n_pages: int, page_bytes: int, stream: int = 0):
+    import torch
+    out = torch.empty(n_pages, dtype=torch.int64, device=t.device)
+    rc = lib().kvfill_page_checksums(t.data_ptr(), n_pages, page_bytes, out.data_ptr(), stream)
+    if rc:
+        raise RuntimeError(f"kvfill_page_checksums failed ({rc})")
+    return out
