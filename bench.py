@@ -1,0 +1,438 @@
+#!/usr/bin/env python
+"""bench.py -- KV checkpoint pack / restore throughput on B200 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+                    [--workload cfg1|cfg2|cfg4] [--kernel auto|warp|bulk]
+
+A "step" is one pass of the whole hot path over one batch:
+  a1 select every running request's delta [t_prev, t_cur)         (vectorised host ints)
+  a2 lumen_kv_plan_build for the pack and for the restore          (host C++ + 1 small H2D)
+  a3 lumen_kv_checkpoint_pack  pool -> HBM staging buffer          (1 kernel)
+  a6 fresh pages for the restore come from the seeded page tables  (input)
+  a7 lumen_kv_restore_unpack   HBM staging buffer -> fresh pages   (1 kernel)
+  plus lumen_kv_plan_free of both plans.
+`value` is payload GB/s (bytes checkpointed + bytes restored per second), device-timed
+with inputs resident in HBM.  `e2e` is the same step through the same C ABI with HOST
+buffers: pack writes mapped pinned host memory (a4), restore reads it back, so P bytes
+cross the host link in each direction inside the timed region.
+Default workload = BASELINE.json configs[1] (Qwen3-14B shape, 64 requests, 16-token
+deltas, pool of 60,000 pages = 146.5 GiB).  Input recipe: DESIGN.md section 4.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+from pathlib import Path
+
+ROOT = Path(__file__).resolve().parent
+if str(ROOT) not in sys.path:
+    sys.path.insert(0, str(ROOT))
+
+import numpy as np  # noqa: E402
+
+CYCLE = 64          # distinct delta sets the steps rotate over (each advances 16 tokens)
+N_STAGE = 4         # rotating HBM staging buffers (4 x 160 MiB > 126 MB L2)
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=300)
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
+    ap.add_argument("--workload", choices=["cfg1", "cfg2", "cfg4"], default="cfg1")
+    ap.add_argument("--kernel", choices=["auto", "warp", "bulk"], default="auto")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--e2e-steps", type=int, default=0, help="default: min(steps, 100)")
+    return ap.parse_args()
+
+
+# ------------------------------------------------------------------------------------
+# workload construction (structure only; see workloads/gen.py)
+# ------------------------------------------------------------------------------------
+def make_workload(name: str, seed: int, pages_cap=None):
+    from workloads import cfg1_qwen14b, cfg2_qwen32b, cfg4_longctx
+    if name == "cfg1":
+        N = 60000 if pages_cap is None else min(60000, pages_cap)
+        w = cfg1_qwen14b(seed, N=N, grow_iters=CYCLE)
+        label = (f"BASELINE.json configs[1]: Qwen3-14B-shaped KV (40 layers, 8 kv_heads, head_dim 128, "
+                 f"bf16, page_size 16, pool {N} pages), 64 requests lognormal(median 2k, sigma 1, "
+                 f"clip 128..16k), 16-token delta per request per step")
+        delta = 16
+    elif name == "cfg2":
+        w = cfg2_qwen32b(seed)
+        label = ("BASELINE.json configs[2]: Qwen3-32B-shaped KV (64 layers), 16 requests x 8k-token "
+                 "full-prefix pack then restore into fresh seeded-random pages, pool 20000 pages")
+        delta = 0
+    else:
+        w = cfg4_longctx(seed, wave_reqs=2)
+        label = ("BASELINE.json configs[4] (wave of 2 of the 8 requests; the as-written 256 GiB does "
+                 "not fit one GPU): Qwen3-32B shape, page_size 1, 128k tokens each, shuffled slots")
+        delta = 0
+    return w, label, delta
+
+
+def iteration_ranges(w, delta: int, cycle: int):
+    """Per cycle position: (t_begin[], t_end[]) for every request (a1)."""
+    tb0 = np.array([tb for _, tb, _ in w.reqs], dtype=np.int64)
+    te0 = np.array([te for _, _, te in w.reqs], dtype=np.int64)
+    if delta == 0:
+        return [(tb0, te0)]
+    return [(tb0 + delta * i, te0 + delta * i) for i in range(cycle)]
+
+
+# ------------------------------------------------------------------------------------
+# clocks during the timed region (NVML polled from a thread)
+# ------------------------------------------------------------------------------------
+class ClockSampler:
+    REASONS = {0x1: "gpu_idle", 0x2: "applications_clocks_setting", 0x4: "sw_power_cap",
+               0x8: "hw_slowdown", 0x10: "sync_boost", 0x20: "sw_thermal_slowdown",
+               0x40: "hw_thermal_slowdown", 0x80: "hw_power_brake_slowdown",
+               0x100: "display_clock_setting"}
+
+    def __init__(self, index: int):
+        self.samples, self.reasons, self._stop, self._th = [], set(), threading.Event(), None
+        self.max_mhz = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+        except Exception:
+            self.nv = None
+
+    def _poll_once(self):
+        nv = self.nv
+        self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+        try:
+            mask = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+        except Exception:
+            mask = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+        for bit, name in self.REASONS.items():
+            if mask & bit and name != "gpu_idle":
+                self.reasons.add(name)
+
+    def _run(self):
+        while not self._stop.is_set():
+            try:
+                self._poll_once()
+            except Exception:
+                break
+            time.sleep(0.0005)
+
+    def start(self):
+        if self.nv is None:
+            return
+        self._stop.clear()
+        self._th = threading.Thread(target=self._run, daemon=True)
+        self._th.start()
+
+    def stop(self):
+        if self._th is not None:
+            self._stop.set()
+            self._th.join()
+            self._th = None
+
+    def summary(self):
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                    "samples": 0}
+        return {"sm_mhz": float(np.median(self.samples)), "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+# ------------------------------------------------------------------------------------
+# CPU oracle legs (the only places bench.py executes oracle/)
+# ------------------------------------------------------------------------------------
+def oracle_sample(workload: str, seed: int):
+    """A bounded sample of the workload on a sparse host pool: one step's pack + restore
+    for cfg1 (2 x 160 MiB); for the 32 GiB configs the first request's first 4096 tokens."""
+    from workloads.hostpool import sparse_host_pool
+    w, label, delta = make_workload(workload, seed)
+    if workload == "cfg1":
+        reqs, rreqs, what = w.reqs, w.restore_reqs, "one full step (64 requests x 16 tokens, pack + restore)"
+    else:
+        n = 4096
+        reqs = [(w.reqs[0][0], 0, n)]
+        rreqs = [(w.restore_reqs[0][0], 0, n)]
+        what = f"first request, first {n} tokens (pack + restore)"
+    K, V, keep = sparse_host_pool(w.geom, seed, list(reqs) + list(rreqs))
+    return w, label, reqs, rreqs, K, V, keep, what
+
+
+def oracle_step(geom, K, V, reqs, rreqs, omp=False):
+    import oracle
+    B = oracle.pack(geom, K, V, reqs, omp=omp)
+    oracle.unpack(geom, K, V, rreqs, B, omp=omp)
+    return 2 * B.size * 2          # payload bytes moved: packed + restored
+
+
+def cpu_baseline(workload: str, seed: int, budget_s: float = 12.0):
+    import oracle
+    w, label, reqs, rreqs, K, V, keep, what = oracle_sample(workload, seed)
+    oracle_step(w.geom, K, V, reqs, rreqs)                       # warm: page-faults the pool
+    t0 = time.perf_counter(); nbytes = oracle_step(w.geom, K, V, reqs, rreqs)
+    one = time.perf_counter() - t0
+    reps = int(max(1, min(64, budget_s / max(one, 1e-3))))
+    t0 = time.perf_counter()
+    for _ in range(reps):
+        oracle_step(w.geom, K, V, reqs, rreqs)
+    dt = time.perf_counter() - t0
+    out = {"value": nbytes * reps / dt / 1e9, "unit": "GB/s", "cores": 1, "kind": "oracle",
+           "sample": f"{what}, {reps} repetitions, plain single-thread C oracle as it stands"}
+    # context only: the OpenMP/memcpy timing variant (asserted equal to the plain one in tests)
+    threads = oracle.omp_threads()
+    oracle_step(w.geom, K, V, reqs, rreqs, omp=True)
+    t0 = time.perf_counter()
+    for _ in range(reps):
+        oracle_step(w.geom, K, V, reqs, rreqs, omp=True)
+    dt = time.perf_counter() - t0
+    out["omp_variant"] = {"value": nbytes * reps / dt / 1e9, "unit": "GB/s", "cores": threads}
+    return out
+
+
+def run_reference(args):
+    """--impl reference: the oracle, as it stands, on the host cores; rank 0 only."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    from workloads import MASTER_SEED
+    w, label, reqs, rreqs, K, V, keep, what = oracle_sample(args.workload, MASTER_SEED)
+    for _ in range(max(1, min(args.warmup, 3))):
+        oracle_step(w.geom, K, V, reqs, rreqs)
+    steps = max(1, args.steps)
+    # keep the whole run within a few minutes whatever K the driver passes
+    t0 = time.perf_counter(); nbytes = oracle_step(w.geom, K, V, reqs, rreqs); one = time.perf_counter() - t0
+    timed = int(max(1, min(steps, 120.0 / max(one, 1e-3))))
+    t0 = time.perf_counter()
+    for _ in range(timed):
+        oracle_step(w.geom, K, V, reqs, rreqs)
+    dt = time.perf_counter() - t0
+    val = nbytes * timed / dt / 1e9
+    line = {"impl": "reference", "metric": "kv_pack_restore_payload_GBps", "value": val, "unit": "GB/s",
+            "n_gpus": args.gpus, "steps": steps, "warmup": args.warmup, "ms_per_step": dt / timed * 1e3,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u16",
+            "data": "synthetic", "config": {"workload": label, "timed_steps": timed},
+            "cpu_baseline": {"value": val, "unit": "GB/s", "cores": 1, "kind": "oracle",
+                             "sample": f"each step = {what}; plain single-thread C oracle"},
+            "e2e": {"value": val, "unit": "GB/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+# ------------------------------------------------------------------------------------
+# the CUDA arm
+# ------------------------------------------------------------------------------------
+def measured_peaks():
+    p = ROOT / "MEASURED_PEAKS.json"
+    if p.exists():
+        try:
+            return float(json.loads(p.read_text())["hbm_gbs"]), "MEASURED_PEAKS.json hbm_gbs (of measured)"
+        except Exception:
+            pass
+    return 6650.0, "B200_PROFILING.md fallback 6.65 TB/s (of fallback)"
+
+
+def ncu_traffic(workload: str, kernel: str):
+    """dram bytes per launch from the committed ncu --set full capture, if any."""
+    p = ROOT / "profiles" / "traffic.json"
+    if p.exists():
+        try:
+            return json.loads(p.read_text()).get(f"{workload}:{kernel}")
+        except Exception:
+            return None
+    return None
+
+
+def memcpy_peaks(torch, nbytes=1 << 30):
+    """Pinned cudaMemcpyAsync D2H / H2D, best of 10, CUDA events: the host-path denominators."""
+    h = torch.empty(nbytes, dtype=torch.uint8, pin_memory=True)
+    d = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+    out = {}
+    for name, dst, src in (("d2h", h, d), ("h2d", d, h)):
+        best = float("inf")
+        for _ in range(10):
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(); dst.copy_(src, non_blocking=True); b.record(); torch.cuda.synchronize()
+            best = min(best, a.elapsed_time(b))
+        out[name] = nbytes / best / 1e6
+    return out
+
+
+def run_ours(args):
+    import torch
+    import paper_2606_17787_b200 as lk            # fails loudly if liblumen_kv.so is missing
+    from paper_2606_17787_b200.pool import KVPool, pinned_buffer
+    from workloads import MASTER_SEED
+    from workloads import device as wdev
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: there is no CPU path for --impl ours")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    wdev.build()
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+
+    # ---- workload (one replica per rank: weak scaling, no data-path collective) ----------
+    seed = MASTER_SEED + rank
+    free_b, _total = torch.cuda.mem_get_info()
+    pages_cap = None
+    if args.workload == "cfg1":
+        page_all = 2 * 40 * 16 * 8 * 128 * 2
+        reserve = N_STAGE * 64 * 16 * 160 * 1024 + (6 << 30)
+        fit = int((free_b - reserve) // page_all // 1000 * 1000)
+        pages_cap = fit if fit < 60000 else None
+    w, label, delta = make_workload(args.workload, seed, pages_cap)
+    L, H, D, S, N = w.geom
+    pool = KVPool(L, H, D, S, N)
+    for i, t in enumerate(pool.planes()):
+        wdev.fill_plane(t, seed, i)
+    torch.cuda.synchronize()
+    P = w.payload_bytes
+    ranges = iteration_ranges(w, delta, CYCLE)
+    n_stage = N_STAGE if P <= (1 << 30) else 1
+    lag = 2 if n_stage > 1 else 0
+    dbufs = [torch.empty(P, dtype=torch.uint8, device="cuda") for _ in range(n_stage)]
+
+    kflag = {"auto": lk.LUMEN_KV_KERNEL_AUTO, "warp": lk.LUMEN_KV_KERNEL_WARP,
+             "bulk": lk.LUMEN_KV_KERNEL_BULK}[args.kernel]
+    ra_p, ra_r = lk.ReqArray(w.reqs), lk.ReqArray(w.restore_reqs)
+    stream = torch.cuda.Stream()
+    sh = stream.cuda_stream
+    geom, kp, vp = pool.geom, pool.k_ptrs, pool.v_ptrs
+    DEV, HOST = lk.LUMEN_KV_MEM_DEVICE, lk.LUMEN_KV_MEM_HOST_MAPPED
+    UNIQUE = lk.LUMEN_KV_VALIDATE_UNIQUE_DST
+
+    def step(i, bufs, kind, lag_, evs=None):
+        nb = len(bufs)
+        tb, te = ranges[i % len(ranges)]
+        ra_p.set_ranges(tb, te)                                           # a1
+        tb, te = ranges[(i - lag_) % len(ranges)]
+        ra_r.set_ranges(tb, te)
+        p = lk.lumen_kv_plan_build(geom, ra_p, kflag, sh)                 # a2
+        r = lk.lumen_kv_plan_build(geom, ra_r, kflag | UNIQUE, sh)
+        if evs is not None:
+            evs[0].record(stream)
+        lk.lumen_kv_checkpoint_pack(p, kp, vp, bufs[i % nb].data_ptr(), P, kind, sh)          # a3 / a4
+        if evs is not None:
+            evs[1].record(stream)
+        lk.lumen_kv_restore_unpack(r, kp, vp, bufs[(i - lag_) % nb].data_ptr(), P, kind, sh)  # a7
+        if evs is not None:
+            evs[2].record(stream)
+        p.close(); r.close()
+
+    def timed_loop(K, W, bufs, kind, lag_, sampler=None):
+        for i in range(-lag_, 0):                      # fill the buffers the first restores read
+            step(i + len(ranges) * len(bufs), bufs, kind, 0)
+        for i in range(W):
+            step(i, bufs, kind, lag_)
+        evs = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(K)]
+        e_start, e_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier(); torch.cuda.synchronize()
+        if sampler:
+            sampler.start()
+        t_wall = time.perf_counter()
+        e_start.record(stream)
+        for i in range(K):
+            step(W + i, bufs, kind, lag_, evs[i])
+        e_end.record(stream)
+        stream.synchronize(); torch.cuda.synchronize()
+        t_wall = time.perf_counter() - t_wall
+        if sampler:
+            sampler.stop()
+        barrier()
+        ms = e_start.elapsed_time(e_end)
+        if dist is not None:
+            t = torch.tensor([ms], device="cuda", dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ms = float(t.item())
+        pack_ms = float(np.mean([e[0].elapsed_time(e[1]) for e in evs]))
+        unpack_ms = float(np.mean([e[1].elapsed_time(e[2]) for e in evs]))
+        return ms, pack_ms, unpack_ms, t_wall * 1e3
+
+    K, W = max(1, args.steps), max(3, args.warmup)
+    sampler = ClockSampler(local)
+    with torch.cuda.stream(stream):
+        ms, pack_ms, unpack_ms, wall_ms = timed_loop(K, W, dbufs, DEV, lag, sampler)
+    value = world * K * 2 * P / (ms * 1e-3) / 1e9
+    token_bytes = 2 * L * H * D * 2
+
+    # ---- roofline of the dominant kernel ------------------------------------------------
+    peak, peak_src = measured_peaks()
+    dom, dom_ms = ("lumen_kv_checkpoint_pack", pack_ms) if pack_ms >= unpack_ms else \
+                  ("lumen_kv_restore_unpack", unpack_ms)
+    achieved = 2 * P / (dom_ms * 1e-3) / 1e9
+    resolved = args.kernel if args.kernel != "auto" else "warp"
+    roofline = {"bound": "hbm", "kernel": f"{dom} ({'kv_copy_' + resolved})", "achieved": achieved,
+                "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                "traffic": ncu_traffic(args.workload, resolved),
+                "algorithmic_bytes_per_launch": 2 * P, "peak_source": peak_src,
+                "pack_ms": pack_ms, "unpack_ms": unpack_ms,
+                "pack_traffic_GBps": 2 * P / pack_ms / 1e6, "unpack_traffic_GBps": 2 * P / unpack_ms / 1e6}
+
+    # ---- e2e: same step, host buffers, bytes cross the host link inside the timed region --
+    e2e = None
+    if not args.no_e2e:
+        est = 2 * P / 50e9
+        Ke = args.e2e_steps or int(max(3, min(K, 100, 20.0 / est)))
+        hb = [pinned_buffer(P) for _ in range(2 if P <= (1 << 30) else 1)]
+        link = memcpy_peaks(torch)
+        with torch.cuda.stream(stream):
+            ms_e, pack_e, unpack_e, _ = timed_loop(Ke, 3, hb, HOST, 1 if len(hb) > 1 else 0)
+        e2e = {"value": world * Ke * 2 * P / (ms_e * 1e-3) / 1e9, "unit": "GB/s",
+               "h2d_bytes_per_step": P, "d2h_bytes_per_step": P, "steps": Ke,
+               "ms_per_step": ms_e / Ke, "gpu_launches": 2 * Ke,
+               "pack_to_host_GBps": P / pack_e / 1e6, "restore_from_host_GBps": P / unpack_e / 1e6,
+               "memcpy_peak_d2h_GBps": link["d2h"], "memcpy_peak_h2d_GBps": link["h2d"],
+               "pack_frac_of_d2h_peak": P / pack_e / 1e6 / link["d2h"],
+               "restore_frac_of_h2d_peak": P / unpack_e / 1e6 / link["h2d"],
+               "path": "kernel stores/loads on mapped pinned host memory (zero-copy over PCIe)"}
+        del hb
+
+    line = {
+        "metric": "kv_pack_restore_payload_GBps", "value": value, "unit": "GB/s",
+        "n_gpus": world, "steps": K, "warmup": W, "ms_per_step": ms / K,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "u16", "data": "synthetic",
+        "config": {"workload": label, "payload_bytes_per_direction_per_step": P,
+                   "tokens_per_step": w.tokens, "runs_per_plan": None,
+                   "l2": (f"inputs larger than L2: steps rotate over {n_stage} staging buffers of "
+                          f"{P / 2**20:.0f} MiB and {len(ranges)} distinct delta sets; the restore reads "
+                          f"the buffer packed {lag} steps earlier"),
+                   "kernel": args.kernel, "replicas": world, "seed": hex(MASTER_SEED)},
+        "tokens_per_s": value * 1e9 / token_bytes,
+        "wall_ms_per_step": wall_ms / K,
+        "roofline": roofline, "e2e": e2e, "gpu_launches": 2 * K, "clocks": sampler.summary(),
+    }
+    if rank == 0:
+        if world == 1 and not args.no_cpu_baseline:
+            line["cpu_baseline"] = cpu_baseline(args.workload, MASTER_SEED)
+        print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -169,9 +169,45 @@ class Plan:
         self.close()
 
 
-def lumen_kv_plan_build(geom: lumen_kv_geom, reqs: Sequence[Req], flags: int = 0,
-                        stream: int = 0) -> Plan:
-    """reqs: sequence of (page_table int32 ndarray, t_begin, t_end)."""
+REQ_DTYPE = np.dtype([("page_table", np.uint64), ("page_table_len", np.int64),
+                      ("t_begin", np.int64), ("t_end", np.int64)])
+assert REQ_DTYPE.itemsize == ctypes.sizeof(lumen_kv_req)
+
+
+class ReqArray:
+    """A C array of lumen_kv_req kept as a numpy structured array, so that a serving loop
+    can advance every request's delta range with one vectorised op per iteration
+    (step a1) instead of re-marshalling Python tuples.  Owns the page tables."""
+
+    def __init__(self, reqs: Sequence[Req]):
+        self._tables = [np.ascontiguousarray(pt, dtype=np.int32) for pt, _, _ in reqs]
+        self.arr = np.zeros(len(reqs), dtype=REQ_DTYPE)
+        for i, ((_, tb, te), pt) in enumerate(zip(reqs, self._tables)):
+            self.arr[i] = (pt.ctypes.data if pt.size else 0, pt.size, int(tb), int(te))
+
+    def __len__(self) -> int:
+        return self.arr.size
+
+    def set_ranges(self, t_begin, t_end) -> None:
+        self.arr["t_begin"] = t_begin
+        self.arr["t_end"] = t_end
+
+    def advance(self, tokens: int) -> None:
+        """[tb, te) <- [te, te + tokens): the next incremental delta."""
+        self.arr["t_begin"] = self.arr["t_end"]
+        self.arr["t_end"] += int(tokens)
+
+
+def lumen_kv_plan_build(geom: lumen_kv_geom, reqs, flags: int = 0, stream: int = 0) -> Plan:
+    """reqs: a ReqArray, or a sequence of (page_table int32 ndarray, t_begin, t_end)."""
+    if isinstance(reqs, ReqArray):
+        out = ctypes.c_void_p()
+        rc = _lib().lumen_kv_plan_build(
+            ctypes.byref(geom), ctypes.cast(reqs.arr.ctypes.data, ctypes.POINTER(lumen_kv_req)),
+            len(reqs), int(flags), ctypes.c_void_p(int(stream)), ctypes.byref(out))
+        if rc:
+            raise LumenKVError(rc, "lumen_kv_plan_build")
+        return Plan(out.value, geom, len(reqs))
     n = len(reqs)
     arr = (lumen_kv_req * max(n, 1))()
     keep = []

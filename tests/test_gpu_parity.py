@@ -86,10 +86,10 @@ def test_random_tiny_geometries(G, kernel):
 @pytest.mark.parametrize("kernel", ["warp", "bulk"])
 def test_mid_cfg1_shape(G, kernel):
     """Qwen3-14B row/page shape, fewer layers/pages: 32 KiB runs, ragged 16-token deltas."""
-    w = cfg1_qwen14b(L=3, N=1024, n_reqs=24, grow_iters=2, hi=512, lo=20)
+    w = cfg1_qwen14b(L=3, N=2048, n_reqs=24, grow_iters=2, median=200, hi=512, lo=20)
     run_case(G, w, kernel, "device")
     run_case(G, w.advanced(16), kernel, "host")
-    run_case(G, cfg1_qwen14b(L=3, N=1024, n_reqs=24, grow_iters=2, hi=512, lo=20, aligned=True), kernel, "device")
+    run_case(G, cfg1_qwen14b(L=3, N=2048, n_reqs=24, grow_iters=2, median=200, hi=512, lo=20, aligned=True), kernel, "device")
 
 
 @pytest.mark.parametrize("kernel", ["warp", "bulk"])
@@ -108,8 +108,8 @@ def test_mid_cfg4_token_granular(G, kernel):
 @pytest.mark.parametrize("kernel", ["warp", "bulk"])
 def test_tp_rank_shape_and_odd_rows(G, kernel):
     # H = 4 (one TP2 rank of an 8-kv-head model); and a 48-byte row
-    run_case(G, cfg1_qwen14b(L=2, H=4, N=512, n_reqs=8, grow_iters=2, hi=256, lo=20), kernel, "device")
-    run_case(G, cfg1_qwen14b(L=2, H=1, D=24, N=512, n_reqs=8, grow_iters=2, hi=256, lo=20), kernel, "device")
+    run_case(G, cfg1_qwen14b(L=2, H=4, N=512, n_reqs=8, grow_iters=2, median=100, hi=256, lo=20), kernel, "device")
+    run_case(G, cfg1_qwen14b(L=2, H=1, D=24, N=512, n_reqs=8, grow_iters=2, median=100, hi=256, lo=20), kernel, "device")
     # page larger than the 32 KiB chunk: S = 64 tokens of 2 KiB
     run_case(G, cfg2_qwen32b(L=1, S=64, N=64, n_reqs=3, prompt=500), kernel, "device")
 
@@ -187,7 +187,7 @@ def test_plan_reuse_and_free_while_in_flight(G):
     """build -> pack -> free in a loop with no host sync: the arena must keep descriptors
     alive until the enqueued work is done, and recycle them afterwards."""
     import torch
-    w = cfg1_qwen14b(L=2, N=2048, n_reqs=32, grow_iters=40, hi=512, lo=20)
+    w = cfg1_qwen14b(L=2, N=8192, n_reqs=32, grow_iters=40, median=200, hi=512, lo=20)
     K, V = G.host_planes(w.geom, 9)
     pool = G.make_pool(w.geom, 9)
     ck = G.Checkpointer(pool)
