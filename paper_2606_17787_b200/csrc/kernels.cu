@@ -16,6 +16,8 @@
 //                  decode descriptors.
 #include "kernels.hpp"
 
+#include <cstdlib>
+
 namespace lumen {
 namespace {
 
@@ -66,7 +68,13 @@ __device__ __forceinline__ Item decode_item(const RunDesc* __restrict__ runs,
 }
 
 // ---------------------------------------------------------------------------------
-// SIMT kernel: warp per (run, plane)
+// SIMT kernel: one warp per (run, plane, sub-chunk)
+//
+// A task is UNROLL*512 bytes of one item: every lane issues its UNROLL independent
+// 16-byte loads, then its UNROLL stores, and the warp retires -- no loop.  Items are
+// cut into 2^sub_shift sub-chunks so that a 64 x 16-token decode delta (about 8,000
+// items of 32 KiB) becomes tens of thousands of equal tasks: the grid has no tail wave,
+// and consecutive warps of a CTA stream consecutive sub-chunks of the same run.
 // ---------------------------------------------------------------------------------
 constexpr int kWarpsPerCta = 8;
 
@@ -74,35 +82,27 @@ template <int UNROLL>
 __global__ void __launch_bounds__(kWarpsPerCta * 32)
 kv_copy_warp(const PlaneTable planes, const RunDesc* __restrict__ runs,
              const ReqDesc* __restrict__ reqs, int64_t n_runs, char* buf, uint32_t row_bytes,
-             int32_t plane0, int pack) {
+             int32_t plane0, int sub_shift, int pack) {
     const int lane = threadIdx.x & 31;
-    const int64_t run = static_cast<int64_t>(blockIdx.x) * kWarpsPerCta + (threadIdx.x >> 5);
+    const int64_t task = static_cast<int64_t>(blockIdx.x) * kWarpsPerCta + (threadIdx.x >> 5);
+    const int64_t run = task >> sub_shift;
     if (run >= n_runs) return;
+    const uint32_t sub = static_cast<uint32_t>(task & ((int64_t{1} << sub_shift) - 1));
     const Item it = decode_item(runs, reqs, run, planes.p[blockIdx.y], plane0 + blockIdx.y, buf,
                                 row_bytes);
-    const char* src = pack ? it.pool : it.buf;
-    char* dst = pack ? it.buf : it.pool;
     const uint32_t nvec = it.bytes >> 4;
+    const uint32_t i = sub * (UNROLL * 32) + lane;
+    if (sub * (UNROLL * 32) >= nvec) return;           // this run is shorter than the longest
+    const char* src = (pack ? it.pool : it.buf) + (static_cast<size_t>(i) << 4);
+    char* dst = (pack ? it.buf : it.pool) + (static_cast<size_t>(i) << 4);
 
-    uint32_t i = lane;
-    // full batches: UNROLL independent 16-byte loads per lane, then the stores
-    for (; i + (UNROLL - 1) * 32 < nvec; i += UNROLL * 32) {
-        uint4 v[UNROLL];
+    uint4 v[UNROLL];
 #pragma unroll
-        for (int u = 0; u < UNROLL; ++u) v[u] = ld_stream16(src + (static_cast<size_t>(i + u * 32) << 4));
+    for (int u = 0; u < UNROLL; ++u)
+        if (i + u * 32 < nvec) v[u] = ld_stream16(src + u * 512);
 #pragma unroll
-        for (int u = 0; u < UNROLL; ++u) st_stream16(dst + (static_cast<size_t>(i + u * 32) << 4), v[u]);
-    }
-    // ragged tail (< UNROLL*32 vectors), still loads-before-stores
-    {
-        uint4 v[UNROLL];
-#pragma unroll
-        for (int u = 0; u < UNROLL; ++u)
-            if (i + u * 32 < nvec) v[u] = ld_stream16(src + (static_cast<size_t>(i + u * 32) << 4));
-#pragma unroll
-        for (int u = 0; u < UNROLL; ++u)
-            if (i + u * 32 < nvec) st_stream16(dst + (static_cast<size_t>(i + u * 32) << 4), v[u]);
-    }
+    for (int u = 0; u < UNROLL; ++u)
+        if (i + u * 32 < nvec) st_stream16(dst + u * 512, v[u]);
 }
 
 // ---------------------------------------------------------------------------------
@@ -258,6 +258,7 @@ BulkCfg bulk_config(int64_t item_bytes_max) {
 }
 
 int g_num_sms = 0;
+int g_warp_unroll = 4;   // LUMEN_KV_WARP_UNROLL=4|8 (tuning knob, read once; 4 measured best)
 
 template <int STAGES>
 cudaError_t launch_bulk(const PlaneTable& pt, const CopyArgs& a, int32_t plane0, int32_t np,
@@ -292,6 +293,7 @@ int resolve_kernel(const CopyArgs& a) {
 cudaError_t launch_kv_copy(const CopyArgs& a) {
     if (a.n_runs == 0 || a.n_planes == 0) return cudaSuccess;
     if (g_num_sms == 0) {
+        if (const char* e = getenv("LUMEN_KV_WARP_UNROLL")) g_warp_unroll = (atoi(e) == 8) ? 8 : 4;
         int dev = 0;
         cudaError_t e = cudaGetDevice(&dev);
         if (e != cudaSuccess) return e;
@@ -319,12 +321,23 @@ cudaError_t launch_kv_copy(const CopyArgs& a) {
                 default: e = launch_bulk<16>(pt, a, plane0, np, c); break;
             }
         } else {
-            const int64_t gx = (a.n_runs + kWarpsPerCta - 1) / kWarpsPerCta;
-            // gridDim.x is limited to 2^31-1 blocks; n_runs < 2^34 is far beyond any plan
+            // sub-chunks per item: smallest power of two covering the longest run
+            const int unroll = g_warp_unroll;
+            const int64_t sub_bytes = int64_t{512} * unroll;
+            int sub_shift = 0;
+            while ((sub_bytes << sub_shift) < item_max) ++sub_shift;
+            const int64_t tasks = a.n_runs << sub_shift;
+            const int64_t gx = (tasks + kWarpsPerCta - 1) / kWarpsPerCta;
+            if (gx > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
             dim3 grid(static_cast<unsigned>(gx), static_cast<unsigned>(np), 1);
-            kv_copy_warp<8><<<grid, kWarpsPerCta * 32, 0, a.stream>>>(
-                pt, a.runs, a.reqs, a.n_runs, static_cast<char*>(a.buf),
-                static_cast<uint32_t>(a.row_bytes), plane0, a.pack ? 1 : 0);
+            if (unroll == 4)
+                kv_copy_warp<4><<<grid, kWarpsPerCta * 32, 0, a.stream>>>(
+                    pt, a.runs, a.reqs, a.n_runs, static_cast<char*>(a.buf),
+                    static_cast<uint32_t>(a.row_bytes), plane0, sub_shift, a.pack ? 1 : 0);
+            else
+                kv_copy_warp<8><<<grid, kWarpsPerCta * 32, 0, a.stream>>>(
+                    pt, a.runs, a.reqs, a.n_runs, static_cast<char*>(a.buf),
+                    static_cast<uint32_t>(a.row_bytes), plane0, sub_shift, a.pack ? 1 : 0);
             e = cudaGetLastError();
         }
         if (e != cudaSuccess) return e;
