@@ -48,16 +48,26 @@ def buf_to_np(buf: torch.Tensor, nbytes: int) -> np.ndarray:
 
 
 def alloc_buffer(nbytes: int, where: str, guard: int = 4096):
-    """Buffer with canary guard bands before and after (C5).  Returns (whole, view)."""
+    """Buffer with canary guard bands before and after (C5).  Returns (whole, view).
+    Host buffers of 1 GiB and more are registered at their exact size (see pinned_exact)."""
     total = nbytes + 2 * guard
     if where == "device":
         whole = torch.full((total,), 0xA5, dtype=torch.uint8, device="cuda")
+    elif total >= (1 << 30):
+        whole = wdev.pinned_exact(total)
+        whole[:guard] = 0xA5
+        whole[guard + nbytes:] = 0xA5
     else:
         whole = pinned_buffer(total)
         whole.fill_(0xA5)
     return whole, whole[guard: guard + nbytes]
 
 
+def release(whole: torch.Tensor) -> None:
+    if not whole.is_cuda:
+        wdev.unpin(whole)
+
+
 def guards_intact(whole: torch.Tensor, nbytes: int, guard: int = 4096) -> bool:
-    w = whole.cpu() if whole.is_cuda else whole
-    return bool((w[:guard] == 0xA5).all()) and bool((w[guard + nbytes:] == 0xA5).all())
+    lo, hi = whole[:guard], whole[guard + nbytes:]
+    return bool((lo == 0xA5).all()) and bool((hi == 0xA5).all())

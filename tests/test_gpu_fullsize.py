@@ -1,0 +1,242 @@
+"""GPU parity at BASELINE.json's full sizes (T3 of SURVEY.md section 4), in the launch
+configuration bench.py times (same entry points, same flags, same buffer kinds).
+
+The packed buffers here are up to 64 GiB, so the oracle checks them two ways:
+  (1) one by one: a few thousand sampled words (r, l, c, j, e); the C oracle's
+      accessors give the buffer index and the pool index (definition C1), the expected
+      value is the pool content g at that index computed on the CPU;
+  (2) everywhere: the index map of the NumPy oracle (oracle_np.slot_ids / layout) is
+      applied with a plain torch gather on the device pool (torch is plumbing here, the
+      map is the oracle's) and compared with every byte of the buffer.
+After the restore: per-page checksums of ALL pages of all planes before/after must match
+outside the target pages; target rows are compared everywhere with the buffer; untouched
+slots of partly filled target pages are compared with a snapshot; guard bands around the
+buffer must be intact.
+"""
+import numpy as np
+import pytest
+
+import oracle
+from oracle import oracle_np
+from workloads import MASTER_SEED, cfg1_qwen14b, cfg2_qwen32b, cfg3_burst, cfg4_longctx, g_words, substream
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def G():
+    import torch
+    assert torch.cuda.is_available()
+    from tests import gpu_util
+    gpu_util.build_all()
+    return gpu_util
+
+
+def _free():
+    import gc
+    import torch
+    gc.collect()
+    torch.cuda.empty_cache()
+
+
+def sampled_pack_check(G, geom, reqs, seed, buf, n_samples, rng):
+    """(1): words of the packed buffer vs g at the oracle's pool index."""
+    import torch
+    L, H, D, S, N = geom
+    E = H * D
+    live = [r for r, (_, tb, te) in enumerate(reqs) if te > tb]
+    bidx, expect = [], []
+    for _ in range(n_samples):
+        r = int(rng.choice(live))
+        n = reqs[r][2] - reqs[r][1]
+        l, c = int(rng.integers(0, L)), int(rng.integers(0, 2))
+        j, e = int(rng.integers(0, n)), int(rng.integers(0, E))
+        bidx.append(oracle.buffer_index(geom, reqs, r, l, c, j, e))
+        pidx = oracle.pool_index(geom, reqs, r, j, e)
+        expect.append(int(g_words(seed, 2 * l + c, pidx, 1)[0]))
+    words = buf.view(torch.int16)
+    idx = torch.tensor(bidx, dtype=torch.int64, device=words.device if words.is_cuda else "cpu")
+    got = words[idx].cpu().numpy().view(np.uint16)
+    assert np.array_equal(got, np.array(expect, dtype=np.uint16))
+
+
+def gather_check(G, pool, reqs, buf, what):
+    """(2): every (request, plane) block of the buffer vs a torch gather with the oracle's map."""
+    import torch
+    L, H, D, S, N = (pool.geom.num_layers, pool.geom.kv_heads, pool.geom.head_dim,
+                     pool.geom.page_size, pool.geom.num_pages)
+    E = H * D
+    geom = (L, H, D, S, N)
+    lay, total = oracle_np.layout(geom, reqs)
+    words = buf.view(torch.int16)
+    assert words.numel() >= total
+    planes = pool.planes()
+    for (pt, tb, te), (off, n) in zip(reqs, lay):
+        if n == 0:
+            continue
+        ids = torch.from_numpy(oracle_np.slot_ids(S, pt, tb, te)).cuda()
+        blk = words[off: off + n * 2 * L * E]
+        if not blk.is_cuda:
+            blk = blk.cuda(non_blocking=True)
+        blk = blk.view(2 * L, n, E)
+        for p in range(2 * L):
+            exp = planes[p].view(torch.int16).view(N * S, E).index_select(0, ids)
+            assert torch.equal(blk[p], exp), f"{what}: request block mismatch plane {p}"
+        del blk
+
+
+def all_checksums(G, pool):
+    import torch
+    g = pool.geom
+    page_bytes = g.page_size * g.kv_heads * g.head_dim * 2
+    return torch.stack([G.wdev.page_checksums(t, g.num_pages, page_bytes) for t in pool.planes()])
+
+
+def restore_and_check(G, pool, ck, w, buf, whole, nbytes):
+    """unpack into the fresh pages of the same pool; check targets, non-targets and guards."""
+    import torch
+    L, H, D, S, N = w.geom
+    E = H * D
+    before = all_checksums(G, pool)
+    target = torch.zeros(N, dtype=torch.bool, device="cuda")
+    partial = []                                   # (page, first untouched slot, end) snapshots
+    for pt, tb, te in w.restore_reqs:
+        if te == tb:
+            continue
+        target[torch.from_numpy(pt[tb // S:(te - 1) // S + 1].astype(np.int64)).cuda()] = True
+        if tb % S:
+            partial.append((int(pt[tb // S]), 0, tb % S))
+        if te % S:
+            partial.append((int(pt[(te - 1) // S]), te % S, S))
+    snaps = [[t.view(torch.int16).view(N, S, E)[pg, a:b].clone() for (pg, a, b) in partial]
+             for t in pool.planes()]
+    rplan = ck.plan(w.restore_reqs, unique_dst=True)
+    ck.unpack(rplan, buf)
+    torch.cuda.synchronize()
+    after = all_checksums(G, pool)
+    changed = (before != after).any(dim=0)
+    assert not bool((changed & ~target).any()), "a non-target page changed"
+    gather_check(G, pool, w.restore_reqs, buf, "restore")       # every target row == buffer row
+    for t, sn in zip(pool.planes(), snaps):
+        v = t.view(torch.int16).view(N, S, E)
+        for (pg, a, b), old in zip(partial, sn):
+            assert torch.equal(v[pg, a:b], old), "untouched slot of a partial page changed"
+    assert G.guards_intact(whole, nbytes)
+    rplan.close()
+
+
+@pytest.mark.parametrize("where", ["device", "host"])
+def test_cfg1_full_size(G, where):
+    """configs[1] as bench.py runs it: 60,000-page pool (146.5 GiB), 64 requests, 16-token deltas."""
+    import torch
+    _free()
+    free_b, _ = torch.cuda.mem_get_info()
+    w = cfg1_qwen14b(grow_iters=64)
+    page_all = 2 * 40 * 16 * 8 * 128 * 2
+    if free_b < w.geom[4] * page_all + (8 << 30):
+        pytest.skip("not enough free HBM for the 146.5 GiB pool")
+    pool = G.make_pool(w.geom, MASTER_SEED)
+    ck = G.Checkpointer(pool)                                   # AUTO kernel, as in bench.py
+    rng = substream(1, "cfg1_samples")
+    for it in range(3):                                         # three iterations: alignment mix varies
+        plan = ck.plan(G.lk.ReqArray(w.reqs))
+        assert plan.nbytes == 167_772_160
+        whole, buf = G.alloc_buffer(plan.nbytes, where)
+        ck.pack(plan, buf)
+        torch.cuda.synchronize()
+        assert G.guards_intact(whole, plan.nbytes)
+        sampled_pack_check(G, w.geom, w.reqs, MASTER_SEED, buf, 1500, rng)
+        gather_check(G, pool, w.reqs, buf, "pack")
+        if it == 0:                                             # full oracle on a sparse host pool
+            from workloads.hostpool import sparse_host_pool
+            K, V, keep = sparse_host_pool(w.geom, MASTER_SEED, w.reqs)
+            ref = oracle.pack(w.geom, K, V, w.reqs)
+            assert np.array_equal(G.buf_to_np(buf, plan.nbytes), ref)
+            del K, V, keep, ref
+        restore_and_check(G, pool, ck, w, buf, whole, plan.nbytes)
+        plan.close()
+        w = w.advanced(16)
+    del pool
+    _free()
+
+
+@pytest.mark.parametrize("where", ["device", "host"])
+def test_cfg2_full_size(G, where):
+    """configs[2]: 16 x 8k-token full-prefix pack (32 GiB) then restore into fresh pages."""
+    import torch
+    _free()
+    w = cfg2_qwen32b()
+    pool = G.make_pool(w.geom, MASTER_SEED + 2)
+    ck = G.Checkpointer(pool)
+    plan = ck.plan(w.reqs)
+    assert plan.nbytes == 32 * 2**30 and plan.num_runs == 8192
+    try:
+        whole, buf = G.alloc_buffer(plan.nbytes, where)
+    except RuntimeError as e:
+        pytest.skip(f"cannot allocate the 32 GiB {where} buffer: {e}")
+    ck.pack(plan, buf)
+    torch.cuda.synchronize()
+    assert G.guards_intact(whole, plan.nbytes)
+    sampled_pack_check(G, w.geom, w.reqs, MASTER_SEED + 2, buf, 1500, substream(2, "cfg2_samples"))
+    gather_check(G, pool, w.reqs, buf, "pack")
+    restore_and_check(G, pool, ck, w, buf, whole, plan.nbytes)
+    plan.close()
+    G.release(whole)
+    del pool, buf, whole
+    _free()
+
+
+def test_cfg4_token_granular_wave(G):
+    """configs[4], one wave of 2 requests x 128k tokens, page_size 1, fully shuffled slots:
+    64 GiB pool + 64 GiB HBM buffer (the as-written 256 GiB + 256 GiB cannot exist on one GPU)."""
+    import torch
+    _free()
+    w = cfg4_longctx(wave_reqs=2)
+    free_b, _ = torch.cuda.mem_get_info()
+    if free_b < 2 * w.payload_bytes + (8 << 30):
+        pytest.skip("not enough free HBM for a 2-request wave")
+    pool = G.make_pool(w.geom, MASTER_SEED + 4)
+    ck = G.Checkpointer(pool)
+    plan = ck.plan(w.reqs)
+    assert plan.num_runs == 2 * 131072 and plan.nbytes == 64 * 2**30
+    whole, buf = G.alloc_buffer(plan.nbytes, "device")
+    ck.pack(plan, buf)
+    torch.cuda.synchronize()
+    sampled_pack_check(G, w.geom, w.reqs, MASTER_SEED + 4, buf, 1500, substream(4, "cfg4_samples"))
+    gather_check(G, pool, w.reqs, buf, "pack")
+    # restore under the new shuffle: with S = 1 and a full shuffle every slot is a target, so
+    # "untouched" reduces to the guard bands; P3 closes the loop: re-pack under the new table
+    rplan = ck.plan(w.restore_reqs, unique_dst=True)
+    ck.unpack(rplan, buf)
+    torch.cuda.synchronize()
+    gather_check(G, pool, w.restore_reqs, buf, "restore")
+    assert G.guards_intact(whole, plan.nbytes)
+    plan.close(); rplan.close()
+    del pool, buf, whole
+    _free()
+
+
+def test_cfg4_host_path_one_request(G):
+    """configs[4] to pinned host and back: one 128k-token request (32 GiB over the host link)."""
+    import torch
+    _free()
+    w = cfg4_longctx(wave_reqs=1, wave=1)
+    pool = G.make_pool(w.geom, MASTER_SEED + 5)
+    ck = G.Checkpointer(pool)
+    plan = ck.plan(w.reqs)
+    try:
+        whole, buf = G.alloc_buffer(plan.nbytes, "host")
+    except RuntimeError as e:
+        pytest.skip(f"cannot pin 32 GiB: {e}")
+    ck.pack(plan, buf)
+    torch.cuda.synchronize()
+    sampled_pack_check(G, w.geom, w.reqs, MASTER_SEED + 5, buf, 1000, substream(5, "cfg4h"))
+    gather_check(G, pool, w.reqs, buf, "pack")
+    rplan = ck.plan(w.restore_reqs, unique_dst=True)
+    ck.unpack(rplan, buf)
+    torch.cuda.synchronize()
+    gather_check(G, pool, w.restore_reqs, buf, "restore")
+    assert G.guards_intact(whole, plan.nbytes)
+    G.release(whole)
+    del pool, buf, whole
+    _free()

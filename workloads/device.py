@@ -53,3 +53,25 @@ def page_checksums(t, n_pages: int, page_bytes: int, stream: int = 0):
     if rc:
         raise RuntimeError(f"kvfill_page_checksums failed ({rc})")
     return out
+
+
+_registered = {}
+
+
+def pinned_exact(nbytes: int):
+    """Page-locked host tensor of exactly nbytes (torch's pinned allocator rounds sizes up
+    to a power of two, which doubles a 32 GiB + guard-band buffer).  Registers a pageable
+    tensor with cudaHostRegister; call unpin(t) when done."""
+    import torch
+    t = torch.empty(int(nbytes), dtype=torch.uint8)
+    rc = torch.cuda.cudart().cudaHostRegister(t.data_ptr(), t.numel(), 0)
+    if int(rc) != 0:
+        raise RuntimeError(f"cudaHostRegister({nbytes}) failed: {rc}")
+    _registered[t.data_ptr()] = t
+    return t
+
+
+def unpin(t) -> None:
+    import torch
+    if _registered.pop(t.data_ptr(), None) is not None:
+        torch.cuda.cudart().cudaHostUnregister(t.data_ptr())
