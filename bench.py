@@ -199,7 +199,7 @@ def cpu_baseline(workload: str, seed: int, budget_s: float = 12.0):
 
 def run_reference(args):
     """--impl reference: the oracle, as it stands, on the host cores; rank 0 only."""
-    if int(os.environ.get("RANK", "0")) != 0:
+    if rank_env()[0] != 0:
         return
     from workloads import MASTER_SEED
     w, label, reqs, rreqs, K, V, keep, what = oracle_sample(args.workload, MASTER_SEED)
@@ -223,6 +223,36 @@ def run_reference(args):
             "e2e": {"value": val, "unit": "GB/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line))
+
+
+# ------------------------------------------------------------------------------------
+# replicas: the path shards with no exchange step, so N ranks are N
+# independent replicas; the only cross-rank traffic is the barrier and the max of the times
+# ------------------------------------------------------------------------------------
+def rank_env():
+    """(rank, world, local_rank) as torchrun exports them; single process otherwise."""
+    return (int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1")),
+            int(os.environ.get("LOCAL_RANK", "0")))
+
+
+def replica_seed(master_seed: int, rank: int) -> int:
+    """Every rank draws its own lengths / page tables / pool content."""
+    return master_seed + rank
+
+
+def max_over_ranks(ms: float, dist, device) -> float:
+    """Device time of the job = the slowest rank's (all_reduce MAX); dist None => 1 rank."""
+    if dist is None:
+        return float(ms)
+    import torch
+    t = torch.tensor([ms], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def job_payload_gbps(world: int, steps: int, payload_bytes: int, ms: float) -> float:
+    """Whole-job payload GB/s: every rank packs P and restores P per step."""
+    return world * steps * 2 * payload_bytes / (ms * 1e-3) / 1e9
 
 
 # ------------------------------------------------------------------------------------
@@ -271,9 +301,7 @@ def run_ours(args):
     from workloads import MASTER_SEED
     from workloads import device as wdev
 
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
+    rank, world, local = rank_env()
     if not torch.cuda.is_available():
         raise RuntimeError("bench.py needs a CUDA device: there is no CPU path for --impl ours")
     torch.cuda.set_device(local)
@@ -288,7 +316,7 @@ def run_ours(args):
             dist.barrier()
 
     # ---- workload (one replica per rank: weak scaling, no data-path collective) ----------
-    seed = MASTER_SEED + rank
+    seed = replica_seed(MASTER_SEED, rank)
     free_b, _total = torch.cuda.mem_get_info()
     pages_cap = None
     if args.workload == "cfg1":
@@ -355,11 +383,7 @@ def run_ours(args):
         if sampler:
             sampler.stop()
         barrier()
-        ms = e_start.elapsed_time(e_end)
-        if dist is not None:
-            t = torch.tensor([ms], device="cuda", dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ms = float(t.item())
+        ms = max_over_ranks(e_start.elapsed_time(e_end), dist, "cuda")
         pack_ms = float(np.mean([e[0].elapsed_time(e[1]) for e in evs]))
         unpack_ms = float(np.mean([e[1].elapsed_time(e[2]) for e in evs]))
         return ms, pack_ms, unpack_ms, t_wall * 1e3
@@ -368,7 +392,7 @@ def run_ours(args):
     sampler = ClockSampler(local)
     with torch.cuda.stream(stream):
         ms, pack_ms, unpack_ms, wall_ms = timed_loop(K, W, dbufs, DEV, lag, sampler)
-    value = world * K * 2 * P / (ms * 1e-3) / 1e9
+    value = job_payload_gbps(world, K, P, ms)
     token_bytes = 2 * L * H * D * 2
 
     # ---- roofline of the dominant kernel ------------------------------------------------
@@ -393,7 +417,7 @@ def run_ours(args):
         link = memcpy_peaks(torch)
         with torch.cuda.stream(stream):
             ms_e, pack_e, unpack_e, _ = timed_loop(Ke, 3, hb, HOST, 1 if len(hb) > 1 else 0)
-        e2e = {"value": world * Ke * 2 * P / (ms_e * 1e-3) / 1e9, "unit": "GB/s",
+        e2e = {"value": job_payload_gbps(world, Ke, P, ms_e), "unit": "GB/s",
                "h2d_bytes_per_step": P, "d2h_bytes_per_step": P, "steps": Ke,
                "ms_per_step": ms_e / Ke, "gpu_launches": 2 * Ke,
                "pack_to_host_GBps": P / pack_e / 1e6, "restore_from_host_GBps": P / unpack_e / 1e6,
