@@ -268,14 +268,20 @@ def measured_peaks():
     return 6650.0, "B200_PROFILING.md fallback 6.65 TB/s (of fallback)"
 
 
-def ncu_traffic(workload: str, kernel: str):
-    """dram bytes per launch from the committed ncu --set full capture, if any."""
-    p = ROOT / "profiles" / "traffic.json"
-    if p.exists():
-        try:
-            return json.loads(p.read_text()).get(f"{workload}:{kernel}")
-        except Exception:
-            return None
+def ncu_traffic(workload: str, kernel: str, direction: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the
+    committed ncu --set full capture (profiles/traffic.csv, see profiles/README.md), else None."""
+    import csv
+    p = ROOT / "profiles" / "traffic.csv"
+    if not p.exists():
+        return None
+    try:
+        with open(p, newline="") as f:
+            for r in csv.DictReader(f):
+                if (r["workload"], r["kernel"], r["direction"]) == (workload, kernel, direction):
+                    return int(r["dram_bytes_read"]) + int(r["dram_bytes_write"])
+    except Exception:
+        return None
     return None
 
 
@@ -403,7 +409,8 @@ def run_ours(args):
     resolved = args.kernel if args.kernel != "auto" else "warp"
     roofline = {"bound": "hbm", "kernel": f"{dom} ({'kv_copy_' + resolved})", "achieved": achieved,
                 "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": ncu_traffic(args.workload, resolved),
+                "traffic": ncu_traffic(args.workload, resolved,
+                                       "pack" if dom.endswith("pack") else "unpack"),
                 "algorithmic_bytes_per_launch": 2 * P, "peak_source": peak_src,
                 "pack_ms": pack_ms, "unpack_ms": unpack_ms,
                 "pack_traffic_GBps": 2 * P / pack_ms / 1e6, "unpack_traffic_GBps": 2 * P / unpack_ms / 1e6}
