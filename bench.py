@@ -46,6 +46,8 @@ def parse_args():
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--workload", choices=["cfg1", "cfg2", "cfg4"], default="cfg1")
     ap.add_argument("--kernel", choices=["auto", "warp", "bulk"], default="auto")
+    ap.add_argument("--upload-descriptors", action="store_true",
+                    help="LUMEN_KV_NO_INLINE: upload small plans to device memory too (A/B evidence)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=0, help="default: min(steps, 100)")
@@ -344,6 +346,8 @@ def run_ours(args):
 
     kflag = {"auto": lk.LUMEN_KV_KERNEL_AUTO, "warp": lk.LUMEN_KV_KERNEL_WARP,
              "bulk": lk.LUMEN_KV_KERNEL_BULK}[args.kernel]
+    if args.upload_descriptors:
+        kflag |= lk.LUMEN_KV_NO_INLINE
     ra_p, ra_r = lk.ReqArray(w.reqs), lk.ReqArray(w.restore_reqs)
     stream = torch.cuda.Stream()
     sh = stream.cuda_stream
@@ -351,30 +355,44 @@ def run_ours(args):
     DEV, HOST = lk.LUMEN_KV_MEM_DEVICE, lk.LUMEN_KV_MEM_HOST_MAPPED
     UNIQUE = lk.LUMEN_KV_VALIDATE_UNIQUE_DST
 
-    def step(i, bufs, kind, lag_, evs=None):
+    def step(i, bufs, kind, lag_, evs=None, only=None):
+        """only=None: the whole step.  only="pack"/"unpack": that direction alone (same plans,
+        same rotation), used to time one kernel as a back-to-back batch of launches."""
         nb = len(bufs)
-        tb, te = ranges[i % len(ranges)]
-        ra_p.set_ranges(tb, te)                                           # a1
-        tb, te = ranges[(i - lag_) % len(ranges)]
-        ra_r.set_ranges(tb, te)
-        p = lk.lumen_kv_plan_build(geom, ra_p, kflag, sh)                 # a2
-        r = lk.lumen_kv_plan_build(geom, ra_r, kflag | UNIQUE, sh)
+        p = r = None
+        if only != "unpack":
+            tb, te = ranges[i % len(ranges)]
+            ra_p.set_ranges(tb, te)                                           # a1
+            p = lk.lumen_kv_plan_build(geom, ra_p, kflag, sh)                 # a2
+        if only != "pack":
+            tb, te = ranges[(i - lag_) % len(ranges)]
+            ra_r.set_ranges(tb, te)
+            r = lk.lumen_kv_plan_build(geom, ra_r, kflag | UNIQUE, sh)
         if evs is not None:
             evs[0].record(stream)
-        lk.lumen_kv_checkpoint_pack(p, kp, vp, bufs[i % nb].data_ptr(), P, kind, sh)          # a3 / a4
+        if p is not None:
+            lk.lumen_kv_checkpoint_pack(p, kp, vp, bufs[i % nb].data_ptr(), P, kind, sh)          # a3 / a4
         if evs is not None:
             evs[1].record(stream)
-        lk.lumen_kv_restore_unpack(r, kp, vp, bufs[(i - lag_) % nb].data_ptr(), P, kind, sh)  # a7
+        if r is not None:
+            lk.lumen_kv_restore_unpack(r, kp, vp, bufs[(i - lag_) % nb].data_ptr(), P, kind, sh)  # a7
         if evs is not None:
             evs[2].record(stream)
-        p.close(); r.close()
+        if p is not None:
+            p.close()
+        if r is not None:
+            r.close()
 
-    def timed_loop(K, W, bufs, kind, lag_, sampler=None):
+    def timed_loop(K, W, bufs, kind, lag_, sampler=None, per_launch=False, only=None):
+        """W warm-up steps, then exactly K steps between one event pair.  per_launch=True adds
+        an event between the launches of every step (kernel durations); those records sit
+        between the kernels, so that variant is never the one `value` comes from."""
         for i in range(-lag_, 0):                      # fill the buffers the first restores read
             step(i + len(ranges) * len(bufs), bufs, kind, 0)
         for i in range(W):
-            step(i, bufs, kind, lag_)
-        evs = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(K)]
+            step(i, bufs, kind, lag_, only=only)
+        evs = ([[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(K)]
+               if per_launch else None)
         e_start, e_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         barrier(); torch.cuda.synchronize()
         if sampler:
@@ -382,22 +400,29 @@ def run_ours(args):
         t_wall = time.perf_counter()
         e_start.record(stream)
         for i in range(K):
-            step(W + i, bufs, kind, lag_, evs[i])
+            step(W + i, bufs, kind, lag_, evs[i] if per_launch else None, only)
         e_end.record(stream)
+        t_host = time.perf_counter() - t_wall          # host time to enqueue K steps
         stream.synchronize(); torch.cuda.synchronize()
         t_wall = time.perf_counter() - t_wall
         if sampler:
             sampler.stop()
         barrier()
         ms = max_over_ranks(e_start.elapsed_time(e_end), dist, "cuda")
-        pack_ms = float(np.mean([e[0].elapsed_time(e[1]) for e in evs]))
-        unpack_ms = float(np.mean([e[1].elapsed_time(e[2]) for e in evs]))
-        return ms, pack_ms, unpack_ms, t_wall * 1e3
+        pack_ms = unpack_ms = None
+        if per_launch:
+            pack_ms = float(np.mean([e[0].elapsed_time(e[1]) for e in evs]))
+            unpack_ms = float(np.mean([e[1].elapsed_time(e[2]) for e in evs]))
+        return ms, pack_ms, unpack_ms, t_wall * 1e3, t_host * 1e3
 
     K, W = max(1, args.steps), max(3, args.warmup)
     sampler = ClockSampler(local)
+    Kk = min(K, 200)                                   # per-launch pass: same steps, instrumented
     with torch.cuda.stream(stream):
-        ms, pack_ms, unpack_ms, wall_ms = timed_loop(K, W, dbufs, DEV, lag, sampler)
+        ms, _, _, wall_ms, host_ms = timed_loop(K, W, dbufs, DEV, lag, sampler)
+        ms_k, pack_1, unpack_1, _, _ = timed_loop(Kk, 3, dbufs, DEV, lag, per_launch=True)
+        pack_ms = timed_loop(Kk, 3, dbufs, DEV, lag, only="pack")[0] / Kk
+        unpack_ms = timed_loop(Kk, 3, dbufs, DEV, lag, only="unpack")[0] / Kk
     value = job_payload_gbps(world, K, P, ms)
     token_bytes = 2 * L * H * D * 2
 
@@ -412,7 +437,13 @@ def run_ours(args):
                 "traffic": ncu_traffic(args.workload, resolved,
                                        "pack" if dom.endswith("pack") else "unpack"),
                 "algorithmic_bytes_per_launch": 2 * P, "peak_source": peak_src,
+                "timing": (f"average launch duration = one CUDA-event pair around {Kk} back-to-back launches "
+                           "of that direction alone (same plans and buffer rotation as the step), on the "
+                           "launching stream, in this run; *_single_ms = one event pair per launch inside "
+                           f"whole steps ({ms_k / Kk:.4f} ms/step: the records between the launches cost a "
+                           "few us each and prevent the overlap of consecutive launches)"),
                 "pack_ms": pack_ms, "unpack_ms": unpack_ms,
+                "pack_single_ms": pack_1, "unpack_single_ms": unpack_1,
                 "pack_traffic_GBps": 2 * P / pack_ms / 1e6, "unpack_traffic_GBps": 2 * P / unpack_ms / 1e6}
 
     # ---- e2e: same step, host buffers, bytes cross the host link inside the timed region --
@@ -423,7 +454,8 @@ def run_ours(args):
         hb = [pinned_buffer(P) for _ in range(2 if P <= (1 << 30) else 1)]
         link = memcpy_peaks(torch)
         with torch.cuda.stream(stream):
-            ms_e, pack_e, unpack_e, _ = timed_loop(Ke, 3, hb, HOST, 1 if len(hb) > 1 else 0)
+            ms_e, pack_e, unpack_e, _, _ = timed_loop(Ke, 3, hb, HOST, 1 if len(hb) > 1 else 0,
+                                                      per_launch=True)
         e2e = {"value": job_payload_gbps(world, Ke, P, ms_e), "unit": "GB/s",
                "h2d_bytes_per_step": P, "d2h_bytes_per_step": P, "steps": Ke,
                "ms_per_step": ms_e / Ke, "gpu_launches": 2 * Ke,
@@ -444,9 +476,11 @@ def run_ours(args):
                    "l2": (f"inputs larger than L2: steps rotate over {n_stage} staging buffers of "
                           f"{P / 2**20:.0f} MiB and {len(ranges)} distinct delta sets; the restore reads "
                           f"the buffer packed {lag} steps earlier"),
-                   "kernel": args.kernel, "replicas": world, "seed": hex(MASTER_SEED)},
+                   "kernel": args.kernel, "replicas": world,
+                   "descriptors": "uploaded" if args.upload_descriptors else "kernel parameters (plans <= 256 runs)",
+                   "pdl": os.environ.get("LUMEN_KV_PDL", "1") != "0", "seed": hex(MASTER_SEED)},
         "tokens_per_s": value * 1e9 / token_bytes,
-        "wall_ms_per_step": wall_ms / K,
+        "wall_ms_per_step": wall_ms / K, "host_enqueue_ms_per_step": host_ms / K,
         "roofline": roofline, "e2e": e2e, "gpu_launches": 2 * K, "clocks": sampler.summary(),
     }
     if rank == 0:

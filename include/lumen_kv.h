@@ -43,8 +43,8 @@
  *     unpack.  The caller owns pools, buffers, streams and page tables (page
  *     tables are copied at build time).  Plans may be used concurrently from
  *     different streams; one plan must not be used from two host threads at once.
- *   - There is no CPU fallback: without a CUDA device every call except the
- *     host-only plan build and the accessors fails with LUMEN_KV_ECUDA.
+ *   - There is no CPU fallback: without a CUDA device pack and unpack fail with
+ *     LUMEN_KV_ECUDA, and so does every plan_build that has descriptors to upload.
  */
 #ifndef LUMEN_KV_H
 #define LUMEN_KV_H
@@ -100,6 +100,11 @@ typedef struct lumen_kv_plan lumen_kv_plan;  /* opaque; library owns its descrip
 #define LUMEN_KV_MERGE_ADJACENT      0x2u /* merge runs whose physical pages are adjacent     */
 #define LUMEN_KV_HOST_ONLY           0x4u /* build descriptors on the host only (no CUDA call);
                                              such a plan can be inspected but not executed   */
+#define LUMEN_KV_NO_INLINE           0x8u /* always upload the descriptors to device memory.
+                                             By default a plan of <= 256 runs and <= 128
+                                             requests (one decode step's deltas) is carried in
+                                             the kernel parameters: no upload, no device memory,
+                                             and plan_build makes no CUDA call for it          */
 /* kernel selection (default 0 = library heuristic); for benchmarking / evidence   */
 #define LUMEN_KV_KERNEL_SHIFT        8
 #define LUMEN_KV_KERNEL_MASK         0xF00u
@@ -119,7 +124,8 @@ typedef struct lumen_kv_plan lumen_kv_plan;  /* opaque; library owns its descrip
  *   geom, reqs : host pointers, read only during the call.  num_reqs >= 0.
  *   stream     : cudaStream_t on which the descriptor upload is enqueued; the plan
  *                may be used on that stream immediately, on other streams after the
- *                caller orders them behind it.  Ignored with LUMEN_KV_HOST_ONLY.
+ *                caller orders them behind it.  Ignored with LUMEN_KV_HOST_ONLY and for
+ *                small plans that need no upload (see LUMEN_KV_NO_INLINE).
  *   out        : receives the plan; release with lumen_kv_plan_free.
  * Zero-length ranges and num_reqs == 0 are legal (A4) and yield 0 bytes.
  * Errors: EINVAL, ERANGE, EOVERLAP (with VALIDATE_UNIQUE_DST), ENOMEM, ECUDA.

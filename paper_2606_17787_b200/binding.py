@@ -25,6 +25,7 @@ LUMEN_KV_EOVERLAP, LUMEN_KV_ESIZE, LUMEN_KV_ENOMEM, LUMEN_KV_ECUDA = -3, -4, -5,
 LUMEN_KV_VALIDATE_UNIQUE_DST = 0x1
 LUMEN_KV_MERGE_ADJACENT = 0x2
 LUMEN_KV_HOST_ONLY = 0x4
+LUMEN_KV_NO_INLINE = 0x8
 LUMEN_KV_KERNEL_AUTO, LUMEN_KV_KERNEL_WARP, LUMEN_KV_KERNEL_BULK = 0x000, 0x100, 0x200
 LUMEN_KV_MEM_DEVICE, LUMEN_KV_MEM_HOST_MAPPED = 0, 1
 

@@ -50,7 +50,8 @@ def build(force: bool = False, verbose: bool = False) -> Path:
     if res.returncode != 0:
         sys.stderr.write(res.stdout + res.stderr)
         raise RuntimeError("nvcc failed building liblumen_kv.so")
-    (PKG / "build_ptxas.log").write_text(" ".join(cmd) + "\n" + res.stdout + res.stderr)
+    log = (" ".join(cmd) + "\n" + res.stdout + res.stderr).replace(str(tmp), str(SO))
+    (PKG / "build_ptxas.log").write_text(log.replace(str(ROOT) + "/", ""))
     if verbose:
         print(res.stdout + res.stderr)
     os.replace(tmp, SO)

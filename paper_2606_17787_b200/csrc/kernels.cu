@@ -17,6 +17,7 @@
 #include "kernels.hpp"
 
 #include <cstdlib>
+#include <cstring>
 
 namespace lumen {
 namespace {
@@ -42,6 +43,41 @@ __device__ __forceinline__ void st_stream16(void* p, const uint4& v) {
                  : "memory");
 }
 
+// Programmatic dependent launch (sm_90+): `launch_dependents` lets the next kernel in the
+// stream become resident while this grid's last wave drains; `wait` blocks until every
+// prerequisite grid has completed and its memory is visible.  A kernel that was not
+// launched with the programmatic attribute executes both as no-ops.
+__device__ __forceinline__ void pdl_launch_dependents() {
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+}
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
+// Where the descriptors live: in global memory (uploaded by plan_build) or, for small
+// plans, in the kernel parameters themselves (constant bank, no upload, no dependent
+// global loads before the first payload load).
+struct GlobalDesc {
+    const RunDesc* runs;
+    const ReqDesc* reqs;
+    static constexpr bool kInline = false;
+};
+struct InlineDesc {
+    RunDesc runs[kInlineRuns];
+    ReqDesc reqs[kInlineReqs];
+    static constexpr bool kInline = true;
+};
+__device__ __forceinline__ uint4 load_run(const GlobalDesc& d, int64_t run) {
+    return __ldg(reinterpret_cast<const uint4*>(d.runs + run));
+}
+__device__ __forceinline__ longlong2 load_req(const GlobalDesc& d, uint32_t r) {
+    return __ldg(reinterpret_cast<const longlong2*>(d.reqs + r));
+}
+__device__ __forceinline__ uint4 load_run(const InlineDesc& d, int64_t run) {
+    return *reinterpret_cast<const uint4*>(d.runs + run);
+}
+__device__ __forceinline__ longlong2 load_req(const InlineDesc& d, uint32_t r) {
+    return *reinterpret_cast<const longlong2*>(d.reqs + r);
+}
+
 // Decode one item into (pool pointer, buffer pointer, bytes).
 struct Item {
     char* pool;
@@ -49,15 +85,15 @@ struct Item {
     uint32_t bytes;
 };
 
-__device__ __forceinline__ Item decode_item(const RunDesc* __restrict__ runs,
-                                            const ReqDesc* __restrict__ reqs, int64_t run,
+template <class Desc>
+__device__ __forceinline__ Item decode_item(const Desc& desc, int64_t run,
                                             const void* plane_base, int32_t plane, char* buf,
                                             uint32_t row_bytes) {
-    const uint4 d = __ldg(reinterpret_cast<const uint4*>(runs + run));
+    const uint4 d = load_run(desc, run);
     // d.x = src_lo, d.y = dst_tok, d.z = req, d.w = count | src_hi << 16
     const uint32_t count = d.w & 0xFFFFu;
     const uint64_t off16 = (static_cast<uint64_t>(d.w >> 16) << 32) | d.x;
-    const longlong2 q = __ldg(reinterpret_cast<const longlong2*>(reqs + d.z));
+    const longlong2 q = load_req(desc, d.z);
     // q.x = row_base, q.y = n
     const int64_t row = q.x + static_cast<int64_t>(plane) * q.y + d.y;
     Item it;
@@ -78,18 +114,24 @@ __device__ __forceinline__ Item decode_item(const RunDesc* __restrict__ runs,
 // ---------------------------------------------------------------------------------
 constexpr int kWarpsPerCta = 8;
 
-template <int UNROLL>
+template <int UNROLL, class Desc>
 __global__ void __launch_bounds__(kWarpsPerCta * 32)
-kv_copy_warp(const PlaneTable planes, const RunDesc* __restrict__ runs,
-             const ReqDesc* __restrict__ reqs, int64_t n_runs, char* buf, uint32_t row_bytes,
-             int32_t plane0, int sub_shift, int pack) {
+kv_copy_warp(const __grid_constant__ PlaneTable planes, const __grid_constant__ Desc desc,
+             int64_t n_runs, char* buf, uint32_t row_bytes, int32_t plane0, int sub_shift,
+             int pack) {
+    pdl_launch_dependents();
     const int lane = threadIdx.x & 31;
     const int64_t task = static_cast<int64_t>(blockIdx.x) * kWarpsPerCta + (threadIdx.x >> 5);
     const int64_t run = task >> sub_shift;
     if (run >= n_runs) return;
     const uint32_t sub = static_cast<uint32_t>(task & ((int64_t{1} << sub_shift) - 1));
-    const Item it = decode_item(runs, reqs, run, planes.p[blockIdx.y], plane0 + blockIdx.y, buf,
+    // descriptors in global memory were written by an earlier copy in the stream; to stay
+    // independent of how that copy was ordered, only parameter-resident ones are decoded
+    // before the wait
+    if (!Desc::kInline) pdl_wait();
+    const Item it = decode_item(desc, run, planes.p[blockIdx.y], plane0 + blockIdx.y, buf,
                                 row_bytes);
+    if (Desc::kInline) pdl_wait();
     const uint32_t nvec = it.bytes >> 4;
     const uint32_t i = sub * (UNROLL * 32) + lane;
     if (sub * (UNROLL * 32) >= nvec) return;           // this run is shorter than the longest
@@ -165,9 +207,9 @@ struct StageMeta {
 // iterations after its load so that LAG loads are in flight per CTA.
 template <int STAGES>
 __global__ void __launch_bounds__(32)
-kv_copy_bulk(const PlaneTable planes, const RunDesc* __restrict__ runs,
-             const ReqDesc* __restrict__ reqs, int64_t n_runs, int32_t n_planes, char* buf,
-             uint32_t row_bytes, uint32_t stage_bytes, int32_t plane0, int pack) {
+kv_copy_bulk(const __grid_constant__ PlaneTable planes, const __grid_constant__ GlobalDesc desc,
+             int64_t n_runs, int32_t n_planes, char* buf, uint32_t row_bytes,
+             uint32_t stage_bytes, int32_t plane0, int pack) {
     constexpr int LAG = (STAGES + 1) / 2;
     extern __shared__ __align__(128) unsigned char smem[];
     __shared__ __align__(8) uint64_t full_bar[STAGES];
@@ -192,7 +234,7 @@ kv_copy_bulk(const PlaneTable planes, const RunDesc* __restrict__ runs,
         if (mine < total) {
             const int32_t pl = static_cast<int32_t>(mine / n_runs);
             const int64_t run = mine - static_cast<int64_t>(pl) * n_runs;
-            my = decode_item(runs, reqs, run, planes.p[pl], plane0 + pl, buf, row_bytes);
+            my = decode_item(desc, run, planes.p[pl], plane0 + pl, buf, row_bytes);
         }
         const char* my_src = pack ? my.pool : my.buf;
         char* my_dst = pack ? my.buf : my.pool;
@@ -275,15 +317,45 @@ cudaError_t launch_bulk(const PlaneTable& pt, const CopyArgs& a, int32_t plane0,
     int64_t grid = static_cast<int64_t>(g_num_sms) * c.ctas_per_sm;
     if (grid > total) grid = total;
     kern<<<static_cast<unsigned>(grid), 32, c.smem, a.stream>>>(
-        pt, a.runs, a.reqs, a.n_runs, np, static_cast<char*>(a.buf),
+        pt, GlobalDesc{a.runs, a.reqs}, a.n_runs, np, static_cast<char*>(a.buf),
         static_cast<uint32_t>(a.row_bytes), c.stage_bytes, plane0, a.pack ? 1 : 0);
     return cudaGetLastError();
+}
+
+struct WarpLaunch {
+    dim3 grid;
+    cudaStream_t stream;
+    int64_t n_runs;
+    char* buf;
+    uint32_t row_bytes;
+    int32_t plane0;
+    int sub_shift;
+    int pack;
+};
+
+int g_pdl = 1;   // LUMEN_KV_PDL=0 launches without the programmatic attribute (A/B evidence)
+
+template <int UNROLL, class Desc>
+cudaError_t launch_warp(const PlaneTable& pt, const Desc& d, const WarpLaunch& w) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = w.grid;
+    cfg.blockDim = dim3(kWarpsPerCta * 32, 1, 1);
+    cfg.dynamicSmemBytes = 0;
+    cfg.stream = w.stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = g_pdl ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, kv_copy_warp<UNROLL, Desc>, pt, d, w.n_runs, w.buf,
+                              w.row_bytes, w.plane0, w.sub_shift, w.pack);
 }
 
 }  // namespace
 
 int resolve_kernel(const CopyArgs& a) {
     int k = a.kernel;
+    if (a.inline_desc) return kKernelWarp;   // parameter-resident plans exist for this kernel only
     const int64_t item_max = static_cast<int64_t>(a.max_count) * a.row_bytes;
     if (k == kKernelBulk && item_max > kChunkBytes) k = kKernelWarp;  // one row > ring slot
     if (k == kKernelAuto) k = kKernelWarp;
@@ -294,6 +366,7 @@ cudaError_t launch_kv_copy(const CopyArgs& a) {
     if (a.n_runs == 0 || a.n_planes == 0) return cudaSuccess;
     if (g_num_sms == 0) {
         if (const char* e = getenv("LUMEN_KV_WARP_UNROLL")) g_warp_unroll = (atoi(e) == 8) ? 8 : 4;
+        if (const char* e = getenv("LUMEN_KV_PDL")) g_pdl = atoi(e) ? 1 : 0;
         int dev = 0;
         cudaError_t e = cudaGetDevice(&dev);
         if (e != cudaSuccess) return e;
@@ -322,23 +395,30 @@ cudaError_t launch_kv_copy(const CopyArgs& a) {
             }
         } else {
             // sub-chunks per item: smallest power of two covering the longest run
-            const int unroll = g_warp_unroll;
-            const int64_t sub_bytes = int64_t{512} * unroll;
+            const int64_t sub_bytes = int64_t{512} * g_warp_unroll;
             int sub_shift = 0;
             while ((sub_bytes << sub_shift) < item_max) ++sub_shift;
             const int64_t tasks = a.n_runs << sub_shift;
             const int64_t gx = (tasks + kWarpsPerCta - 1) / kWarpsPerCta;
             if (gx > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
-            dim3 grid(static_cast<unsigned>(gx), static_cast<unsigned>(np), 1);
-            if (unroll == 4)
-                kv_copy_warp<4><<<grid, kWarpsPerCta * 32, 0, a.stream>>>(
-                    pt, a.runs, a.reqs, a.n_runs, static_cast<char*>(a.buf),
-                    static_cast<uint32_t>(a.row_bytes), plane0, sub_shift, a.pack ? 1 : 0);
-            else
-                kv_copy_warp<8><<<grid, kWarpsPerCta * 32, 0, a.stream>>>(
-                    pt, a.runs, a.reqs, a.n_runs, static_cast<char*>(a.buf),
-                    static_cast<uint32_t>(a.row_bytes), plane0, sub_shift, a.pack ? 1 : 0);
-            e = cudaGetLastError();
+            WarpLaunch w;
+            w.grid = dim3(static_cast<unsigned>(gx), static_cast<unsigned>(np), 1);
+            w.stream = a.stream;
+            w.n_runs = a.n_runs;
+            w.buf = static_cast<char*>(a.buf);
+            w.row_bytes = static_cast<uint32_t>(a.row_bytes);
+            w.plane0 = plane0;
+            w.sub_shift = sub_shift;
+            w.pack = a.pack ? 1 : 0;
+            if (a.inline_desc) {
+                InlineDesc d;   // unused tail entries are never indexed (run < n_runs)
+                std::memcpy(d.runs, a.runs, static_cast<size_t>(a.n_runs) * sizeof(RunDesc));
+                std::memcpy(d.reqs, a.reqs, static_cast<size_t>(a.n_reqs) * sizeof(ReqDesc));
+                e = (g_warp_unroll == 4) ? launch_warp<4>(pt, d, w) : launch_warp<8>(pt, d, w);
+            } else {
+                const GlobalDesc d{a.runs, a.reqs};
+                e = (g_warp_unroll == 4) ? launch_warp<4>(pt, d, w) : launch_warp<8>(pt, d, w);
+            }
         }
         if (e != cudaSuccess) return e;
     }

@@ -10,11 +10,19 @@ namespace lumen {
 
 constexpr int kMaxPlanesPerLaunch = 256;  // plane pointers travel as kernel parameters
 
+// Small plans (one decode step: 64 requests x 1-2 runs) travel entirely in the kernel
+// parameters: no descriptor upload, no device blob, and a CTA starts its payload loads
+// without first waiting on two dependent descriptor loads from global memory.
+constexpr int kInlineRuns = 256;
+constexpr int kInlineReqs = 128;
+
 enum KernelKind : int { kKernelAuto = 0, kKernelWarp = 1, kKernelBulk = 2 };
 
 struct CopyArgs {
-    const RunDesc* runs = nullptr;   // device
-    const ReqDesc* reqs = nullptr;   // device
+    const RunDesc* runs = nullptr;   // device (or host when inline_desc)
+    const ReqDesc* reqs = nullptr;   // device (or host when inline_desc)
+    int32_t n_reqs = 0;
+    bool inline_desc = false;        // descriptors are HOST pointers, passed as kernel parameters
     int64_t n_runs = 0;
     int64_t row_bytes = 0;
     int32_t max_count = 0;           // longest run in tokens

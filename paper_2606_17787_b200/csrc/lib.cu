@@ -129,6 +129,7 @@ struct lumen_kv_plan {
     int64_t n_runs = 0;
     int32_t n_reqs = 0;
     uint32_t flags = 0;
+    bool inline_desc = false;  // small plan: descriptors stay in hp and travel as kernel parameters
 };
 
 namespace lumen {
@@ -186,9 +187,11 @@ int run_copy(const lumen_kv_plan* plan, const void* const* k_planes, const void*
     if (reinterpret_cast<uintptr_t>(dev_buf) & 15) return LUMEN_KV_EINVAL;
 
     CopyArgs a;
-    a.runs = plan->d_runs;
-    a.reqs = plan->d_reqs;
+    a.inline_desc = plan->inline_desc;
+    a.runs = plan->inline_desc ? plan->h_runs : plan->d_runs;
+    a.reqs = plan->inline_desc ? plan->h_reqs : plan->d_reqs;
     a.n_runs = plan->n_runs;
+    a.n_reqs = plan->n_reqs;
     a.row_bytes = plan->hp.row_bytes;
     a.max_count = plan->hp.max_count;
     a.planes = planes.data();
@@ -200,6 +203,7 @@ int run_copy(const lumen_kv_plan* plan, const void* const* k_planes, const void*
     a.stream = static_cast<cudaStream_t>(stream);
     cudaError_t e = launch_kv_copy(a);
     if (e != cudaSuccess) return cuda_fail(e);
+    if (plan->inline_desc) return LUMEN_KV_OK;   // nothing on the device to keep alive
     return note_use(const_cast<lumen_kv_plan*>(plan), a.stream);
 }
 
@@ -235,6 +239,17 @@ int lumen_kv_plan_build(const lumen_kv_geom* geom, const lumen_kv_req* reqs, int
     const size_t run_bytes = p->hp.runs.size() * sizeof(RunDesc);
     const size_t req_bytes = p->hp.reqs.size() * sizeof(ReqDesc);
     const size_t total = run_bytes + req_bytes;
+
+    // Small plans (a decode step's deltas) need no device copy at all: the kernel receives
+    // the descriptors in its parameters.  Only the SIMT kernel has that variant.
+    if (!(flags & (LUMEN_KV_HOST_ONLY | LUMEN_KV_NO_INLINE)) && ksel != LUMEN_KV_KERNEL_BULK &&
+        p->n_runs <= kInlineRuns && num_reqs <= kInlineReqs) {
+        p->inline_desc = true;
+        p->h_runs = p->hp.runs.data();
+        p->h_reqs = p->hp.reqs.data();
+        *out = p;
+        return LUMEN_KV_OK;
+    }
 
     if (flags & LUMEN_KV_HOST_ONLY) {
         Blob* b = new (std::nothrow) Blob();

@@ -42,7 +42,7 @@ int build_host_plan(const lumen_kv_geom* g, const lumen_kv_req* reqs, int32_t nu
     if (!g || !hp) return LUMEN_KV_EINVAL;
     if (num_reqs < 0 || (num_reqs > 0 && !reqs)) return LUMEN_KV_EINVAL;
     const uint32_t known = LUMEN_KV_VALIDATE_UNIQUE_DST | LUMEN_KV_MERGE_ADJACENT |
-                           LUMEN_KV_HOST_ONLY | LUMEN_KV_KERNEL_MASK;
+                           LUMEN_KV_HOST_ONLY | LUMEN_KV_NO_INLINE | LUMEN_KV_KERNEL_MASK;
     if (flags & ~known) return LUMEN_KV_EINVAL;
     if (g->num_layers < 1 || g->kv_heads < 1 || g->head_dim < 1 || g->page_size < 1 ||
         g->elem_bytes < 1 || g->reserved != 0)

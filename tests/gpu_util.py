@@ -9,8 +9,11 @@ from paper_2606_17787_b200.pool import KVPool, Checkpointer, pinned_buffer
 from workloads import device as wdev
 from workloads import fill_plane_np
 
+# "warp": plans of <= 256 runs travel in the kernel parameters; "warp_upload" forces the
+# descriptor upload to device memory for those too, so both descriptor paths are compared
 KERNELS = {"warp": lk.LUMEN_KV_KERNEL_WARP, "bulk": lk.LUMEN_KV_KERNEL_BULK,
-           "auto": lk.LUMEN_KV_KERNEL_AUTO}
+           "auto": lk.LUMEN_KV_KERNEL_AUTO,
+           "warp_upload": lk.LUMEN_KV_KERNEL_WARP | lk.LUMEN_KV_NO_INLINE}
 
 
 def build_all():

@@ -65,13 +65,13 @@ def run_case(G, w, kernel, where, *, merge=False, seed=MASTER_SEED):
 
 
 @pytest.mark.parametrize("where", ["device", "host"])
-@pytest.mark.parametrize("kernel", ["warp", "bulk", "auto"])
+@pytest.mark.parametrize("kernel", ["warp", "warp_upload", "bulk", "auto"])
 def test_cfg0_tiny(G, kernel, where):
     run_case(G, cfg0_tiny(), kernel, where)
     run_case(G, cfg0_tiny(full_prefix=True), kernel, where)
 
 
-@pytest.mark.parametrize("kernel", ["warp", "bulk"])
+@pytest.mark.parametrize("kernel", ["warp", "warp_upload", "bulk"])
 def test_random_tiny_geometries(G, kernel):
     rng = substream(2024, "gpu_tiny")
     n = 0
@@ -83,7 +83,7 @@ def test_random_tiny_geometries(G, kernel):
         n += 1
 
 
-@pytest.mark.parametrize("kernel", ["warp", "bulk"])
+@pytest.mark.parametrize("kernel", ["warp", "warp_upload", "bulk"])
 def test_mid_cfg1_shape(G, kernel):
     """Qwen3-14B row/page shape, fewer layers/pages: 32 KiB runs, ragged 16-token deltas."""
     w = cfg1_qwen14b(L=3, N=2048, n_reqs=24, grow_iters=2, median=200, hi=512, lo=20)

@@ -194,15 +194,24 @@ def test_empty_plans(lk):
 
 
 def test_no_cpu_fallback(lk):
-    """Without a CUDA device the executable plan build must fail loudly (ECUDA)."""
+    """Without a CUDA device everything that would touch the device fails loudly (ECUDA):
+    the descriptor upload of plan_build, and pack/unpack of a parameter-resident plan
+    (whose build makes no CUDA call)."""
     import torch
     if torch.cuda.is_available():
         pytest.skip("GPU present")
     g = lk.make_geom(2, 2, 8, 4, 16)
     pt = np.array([1], dtype=np.int32)
     with pytest.raises(lk.LumenKVError) as e:
-        lk.lumen_kv_plan_build(g, [(pt, 0, 2)], 0)
+        lk.lumen_kv_plan_build(g, [(pt, 0, 2)], lk.LUMEN_KV_NO_INLINE)
     assert e.value.status == lk.LUMEN_KV_ECUDA
+    small = lk.lumen_kv_plan_build(g, [(pt, 0, 2)], 0)
+    assert small.nbytes == 2 * 2 * 2 * 32 and small.num_runs == 1
+    for call in (lk.lumen_kv_checkpoint_pack, lk.lumen_kv_restore_unpack):
+        with pytest.raises(lk.LumenKVError) as e:
+            call(small, [16, 16], [16, 16], 16, 1 << 20)
+        assert e.value.status == lk.LUMEN_KV_ECUDA
+    small.close()
     # a host-only plan cannot be executed
     p = lk.lumen_kv_plan_build(g, [(pt, 0, 2)], lk.LUMEN_KV_HOST_ONLY)
     with pytest.raises(lk.LumenKVError) as e:
