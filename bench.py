@@ -44,7 +44,7 @@ def parse_args():
     ap.add_argument("--steps", type=int, default=300)
     ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
-    ap.add_argument("--workload", choices=["cfg1", "cfg2", "cfg4"], default="cfg1")
+    ap.add_argument("--workload", choices=["cfg1", "cfg2", "cfg3", "cfg4"], default="cfg1")
     ap.add_argument("--kernel", choices=["auto", "warp", "bulk"], default="auto")
     ap.add_argument("--upload-descriptors", action="store_true",
                     help="LUMEN_KV_NO_INLINE: upload small plans to device memory too (A/B evidence)")
@@ -156,6 +156,17 @@ def oracle_sample(workload: str, seed: int):
     """A bounded sample of the workload on a sparse host pool: one step's pack + restore
     for cfg1 (2 x 160 MiB); for the 32 GiB configs the first request's first 4096 tokens."""
     from workloads.hostpool import sparse_host_pool
+    if workload == "cfg3":
+        # burst sample: one 1-token delta pack of the 64 running requests + the restore of the
+        # first interrupted request's first 4096 tokens into its free-list pages
+        from workloads import Workload, cfg3_burst
+        b = cfg3_burst(seed)
+        pt, _, _ = b.waves[0][0]
+        n = min(4096, b.waves[0][0][2])
+        w = Workload("cfg3_burst", b.geom, list(b.running), [(pt, 0, n)])
+        K, V, keep = sparse_host_pool(w.geom, seed, list(w.reqs) + list(w.restore_reqs))
+        return (w, "BASELINE.json configs[3] (recovery burst, Qwen3-32B shape)", w.reqs, w.restore_reqs,
+                K, V, keep, f"1-token pack of 64 running requests + restore of {n} tokens of one request")
     w, label, delta = make_workload(workload, seed)
     if workload == "cfg1":
         reqs, rreqs, what = w.reqs, w.restore_reqs, "one full step (64 requests x 16 tokens, pack + restore)"
@@ -171,6 +182,11 @@ def oracle_sample(workload: str, seed: int):
 def oracle_step(geom, K, V, reqs, rreqs, omp=False):
     import oracle
     B = oracle.pack(geom, K, V, reqs, omp=omp)
+    n_restore = oracle.total_elems(geom, rreqs)
+    if n_restore != B.size:        # burst sample: the restored checkpoint is not the packed delta
+        R = np.zeros(n_restore, dtype=np.uint16)
+        oracle.unpack(geom, K, V, rreqs, R, omp=omp)
+        return (B.size + n_restore) * 2
     oracle.unpack(geom, K, V, rreqs, B, omp=omp)
     return 2 * B.size * 2          # payload bytes moved: packed + restored
 
@@ -463,7 +479,54 @@ def run_ours(args):
                "memcpy_peak_d2h_GBps": link["d2h"], "memcpy_peak_h2d_GBps": link["h2d"],
                "pack_frac_of_d2h_peak": P / pack_e / 1e6 / link["d2h"],
                "restore_frac_of_h2d_peak": P / unpack_e / 1e6 / link["h2d"],
-               "path": "kernel stores/loads on mapped pinned host memory (zero-copy over PCIe)"}
+               "path": ("kernel stores/loads on mapped pinned host memory (zero-copy over PCIe), pack then "
+                        "restore on one stream")}
+        if len(hb) > 1:
+            # a8: the link is full duplex -- step i's pack (D2H) and the restore of the buffer packed
+            # in step i-1 (H2D) run on two streams, ordered only by the events on the two buffers
+            sA, sB = torch.cuda.Stream(), torch.cuda.Stream()
+            packed = [torch.cuda.Event() for _ in hb]
+            restored = [torch.cuda.Event() for _ in hb]
+
+            def duplex_step(i):
+                cur, prev = i % 2, (i - 1) % 2
+                tb, te = ranges[i % len(ranges)]
+                ra_p.set_ranges(tb, te)
+                tb, te = ranges[(i - 1) % len(ranges)]
+                ra_r.set_ranges(tb, te)
+                p = lk.lumen_kv_plan_build(geom, ra_p, kflag, sA.cuda_stream)
+                r = lk.lumen_kv_plan_build(geom, ra_r, kflag | UNIQUE, sB.cuda_stream)
+                sA.wait_event(restored[cur])            # the restore that last read this buffer
+                lk.lumen_kv_checkpoint_pack(p, kp, vp, hb[cur].data_ptr(), P, HOST, sA.cuda_stream)
+                packed[cur].record(sA)
+                sB.wait_event(packed[prev])
+                lk.lumen_kv_restore_unpack(r, kp, vp, hb[prev].data_ptr(), P, HOST, sB.cuda_stream)
+                restored[prev].record(sB)
+                p.close(); r.close()
+
+            for ev in packed + restored:
+                ev.record(sA)
+            for i in range(3):
+                duplex_step(i)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            barrier(); torch.cuda.synchronize()
+            e0.record(sA)
+            sB.wait_event(e0)
+            for i in range(3, 3 + Ke):
+                duplex_step(i)
+            done_b = torch.cuda.Event(); done_b.record(sB)
+            sA.wait_event(done_b)
+            e1.record(sA)
+            torch.cuda.synchronize(); barrier()
+            ms_d = max_over_ranks(e0.elapsed_time(e1), dist, "cuda")
+            e2e["one_stream_value"] = e2e["value"]
+            e2e["one_stream_ms_per_step"] = e2e["ms_per_step"]
+            e2e["value"] = job_payload_gbps(world, Ke, P, ms_d)
+            e2e["ms_per_step"] = ms_d / Ke
+            e2e["duplex_frac_of_d2h_plus_h2d_peak"] = e2e["value"] / world / (link["d2h"] + link["h2d"])
+            e2e["path"] = ("kernel stores/loads on mapped pinned host memory (zero-copy over PCIe); value = "
+                           "pack of step i (D2H) and restore of step i-1's buffer (H2D) on two streams, "
+                           "full duplex; one_stream_* = the same calls back to back on one stream")
         del hb
 
     line = {
@@ -491,10 +554,117 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def run_cfg3(args):
+    """BASELINE.json configs[3], the recovery burst (a6-a8): every wave of interrupted requests
+    is restored from pinned host memory into pages popped from the seeded shuffled free list,
+    first alone, then again while a second stream keeps packing 1-token deltas of the 64
+    running requests to pinned host memory.  `value` = restored payload GB/s with the
+    concurrent packs running, summed over the waves (bytes / device time)."""
+    import torch
+    import paper_2606_17787_b200 as lk
+    from paper_2606_17787_b200.pool import KVPool, pinned_buffer
+    from workloads import MASTER_SEED, cfg3_burst
+    from workloads import device as wdev
+
+    rank, world, local = rank_env()
+    if world != 1:
+        raise RuntimeError("--workload cfg3 is a 1-GPU workload")
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: there is no CPU path for --impl ours")
+    torch.cuda.set_device(local)
+    wdev.build()
+    b = cfg3_burst(MASTER_SEED)
+    L, H, D, S, N = b.geom
+    tok_bytes = 2 * L * H * D * 2
+    pool = KVPool(L, H, D, S, N)
+    for i, t in enumerate(pool.planes()):
+        wdev.fill_plane(t, MASTER_SEED, i)
+    wave_bytes = [sum(te for _, _, te in w) * tok_bytes for w in b.waves]
+    hbuf = wdev.pinned_exact(max(wave_bytes))
+    wdev.fill_host_checkpoint(hbuf, max(wave_bytes), MASTER_SEED + 30, 0xC3)
+    link = memcpy_peaks(torch)
+    n_pb = 8
+    pbytes = len(b.running) * tok_bytes
+    pbufs = [pinned_buffer(pbytes) for _ in range(n_pb)]
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    geom, kp, vp, HOST = pool.geom, pool.k_ptrs, pool.v_ptrs, lk.LUMEN_KV_MEM_HOST_MAPPED
+    ra = lk.ReqArray(b.running)
+    te0 = np.array([te for _, _, te in b.running], dtype=np.int64)
+    sampler = ClockSampler(local)
+
+    def restore(wave, nbytes, concurrent):
+        plan = lk.lumen_kv_plan_build(geom, wave, lk.LUMEN_KV_VALIDATE_UNIQUE_DST, s1.cuda_stream)
+        a, z = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        pa, pz = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        a.record(s1)
+        lk.lumen_kv_restore_unpack(plan, kp, vp, hbuf.data_ptr(), nbytes, HOST, s1.cuda_stream)
+        z.record(s1)
+        it = 0
+        if concurrent:
+            pa.record(s2)
+            while not z.query():                        # a2-a4 on stream 2 until the restore ends
+                ra.set_ranges(te0 + (it % 48), te0 + (it % 48) + 1)
+                p = lk.lumen_kv_plan_build(geom, ra, 0, s2.cuda_stream)
+                lk.lumen_kv_checkpoint_pack(p, kp, vp, pbufs[it % n_pb].data_ptr(), pbytes, HOST,
+                                            s2.cuda_stream)
+                p.close()
+                it += 1
+                if it % n_pb == 0:
+                    s2.synchronize()                    # bound the queue: n_pb packs in flight
+            pz.record(s2)
+        torch.cuda.synchronize()
+        plan.close()
+        return a.elapsed_time(z), it, (pa.elapsed_time(pz) if concurrent else 0.0)
+
+    restore(b.waves[-1], wave_bytes[-1], False)         # warm-up
+    alone = [restore(w, nb, False)[0] for w, nb in zip(b.waves, wave_bytes)]
+    sampler.start()
+    conc = [restore(w, nb, True) for w, nb in zip(b.waves, wave_bytes)]
+    sampler.stop()
+    total = sum(wave_bytes)
+    t_alone, t_conc = sum(alone), sum(c[0] for c in conc)
+    packs, t_pack = sum(c[1] for c in conc), sum(c[2] for c in conc)
+    value = total / t_conc / 1e6
+    line = {
+        "metric": "kv_pack_restore_payload_GBps", "value": value, "unit": "GB/s", "n_gpus": 1,
+        "steps": len(b.waves), "warmup": 1, "ms_per_step": t_conc / len(b.waves),
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u16",
+        "data": "synthetic",
+        "config": {"workload": ("BASELINE.json configs[3]: recovery burst, Qwen3-32B shape, pool "
+                                f"{N} pages 40 % occupied by 64 running requests, 48 interrupted prefixes "
+                                f"U{{1024..32768}} = {total / 2**30:.1f} GiB restored from pinned host in "
+                                f"{len(b.waves)} waves (the as-written single shot needs a 330 GiB pool), "
+                                "concurrent 1-token delta packs to pinned host on a second stream"),
+                   "wave_GiB": [x / 2**30 for x in wave_bytes], "seed": hex(MASTER_SEED),
+                   "l2": "inputs larger than L2: every wave is tens of GiB read once over the host link"},
+        "tokens_per_s": value * 1e9 / tok_bytes,
+        "restore_alone_GBps": total / t_alone / 1e6,
+        "restore_concurrent_GBps": value,
+        "concurrent_packs": {"iterations": packs, "bytes_each": pbytes,
+                             "GBps": packs * pbytes / t_pack / 1e6 if t_pack else None,
+                             "ms_each": t_pack / packs if packs else None},
+        "roofline": {"bound": "host_link", "kernel": "lumen_kv_restore_unpack (kv_copy_warp, mapped host source)",
+                     "achieved": total / t_alone / 1e6, "peak": link["h2d"], "unit": "GB/s",
+                     "frac": total / t_alone / 1e6 / link["h2d"], "traffic": None,
+                     "peak_source": "pinned cudaMemcpyAsync H2D, 1 GiB, best of 10, this run",
+                     "frac_with_concurrent_packs": value / link["h2d"],
+                     "memcpy_peak_d2h_GBps": link["d2h"]},
+        "e2e": {"value": value, "unit": "GB/s", "h2d_bytes_per_step": total // len(b.waves),
+                "d2h_bytes_per_step": packs * pbytes // len(b.waves),
+                "note": "this workload is the host path: the timed region is the H2D restore itself"},
+        "gpu_launches": 2 * len(b.waves) + 1 + packs, "clocks": sampler.summary(),
+    }
+    print(json.dumps(line), flush=True)
+    wdev.unpin(hbuf)
+
+
 def main():
     args = parse_args()
     if args.impl == "reference":
         run_reference(args)
+    elif args.workload == "cfg3":
+        run_cfg3(args)
     else:
         run_ours(args)
 

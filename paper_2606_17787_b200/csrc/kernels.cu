@@ -205,9 +205,9 @@ struct StageMeta {
 
 // STAGES ring slots of stage_bytes each; the store of item i is issued LAG
 // iterations after its load so that LAG loads are in flight per CTA.
-template <int STAGES>
+template <int STAGES, class Desc>
 __global__ void __launch_bounds__(32)
-kv_copy_bulk(const __grid_constant__ PlaneTable planes, const __grid_constant__ GlobalDesc desc,
+kv_copy_bulk(const __grid_constant__ PlaneTable planes, const __grid_constant__ Desc desc,
              int64_t n_runs, int32_t n_planes, char* buf, uint32_t row_bytes,
              uint32_t stage_bytes, int32_t plane0, int pack) {
     constexpr int LAG = (STAGES + 1) / 2;
@@ -283,6 +283,7 @@ struct BulkCfg {
     uint32_t stage_bytes;
     size_t smem;
     int ctas_per_sm;
+    int host_ctas;
 };
 
 BulkCfg bulk_config(int64_t item_bytes_max) {
@@ -290,11 +291,15 @@ BulkCfg bulk_config(int64_t item_bytes_max) {
     const uint32_t sb = static_cast<uint32_t>((item_bytes_max + 127) & ~int64_t{127});
     BulkCfg c{};
     c.stage_bytes = sb;
-    if (sb > 16384)      { c.stages = 3;  c.ctas_per_sm = 2; }
-    else if (sb > 8192)  { c.stages = 4;  c.ctas_per_sm = 3; }
-    else if (sb > 4096)  { c.stages = 6;  c.ctas_per_sm = 4; }
-    else if (sb > 2048)  { c.stages = 8;  c.ctas_per_sm = 6; }
-    else                 { c.stages = 16; c.ctas_per_sm = 6; }
+    // host_ctas: grid when the buffer is host memory, sized for about 1.5 MB of loads in flight
+    // (LAG x slot x CTAs) -- ten times the bandwidth-delay product of the Gen5 x16 link, and
+    // little enough that the queued host traffic does not get in the way of HBM traffic
+    // (measured: a full grid slows a concurrent HBM copy 1.87x).
+    if (sb > 16384)      { c.stages = 3;  c.ctas_per_sm = 2; c.host_ctas = 24; }
+    else if (sb > 8192)  { c.stages = 4;  c.ctas_per_sm = 3; c.host_ctas = 48; }
+    else if (sb > 4096)  { c.stages = 6;  c.ctas_per_sm = 4; c.host_ctas = 64; }
+    else if (sb > 2048)  { c.stages = 8;  c.ctas_per_sm = 6; c.host_ctas = 96; }
+    else                 { c.stages = 16; c.ctas_per_sm = 6; c.host_ctas = 96; }
     c.smem = static_cast<size_t>(c.stages) * sb;
     return c;
 }
@@ -302,10 +307,12 @@ BulkCfg bulk_config(int64_t item_bytes_max) {
 int g_num_sms = 0;
 int g_warp_unroll = 4;   // LUMEN_KV_WARP_UNROLL=4|8 (tuning knob, read once; 4 measured best)
 
-template <int STAGES>
-cudaError_t launch_bulk(const PlaneTable& pt, const CopyArgs& a, int32_t plane0, int32_t np,
-                        const BulkCfg& c) {
-    auto kern = kv_copy_bulk<STAGES>;
+int g_host_ctas = 0;   // grid of the bulk kernel when the buffer is host memory (0: default)
+
+template <int STAGES, class Desc>
+cudaError_t launch_bulk_desc(const PlaneTable& pt, const Desc& d, const CopyArgs& a, int32_t plane0,
+                             int32_t np, const BulkCfg& c) {
+    auto kern = kv_copy_bulk<STAGES, Desc>;
     static bool attr_set = false;
     if (!attr_set) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -315,11 +322,27 @@ cudaError_t launch_bulk(const PlaneTable& pt, const CopyArgs& a, int32_t plane0,
     }
     const int64_t total = a.n_runs * np;
     int64_t grid = static_cast<int64_t>(g_num_sms) * c.ctas_per_sm;
+    // A host-memory buffer is bound by the host link (~55 GB/s): a few dozen single-warp
+    // CTAs keep it full, and the SMs stay free for whatever else the device is running
+    // (checkpointing must stay off the GPU critical path).
+    if (a.buf_is_host) grid = g_host_ctas > 0 ? g_host_ctas : c.host_ctas;
     if (grid > total) grid = total;
     kern<<<static_cast<unsigned>(grid), 32, c.smem, a.stream>>>(
-        pt, GlobalDesc{a.runs, a.reqs}, a.n_runs, np, static_cast<char*>(a.buf),
-        static_cast<uint32_t>(a.row_bytes), c.stage_bytes, plane0, a.pack ? 1 : 0);
+        pt, d, a.n_runs, np, static_cast<char*>(a.buf), static_cast<uint32_t>(a.row_bytes),
+        c.stage_bytes, plane0, a.pack ? 1 : 0);
     return cudaGetLastError();
+}
+
+template <int STAGES>
+cudaError_t launch_bulk(const PlaneTable& pt, const CopyArgs& a, int32_t plane0, int32_t np,
+                        const BulkCfg& c) {
+    if (a.inline_desc) {
+        InlineDesc d;
+        std::memcpy(d.runs, a.runs, static_cast<size_t>(a.n_runs) * sizeof(RunDesc));
+        std::memcpy(d.reqs, a.reqs, static_cast<size_t>(a.n_reqs) * sizeof(ReqDesc));
+        return launch_bulk_desc<STAGES>(pt, d, a, plane0, np, c);
+    }
+    return launch_bulk_desc<STAGES>(pt, GlobalDesc{a.runs, a.reqs}, a, plane0, np, c);
 }
 
 struct WarpLaunch {
@@ -353,12 +376,13 @@ cudaError_t launch_warp(const PlaneTable& pt, const Desc& d, const WarpLaunch& w
 
 }  // namespace
 
+int g_host_kernel = kKernelBulk;   // LUMEN_KV_HOST_KERNEL=warp|bulk: what AUTO picks for host buffers
+
 int resolve_kernel(const CopyArgs& a) {
     int k = a.kernel;
-    if (a.inline_desc) return kKernelWarp;   // parameter-resident plans exist for this kernel only
     const int64_t item_max = static_cast<int64_t>(a.max_count) * a.row_bytes;
+    if (k == kKernelAuto) k = a.buf_is_host ? g_host_kernel : kKernelWarp;
     if (k == kKernelBulk && item_max > kChunkBytes) k = kKernelWarp;  // one row > ring slot
-    if (k == kKernelAuto) k = kKernelWarp;
     return k;
 }
 
@@ -367,12 +391,15 @@ cudaError_t launch_kv_copy(const CopyArgs& a) {
     if (g_num_sms == 0) {
         if (const char* e = getenv("LUMEN_KV_WARP_UNROLL")) g_warp_unroll = (atoi(e) == 8) ? 8 : 4;
         if (const char* e = getenv("LUMEN_KV_PDL")) g_pdl = atoi(e) ? 1 : 0;
+        if (const char* e = getenv("LUMEN_KV_HOST_KERNEL"))
+            g_host_kernel = (e[0] == 'w') ? kKernelWarp : kKernelBulk;
         int dev = 0;
         cudaError_t e = cudaGetDevice(&dev);
         if (e != cudaSuccess) return e;
         e = cudaDeviceGetAttribute(&g_num_sms, cudaDevAttrMultiProcessorCount, dev);
         if (e != cudaSuccess) return e;
     }
+    if (const char* e = getenv("LUMEN_KV_HOST_CTAS")) g_host_ctas = atoi(e);   // sweep knob
     const int kernel = resolve_kernel(a);
     const int64_t item_max = static_cast<int64_t>(a.max_count) * a.row_bytes;
 

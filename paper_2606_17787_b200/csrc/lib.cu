@@ -241,9 +241,8 @@ int lumen_kv_plan_build(const lumen_kv_geom* geom, const lumen_kv_req* reqs, int
     const size_t total = run_bytes + req_bytes;
 
     // Small plans (a decode step's deltas) need no device copy at all: the kernel receives
-    // the descriptors in its parameters.  Only the SIMT kernel has that variant.
-    if (!(flags & (LUMEN_KV_HOST_ONLY | LUMEN_KV_NO_INLINE)) && ksel != LUMEN_KV_KERNEL_BULK &&
-        p->n_runs <= kInlineRuns && num_reqs <= kInlineReqs) {
+    // the descriptors in its parameters.
+    if (!(flags & (LUMEN_KV_HOST_ONLY | LUMEN_KV_NO_INLINE)) && p->n_runs <= kInlineRuns && num_reqs <= kInlineReqs) {
         p->inline_desc = true;
         p->h_runs = p->hp.runs.data();
         p->h_reqs = p->hp.reqs.data();

@@ -46,6 +46,33 @@ def fill_plane(t, seed: int, plane: int, stream: int = 0) -> None:
         raise RuntimeError(f"kvfill_fill failed ({rc})")
 
 
+def fill_words(t, first_word: int, seed: int, plane: int, stream: int = 0) -> None:
+    """Fills t (a chunk of a larger logical array) with words [first_word, first_word + n) of
+    g(seed, plane, .): lets a host-resident checkpoint be generated chunk by chunk on the device."""
+    n_words = t.numel() * t.element_size() // 2
+    if first_word % 4:
+        raise ValueError("first_word must be a multiple of 4 (one 64-bit hash = 4 words)")
+    rc = lib().kvfill_fill(t.data_ptr(), int(first_word), n_words, seed & 0xFFFFFFFFFFFFFFFF, plane,
+                           stream)
+    if rc:
+        raise RuntimeError(f"kvfill_fill failed ({rc})")
+
+
+def fill_host_checkpoint(host_buf, nbytes: int, seed: int, plane: int, chunk_bytes: int = 1 << 30):
+    """host_buf[:nbytes] (pinned uint8 tensor) <- g(seed, plane, word index), generated on the
+    device in chunks and copied down (a 72 GiB checkpoint would take minutes with numpy)."""
+    import torch
+    scratch = torch.empty(min(chunk_bytes, max(nbytes, 8)), dtype=torch.uint8, device="cuda")
+    at = 0
+    while at < nbytes:
+        n = min(scratch.numel(), nbytes - at)
+        fill_words(scratch[:n], at // 2, seed, plane)
+        host_buf[at: at + n].copy_(scratch[:n], non_blocking=True)
+        torch.cuda.synchronize()
+        at += n
+    del scratch
+
+
 def page_checksums(t, n_pages: int, page_bytes: int, stream: int = 0):
     import torch
     out = torch.empty(n_pages, dtype=torch.int64, device=t.device)
