@@ -171,6 +171,59 @@ LUMEN_KV_API int lumen_kv_restore_unpack(const lumen_kv_plan* plan,
                             void* const* k_planes, void* const* v_planes,
                             const void* src, int64_t src_bytes, int src_kind, void* stream);
 
+/*
+ * Two-stage host path (steps a4 / a7 through the copy engines).
+ *
+ * PAPER.md:145 step 3 copies the new KV "from GPU memory to the local pinned buffer" in
+ * the background and PAPER.md:122 requires that this stays off the GPU critical path.
+ * lumen_kv_checkpoint_pack with LUMEN_KV_MEM_HOST_MAPPED does it with SM stores over the
+ * host link.  The staged form cuts the plan into chunks that are contiguous in the
+ * checkpoint buffer, packs chunk c into slot c % n_slots of a caller-provided DEVICE
+ * staging ring with the HBM-speed kernel (microseconds of SM time), and moves the slot to
+ * dst + chunk offset with cudaMemcpyAsync on the stager's own copy stream while the next
+ * chunk is being packed; restore runs the mirror image (H2D copy, then unpack).  The
+ * bytes that arrive are identical to the one-shot call's.
+ *
+ * A stager owns one non-blocking copy stream and 2*n_slots events; it holds no payload
+ * memory.  staging: device pointer, 16-byte aligned, n_slots*slot_bytes bytes, owned by
+ * the caller and not touched by anything else while a staged call is in flight.
+ * slot_bytes must be a multiple of 16 and at least as large as the longest run of every
+ * plan used with it (32 KiB unless a single row is larger), else ESIZE.  2 <= n_slots <= 16.
+ * One stager serves one staged call at a time (calls on it are serialised by its events);
+ * use one stager per direction to run pack and restore concurrently.
+ *
+ * Stream semantics are those of the one-shot calls: the work is ordered after everything
+ * enqueued on `stream` before the call, and work enqueued on `stream` after the call sees
+ * the complete result (host buffer for pack, pool for restore).  host buffers: pinned
+ * host memory (cudaHostAlloc / cudaHostRegister); pass the HOST pointer.
+ * Errors: EINVAL, ESIZE, ECUDA.
+ */
+typedef struct lumen_kv_stager lumen_kv_stager;
+LUMEN_KV_API int lumen_kv_stager_create(void* staging, int64_t slot_bytes, int32_t n_slots,
+                                        lumen_kv_stager** out);
+LUMEN_KV_API void lumen_kv_stager_destroy(lumen_kv_stager* stager);   /* synchronises its copy stream */
+LUMEN_KV_API int lumen_kv_checkpoint_pack_staged(const lumen_kv_plan* plan,
+                             const void* const* k_planes, const void* const* v_planes,
+                             void* dst_host, int64_t dst_bytes, lumen_kv_stager* stager,
+                             void* stream);
+LUMEN_KV_API int lumen_kv_restore_unpack_staged(const lumen_kv_plan* plan,
+                             void* const* k_planes, void* const* v_planes,
+                             const void* src_host, int64_t src_bytes, lumen_kv_stager* stager,
+                             void* stream);
+/* number of chunks a staged call on this plan would be cut into for the given slot size
+ * (host arithmetic only; ESIZE if a run does not fit a slot) */
+LUMEN_KV_API int64_t lumen_kv_plan_num_chunks(const lumen_kv_plan* plan, int64_t slot_bytes);
+/* The chunks themselves, for inspection: chunk i = runs [run_begin, run_end) replicated over
+ * planes [plane_begin, plane_end) = buffer bytes [byte_begin, byte_end).  Writes at most cap
+ * entries to out (may be NULL when cap == 0); returns the number of chunks or a status. */
+typedef struct {
+    int64_t run_begin, run_end;
+    int32_t plane_begin, plane_end;
+    int64_t byte_begin, byte_end;
+} lumen_kv_chunk_info;
+LUMEN_KV_API int64_t lumen_kv_plan_get_chunks(const lumen_kv_plan* plan, int64_t slot_bytes,
+                                              lumen_kv_chunk_info* out, int64_t cap);
+
 /* Release a plan.  Safe to call while work using the plan is still in flight on a
  * stream: the descriptors are recycled only after that work has completed.       */
 LUMEN_KV_API void lumen_kv_plan_free(lumen_kv_plan* plan);

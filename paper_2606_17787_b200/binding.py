@@ -34,6 +34,8 @@ EXPORTS = (
     "lumen_kv_plan_num_runs", "lumen_kv_plan_get_run", "lumen_kv_checkpoint_pack",
     "lumen_kv_restore_unpack", "lumen_kv_plan_free", "lumen_kv_trim",
     "lumen_kv_strerror", "lumen_kv_last_cuda_error", "lumen_kv_version",
+    "lumen_kv_stager_create", "lumen_kv_stager_destroy", "lumen_kv_checkpoint_pack_staged",
+    "lumen_kv_restore_unpack_staged", "lumen_kv_plan_num_chunks", "lumen_kv_plan_get_chunks",
 )
 
 
@@ -52,6 +54,12 @@ class lumen_kv_req(ctypes.Structure):
 class lumen_kv_run_info(ctypes.Structure):
     _fields_ = [("src_slot", ctypes.c_int64), ("dst_token", ctypes.c_int64),
                 ("req", ctypes.c_int32), ("count", ctypes.c_int32)]
+
+
+class lumen_kv_chunk_info(ctypes.Structure):
+    _fields_ = [("run_begin", ctypes.c_int64), ("run_end", ctypes.c_int64),
+                ("plane_begin", ctypes.c_int32), ("plane_end", ctypes.c_int32),
+                ("byte_begin", ctypes.c_int64), ("byte_end", ctypes.c_int64)]
 
 
 class LumenKVError(RuntimeError):
@@ -92,6 +100,18 @@ def _lib() -> ctypes.CDLL:
         f = getattr(L, name)
         f.restype = ctypes.c_int
         f.argtypes = [vp, ctypes.POINTER(vp), ctypes.POINTER(vp), vp, i64, ctypes.c_int, vp]
+    L.lumen_kv_stager_create.restype = ctypes.c_int
+    L.lumen_kv_stager_create.argtypes = [vp, i64, i32, ctypes.POINTER(vp)]
+    L.lumen_kv_stager_destroy.restype = None
+    L.lumen_kv_stager_destroy.argtypes = [vp]
+    for name in ("lumen_kv_checkpoint_pack_staged", "lumen_kv_restore_unpack_staged"):
+        f = getattr(L, name)
+        f.restype = ctypes.c_int
+        f.argtypes = [vp, ctypes.POINTER(vp), ctypes.POINTER(vp), vp, i64, vp, vp]
+    L.lumen_kv_plan_num_chunks.restype = i64
+    L.lumen_kv_plan_num_chunks.argtypes = [vp, i64]
+    L.lumen_kv_plan_get_chunks.restype = i64
+    L.lumen_kv_plan_get_chunks.argtypes = [vp, i64, ctypes.POINTER(lumen_kv_chunk_info), i64]
     L.lumen_kv_plan_free.restype = None
     L.lumen_kv_plan_free.argtypes = [vp]
     L.lumen_kv_trim.restype = None
@@ -151,6 +171,17 @@ class Plan:
         if rc:
             raise LumenKVError(rc, "lumen_kv_plan_get_run")
         return info
+
+    def chunks(self, slot_bytes: int):
+        """The chunks a staged call with this slot size is cut into (list of lumen_kv_chunk_info)."""
+        n = int(_lib().lumen_kv_plan_num_chunks(self.handle, int(slot_bytes)))
+        if n < 0:
+            raise LumenKVError(n, "lumen_kv_plan_num_chunks")
+        arr = (lumen_kv_chunk_info * max(n, 1))()
+        m = int(_lib().lumen_kv_plan_get_chunks(self.handle, int(slot_bytes), arr, n))
+        if m != n:
+            raise LumenKVError(min(m, -1), "lumen_kv_plan_get_chunks")
+        return [arr[i] for i in range(n)]
 
     def close(self) -> None:
         if self._h:
@@ -263,6 +294,56 @@ def lumen_kv_restore_unpack(plan: Plan, k_planes, v_planes, src: int, src_bytes:
                                         ctypes.c_void_p(int(stream)))
     if rc:
         raise LumenKVError(rc, "lumen_kv_restore_unpack")
+
+
+class Stager:
+    """Owner of a `lumen_kv_stager*` over caller-provided device staging memory."""
+
+    def __init__(self, staging_ptr: int, slot_bytes: int, n_slots: int):
+        out = ctypes.c_void_p()
+        rc = _lib().lumen_kv_stager_create(ctypes.c_void_p(int(staging_ptr)), int(slot_bytes),
+                                           int(n_slots), ctypes.byref(out))
+        if rc:
+            raise LumenKVError(rc, "lumen_kv_stager_create")
+        self._h = out
+        self.slot_bytes, self.n_slots = int(slot_bytes), int(n_slots)
+
+    @property
+    def handle(self) -> ctypes.c_void_p:
+        if not self._h:
+            raise ValueError("stager already destroyed")
+        return self._h
+
+    def close(self) -> None:
+        if self._h:
+            _lib().lumen_kv_stager_destroy(self._h)
+            self._h = ctypes.c_void_p(None)
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def lumen_kv_checkpoint_pack_staged(plan: Plan, k_planes, v_planes, dst_host: int, dst_bytes: int,
+                                    stager: Stager, stream: int = 0) -> None:
+    L = plan.geom.num_layers
+    rc = _lib().lumen_kv_checkpoint_pack_staged(
+        plan.handle, _as_ptr_array(k_planes, L), _as_ptr_array(v_planes, L),
+        ctypes.c_void_p(int(dst_host)), int(dst_bytes), stager.handle, ctypes.c_void_p(int(stream)))
+    if rc:
+        raise LumenKVError(rc, "lumen_kv_checkpoint_pack_staged")
+
+
+def lumen_kv_restore_unpack_staged(plan: Plan, k_planes, v_planes, src_host: int, src_bytes: int,
+                                   stager: Stager, stream: int = 0) -> None:
+    L = plan.geom.num_layers
+    rc = _lib().lumen_kv_restore_unpack_staged(
+        plan.handle, _as_ptr_array(k_planes, L), _as_ptr_array(v_planes, L),
+        ctypes.c_void_p(int(src_host)), int(src_bytes), stager.handle, ctypes.c_void_p(int(stream)))
+    if rc:
+        raise LumenKVError(rc, "lumen_kv_restore_unpack_staged")
 
 
 def lumen_kv_plan_free(plan: Plan) -> None:

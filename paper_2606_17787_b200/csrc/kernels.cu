@@ -329,7 +329,7 @@ cudaError_t launch_bulk_desc(const PlaneTable& pt, const Desc& d, const CopyArgs
     if (grid > total) grid = total;
     kern<<<static_cast<unsigned>(grid), 32, c.smem, a.stream>>>(
         pt, d, a.n_runs, np, static_cast<char*>(a.buf), static_cast<uint32_t>(a.row_bytes),
-        c.stage_bytes, plane0, a.pack ? 1 : 0);
+        c.stage_bytes, a.plane_base + plane0, a.pack ? 1 : 0);
     return cudaGetLastError();
 }
 
@@ -434,7 +434,7 @@ cudaError_t launch_kv_copy(const CopyArgs& a) {
             w.n_runs = a.n_runs;
             w.buf = static_cast<char*>(a.buf);
             w.row_bytes = static_cast<uint32_t>(a.row_bytes);
-            w.plane0 = plane0;
+            w.plane0 = a.plane_base + plane0;
             w.sub_shift = sub_shift;
             w.pack = a.pack ? 1 : 0;
             if (a.inline_desc) {

@@ -28,6 +28,7 @@ struct CopyArgs {
     int32_t max_count = 0;           // longest run in tokens
     const void* const* planes = nullptr;  // HOST array of n_planes device pointers (K0,V0,K1,V1,..)
     int32_t n_planes = 0;
+    int32_t plane_base = 0;          // absolute index of planes[0] (a launch over a plane sub-range)
     void* buf = nullptr;             // device-accessible checkpoint buffer
     bool buf_is_host = false;        // mapped pinned host memory
     bool pack = true;                // true: planes -> buf, false: buf -> planes

@@ -155,6 +155,54 @@ int note_use(lumen_kv_plan* p, cudaStream_t stream) {
     return LUMEN_KV_OK;
 }
 
+// validation shared by the one-shot and the staged calls: interleaves the plane pointers
+// (K0,V0,K1,V1,..) into `planes`
+int gather_planes(const lumen_kv_plan* plan, const void* const* k_planes,
+                  const void* const* v_planes, std::vector<const void*>* planes) {
+    if (!k_planes || !v_planes) return LUMEN_KV_EINVAL;
+    const int32_t L = plan->hp.geom.num_layers;
+    planes->resize(static_cast<size_t>(2 * L));
+    for (int32_t l = 0; l < L; ++l) {
+        const void* k = k_planes[l];
+        const void* v = v_planes[l];
+        if (!k || !v) return LUMEN_KV_EINVAL;
+        if ((reinterpret_cast<uintptr_t>(k) | reinterpret_cast<uintptr_t>(v)) & 15)
+            return LUMEN_KV_EINVAL;
+        (*planes)[2 * l] = k;
+        (*planes)[2 * l + 1] = v;
+    }
+    return LUMEN_KV_OK;
+}
+
+// Enqueue runs [ra, rb) x planes [p0, p1) of the plan.  `buf` is the address that byte 0 of
+// the plan's checkpoint buffer would have (for a staging slot: slot base - chunk offset, so
+// it may lie outside any allocation; only bytes of the chunk are ever addressed).
+int launch_part(const lumen_kv_plan* plan, const std::vector<const void*>& planes, uintptr_t buf,
+                bool buf_is_host, cudaStream_t stream, bool pack, int64_t ra, int64_t rb,
+                int32_t p0, int32_t p1) {
+    if (rb <= ra || p1 <= p0) return LUMEN_KV_OK;
+    CopyArgs a;
+    a.inline_desc = plan->inline_desc;
+    a.runs = (plan->inline_desc ? plan->h_runs : plan->d_runs) + ra;
+    a.reqs = plan->inline_desc ? plan->h_reqs : plan->d_reqs;
+    a.n_runs = rb - ra;
+    a.n_reqs = plan->n_reqs;
+    a.row_bytes = plan->hp.row_bytes;
+    a.max_count = plan->hp.max_count;
+    a.planes = planes.data() + p0;
+    a.n_planes = p1 - p0;
+    a.plane_base = p0;
+    a.buf = reinterpret_cast<void*>(buf);
+    a.buf_is_host = buf_is_host;
+    a.pack = pack;
+    a.kernel = static_cast<int>((plan->flags & LUMEN_KV_KERNEL_MASK) >> LUMEN_KV_KERNEL_SHIFT);
+    a.stream = stream;
+    cudaError_t e = launch_kv_copy(a);
+    if (e != cudaSuccess) return cuda_fail(e);
+    if (plan->inline_desc) return LUMEN_KV_OK;   // nothing on the device to keep alive
+    return note_use(const_cast<lumen_kv_plan*>(plan), stream);
+}
+
 int run_copy(const lumen_kv_plan* plan, const void* const* k_planes, const void* const* v_planes,
              void* buf, int64_t buf_bytes, int kind, void* stream, bool pack) {
     if (!plan) return LUMEN_KV_EINVAL;
@@ -162,19 +210,10 @@ int run_copy(const lumen_kv_plan* plan, const void* const* k_planes, const void*
     if (kind != LUMEN_KV_MEM_DEVICE && kind != LUMEN_KV_MEM_HOST_MAPPED) return LUMEN_KV_EINVAL;
     if (buf_bytes < plan->hp.total_bytes) return LUMEN_KV_ESIZE;
     if (plan->hp.total_bytes == 0) return LUMEN_KV_OK;  // A4: empty plan launches nothing
-    if (!k_planes || !v_planes || !buf) return LUMEN_KV_EINVAL;
-
-    const int32_t L = plan->hp.geom.num_layers;
-    std::vector<const void*> planes(static_cast<size_t>(2 * L));
-    for (int32_t l = 0; l < L; ++l) {
-        const void* k = k_planes[l];
-        const void* v = v_planes[l];
-        if (!k || !v) return LUMEN_KV_EINVAL;
-        if ((reinterpret_cast<uintptr_t>(k) | reinterpret_cast<uintptr_t>(v)) & 15)
-            return LUMEN_KV_EINVAL;
-        planes[2 * l] = k;
-        planes[2 * l + 1] = v;
-    }
+    if (!buf) return LUMEN_KV_EINVAL;
+    std::vector<const void*> planes;
+    int rc = gather_planes(plan, k_planes, v_planes, &planes);
+    if (rc != LUMEN_KV_OK) return rc;
     void* dev_buf = buf;
     if (kind == LUMEN_KV_MEM_HOST_MAPPED) {
         cudaError_t e = cudaHostGetDevicePointer(&dev_buf, buf, 0);
@@ -185,32 +224,171 @@ int run_copy(const lumen_kv_plan* plan, const void* const* k_planes, const void*
         }
     }
     if (reinterpret_cast<uintptr_t>(dev_buf) & 15) return LUMEN_KV_EINVAL;
+    return launch_part(plan, planes, reinterpret_cast<uintptr_t>(dev_buf),
+                       kind == LUMEN_KV_MEM_HOST_MAPPED, static_cast<cudaStream_t>(stream), pack, 0,
+                       plan->n_runs, 0, 2 * plan->hp.geom.num_layers);
+}
 
-    CopyArgs a;
-    a.inline_desc = plan->inline_desc;
-    a.runs = plan->inline_desc ? plan->h_runs : plan->d_runs;
-    a.reqs = plan->inline_desc ? plan->h_reqs : plan->d_reqs;
-    a.n_runs = plan->n_runs;
-    a.n_reqs = plan->n_reqs;
-    a.row_bytes = plan->hp.row_bytes;
-    a.max_count = plan->hp.max_count;
-    a.planes = planes.data();
-    a.n_planes = 2 * L;
-    a.buf = dev_buf;
-    a.buf_is_host = (kind == LUMEN_KV_MEM_HOST_MAPPED);
-    a.pack = pack;
-    a.kernel = static_cast<int>((plan->flags & LUMEN_KV_KERNEL_MASK) >> LUMEN_KV_KERNEL_SHIFT);
-    a.stream = static_cast<cudaStream_t>(stream);
-    cudaError_t e = launch_kv_copy(a);
-    if (e != cudaSuccess) return cuda_fail(e);
-    if (plan->inline_desc) return LUMEN_KV_OK;   // nothing on the device to keep alive
-    return note_use(const_cast<lumen_kv_plan*>(plan), a.stream);
+}  // namespace
+}  // namespace lumen
+
+// Two-stage host path: device staging ring + copy-engine transfers (include/lumen_kv.h).
+struct lumen_kv_stager {
+    char* base = nullptr;          // caller's device staging memory
+    int64_t slot_bytes = 0;
+    int32_t n_slots = 0;
+    int64_t next = 0;              // chunks issued so far: chunk i uses slot i % n_slots
+    cudaStream_t copy = nullptr;   // the stager's copy stream (non-blocking)
+    cudaEvent_t full[16];          // slot holds a complete chunk (producer done)
+    cudaEvent_t free_[16];         // slot may be overwritten (consumer done)
+    cudaEvent_t join = nullptr;
+};
+
+namespace lumen {
+namespace {
+
+#define LUMEN_CUDA(x)                                  \
+    do {                                               \
+        cudaError_t e_ = (x);                          \
+        if (e_ != cudaSuccess) return cuda_fail(e_);   \
+    } while (0)
+
+int run_staged(const lumen_kv_plan* plan, const void* const* k_planes, const void* const* v_planes,
+               void* host, int64_t host_bytes, lumen_kv_stager* st, void* stream_, bool pack) {
+    if (!plan || !st) return LUMEN_KV_EINVAL;
+    if (plan->flags & LUMEN_KV_HOST_ONLY) return LUMEN_KV_EINVAL;
+    if (host_bytes < plan->hp.total_bytes) return LUMEN_KV_ESIZE;
+    if (plan->hp.total_bytes == 0) return LUMEN_KV_OK;
+    if (!host || (reinterpret_cast<uintptr_t>(host) & 15)) return LUMEN_KV_EINVAL;
+    std::vector<const void*> planes;
+    int rc = gather_planes(plan, k_planes, v_planes, &planes);
+    if (rc != LUMEN_KV_OK) return rc;
+    void* alias = nullptr;         // only to reject pageable memory: the copies must be asynchronous
+    if (cudaHostGetDevicePointer(&alias, host, 0) != cudaSuccess) {
+        (void)cudaGetLastError();
+        return LUMEN_KV_EINVAL;
+    }
+    std::vector<Chunk> chunks;
+    rc = build_chunks(plan->hp, plan->h_runs, st->slot_bytes, &chunks);
+    if (rc != LUMEN_KV_OK) return rc;
+
+    cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+    char* h = static_cast<char*>(host);
+    if (!pack) {   // the host buffer may have been produced by earlier work on `stream`
+        LUMEN_CUDA(cudaEventRecord(st->join, stream));
+        LUMEN_CUDA(cudaStreamWaitEvent(st->copy, st->join, 0));
+    }
+    for (const Chunk& c : chunks) {
+        const int slot = static_cast<int>(st->next++ % st->n_slots);
+        char* sbase = st->base + int64_t{slot} * st->slot_bytes;
+        // the address byte 0 of the checkpoint buffer would have if the chunk sat in this slot
+        const uintptr_t shifted = reinterpret_cast<uintptr_t>(sbase) - static_cast<uintptr_t>(c.b0);
+        const size_t bytes = static_cast<size_t>(c.b1 - c.b0);
+        if (pack) {
+            LUMEN_CUDA(cudaStreamWaitEvent(stream, st->free_[slot], 0));
+            rc = launch_part(plan, planes, shifted, false, stream, true, c.ra, c.rb, c.p0, c.p1);
+            if (rc != LUMEN_KV_OK) return rc;
+            LUMEN_CUDA(cudaEventRecord(st->full[slot], stream));
+            LUMEN_CUDA(cudaStreamWaitEvent(st->copy, st->full[slot], 0));
+            LUMEN_CUDA(cudaMemcpyAsync(h + c.b0, sbase, bytes, cudaMemcpyDeviceToHost, st->copy));
+            LUMEN_CUDA(cudaEventRecord(st->free_[slot], st->copy));
+        } else {
+            LUMEN_CUDA(cudaStreamWaitEvent(st->copy, st->free_[slot], 0));
+            LUMEN_CUDA(cudaMemcpyAsync(sbase, h + c.b0, bytes, cudaMemcpyHostToDevice, st->copy));
+            LUMEN_CUDA(cudaEventRecord(st->full[slot], st->copy));
+            LUMEN_CUDA(cudaStreamWaitEvent(stream, st->full[slot], 0));
+            rc = launch_part(plan, planes, shifted, false, stream, false, c.ra, c.rb, c.p0, c.p1);
+            if (rc != LUMEN_KV_OK) return rc;
+            LUMEN_CUDA(cudaEventRecord(st->free_[slot], stream));
+        }
+    }
+    if (pack) {    // work enqueued on `stream` after this call sees the complete host buffer
+        LUMEN_CUDA(cudaEventRecord(st->join, st->copy));
+        LUMEN_CUDA(cudaStreamWaitEvent(stream, st->join, 0));
+    }
+    return LUMEN_KV_OK;
 }
 
 }  // namespace
 }  // namespace lumen
 
 extern "C" {
+
+int lumen_kv_stager_create(void* staging, int64_t slot_bytes, int32_t n_slots,
+                           lumen_kv_stager** out) {
+    using namespace lumen;
+    if (!out) return LUMEN_KV_EINVAL;
+    *out = nullptr;
+    if (!staging || (reinterpret_cast<uintptr_t>(staging) & 15) || slot_bytes < 16 ||
+        slot_bytes % 16 != 0 || n_slots < 2 || n_slots > 16)
+        return LUMEN_KV_EINVAL;
+    lumen_kv_stager* st = new (std::nothrow) lumen_kv_stager();
+    if (!st) return LUMEN_KV_ENOMEM;
+    st->base = static_cast<char*>(staging);
+    st->slot_bytes = slot_bytes;
+    st->n_slots = n_slots;
+    for (int i = 0; i < 16; ++i) st->full[i] = st->free_[i] = nullptr;
+    cudaError_t e = cudaStreamCreateWithFlags(&st->copy, cudaStreamNonBlocking);
+    for (int i = 0; i < n_slots && e == cudaSuccess; ++i) {
+        e = cudaEventCreateWithFlags(&st->full[i], cudaEventDisableTiming);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&st->free_[i], cudaEventDisableTiming);
+    }
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&st->join, cudaEventDisableTiming);
+    if (e != cudaSuccess) {
+        lumen_kv_stager_destroy(st);
+        return cuda_fail(e);
+    }
+    *out = st;
+    return LUMEN_KV_OK;
+}
+
+void lumen_kv_stager_destroy(lumen_kv_stager* st) {
+    if (!st) return;
+    if (st->copy) {
+        cudaStreamSynchronize(st->copy);
+        cudaStreamDestroy(st->copy);
+    }
+    for (int i = 0; i < 16; ++i) {
+        if (st->full[i]) cudaEventDestroy(st->full[i]);
+        if (st->free_[i]) cudaEventDestroy(st->free_[i]);
+    }
+    if (st->join) cudaEventDestroy(st->join);
+    (void)cudaGetLastError();
+    delete st;
+}
+
+int lumen_kv_checkpoint_pack_staged(const lumen_kv_plan* plan, const void* const* k_planes,
+                                    const void* const* v_planes, void* dst_host,
+                                    int64_t dst_bytes, lumen_kv_stager* stager, void* stream) {
+    return lumen::run_staged(plan, k_planes, v_planes, dst_host, dst_bytes, stager, stream, true);
+}
+
+int lumen_kv_restore_unpack_staged(const lumen_kv_plan* plan, void* const* k_planes,
+                                   void* const* v_planes, const void* src_host,
+                                   int64_t src_bytes, lumen_kv_stager* stager, void* stream) {
+    return lumen::run_staged(plan, const_cast<const void* const*>(k_planes),
+                             const_cast<const void* const*>(v_planes),
+                             const_cast<void*>(src_host), src_bytes, stager, stream, false);
+}
+
+int64_t lumen_kv_plan_get_chunks(const lumen_kv_plan* plan, int64_t slot_bytes,
+                                 lumen_kv_chunk_info* out, int64_t cap) {
+    if (!plan || cap < 0 || (cap > 0 && !out)) return LUMEN_KV_EINVAL;
+    std::vector<lumen::Chunk> chunks;
+    const int rc = lumen::build_chunks(plan->hp, plan->h_runs, slot_bytes, &chunks);
+    if (rc != LUMEN_KV_OK) return rc;
+    const int64_t n = static_cast<int64_t>(chunks.size());
+    for (int64_t i = 0; i < n && i < cap; ++i) {
+        const lumen::Chunk& c = chunks[static_cast<size_t>(i)];
+        out[i] = lumen_kv_chunk_info{c.ra, c.rb, c.p0, c.p1, c.b0, c.b1};
+    }
+    return n;
+}
+
+int64_t lumen_kv_plan_num_chunks(const lumen_kv_plan* plan, int64_t slot_bytes) {
+    return lumen_kv_plan_get_chunks(plan, slot_bytes, nullptr, 0);
+}
+
 
 int lumen_kv_plan_build(const lumen_kv_geom* geom, const lumen_kv_req* reqs, int32_t num_reqs,
                         uint32_t flags, void* stream, lumen_kv_plan** out) {

@@ -136,8 +136,10 @@ int build_host_plan(const lumen_kv_geom* g, const lumen_kv_req* reqs, int32_t nu
 
     // pass 2: flatten into runs
     hp->runs.reserve(static_cast<size_t>(touched * std::max<int64_t>(1, (dense + kChunkBytes - 1) / kChunkBytes)));
+    hp->req_run_begin.assign(static_cast<size_t>(num_reqs) + 1, 0);
     for (int32_t r = 0; r < num_reqs; ++r) {
         const lumen_kv_req& q = reqs[r];
+        hp->req_run_begin[r] = static_cast<int64_t>(hp->runs.size());
         if (q.t_end == q.t_begin) continue;
         Extent cur;
         int64_t t = q.t_begin;
@@ -157,6 +159,62 @@ int build_host_plan(const lumen_kv_geom* g, const lumen_kv_req* reqs, int32_t nu
         }
         if (cur.count > 0) emit(hp, cur, r, chunk_tokens);
     }
+    hp->req_run_begin[num_reqs] = static_cast<int64_t>(hp->runs.size());
+    return LUMEN_KV_OK;
+}
+
+int build_chunks(const HostPlan& hp, const RunDesc* runs, int64_t slot_bytes,
+                 std::vector<Chunk>* out) {
+    out->clear();
+    if (slot_bytes < 16 || slot_bytes % 16 != 0) return LUMEN_KV_EINVAL;
+    const int64_t row = hp.row_bytes;
+    const int32_t planes = 2 * hp.geom.num_layers;
+    if (int64_t{hp.max_count} * row > slot_bytes) return LUMEN_KV_ESIZE;
+    const int64_t R = static_cast<int64_t>(hp.req_offset.size()) - 1;
+    Chunk group{0, 0, 0, planes, 0, 0};          // whole requests accumulated so far
+    auto flush = [&]() {
+        if (group.b1 > group.b0) out->push_back(group);
+    };
+    for (int64_t r = 0; r < R; ++r) {
+        const int64_t off = hp.req_offset[r], bytes = hp.req_offset[r + 1] - off;
+        const int64_t ra = hp.req_run_begin[r], rb = hp.req_run_begin[r + 1];
+        if (bytes == 0) continue;
+        if (bytes <= slot_bytes) {
+            if (group.b1 > group.b0 && group.b1 - group.b0 + bytes > slot_bytes) {
+                flush();
+                group.b0 = group.b1 = off;
+            }
+            if (group.b1 == group.b0) { group.ra = ra; group.b0 = off; }
+            group.rb = rb;
+            group.b1 = off + bytes;
+            continue;
+        }
+        flush();
+        group.b0 = group.b1 = off + bytes;
+        const int64_t pb = bytes / planes;       // one plane of this request: n_r * row
+        if (pb <= slot_bytes) {
+            const int32_t k = static_cast<int32_t>(std::min<int64_t>(planes, slot_bytes / pb));
+            for (int32_t p0 = 0; p0 < planes; p0 += k) {
+                const int32_t p1 = std::min(planes, p0 + k);
+                out->push_back(Chunk{ra, rb, p0, p1, off + p0 * pb, off + p1 * pb});
+            }
+            continue;
+        }
+        for (int32_t p = 0; p < planes; ++p) {   // split the token axis at run boundaries
+            int64_t a = ra;
+            while (a < rb) {
+                int64_t b = a, sz = 0;
+                while (b < rb && sz + int64_t{runs[b].count} * row <= slot_bytes) {
+                    sz += int64_t{runs[b].count} * row;
+                    ++b;
+                }
+                const int64_t b0 = off + p * pb + int64_t{runs[a].dst_tok} * row;
+                out->push_back(Chunk{a, b, p, p + 1, b0, b0 + sz});
+                a = b;
+            }
+        }
+    }
+    flush();
     return LUMEN_KV_OK;
 }
 

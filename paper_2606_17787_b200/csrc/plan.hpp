@@ -43,7 +43,23 @@ struct HostPlan {
     std::vector<RunDesc> runs;
     std::vector<ReqDesc> reqs;
     std::vector<int64_t> req_offset;  // num_reqs + 1 byte offsets
+    std::vector<int64_t> req_run_begin;  // num_reqs + 1: runs of request r are [begin[r], begin[r+1])
 };
+
+// A piece of a plan that is contiguous in the checkpoint buffer: runs [ra, rb) replicated
+// over planes [p0, p1) cover exactly the buffer bytes [b0, b1).  Either whole requests over
+// all planes, or one request over a plane range, or one plane of one request over a token
+// range (buffer layout [req][plane][token], include/lumen_kv.h).
+struct Chunk {
+    int64_t ra, rb;
+    int32_t p0, p1;
+    int64_t b0, b1;
+};
+
+// Cuts the plan into chunks of at most slot_bytes each (the two-stage host path).  `runs` are
+// the plan's run descriptors on the host.  ESIZE if a single run is larger than slot_bytes.
+int build_chunks(const HostPlan& hp, const RunDesc* runs, int64_t slot_bytes,
+                 std::vector<Chunk>* out);
 
 // Validates and flattens.  Returns a lumen_kv_status.
 int build_host_plan(const lumen_kv_geom* geom, const lumen_kv_req* reqs,

@@ -68,6 +68,20 @@ def _kind_of(buf: torch.Tensor) -> int:
     raise ValueError("checkpoint buffer must be a CUDA tensor or a pinned host tensor")
 
 
+class StagingRing:
+    """Device staging memory + the library's stager for the two-stage host path
+    (lumen_kv_checkpoint_pack_staged / lumen_kv_restore_unpack_staged)."""
+
+    def __init__(self, slot_bytes: int = 32 << 20, n_slots: int = 3,
+                 device: Optional[torch.device] = None):
+        self.mem = torch.empty(int(slot_bytes) * int(n_slots), dtype=torch.uint8,
+                               device=torch.device(device if device is not None else "cuda"))
+        self.stager = B.Stager(self.mem.data_ptr(), slot_bytes, n_slots)
+
+    def close(self) -> None:
+        self.stager.close()
+
+
 class Checkpointer:
     """pack()/unpack() on the current torch CUDA stream (or an explicit one)."""
 
@@ -89,3 +103,15 @@ class Checkpointer:
         s = stream if stream is not None else torch.cuda.current_stream(self.pool.device)
         B.lumen_kv_restore_unpack(plan, self.pool.k_ptrs, self.pool.v_ptrs, buf.data_ptr(),
                                   buf.numel() * buf.element_size(), _kind_of(buf), s.cuda_stream)
+
+    def pack_staged(self, plan: B.Plan, host_buf: torch.Tensor, ring: StagingRing, *, stream=None) -> None:
+        s = stream if stream is not None else torch.cuda.current_stream(self.pool.device)
+        B.lumen_kv_checkpoint_pack_staged(plan, self.pool.k_ptrs, self.pool.v_ptrs,
+                                          host_buf.data_ptr(), host_buf.numel() * host_buf.element_size(),
+                                          ring.stager, s.cuda_stream)
+
+    def unpack_staged(self, plan: B.Plan, host_buf: torch.Tensor, ring: StagingRing, *, stream=None) -> None:
+        s = stream if stream is not None else torch.cuda.current_stream(self.pool.device)
+        B.lumen_kv_restore_unpack_staged(plan, self.pool.k_ptrs, self.pool.v_ptrs,
+                                         host_buf.data_ptr(), host_buf.numel() * host_buf.element_size(),
+                                         ring.stager, s.cuda_stream)

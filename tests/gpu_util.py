@@ -5,7 +5,7 @@ import numpy as np
 import torch
 
 import paper_2606_17787_b200 as lk
-from paper_2606_17787_b200.pool import KVPool, Checkpointer, pinned_buffer
+from paper_2606_17787_b200.pool import KVPool, Checkpointer, StagingRing, pinned_buffer
 from workloads import device as wdev
 from workloads import fill_plane_np
 

@@ -230,3 +230,102 @@ def test_two_streams_concurrent(G):
     assert np.array_equal(G.buf_to_np(out, out.numel()), B_run)
     for t, ref in zip(pool.planes(), [x for kv in zip(K, V) for x in kv]):
         assert np.array_equal(G.plane_to_np(t), ref)
+
+
+# ---- two-stage host path (device staging ring + copy engines) -----------------------------
+def run_staged_case(G, w, slot_bytes, n_slots, *, seed=MASTER_SEED, kernel="auto"):
+    """pack_staged -> pinned host buffer == oracle.pack; unpack_staged -> whole pool == oracle's;
+    the one-shot mapped-host call reads back what the staged call wrote and vice versa."""
+    import torch
+    K, V = G.host_planes(w.geom, seed)
+    B_ref = oracle.pack(w.geom, K, V, w.reqs)
+    K2, V2 = G.host_planes(w.geom, seed + 1)
+    oracle.unpack(w.geom, K2, V2, w.restore_reqs, B_ref)
+    pool_a, pool_b = G.make_pool(w.geom, seed), G.make_pool(w.geom, seed + 1)
+    ck_a, ck_b = G.Checkpointer(pool_a, G.KERNELS[kernel]), G.Checkpointer(pool_b, G.KERNELS[kernel])
+    ring = G.StagingRing(slot_bytes, n_slots)
+    ring.mem.fill_(0x5A)
+    plan = ck_a.plan(w.reqs)
+    n_chunks = len(plan.chunks(slot_bytes))
+    whole, buf = G.alloc_buffer(plan.nbytes, "host")
+    side = torch.cuda.Stream()
+    with torch.cuda.stream(side):                       # not the default stream
+        ck_a.pack_staged(plan, buf, ring)
+        done = torch.cuda.Event(); done.record(side)    # stream order alone must imply completion
+    done.synchronize()
+    assert np.array_equal(G.buf_to_np(buf, plan.nbytes), B_ref), "staged pack mismatch"
+    assert G.guards_intact(whole, plan.nbytes)
+    rplan = ck_b.plan(w.restore_reqs, unique_dst=True)
+    with torch.cuda.stream(side):
+        ck_b.unpack_staged(rplan, buf, ring)            # same ring, other direction
+        done.record(side)
+    done.synchronize()
+    for t, ref in zip(pool_b.planes(), [x for kv in zip(K2, V2) for x in kv]):
+        assert np.array_equal(G.plane_to_np(t), ref), "staged unpack mismatch"
+    # two staged calls back to back on one stream reuse the slots while copies are in flight
+    whole2, buf2 = G.alloc_buffer(plan.nbytes, "host")
+    with torch.cuda.stream(side):
+        ck_b.pack_staged(rplan, buf2, ring)
+        ck_b.pack_staged(rplan, buf, ring)
+        done.record(side)
+    done.synchronize()
+    assert np.array_equal(G.buf_to_np(buf2, plan.nbytes), B_ref)
+    assert np.array_equal(G.buf_to_np(buf, plan.nbytes), B_ref)
+    assert G.guards_intact(whole2, plan.nbytes)
+    plan.close(); rplan.close(); ring.close()
+    return n_chunks
+
+
+def test_staged_cfg0_and_tiny(G):
+    assert run_staged_case(G, cfg0_tiny(), 4096, 2) > 8           # 256 B rows, 16-token pages
+    assert run_staged_case(G, cfg0_tiny(full_prefix=True), 1 << 20, 3) == 1
+    rng = substream(4242, "gpu_staged")
+    n = 0
+    while n < 25:
+        w = random_tiny(rng)
+        row = w.geom[1] * w.geom[2] * 2
+        if row % 16 or not w.tokens:
+            continue
+        max_run = max(min(w.geom[3], te - tb) for _, tb, te in w.reqs if te > tb) * row
+        slot = (max_run * int(rng.integers(1, 6)) + 15) // 16 * 16
+        run_staged_case(G, w, slot, int(rng.integers(2, 5)), seed=n)
+        n += 1
+
+
+@pytest.mark.parametrize("kernel", ["auto", "warp_upload", "bulk"])
+def test_staged_mid_shapes(G, kernel):
+    """All three chunk kinds on the paper's shapes: groups of whole requests (cfg 1 deltas),
+    plane ranges of one request (cfg 2 prefixes), token ranges of one plane (cfg 4, S = 1)."""
+    w = cfg1_qwen14b(L=3, N=2048, n_reqs=24, grow_iters=2, median=200, hi=512, lo=20)
+    assert run_staged_case(G, w, 1 << 20, 3, kernel=kernel) == 5        # 24 x 192 KiB requests, 5 per slot
+    w = cfg2_qwen32b(L=2, N=1200, n_reqs=3, prompt=1000)                # 1000 x 2 KiB per plane
+    assert run_staged_case(G, w, 5 << 20, 2, kernel=kernel) == 2 * 3    # 2 planes per chunk
+    w = cfg4_longctx(L=2, tokens=3001, wave_reqs=2)
+    assert run_staged_case(G, w, 1 << 20, 4, kernel=kernel) == 2 * 4 * 6  # 512 tokens per chunk
+
+
+def test_staged_errors(G):
+    import torch
+    lk = G.lk
+    w = cfg0_tiny()
+    pool = G.make_pool(w.geom, 1)
+    ck = G.Checkpointer(pool)
+    plan = ck.plan(w.reqs)
+    ring = G.StagingRing(1024, 2)                       # smaller than one 16-token run (4 KiB)
+    whole, buf = G.alloc_buffer(plan.nbytes, "host")
+    with pytest.raises(lk.LumenKVError) as e:
+        ck.pack_staged(plan, buf, ring)
+    assert e.value.status == lk.LUMEN_KV_ESIZE
+    ring2 = G.StagingRing(8192, 2)
+    with pytest.raises(lk.LumenKVError) as e:
+        ck.pack_staged(plan, buf[: plan.nbytes - 16], ring2)
+    assert e.value.status == lk.LUMEN_KV_ESIZE
+    pageable = torch.empty(plan.nbytes, dtype=torch.uint8)
+    with pytest.raises(lk.LumenKVError) as e:
+        lk.lumen_kv_checkpoint_pack_staged(plan, pool.k_ptrs, pool.v_ptrs, pageable.data_ptr(),
+                                           plan.nbytes, ring2.stager, 0)
+    assert e.value.status == lk.LUMEN_KV_EINVAL
+    empty = ck.plan([])
+    ck.pack_staged(empty, buf, ring2)                   # A4: nothing to do, returns OK
+    torch.cuda.synchronize()
+    assert G.guards_intact(whole, plan.nbytes)

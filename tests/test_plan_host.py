@@ -212,6 +212,14 @@ def test_no_cpu_fallback(lk):
             call(small, [16, 16], [16, 16], 16, 1 << 20)
         assert e.value.status == lk.LUMEN_KV_ECUDA
     small.close()
+    # the stager validates its arguments on the host, then needs a device for its copy stream
+    for bad in ((0, 1024, 2), (16, 1000, 2), (16, 1024, 1), (16, 1024, 17), (24, 1024, 2)):
+        with pytest.raises(lk.LumenKVError) as e:
+            lk.Stager(*bad)
+        assert e.value.status == lk.LUMEN_KV_EINVAL
+    with pytest.raises(lk.LumenKVError) as e:
+        lk.Stager(16, 1024, 2)
+    assert e.value.status == lk.LUMEN_KV_ECUDA
     # a host-only plan cannot be executed
     p = lk.lumen_kv_plan_build(g, [(pt, 0, 2)], lk.LUMEN_KV_HOST_ONLY)
     with pytest.raises(lk.LumenKVError) as e:
@@ -240,3 +248,75 @@ def test_plan_build_speed_host(lk):
         lk.lumen_kv_plan_build(g, w.reqs, lk.LUMEN_KV_HOST_ONLY).close()
     dt = (time.perf_counter() - t0) / 200
     assert dt < 2e-3, dt      # includes the ctypes marshalling of 64 requests
+
+
+# ---- two-stage host path: the chunker (host arithmetic only) ---------------------------
+def _check_chunks(plan, geom, reqs, slot):
+    """Chunks tile the buffer in ascending order, fit the slot, and chunk (runs, planes) covers
+    exactly its byte range according to the NumPy oracle's layout."""
+    L, H, D, S, N = geom
+    row = H * D * 2
+    lay, total = oracle_np.layout(geom, reqs)             # (offset, n) per request, in words
+    chunks = plan.chunks(slot)
+    runs = [plan.run(i) for i in range(plan.num_runs)]
+    at = 0
+    for c in chunks:
+        assert c.byte_begin == at and c.byte_end > c.byte_begin
+        assert c.byte_end - c.byte_begin <= slot
+        assert 0 <= c.plane_begin < c.plane_end <= 2 * L and c.run_begin < c.run_end
+        covered = []
+        for p in range(c.plane_begin, c.plane_end):
+            for i in range(c.run_begin, c.run_end):
+                r = runs[i]
+                off_words, n = lay[r.req]
+                b0 = off_words * 2 + (p * n + r.dst_token) * row
+                covered.append((b0, b0 + r.count * row))
+        covered.sort()
+        assert covered[0][0] == c.byte_begin and covered[-1][1] == c.byte_end
+        for (a0, a1), (b0, b1) in zip(covered, covered[1:]):
+            assert a1 == b0, "chunk is not contiguous in the buffer"
+        at = c.byte_end
+    assert at == total * 2 == plan.nbytes
+    return len(chunks)
+
+
+def test_chunks_tile_the_buffer(lk):
+    rng = substream(77, "chunks")
+    seen = 0
+    for _ in range(60):
+        w = random_tiny(rng)
+        row = w.geom[1] * w.geom[2] * 2
+        if row % 16:
+            continue
+        plan = lk.lumen_kv_plan_build(geom_of(lk, w), w.reqs, lk.LUMEN_KV_HOST_ONLY)
+        max_run = max([plan.run(i).count for i in range(plan.num_runs)] + [1]) * row
+        for slot in (max_run, 2 * max_run + 16, 7 * row + max_run, 1 << 20):
+            slot = (slot + 15) // 16 * 16
+            seen += _check_chunks(plan, w.geom, w.reqs, slot)
+        if plan.num_runs and max_run > 16:
+            with pytest.raises(lk.LumenKVError) as e:       # a run must fit a slot
+                plan.chunks(max_run - 16)
+            assert e.value.status == lk.LUMEN_KV_ESIZE
+    assert seen > 200
+
+
+def test_chunks_of_the_big_configs(lk):
+    """Closed forms: cfg1 step (64 x 2.5 MiB requests) in 32 MiB slots = whole-request groups of
+    12; cfg2 request (2 GiB, 16 MiB per plane) = 2 planes per chunk; cfg4 (256 MiB per plane,
+    one 2 KiB run per token) = 8 token ranges per plane."""
+    slot = 32 << 20
+    w = cfg1_qwen14b()
+    p = lk.lumen_kv_plan_build(geom_of(lk, w), w.reqs, lk.LUMEN_KV_HOST_ONLY)
+    ch = p.chunks(slot)
+    assert len(ch) == 6 and all(c.plane_begin == 0 and c.plane_end == 80 for c in ch)
+    assert [c.byte_end - c.byte_begin for c in ch] == [12 * 2621440] * 5 + [4 * 2621440]
+    w = cfg2_qwen32b(n_reqs=2, N=4096)
+    p = lk.lumen_kv_plan_build(geom_of(lk, w), w.reqs, lk.LUMEN_KV_HOST_ONLY)
+    ch = p.chunks(slot)
+    assert len(ch) == 2 * 64 and all(c.plane_end - c.plane_begin == 2 for c in ch)
+    assert all(c.run_end - c.run_begin == 512 for c in ch)
+    w = cfg4_longctx(wave_reqs=1)
+    p = lk.lumen_kv_plan_build(geom_of(lk, w), w.reqs, lk.LUMEN_KV_HOST_ONLY)
+    ch = p.chunks(slot)
+    assert len(ch) == 128 * 8 and all(c.run_end - c.run_begin == 16384 for c in ch)
+    assert p.chunks(1 << 40)[0].byte_end == 32 << 30 and len(p.chunks(1 << 40)) == 1
