@@ -18,6 +18,7 @@
 
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 
 namespace lumen {
 namespace {
@@ -312,14 +313,7 @@ int g_host_ctas = 0;   // grid of the bulk kernel when the buffer is host memory
 template <int STAGES, class Desc>
 cudaError_t launch_bulk_desc(const PlaneTable& pt, const Desc& d, const CopyArgs& a, int32_t plane0,
                              int32_t np, const BulkCfg& c) {
-    auto kern = kv_copy_bulk<STAGES, Desc>;
-    static bool attr_set = false;
-    if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             200 * 1024);
-        if (e != cudaSuccess) return e;
-        attr_set = true;
-    }
+    auto kern = kv_copy_bulk<STAGES, Desc>;   // dynamic shared memory limit set by preload_all()
     const int64_t total = a.n_runs * np;
     int64_t grid = static_cast<int64_t>(g_num_sms) * c.ctas_per_sm;
     // A host-memory buffer is bound by the host link (~55 GB/s): a few dozen single-warp
@@ -374,6 +368,37 @@ cudaError_t launch_warp(const PlaneTable& pt, const Desc& d, const WarpLaunch& w
                               w.row_bytes, w.plane0, w.sub_shift, w.pack);
 }
 
+// CUDA loads a kernel lazily at its first launch, and that load can wait for kernels that are
+// already running -- measured here: the first 1-token delta pack issued while a 70 GiB restore
+// was in flight took 1.49 s instead of 0.44 ms.  Touch every variant once, up front.
+template <class K>
+cudaError_t preload(K kernel, bool big_smem) {
+    cudaFuncAttributes fa;
+    cudaError_t e = cudaFuncGetAttributes(&fa, kernel);
+    if (e == cudaSuccess && big_smem)
+        e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+    return e;
+}
+
+template <int STAGES>
+cudaError_t preload_bulk() {
+    cudaError_t e = preload(kv_copy_bulk<STAGES, GlobalDesc>, true);
+    return e != cudaSuccess ? e : preload(kv_copy_bulk<STAGES, InlineDesc>, true);
+}
+
+cudaError_t preload_all() {
+    cudaError_t e = preload(kv_copy_warp<4, GlobalDesc>, false);
+    if (e == cudaSuccess) e = preload(kv_copy_warp<4, InlineDesc>, false);
+    if (e == cudaSuccess) e = preload(kv_copy_warp<8, GlobalDesc>, false);
+    if (e == cudaSuccess) e = preload(kv_copy_warp<8, InlineDesc>, false);
+    if (e == cudaSuccess) e = preload_bulk<3>();
+    if (e == cudaSuccess) e = preload_bulk<4>();
+    if (e == cudaSuccess) e = preload_bulk<6>();
+    if (e == cudaSuccess) e = preload_bulk<8>();
+    if (e == cudaSuccess) e = preload_bulk<16>();
+    return e;
+}
+
 }  // namespace
 
 int g_host_kernel = kKernelBulk;   // LUMEN_KV_HOST_KERNEL=warp|bulk: what AUTO picks for host buffers
@@ -388,18 +413,22 @@ int resolve_kernel(const CopyArgs& a) {
 
 cudaError_t launch_kv_copy(const CopyArgs& a) {
     if (a.n_runs == 0 || a.n_planes == 0) return cudaSuccess;
-    if (g_num_sms == 0) {
+    // one-time, thread-safe: tuning knobs, SM count, kernel preload
+    static std::once_flag once;
+    static cudaError_t init_err = cudaSuccess;
+    std::call_once(once, [] {
         if (const char* e = getenv("LUMEN_KV_WARP_UNROLL")) g_warp_unroll = (atoi(e) == 8) ? 8 : 4;
         if (const char* e = getenv("LUMEN_KV_PDL")) g_pdl = atoi(e) ? 1 : 0;
         if (const char* e = getenv("LUMEN_KV_HOST_KERNEL"))
             g_host_kernel = (e[0] == 'w') ? kKernelWarp : kKernelBulk;
+        if (const char* e = getenv("LUMEN_KV_HOST_CTAS")) g_host_ctas = atoi(e);
         int dev = 0;
-        cudaError_t e = cudaGetDevice(&dev);
-        if (e != cudaSuccess) return e;
-        e = cudaDeviceGetAttribute(&g_num_sms, cudaDevAttrMultiProcessorCount, dev);
-        if (e != cudaSuccess) return e;
-    }
-    if (const char* e = getenv("LUMEN_KV_HOST_CTAS")) g_host_ctas = atoi(e);   // sweep knob
+        init_err = cudaGetDevice(&dev);
+        if (init_err == cudaSuccess)
+            init_err = cudaDeviceGetAttribute(&g_num_sms, cudaDevAttrMultiProcessorCount, dev);
+        if (init_err == cudaSuccess) init_err = preload_all();
+    });
+    if (init_err != cudaSuccess) return init_err;
     const int kernel = resolve_kernel(a);
     const int64_t item_max = static_cast<int64_t>(a.max_count) * a.row_bytes;
 
