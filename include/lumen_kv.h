@@ -210,6 +210,30 @@ LUMEN_KV_API int lumen_kv_restore_unpack_staged(const lumen_kv_plan* plan,
                              void* const* k_planes, void* const* v_planes,
                              const void* src_host, int64_t src_bytes, lumen_kv_stager* stager,
                              void* stream);
+/*
+ * Per-chunk commit / ready flags (checkpointed pages "become visible ... only
+ * upon complete reception"; the sender of step (4), consumes the pinned buffer
+ * while later pages are still being copied).
+ *   flags : pinned host array of at least lumen_kv_plan_num_chunks(plan, slot_bytes) 64-bit
+ *           words, 8-byte aligned, owned by the caller; NULL = the plain staged call.
+ *   pack  : flags[c] = epoch is written in stream order AFTER chunk c's bytes
+ *           [byte_begin, byte_end) are complete in dst_host (a release: a host thread that
+ *           reads flags[c] == epoch with acquire semantics may read the chunk).
+ *   restore: the H2D copy of chunk c waits until flags[c] >= epoch (written by a host
+ *           thread after it has filled the chunk, e.g. on reception); chunks are consumed
+ *           in order, so a flag that is never raised stalls the call's streams for ever.
+ * Chunk c is entry c of lumen_kv_plan_get_chunks.  ECUDA if the driver lacks 64-bit stream
+ * memory operations.
+ */
+LUMEN_KV_API int lumen_kv_checkpoint_pack_staged_commit(const lumen_kv_plan* plan,
+                             const void* const* k_planes, const void* const* v_planes,
+                             void* dst_host, int64_t dst_bytes, lumen_kv_stager* stager,
+                             void* stream, uint64_t* flags, uint64_t epoch);
+LUMEN_KV_API int lumen_kv_restore_unpack_staged_ready(const lumen_kv_plan* plan,
+                             void* const* k_planes, void* const* v_planes,
+                             const void* src_host, int64_t src_bytes, lumen_kv_stager* stager,
+                             void* stream, const uint64_t* flags, uint64_t epoch);
+
 /* number of chunks a staged call on this plan would be cut into for the given slot size
  * (host arithmetic only; ESIZE if a run does not fit a slot) */
 LUMEN_KV_API int64_t lumen_kv_plan_num_chunks(const lumen_kv_plan* plan, int64_t slot_bytes);

@@ -36,6 +36,7 @@ EXPORTS = (
     "lumen_kv_strerror", "lumen_kv_last_cuda_error", "lumen_kv_version",
     "lumen_kv_stager_create", "lumen_kv_stager_destroy", "lumen_kv_checkpoint_pack_staged",
     "lumen_kv_restore_unpack_staged", "lumen_kv_plan_num_chunks", "lumen_kv_plan_get_chunks",
+    "lumen_kv_checkpoint_pack_staged_commit", "lumen_kv_restore_unpack_staged_ready",
 )
 
 
@@ -108,6 +109,10 @@ def _lib() -> ctypes.CDLL:
         f = getattr(L, name)
         f.restype = ctypes.c_int
         f.argtypes = [vp, ctypes.POINTER(vp), ctypes.POINTER(vp), vp, i64, vp, vp]
+    for name in ("lumen_kv_checkpoint_pack_staged_commit", "lumen_kv_restore_unpack_staged_ready"):
+        f = getattr(L, name)
+        f.restype = ctypes.c_int
+        f.argtypes = [vp, ctypes.POINTER(vp), ctypes.POINTER(vp), vp, i64, vp, vp, vp, ctypes.c_uint64]
     L.lumen_kv_plan_num_chunks.restype = i64
     L.lumen_kv_plan_num_chunks.argtypes = [vp, i64]
     L.lumen_kv_plan_get_chunks.restype = i64
@@ -344,6 +349,31 @@ def lumen_kv_restore_unpack_staged(plan: Plan, k_planes, v_planes, src_host: int
         ctypes.c_void_p(int(src_host)), int(src_bytes), stager.handle, ctypes.c_void_p(int(stream)))
     if rc:
         raise LumenKVError(rc, "lumen_kv_restore_unpack_staged")
+
+
+def lumen_kv_checkpoint_pack_staged_commit(plan: Plan, k_planes, v_planes, dst_host: int,
+                                           dst_bytes: int, stager: Stager, stream: int,
+                                           flags_host: int, epoch: int) -> None:
+    """flags_host: host pointer of a pinned uint64 array, one word per chunk."""
+    L = plan.geom.num_layers
+    rc = _lib().lumen_kv_checkpoint_pack_staged_commit(
+        plan.handle, _as_ptr_array(k_planes, L), _as_ptr_array(v_planes, L),
+        ctypes.c_void_p(int(dst_host)), int(dst_bytes), stager.handle, ctypes.c_void_p(int(stream)),
+        ctypes.c_void_p(int(flags_host)), int(epoch))
+    if rc:
+        raise LumenKVError(rc, "lumen_kv_checkpoint_pack_staged_commit")
+
+
+def lumen_kv_restore_unpack_staged_ready(plan: Plan, k_planes, v_planes, src_host: int,
+                                         src_bytes: int, stager: Stager, stream: int,
+                                         flags_host: int, epoch: int) -> None:
+    L = plan.geom.num_layers
+    rc = _lib().lumen_kv_restore_unpack_staged_ready(
+        plan.handle, _as_ptr_array(k_planes, L), _as_ptr_array(v_planes, L),
+        ctypes.c_void_p(int(src_host)), int(src_bytes), stager.handle, ctypes.c_void_p(int(stream)),
+        ctypes.c_void_p(int(flags_host)), int(epoch))
+    if rc:
+        raise LumenKVError(rc, "lumen_kv_restore_unpack_staged_ready")
 
 
 def lumen_kv_plan_free(plan: Plan) -> None:

@@ -253,8 +253,35 @@ namespace {
         if (e_ != cudaSuccess) return cuda_fail(e_);   \
     } while (0)
 
+// 64-bit stream memory operations (driver API), fetched at run time so that the library has
+// no link-time dependency on libcuda: (stream, device address, value, flags)
+typedef int (*StreamMemOp64)(cudaStream_t, unsigned long long, unsigned long long, unsigned int);
+StreamMemOp64 g_write64 = nullptr, g_wait64 = nullptr;
+
+int load_stream_memops() {
+    static std::once_flag once;
+    static cudaError_t err = cudaSuccess;
+    std::call_once(once, [] {
+        void* w = nullptr;
+        void* q = nullptr;
+        cudaDriverEntryPointQueryResult r1, r2;
+        err = cudaGetDriverEntryPoint("cuStreamWriteValue64", &w, cudaEnableDefault, &r1);
+        if (err == cudaSuccess)
+            err = cudaGetDriverEntryPoint("cuStreamWaitValue64", &q, cudaEnableDefault, &r2);
+        if (err == cudaSuccess && (r1 != cudaDriverEntryPointSuccess ||
+                                   r2 != cudaDriverEntryPointSuccess || !w || !q))
+            err = cudaErrorNotSupported;
+        if (err == cudaSuccess) {
+            g_write64 = reinterpret_cast<StreamMemOp64>(w);
+            g_wait64 = reinterpret_cast<StreamMemOp64>(q);
+        }
+    });
+    return err == cudaSuccess ? LUMEN_KV_OK : cuda_fail(err);
+}
+
 int run_staged(const lumen_kv_plan* plan, const void* const* k_planes, const void* const* v_planes,
-               void* host, int64_t host_bytes, lumen_kv_stager* st, void* stream_, bool pack) {
+               void* host, int64_t host_bytes, lumen_kv_stager* st, void* stream_, bool pack,
+               const uint64_t* flags = nullptr, uint64_t epoch = 0) {
     if (!plan || !st) return LUMEN_KV_EINVAL;
     if (plan->flags & LUMEN_KV_HOST_ONLY) return LUMEN_KV_EINVAL;
     if (host_bytes < plan->hp.total_bytes) return LUMEN_KV_ESIZE;
@@ -271,8 +298,21 @@ int run_staged(const lumen_kv_plan* plan, const void* const* k_planes, const voi
     std::vector<Chunk> chunks;
     rc = build_chunks(plan->hp, plan->h_runs, st->slot_bytes, &chunks);
     if (rc != LUMEN_KV_OK) return rc;
+    unsigned long long flags_dev = 0;   // device alias of the caller's pinned flag array
+    if (flags) {
+        if (reinterpret_cast<uintptr_t>(flags) & 7) return LUMEN_KV_EINVAL;
+        void* fa = nullptr;
+        if (cudaHostGetDevicePointer(&fa, const_cast<uint64_t*>(flags), 0) != cudaSuccess) {
+            (void)cudaGetLastError();
+            return LUMEN_KV_EINVAL;
+        }
+        flags_dev = reinterpret_cast<unsigned long long>(fa);
+        rc = load_stream_memops();
+        if (rc != LUMEN_KV_OK) return rc;
+    }
 
     cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+    int64_t ci = 0;                     // chunk index = entry of lumen_kv_plan_get_chunks
     char* h = static_cast<char*>(host);
     if (!pack) {   // the host buffer may have been produced by earlier work on `stream`
         LUMEN_CUDA(cudaEventRecord(st->join, stream));
@@ -292,8 +332,12 @@ int run_staged(const lumen_kv_plan* plan, const void* const* k_planes, const voi
             LUMEN_CUDA(cudaStreamWaitEvent(st->copy, st->full[slot], 0));
             LUMEN_CUDA(cudaMemcpyAsync(h + c.b0, sbase, bytes, cudaMemcpyDeviceToHost, st->copy));
             LUMEN_CUDA(cudaEventRecord(st->free_[slot], st->copy));
+            if (flags && g_write64(st->copy, flags_dev + 8ull * ci, epoch, 0) != 0)
+                return cuda_fail(cudaErrorUnknown);
         } else {
             LUMEN_CUDA(cudaStreamWaitEvent(st->copy, st->free_[slot], 0));
+            if (flags && g_wait64(st->copy, flags_dev + 8ull * ci, epoch, 0 /* >= */) != 0)
+                return cuda_fail(cudaErrorUnknown);
             LUMEN_CUDA(cudaMemcpyAsync(sbase, h + c.b0, bytes, cudaMemcpyHostToDevice, st->copy));
             LUMEN_CUDA(cudaEventRecord(st->full[slot], st->copy));
             LUMEN_CUDA(cudaStreamWaitEvent(stream, st->full[slot], 0));
@@ -301,6 +345,7 @@ int run_staged(const lumen_kv_plan* plan, const void* const* k_planes, const voi
             if (rc != LUMEN_KV_OK) return rc;
             LUMEN_CUDA(cudaEventRecord(st->free_[slot], stream));
         }
+        ++ci;
     }
     if (pack) {    // work enqueued on `stream` after this call sees the complete host buffer
         LUMEN_CUDA(cudaEventRecord(st->join, st->copy));
@@ -369,6 +414,24 @@ int lumen_kv_restore_unpack_staged(const lumen_kv_plan* plan, void* const* k_pla
     return lumen::run_staged(plan, const_cast<const void* const*>(k_planes),
                              const_cast<const void* const*>(v_planes),
                              const_cast<void*>(src_host), src_bytes, stager, stream, false);
+}
+
+int lumen_kv_checkpoint_pack_staged_commit(const lumen_kv_plan* plan, const void* const* k_planes,
+                                           const void* const* v_planes, void* dst_host,
+                                           int64_t dst_bytes, lumen_kv_stager* stager, void* stream,
+                                           uint64_t* flags, uint64_t epoch) {
+    return lumen::run_staged(plan, k_planes, v_planes, dst_host, dst_bytes, stager, stream, true,
+                             flags, epoch);
+}
+
+int lumen_kv_restore_unpack_staged_ready(const lumen_kv_plan* plan, void* const* k_planes,
+                                         void* const* v_planes, const void* src_host,
+                                         int64_t src_bytes, lumen_kv_stager* stager, void* stream,
+                                         const uint64_t* flags, uint64_t epoch) {
+    return lumen::run_staged(plan, const_cast<const void* const*>(k_planes),
+                             const_cast<const void* const*>(v_planes),
+                             const_cast<void*>(src_host), src_bytes, stager, stream, false, flags,
+                             epoch);
 }
 
 int64_t lumen_kv_plan_get_chunks(const lumen_kv_plan* plan, int64_t slot_bytes,

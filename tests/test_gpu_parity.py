@@ -329,3 +329,80 @@ def test_staged_errors(G):
     ck.pack_staged(empty, buf, ring2)                   # A4: nothing to do, returns OK
     torch.cuda.synchronize()
     assert G.guards_intact(whole, plan.nbytes)
+
+
+def test_staged_commit_and_ready_flags(G):
+    """Per-chunk flags: a host consumer that sees flags[c] == epoch finds chunk c
+    complete in the pinned buffer while later chunks are still in flight; a restore whose
+    ready flags are raised chunk by chunk by a host producer never reads a chunk early."""
+    import threading
+    import time
+    import torch
+    lk = G.lk
+    w = cfg2_qwen32b(L=3, N=1500, n_reqs=4, prompt=1200)               # 4 x 14 MiB
+    slot = 1 << 20
+    K, V = G.host_planes(w.geom, 11)
+    B_ref = oracle.pack(w.geom, K, V, w.reqs)
+    K2, V2 = G.host_planes(w.geom, 12)
+    oracle.unpack(w.geom, K2, V2, w.restore_reqs, B_ref)
+    ref_bytes = B_ref.view(np.uint8)
+    pool_a, pool_b = G.make_pool(w.geom, 11), G.make_pool(w.geom, 12)
+    ring = G.StagingRing(slot, 3)
+    plan = lk.lumen_kv_plan_build(pool_a.geom, w.reqs, 0, 0)
+    chunks = plan.chunks(slot)
+    assert len(chunks) > 40
+    whole, buf = G.alloc_buffer(plan.nbytes, "host")
+    buf.fill_(0xEE)
+    host = buf.numpy()
+    flags_t = torch.zeros(len(chunks), dtype=torch.int64, pin_memory=True)
+    flags = flags_t.numpy()
+    EPOCH = 7
+    seen, bad, stop = [], [], threading.Event()
+
+    def consumer():                                     # stands in for the sender of step (4)
+        nxt = 0
+        while nxt < len(chunks) and not stop.is_set():
+            if flags[nxt] == EPOCH:
+                c = chunks[nxt]
+                if not np.array_equal(host[c.byte_begin:c.byte_end], ref_bytes[c.byte_begin:c.byte_end]):
+                    bad.append(nxt)
+                seen.append((nxt, int((flags == EPOCH).sum())))
+                nxt += 1
+
+    th = threading.Thread(target=consumer)
+    th.start()
+    side = torch.cuda.Stream()
+    try:
+        lk.lumen_kv_checkpoint_pack_staged_commit(plan, pool_a.k_ptrs, pool_a.v_ptrs, buf.data_ptr(),
+                                                  plan.nbytes, ring.stager, side.cuda_stream,
+                                                  flags_t.data_ptr(), EPOCH)
+        side.synchronize()
+        th.join(timeout=60)
+    finally:
+        stop.set()
+    assert not th.is_alive() and len(seen) == len(chunks) and not bad
+    assert np.array_equal(G.buf_to_np(buf, plan.nbytes), B_ref) and G.guards_intact(whole, plan.nbytes)
+
+    # ---- restore side: chunks become ready one by one, out of a buffer that starts as garbage ----
+    rplan = lk.lumen_kv_plan_build(pool_b.geom, w.restore_reqs, lk.LUMEN_KV_VALIDATE_UNIQUE_DST, 0)
+    rchunks = rplan.chunks(slot)
+    buf.fill_(0xEE)
+    flags[:] = 0
+    READY = 9
+    lk.lumen_kv_restore_unpack_staged_ready(rplan, pool_b.k_ptrs, pool_b.v_ptrs, buf.data_ptr(),
+                                            rplan.nbytes, ring.stager, side.cuda_stream,
+                                            flags_t.data_ptr(), READY)
+    done = torch.cuda.Event(); done.record(side)
+    try:
+        for i, c in enumerate(rchunks):                 # "reception": fill the chunk, then raise its flag
+            assert not done.query(), "restore finished before all chunks were ready"
+            host[c.byte_begin:c.byte_end] = ref_bytes[c.byte_begin:c.byte_end]
+            if i % 16 == 0:
+                time.sleep(0.002)
+            flags[i] = READY
+    finally:
+        flags[:] = READY                                # never leave the stream waiting
+    side.synchronize()
+    for t, ref in zip(pool_b.planes(), [x for kv in zip(K2, V2) for x in kv]):
+        assert np.array_equal(G.plane_to_np(t), ref), "restore read a chunk before it was ready"
+    plan.close(); rplan.close(); ring.close()
