@@ -248,6 +248,44 @@ typedef struct {
 LUMEN_KV_API int64_t lumen_kv_plan_get_chunks(const lumen_kv_plan* plan, int64_t slot_bytes,
                                               lumen_kv_chunk_info* out, int64_t cap);
 
+/*
+ * Page tags (section 4.2): "each transferred page carries a page tag: a hash
+ * value of the token IDs stored in page i, paired with the page's end position in the request
+ * token sequence (i.e., the cumulative token length after page i)", regenerated from the
+ * token history at recovery to find "the longest contiguous checkpointed prefix"
+ * (PAPER.md:157).  The paper does not name the hash; this library uses 64-bit FNV-1a over
+ * the little-endian bytes of the page's int32 token IDs, of that page only (DESIGN.md
+ * reading A12).  A last page that is not full is hashed over the tokens it holds.
+ */
+typedef struct {
+    uint64_t hash;     /* FNV-1a 64 of the token IDs stored in the page        */
+    int64_t  end_pos;  /* cumulative token length after the page               */
+} lumen_kv_tag;
+
+/* pages of all requests = sum_r ceil((tok_offset[r+1] - tok_offset[r]) / page_size); host arithmetic.
+ * EINVAL for null / decreasing offsets / page_size < 1. */
+LUMEN_KV_API int64_t lumen_kv_tags_num_pages(const int64_t* tok_offset, int32_t num_reqs,
+                                             int32_t page_size);
+/*
+ * lumen_kv_page_tags -- tags of every page of num_reqs requests, on the device.
+ *   token_ids  : DEVICE array; request r's token IDs are [tok_offset[r], tok_offset[r+1]).
+ *   tok_offset : HOST array of num_reqs + 1 non-decreasing offsets (read during the call).
+ *   tags_out   : DEVICE array, 16-byte aligned, of tags_cap >= lumen_kv_tags_num_pages(..)
+ *                entries; request r's tags follow request r-1's, in page order.
+ * Asynchronous on `stream`.  Errors: EINVAL, ESIZE (tags_cap too small), ECUDA.
+ */
+LUMEN_KV_API int lumen_kv_page_tags(const int32_t* token_ids, const int64_t* tok_offset,
+                                    int32_t num_reqs, int32_t page_size, lumen_kv_tag* tags_out,
+                                    int64_t tags_cap, void* stream);
+/*
+ * lumen_kv_longest_prefix -- host lookup: walk the regenerated tags of one request in page
+ * order and halt at the first that is not among `stored` (any order, duplicates allowed);
+ * returns the end position of the last tag found = tokens of the longest contiguous
+ * checkpointed prefix (0 if none), or EINVAL / ENOMEM.  Both arrays are HOST memory.
+ */
+LUMEN_KV_API int64_t lumen_kv_longest_prefix(const lumen_kv_tag* regen, int64_t n_regen,
+                                             const lumen_kv_tag* stored, int64_t n_stored);
+
 /* Release a plan.  Safe to call while work using the plan is still in flight on a
  * stream: the descriptors are recycled only after that work has completed.       */
 LUMEN_KV_API void lumen_kv_plan_free(lumen_kv_plan* plan);

@@ -27,6 +27,7 @@ import numpy as np
 
 _HERE = Path(__file__).resolve().parent
 _SRC = _HERE / "lumen_oracle.c"
+_SRCS = [_HERE / "lumen_oracle.c", _HERE / "tags_oracle.c"]
 _SO = _HERE / "liblumen_oracle.so"
 
 OK, EARG, EPAGE, ESIZE, EOVERLAP = 0, -1, -2, -3, -4
@@ -40,11 +41,11 @@ class OracleError(RuntimeError):
 
 def build(force: bool = False) -> Path:
     """Compile lumen_oracle.c into oracle/liblumen_oracle.so with gcc."""
-    if force or not _SO.exists() or _SO.stat().st_mtime < _SRC.stat().st_mtime:
+    if force or not _SO.exists() or any(_SO.stat().st_mtime < p.stat().st_mtime for p in _SRCS):
         tmp = _SO.with_suffix(f".so.tmp{os.getpid()}")
         subprocess.check_call(
             ["gcc", "-O2", "-fopenmp", "-shared", "-fPIC", "-Wall", "-Wextra",
-             "-o", str(tmp), str(_SRC)])
+             "-o", str(tmp), *map(str, _SRCS)])
         os.replace(tmp, _SO)
     return _SO
 
@@ -60,6 +61,12 @@ class _Req(ctypes.Structure):
                 ("PT_len", ctypes.c_int64),
                 ("tb", ctypes.c_int64), ("te", ctypes.c_int64)]
 
+
+class _Tag(ctypes.Structure):
+    _fields_ = [("hash", ctypes.c_uint64), ("end_pos", ctypes.c_int64)]
+
+
+TAG_DTYPE = np.dtype([("hash", np.uint64), ("end_pos", np.int64)])
 
 _lib = None
 
@@ -88,6 +95,15 @@ def lib() -> ctypes.CDLL:
         _lib.lumen_oracle_pool_index.restype = i64
         _lib.lumen_oracle_pool_index.argtypes = [G, Rq, i32, i64, i64]
         _lib.lumen_oracle_omp_threads.restype = ctypes.c_int
+        T = ctypes.POINTER(_Tag)
+        _lib.tags_oracle_fnv1a64.restype = ctypes.c_uint64
+        _lib.tags_oracle_fnv1a64.argtypes = [ctypes.c_char_p, i64]
+        _lib.tags_oracle_num_pages.restype = i64
+        _lib.tags_oracle_num_pages.argtypes = [i64, i64]
+        _lib.tags_oracle_page_tags.restype = ctypes.c_int
+        _lib.tags_oracle_page_tags.argtypes = [ctypes.POINTER(ctypes.c_int32), i64, i64, T]
+        _lib.tags_oracle_longest_prefix.restype = i64
+        _lib.tags_oracle_longest_prefix.argtypes = [T, i64, T, i64]
     return _lib
 
 
@@ -193,3 +209,32 @@ def pool_index(geom, reqs, r, j, e) -> int:
 
 def omp_threads() -> int:
     return int(lib().lumen_oracle_omp_threads())
+
+
+# ---------------------------------------------------------------------------
+# page tags (tags_oracle.c)
+# ---------------------------------------------------------------------------
+
+def fnv1a64(data: bytes) -> int:
+    return int(lib().tags_oracle_fnv1a64(data, len(data)))
+
+
+def page_tags(token_ids, S: int) -> np.ndarray:
+    """Tags of every page of one request: structured array (hash u64, end_pos i64)."""
+    tok = np.ascontiguousarray(token_ids, dtype=np.int32)
+    n = int(lib().tags_oracle_num_pages(tok.size, int(S)))
+    out = np.zeros(max(n, 0), dtype=TAG_DTYPE)
+    rc = lib().tags_oracle_page_tags(tok.ctypes.data_as(ctypes.POINTER(ctypes.c_int32)), tok.size,
+                                     int(S), out.ctypes.data_as(ctypes.POINTER(_Tag)))
+    if rc:
+        raise OracleError(rc)
+    return out
+
+
+def longest_prefix(regen: np.ndarray, stored: np.ndarray) -> int:
+    """Tokens of the longest contiguous checkpointed prefix."""
+    regen = np.ascontiguousarray(regen, dtype=TAG_DTYPE)
+    stored = np.ascontiguousarray(stored, dtype=TAG_DTYPE)
+    return int(lib().tags_oracle_longest_prefix(
+        regen.ctypes.data_as(ctypes.POINTER(_Tag)), regen.size,
+        stored.ctypes.data_as(ctypes.POINTER(_Tag)), stored.size))

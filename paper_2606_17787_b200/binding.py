@@ -37,6 +37,7 @@ EXPORTS = (
     "lumen_kv_stager_create", "lumen_kv_stager_destroy", "lumen_kv_checkpoint_pack_staged",
     "lumen_kv_restore_unpack_staged", "lumen_kv_plan_num_chunks", "lumen_kv_plan_get_chunks",
     "lumen_kv_checkpoint_pack_staged_commit", "lumen_kv_restore_unpack_staged_ready",
+    "lumen_kv_tags_num_pages", "lumen_kv_page_tags", "lumen_kv_longest_prefix",
 )
 
 
@@ -113,6 +114,12 @@ def _lib() -> ctypes.CDLL:
         f = getattr(L, name)
         f.restype = ctypes.c_int
         f.argtypes = [vp, ctypes.POINTER(vp), ctypes.POINTER(vp), vp, i64, vp, vp, vp, ctypes.c_uint64]
+    L.lumen_kv_tags_num_pages.restype = i64
+    L.lumen_kv_tags_num_pages.argtypes = [vp, i32, i32]
+    L.lumen_kv_page_tags.restype = ctypes.c_int
+    L.lumen_kv_page_tags.argtypes = [vp, vp, i32, i32, vp, i64, vp]
+    L.lumen_kv_longest_prefix.restype = i64
+    L.lumen_kv_longest_prefix.argtypes = [vp, i64, vp, i64]
     L.lumen_kv_plan_num_chunks.restype = i64
     L.lumen_kv_plan_num_chunks.argtypes = [vp, i64]
     L.lumen_kv_plan_get_chunks.restype = i64
@@ -374,6 +381,38 @@ def lumen_kv_restore_unpack_staged_ready(plan: Plan, k_planes, v_planes, src_hos
         ctypes.c_void_p(int(flags_host)), int(epoch))
     if rc:
         raise LumenKVError(rc, "lumen_kv_restore_unpack_staged_ready")
+
+
+TAG_DTYPE = np.dtype([("hash", np.uint64), ("end_pos", np.int64)])   # lumen_kv_tag
+
+
+def lumen_kv_tags_num_pages(tok_offset, page_size: int) -> int:
+    off = np.ascontiguousarray(tok_offset, dtype=np.int64)
+    n = int(_lib().lumen_kv_tags_num_pages(off.ctypes.data, off.size - 1, int(page_size)))
+    if n < 0:
+        raise LumenKVError(n, "lumen_kv_tags_num_pages")
+    return n
+
+
+def lumen_kv_page_tags(token_ids_dev: int, tok_offset, page_size: int, tags_out_dev: int,
+                       tags_cap: int, stream: int = 0) -> None:
+    """token_ids_dev / tags_out_dev: device pointers; tok_offset: host int64 array (R + 1)."""
+    off = np.ascontiguousarray(tok_offset, dtype=np.int64)
+    rc = _lib().lumen_kv_page_tags(ctypes.c_void_p(int(token_ids_dev)), off.ctypes.data, off.size - 1,
+                                   int(page_size), ctypes.c_void_p(int(tags_out_dev)), int(tags_cap),
+                                   ctypes.c_void_p(int(stream)))
+    if rc:
+        raise LumenKVError(rc, "lumen_kv_page_tags")
+
+
+def lumen_kv_longest_prefix(regen: np.ndarray, stored: np.ndarray) -> int:
+    """regen, stored: host arrays of TAG_DTYPE.  Returns tokens of the longest contiguous prefix."""
+    a = np.ascontiguousarray(regen, dtype=TAG_DTYPE)
+    b = np.ascontiguousarray(stored, dtype=TAG_DTYPE)
+    n = int(_lib().lumen_kv_longest_prefix(a.ctypes.data, a.size, b.ctypes.data, b.size))
+    if n < 0:
+        raise LumenKVError(n, "lumen_kv_longest_prefix")
+    return n
 
 
 def lumen_kv_plan_free(plan: Plan) -> None:
