@@ -62,6 +62,10 @@ class _Req(ctypes.Structure):
                 ("tb", ctypes.c_int64), ("te", ctypes.c_int64)]
 
 
+class _Layout(ctypes.Structure):
+    _fields_ = [("off_elems", ctypes.c_int64), ("stride_tokens", ctypes.c_int64)]
+
+
 class _Tag(ctypes.Structure):
     _fields_ = [("hash", ctypes.c_uint64), ("end_pos", ctypes.c_int64)]
 
@@ -95,6 +99,11 @@ def lib() -> ctypes.CDLL:
         _lib.lumen_oracle_pool_index.restype = i64
         _lib.lumen_oracle_pool_index.argtypes = [G, Rq, i32, i64, i64]
         _lib.lumen_oracle_omp_threads.restype = ctypes.c_int
+        Ly = ctypes.POINTER(_Layout)
+        for name in ("lumen_oracle_pack_layout", "lumen_oracle_unpack_layout"):
+            f = getattr(_lib, name)
+            f.restype = ctypes.c_int
+            f.argtypes = [G, PP, PP, Rq, Ly, i32, vp, i64]
         T = ctypes.POINTER(_Tag)
         _lib.tags_oracle_fnv1a64.restype = ctypes.c_uint64
         _lib.tags_oracle_fnv1a64.argtypes = [ctypes.c_char_p, i64]
@@ -191,6 +200,44 @@ def unpack(geom, k_planes, v_planes, reqs, B, *, omp: bool = False,
         rc = lib().lumen_oracle_unpack(ctypes.byref(g), kp, vp, arr, len(reqs),
                                        B.ctypes.data, B.size,
                                        1 if check_overlap else 0)
+    if rc:
+        raise OracleError(rc)
+
+
+def _layouts(layouts):
+    arr = (_Layout * max(len(layouts), 1))()
+    for i, (off, stride) in enumerate(layouts):
+        arr[i].off_elems, arr[i].stride_tokens = int(off), int(stride)
+    return arr
+
+
+def pack_layout(geom, k_planes, v_planes, reqs, layouts, B: np.ndarray) -> None:
+    """Pack into B (uint16, modified in place) with request r's block at element offset
+    layouts[r][0] and plane stride layouts[r][1] tokens; other words of B are left alone."""
+    g = _geom(geom)
+    L, H, D, S, N = (int(x) for x in geom)
+    arr, _keep = _reqs(reqs)
+    words = N * S * H * D
+    kp = _planes(k_planes, L, words, False)
+    vp = _planes(v_planes, L, words, False)
+    if B.dtype != np.uint16 or not B.flags.c_contiguous or not B.flags.writeable:
+        raise ValueError("B must be a writable C-contiguous uint16 array")
+    rc = lib().lumen_oracle_pack_layout(ctypes.byref(g), kp, vp, arr, _layouts(layouts), len(reqs),
+                                        B.ctypes.data, B.size)
+    if rc:
+        raise OracleError(rc)
+
+
+def unpack_layout(geom, k_planes, v_planes, reqs, layouts, B: np.ndarray) -> None:
+    g = _geom(geom)
+    L, H, D, S, N = (int(x) for x in geom)
+    arr, _keep = _reqs(reqs)
+    words = N * S * H * D
+    kp = _planes(k_planes, L, words, True)
+    vp = _planes(v_planes, L, words, True)
+    B = np.ascontiguousarray(B, dtype=np.uint16)
+    rc = lib().lumen_oracle_unpack_layout(ctypes.byref(g), kp, vp, arr, _layouts(layouts), len(reqs),
+                                          B.ctypes.data, B.size)
     if rc:
         raise OracleError(rc)
 

@@ -294,3 +294,92 @@ int lumen_oracle_omp_threads(void)
 #endif
     return n;
 }
+
+/* ---- explicit buffer layout (checkpoint store) ---------------
+ * A checkpoint store keeps what it received: a request's checkpoint is the sequence of its
+ * delta buffers ("transmit only newly generated KV pages"; one checkpoint per
+ * request), and a recovery restores the longest checkpointed prefix
+ * (PAPER.md:157), which may end inside the last delta.  So pack / unpack are also defined
+ * for a buffer in which request r's block sits at an explicit element offset off_r with an
+ * explicit plane stride st_r >= n_r (in tokens):
+ *     B[off_r + ((l*2 + c)*st_r + j)*E + e]  <->  plane(l,c)[PT_r[t div S]][t mod S][e]
+ * The dense layout of C1 is the special case off_r = prefix sum, st_r = n_r.  Words of B
+ * that no (r, l, c, j, e) addresses are never read or written.
+ */
+typedef struct {
+    int64_t off_elems;      /* element offset of the request's block in B */
+    int64_t stride_tokens;  /* tokens between consecutive planes, >= n_r  */
+} oracle_layout;
+
+static int check_layout(const oracle_geom *g, const oracle_req *reqs, const oracle_layout *lay,
+                        int32_t R, int64_t B_elems)
+{
+    const int64_t E = (int64_t)g->H * g->D;
+    if (R > 0 && !lay) return ORACLE_EARG;
+    for (int32_t r = 0; r < R; ++r) {
+        const int64_t n = reqs[r].te - reqs[r].tb;
+        if (lay[r].off_elems < 0 || lay[r].stride_tokens < n) return ORACLE_EARG;
+        if (n > 0 &&
+            lay[r].off_elems + (((int64_t)2 * g->L - 1) * lay[r].stride_tokens + n) * E > B_elems)
+            return ORACLE_ESIZE;
+    }
+    return ORACLE_OK;
+}
+
+int lumen_oracle_pack_layout(const oracle_geom *g,
+                             const uint16_t *const *Kp, const uint16_t *const *Vp,
+                             const oracle_req *reqs, const oracle_layout *lay, int32_t R,
+                             uint16_t *B, int64_t B_elems)
+{
+    int rc = check_inputs(g, reqs, R);
+    if (rc) return rc;
+    rc = check_layout(g, reqs, lay, R, B_elems);
+    if (rc) return rc;
+    const int64_t E = (int64_t)g->H * g->D;
+    const int64_t S = g->S;
+    for (int32_t r = 0; r < R; ++r) {
+        const int64_t n = reqs[r].te - reqs[r].tb;
+        for (int32_t l = 0; l < g->L; ++l)
+            for (int32_t c = 0; c < 2; ++c) {
+                const uint16_t *plane = (c == 0) ? Kp[l] : Vp[l];
+                for (int64_t j = 0; j < n; ++j) {
+                    const int64_t t = reqs[r].tb + j;
+                    const int64_t p = reqs[r].PT[t / S];
+                    const int64_t s = t % S;
+                    for (int64_t e = 0; e < E; ++e)
+                        B[lay[r].off_elems + (((int64_t)l * 2 + c) * lay[r].stride_tokens + j) * E + e] =
+                            plane[((p * S) + s) * E + e];
+                }
+            }
+    }
+    return ORACLE_OK;
+}
+
+int lumen_oracle_unpack_layout(const oracle_geom *g,
+                               uint16_t *const *Kp, uint16_t *const *Vp,
+                               const oracle_req *reqs, const oracle_layout *lay, int32_t R,
+                               const uint16_t *B, int64_t B_elems)
+{
+    int rc = check_inputs(g, reqs, R);
+    if (rc) return rc;
+    rc = check_layout(g, reqs, lay, R, B_elems);
+    if (rc) return rc;
+    const int64_t E = (int64_t)g->H * g->D;
+    const int64_t S = g->S;
+    for (int32_t r = 0; r < R; ++r) {
+        const int64_t n = reqs[r].te - reqs[r].tb;
+        for (int32_t l = 0; l < g->L; ++l)
+            for (int32_t c = 0; c < 2; ++c) {
+                uint16_t *plane = (c == 0) ? Kp[l] : Vp[l];
+                for (int64_t j = 0; j < n; ++j) {
+                    const int64_t t = reqs[r].tb + j;
+                    const int64_t p = reqs[r].PT[t / S];
+                    const int64_t s = t % S;
+                    for (int64_t e = 0; e < E; ++e)
+                        plane[((p * S) + s) * E + e] =
+                            B[lay[r].off_elems + (((int64_t)l * 2 + c) * lay[r].stride_tokens + j) * E + e];
+                }
+            }
+    }
+    return ORACLE_OK;
+}

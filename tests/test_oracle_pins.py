@@ -336,3 +336,89 @@ def test_omp_variants_equal_plain():
         oracle.unpack(w.geom, K3, V3, w.restore_reqs, a, omp=True)
         for x, y in zip(K2 + V2, K3 + V3):
             assert np.array_equal(x, y)
+
+
+# ---- explicit buffer layout (checkpoint store, f3) ------------------------------------------
+def _dense_layouts(geom, reqs):
+    L, H, D, S, N = geom
+    E, off, out = H * D, 0, []
+    for _, tb, te in reqs:
+        out.append((off, te - tb))
+        off += (te - tb) * 2 * L * E
+    return out, off
+
+
+def test_layout_dense_special_case_equals_c1():
+    rng = substream(31, "layout")
+    for _ in range(40):
+        w = random_tiny(rng)
+        K, V = make_pool(w.geom, 5)
+        lays, total = _dense_layouts(w.geom, w.reqs)
+        B = np.full(total, 0xDEAD, dtype=np.uint16)
+        oracle.pack_layout(w.geom, K, V, w.reqs, lays, B)
+        assert np.array_equal(B, oracle.pack(w.geom, K, V, w.reqs))
+        K2, V2 = make_pool(w.geom, 6)
+        K3, V3 = [k.copy() for k in K2], [v.copy() for v in V2]
+        oracle.unpack_layout(w.geom, K2, V2, w.restore_reqs, lays, B)
+        oracle.unpack(w.geom, K3, V3, w.restore_reqs, B)
+        assert all(np.array_equal(a, b) for a, b in zip(K2 + V2, K3 + V3))
+
+
+def test_layout_strided_blocks_and_untouched_gaps():
+    rng = substream(32, "layout2")
+    for _ in range(40):
+        w = random_tiny(rng)
+        L, H, D, S, N = w.geom
+        E = H * D
+        K, V = make_pool(w.geom, 7)
+        dense = oracle.pack(w.geom, K, V, w.reqs)
+        lays, at, written = [], int(rng.integers(0, 9)), 0
+        for _, tb, te in w.reqs:
+            stride = (te - tb) + int(rng.integers(0, 5))
+            lays.append((at, stride))
+            at += 2 * L * stride * E + int(rng.integers(0, 7))
+            written += (te - tb) * 2 * L * E
+        B = np.full(at + 3, 0xDEAD, dtype=np.uint16)
+        oracle.pack_layout(w.geom, K, V, w.reqs, lays, B)
+        mask = np.zeros(B.size, dtype=bool)
+        d_off = 0
+        for (off, stride), (_, tb, te) in zip(lays, w.reqs):
+            n = te - tb
+            for p in range(2 * L):
+                blk = slice(off + p * stride * E, off + p * stride * E + n * E)
+                assert np.array_equal(B[blk], dense[d_off + p * n * E: d_off + (p + 1) * n * E])
+                mask[blk] = True
+            d_off += n * 2 * L * E
+        assert mask.sum() == written and (B[~mask] == 0xDEAD).all()
+        # round trip through the strided buffer == round trip through the dense one
+        K2, V2 = make_pool(w.geom, 8)
+        K3, V3 = [k.copy() for k in K2], [v.copy() for v in V2]
+        oracle.unpack_layout(w.geom, K2, V2, w.restore_reqs, lays, B)
+        oracle.unpack(w.geom, K3, V3, w.restore_reqs, dense)
+        assert all(np.array_equal(a, b) for a, b in zip(K2 + V2, K3 + V3))
+
+
+def test_layout_delta_append_in_place_and_prefix_cut():
+    """P4 end to end: deltas packed one after another into ONE region (stride = final length)
+    give the dense pack of the whole prefix; and a prefix that ends inside a stored delta is
+    restored from that delta's own buffer through its plane stride."""
+    w = cfg0_tiny(full_prefix=True)
+    L, H, D, S, N = w.geom
+    E = H * D
+    K, V = make_pool(w.geom, 9)
+    pt, _, n = w.reqs[1]                                     # 100 tokens
+    full = oracle.pack(w.geom, K, V, [(pt, 0, n)])
+    region = np.full(full.size, 0xDEAD, dtype=np.uint16)
+    for tb, te in ((0, 37), (37, 53), (53, 100)):
+        oracle.pack_layout(w.geom, K, V, [(pt, tb, te)], [(tb * E, n)], region)
+    assert np.array_equal(region, full)
+    # store keeps the delta [37, 53) as it arrived (dense, stride 16); recovery wants [37, 48)
+    seg = oracle.pack(w.geom, K, V, [(pt, 37, 53)])
+    pt2 = w.restore_reqs[1][0]
+    K2, V2 = make_pool(w.geom, 10)
+    K3, V3 = [k.copy() for k in K2], [v.copy() for v in V2]
+    oracle.unpack_layout(w.geom, K2, V2, [(pt2, 37, 48)], [(0, 16)], seg)
+    oracle.unpack(w.geom, K3, V3, [(pt2, 37, 48)], oracle.pack(w.geom, K, V, [(pt, 37, 48)]))
+    assert all(np.array_equal(a, b) for a, b in zip(K2 + V2, K3 + V3))
+    with pytest.raises(oracle.OracleError):                  # stride shorter than the range
+        oracle.unpack_layout(w.geom, K2, V2, [(pt2, 37, 53)], [(0, 15)], seg)

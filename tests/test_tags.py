@@ -137,6 +137,9 @@ def test_gpu_page_tags_equal_oracle(lk):
         ref = np.concatenate([oracle.page_tags(tok[off[r]:off[r + 1]], S) for r in range(R)]
                              + [np.zeros(0, oracle.TAG_DTYPE)])
         assert np.array_equal(got, ref), f"case {case}"
-    with pytest.raises(lk.LumenKVError) as e:
-        lk.lumen_kv_page_tags(d_tok.data_ptr(), off, S, d_out.data_ptr(), n - 1, 0)
-    assert e.value.status == lk.LUMEN_KV_ESIZE or n == 0
+    d_tok = torch.zeros(100, dtype=torch.int32, device="cuda")
+    d_out = torch.zeros((8, 2), dtype=torch.int64, device="cuda")
+    with pytest.raises(lk.LumenKVError) as e:                         # 7 pages, room for 6
+        lk.lumen_kv_page_tags(d_tok.data_ptr(), [0, 100], 16, d_out.data_ptr(), 6, 0)
+    assert e.value.status == lk.LUMEN_KV_ESIZE
+    lk.lumen_kv_page_tags(d_tok.data_ptr(), [0, 0, 0], 16, 0, 0, 0)   # no pages: nothing to do
