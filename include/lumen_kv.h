@@ -134,6 +134,27 @@ LUMEN_KV_API int lumen_kv_plan_build(const lumen_kv_geom* geom, const lumen_kv_r
                         int32_t num_reqs, uint32_t flags, void* stream,
                         lumen_kv_plan** out);
 
+/*
+ * Explicit buffer layout.  A checkpoint store keeps a request's checkpoint as the deltas it
+ * received (one checkpoint per request) and a recovery restores
+ * the longest checkpointed prefix, which may end inside the last delta.  With
+ * a layout, request r's block sits at byte offset buf_offset of the buffer and consecutive
+ * planes are plane_stride_tokens rows apart:
+ *     B[buf_offset_r + ((plane*plane_stride_tokens_r) + j)*row + b]
+ * buf_offset must be a multiple of row, plane_stride_tokens >= n_r.  layouts == NULL is the
+ * dense layout of lumen_kv_plan_build.  lumen_kv_plan_bytes() is then the extent (largest
+ * byte addressed + 1) and lumen_kv_plan_req_offset(r) returns buf_offset_r (r == num_reqs:
+ * the extent).  Blocks of different requests may not overlap for pack; the library does
+ * not check that.  Errors as lumen_kv_plan_build.
+ */
+typedef struct {
+    int64_t buf_offset;           /* bytes, multiple of row                       */
+    int64_t plane_stride_tokens;  /* >= t_end - t_begin                           */
+} lumen_kv_req_layout;
+LUMEN_KV_API int lumen_kv_plan_build_layout(const lumen_kv_geom* geom, const lumen_kv_req* reqs,
+                        const lumen_kv_req_layout* layouts, int32_t num_reqs, uint32_t flags,
+                        void* stream, lumen_kv_plan** out);
+
 /* total checkpoint-buffer bytes = sum_r n_r * 2L * row */
 LUMEN_KV_API int64_t lumen_kv_plan_bytes(const lumen_kv_plan* plan);
 /* byte offset of request r in the buffer (exclusive prefix sum); r == num_reqs gives the total */

@@ -30,7 +30,7 @@ LUMEN_KV_KERNEL_AUTO, LUMEN_KV_KERNEL_WARP, LUMEN_KV_KERNEL_BULK = 0x000, 0x100,
 LUMEN_KV_MEM_DEVICE, LUMEN_KV_MEM_HOST_MAPPED = 0, 1
 
 EXPORTS = (
-    "lumen_kv_plan_build", "lumen_kv_plan_bytes", "lumen_kv_plan_req_offset",
+    "lumen_kv_plan_build", "lumen_kv_plan_build_layout", "lumen_kv_plan_bytes", "lumen_kv_plan_req_offset",
     "lumen_kv_plan_num_runs", "lumen_kv_plan_get_run", "lumen_kv_checkpoint_pack",
     "lumen_kv_restore_unpack", "lumen_kv_plan_free", "lumen_kv_trim",
     "lumen_kv_strerror", "lumen_kv_last_cuda_error", "lumen_kv_version",
@@ -51,6 +51,10 @@ class lumen_kv_geom(ctypes.Structure):
 class lumen_kv_req(ctypes.Structure):
     _fields_ = [("page_table", ctypes.c_void_p), ("page_table_len", ctypes.c_int64),
                 ("t_begin", ctypes.c_int64), ("t_end", ctypes.c_int64)]
+
+
+class lumen_kv_req_layout(ctypes.Structure):
+    _fields_ = [("buf_offset", ctypes.c_int64), ("plane_stride_tokens", ctypes.c_int64)]
 
 
 class lumen_kv_run_info(ctypes.Structure):
@@ -90,6 +94,10 @@ def _lib() -> ctypes.CDLL:
     L.lumen_kv_plan_build.restype = ctypes.c_int
     L.lumen_kv_plan_build.argtypes = [ctypes.POINTER(lumen_kv_geom), ctypes.POINTER(lumen_kv_req),
                                       i32, u32, vp, ctypes.POINTER(vp)]
+    L.lumen_kv_plan_build_layout.restype = ctypes.c_int
+    L.lumen_kv_plan_build_layout.argtypes = [ctypes.POINTER(lumen_kv_geom), ctypes.POINTER(lumen_kv_req),
+                                             ctypes.POINTER(lumen_kv_req_layout), i32, u32, vp,
+                                             ctypes.POINTER(vp)]
     L.lumen_kv_plan_bytes.restype = i64
     L.lumen_kv_plan_bytes.argtypes = [vp]
     L.lumen_kv_plan_req_offset.restype = i64
@@ -242,28 +250,34 @@ class ReqArray:
         self.arr["t_end"] += int(tokens)
 
 
-def lumen_kv_plan_build(geom: lumen_kv_geom, reqs, flags: int = 0, stream: int = 0) -> Plan:
-    """reqs: a ReqArray, or a sequence of (page_table int32 ndarray, t_begin, t_end)."""
-    if isinstance(reqs, ReqArray):
-        out = ctypes.c_void_p()
-        rc = _lib().lumen_kv_plan_build(
-            ctypes.byref(geom), ctypes.cast(reqs.arr.ctypes.data, ctypes.POINTER(lumen_kv_req)),
-            len(reqs), int(flags), ctypes.c_void_p(int(stream)), ctypes.byref(out))
-        if rc:
-            raise LumenKVError(rc, "lumen_kv_plan_build")
-        return Plan(out.value, geom, len(reqs))
-    n = len(reqs)
-    arr = (lumen_kv_req * max(n, 1))()
+def lumen_kv_plan_build(geom: lumen_kv_geom, reqs, flags: int = 0, stream: int = 0,
+                        layouts=None) -> Plan:
+    """reqs: a ReqArray, or a sequence of (page_table int32 ndarray, t_begin, t_end).
+    layouts: None (dense buffer) or one (buf_offset bytes, plane_stride_tokens) per request
+    (lumen_kv_plan_build_layout)."""
+    lay = None
+    if layouts is not None:
+        if len(layouts) != len(reqs):
+            raise ValueError("one layout per request")
+        lay = (lumen_kv_req_layout * max(len(layouts), 1))()
+        for i, (off, stride) in enumerate(layouts):
+            lay[i].buf_offset, lay[i].plane_stride_tokens = int(off), int(stride)
     keep = []
-    for i, (pt, tb, te) in enumerate(reqs):
-        pt = np.ascontiguousarray(pt, dtype=np.int32)
-        keep.append(pt)
-        arr[i].page_table = pt.ctypes.data if pt.size else None
-        arr[i].page_table_len = pt.size
-        arr[i].t_begin, arr[i].t_end = int(tb), int(te)
+    if isinstance(reqs, ReqArray):
+        n = len(reqs)
+        arr = ctypes.cast(reqs.arr.ctypes.data, ctypes.POINTER(lumen_kv_req))
+    else:
+        n = len(reqs)
+        arr = (lumen_kv_req * max(n, 1))()
+        for i, (pt, tb, te) in enumerate(reqs):
+            pt = np.ascontiguousarray(pt, dtype=np.int32)
+            keep.append(pt)
+            arr[i].page_table = pt.ctypes.data if pt.size else None
+            arr[i].page_table_len = pt.size
+            arr[i].t_begin, arr[i].t_end = int(tb), int(te)
     out = ctypes.c_void_p()
-    rc = _lib().lumen_kv_plan_build(ctypes.byref(geom), arr, n, int(flags),
-                                    ctypes.c_void_p(int(stream)), ctypes.byref(out))
+    rc = _lib().lumen_kv_plan_build_layout(ctypes.byref(geom), arr, lay, n, int(flags),
+                                           ctypes.c_void_p(int(stream)), ctypes.byref(out))
     del keep
     if rc:
         raise LumenKVError(rc, "lumen_kv_plan_build")

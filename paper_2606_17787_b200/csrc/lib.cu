@@ -455,6 +455,12 @@ int64_t lumen_kv_plan_num_chunks(const lumen_kv_plan* plan, int64_t slot_bytes) 
 
 int lumen_kv_plan_build(const lumen_kv_geom* geom, const lumen_kv_req* reqs, int32_t num_reqs,
                         uint32_t flags, void* stream, lumen_kv_plan** out) {
+    return lumen_kv_plan_build_layout(geom, reqs, nullptr, num_reqs, flags, stream, out);
+}
+
+int lumen_kv_plan_build_layout(const lumen_kv_geom* geom, const lumen_kv_req* reqs,
+                               const lumen_kv_req_layout* layouts, int32_t num_reqs,
+                               uint32_t flags, void* stream, lumen_kv_plan** out) {
     using namespace lumen;
     if (!out) return LUMEN_KV_EINVAL;
     *out = nullptr;
@@ -465,7 +471,7 @@ int lumen_kv_plan_build(const lumen_kv_geom* geom, const lumen_kv_req* reqs, int
     if (!p) return LUMEN_KV_ENOMEM;
     int rc;
     try {
-        rc = build_host_plan(geom, reqs, num_reqs, flags, &p->hp);
+        rc = build_host_plan(geom, reqs, layouts, num_reqs, flags, &p->hp);
     } catch (const std::bad_alloc&) {
         rc = LUMEN_KV_ENOMEM;
     }

@@ -37,8 +37,9 @@ inline void emit(HostPlan* hp, const Extent& x, int32_t req, int64_t chunk_token
 
 }  // namespace
 
-int build_host_plan(const lumen_kv_geom* g, const lumen_kv_req* reqs, int32_t num_reqs,
-                    uint32_t flags, HostPlan* hp) {
+int build_host_plan(const lumen_kv_geom* g, const lumen_kv_req* reqs,
+                    const lumen_kv_req_layout* layouts, int32_t num_reqs, uint32_t flags,
+                    HostPlan* hp) {
     if (!g || !hp) return LUMEN_KV_EINVAL;
     if (num_reqs < 0 || (num_reqs > 0 && !reqs)) return LUMEN_KV_EINVAL;
     const uint32_t known = LUMEN_KV_VALIDATE_UNIQUE_DST | LUMEN_KV_MERGE_ADJACENT |
@@ -69,6 +70,8 @@ int build_host_plan(const lumen_kv_geom* g, const lumen_kv_req* reqs, int32_t nu
     hp->runs.clear();
     hp->reqs.assign(static_cast<size_t>(num_reqs), ReqDesc{0, 0});
     hp->req_offset.assign(static_cast<size_t>(num_reqs) + 1, 0);
+    hp->req_tokens.assign(static_cast<size_t>(num_reqs), 0);
+    hp->req_stride.assign(static_cast<size_t>(num_reqs), 0);
     hp->max_count = 0;
 
     const bool merge = (flags & LUMEN_KV_MERGE_ADJACENT) && stride == dense;
@@ -78,15 +81,32 @@ int build_host_plan(const lumen_kv_geom* g, const lumen_kv_req* reqs, int32_t nu
     const int64_t planes = 2 * int64_t{g->num_layers};
 
     // pass 1: validate ranges, sizes and page indices; count touched pages
-    int64_t tokens = 0, touched = 0;
+    int64_t tokens = 0, touched = 0, extent = 0;
     for (int32_t r = 0; r < num_reqs; ++r) {
         const lumen_kv_req& q = reqs[r];
         if (q.t_begin < 0 || q.t_end < q.t_begin || q.page_table_len < 0) return LUMEN_KV_EINVAL;
         const int64_t n = q.t_end - q.t_begin;
         if (n >= (int64_t{1} << 32)) return LUMEN_KV_EINVAL;
-        hp->reqs[r].row_base = tokens * planes;
-        hp->reqs[r].n = n;
-        hp->req_offset[r] = tokens * planes * row;
+        hp->req_tokens[r] = n;
+        if (layouts) {
+            const lumen_kv_req_layout& ly = layouts[r];
+            if (ly.buf_offset < 0 || ly.buf_offset % row != 0 || ly.plane_stride_tokens < n ||
+                ly.plane_stride_tokens >= (int64_t{1} << 40) ||
+                ly.buf_offset > (std::numeric_limits<int64_t>::max() / 4))
+                return LUMEN_KV_EINVAL;
+            hp->reqs[r].row_base = ly.buf_offset / row;
+            hp->reqs[r].n = ly.plane_stride_tokens;
+            hp->req_offset[r] = ly.buf_offset;
+            hp->req_stride[r] = ly.plane_stride_tokens;
+            if (n > 0)
+                extent = std::max(extent, ly.buf_offset +
+                                              ((planes - 1) * ly.plane_stride_tokens + n) * row);
+        } else {
+            hp->reqs[r].row_base = tokens * planes;
+            hp->reqs[r].n = n;
+            hp->req_offset[r] = tokens * planes * row;
+            hp->req_stride[r] = n;
+        }
         if (n == 0) continue;
         const int64_t lp0 = q.t_begin / S, lp1 = (q.t_end - 1) / S;
         if (!q.page_table || lp1 >= q.page_table_len) return LUMEN_KV_ERANGE;
@@ -100,7 +120,7 @@ int build_host_plan(const lumen_kv_geom* g, const lumen_kv_req* reqs, int32_t nu
             return LUMEN_KV_EINVAL;
     }
     hp->total_tokens = tokens;
-    hp->total_bytes = tokens * planes * row;
+    hp->total_bytes = layouts ? extent : tokens * planes * row;
     hp->req_offset[num_reqs] = hp->total_bytes;
 
     // optional: every physical page addressed at most once across the whole plan (A5)
@@ -170,33 +190,36 @@ int build_chunks(const HostPlan& hp, const RunDesc* runs, int64_t slot_bytes,
     const int64_t row = hp.row_bytes;
     const int32_t planes = 2 * hp.geom.num_layers;
     if (int64_t{hp.max_count} * row > slot_bytes) return LUMEN_KV_ESIZE;
-    const int64_t R = static_cast<int64_t>(hp.req_offset.size()) - 1;
-    Chunk group{0, 0, 0, planes, 0, 0};          // whole requests accumulated so far
+    const int64_t R = static_cast<int64_t>(hp.req_tokens.size());
+    Chunk group{0, 0, 0, planes, 0, 0};          // whole, buffer-adjacent requests accumulated so far
     auto flush = [&]() {
         if (group.b1 > group.b0) out->push_back(group);
+        group.b0 = group.b1 = 0;
     };
     for (int64_t r = 0; r < R; ++r) {
-        const int64_t off = hp.req_offset[r], bytes = hp.req_offset[r + 1] - off;
+        const int64_t n = hp.req_tokens[r];
+        if (n == 0) continue;
+        const int64_t off = hp.req_offset[r];
+        const int64_t pitch = hp.req_stride[r] * row;   // bytes between consecutive planes
+        const int64_t pb = n * row;                      // bytes of one plane of this request
+        const bool dense = (hp.req_stride[r] == n);
+        const int64_t bytes = pb * planes;
         const int64_t ra = hp.req_run_begin[r], rb = hp.req_run_begin[r + 1];
-        if (bytes == 0) continue;
-        if (bytes <= slot_bytes) {
-            if (group.b1 > group.b0 && group.b1 - group.b0 + bytes > slot_bytes) {
-                flush();
-                group.b0 = group.b1 = off;
-            }
+        if (dense && bytes <= slot_bytes) {
+            const bool open = group.b1 > group.b0;
+            if (open && (off != group.b1 || group.b1 - group.b0 + bytes > slot_bytes)) flush();
             if (group.b1 == group.b0) { group.ra = ra; group.b0 = off; }
             group.rb = rb;
             group.b1 = off + bytes;
             continue;
         }
         flush();
-        group.b0 = group.b1 = off + bytes;
-        const int64_t pb = bytes / planes;       // one plane of this request: n_r * row
         if (pb <= slot_bytes) {
-            const int32_t k = static_cast<int32_t>(std::min<int64_t>(planes, slot_bytes / pb));
+            // dense blocks: as many whole planes as fit; strided blocks: one plane per chunk
+            const int32_t k = dense ? static_cast<int32_t>(std::min<int64_t>(planes, slot_bytes / pb)) : 1;
             for (int32_t p0 = 0; p0 < planes; p0 += k) {
                 const int32_t p1 = std::min(planes, p0 + k);
-                out->push_back(Chunk{ra, rb, p0, p1, off + p0 * pb, off + p1 * pb});
+                out->push_back(Chunk{ra, rb, p0, p1, off + p0 * pitch, off + (p1 - 1) * pitch + pb});
             }
             continue;
         }
@@ -208,7 +231,7 @@ int build_chunks(const HostPlan& hp, const RunDesc* runs, int64_t slot_bytes,
                     sz += int64_t{runs[b].count} * row;
                     ++b;
                 }
-                const int64_t b0 = off + p * pb + int64_t{runs[a].dst_tok} * row;
+                const int64_t b0 = off + p * pitch + int64_t{runs[a].dst_tok} * row;
                 out->push_back(Chunk{a, b, p, p + 1, b0, b0 + sz});
                 a = b;
             }

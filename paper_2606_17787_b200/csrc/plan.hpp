@@ -25,8 +25,8 @@ struct alignas(16) RunDesc {
 static_assert(sizeof(RunDesc) == 16, "RunDesc must be 16 bytes");
 
 struct alignas(16) ReqDesc {
-    int64_t row_base;   // (sum of n over earlier requests) * 2L, in rows
-    int64_t n;          // tokens of this request in the plan
+    int64_t row_base;   // first row of the request's block in the buffer (dense: sum of n * 2L)
+    int64_t n;          // rows between consecutive planes (dense: tokens of this request)
 };
 static_assert(sizeof(ReqDesc) == 16, "ReqDesc must be 16 bytes");
 
@@ -42,7 +42,9 @@ struct HostPlan {
     int32_t max_count = 0;            // longest run, tokens
     std::vector<RunDesc> runs;
     std::vector<ReqDesc> reqs;
-    std::vector<int64_t> req_offset;  // num_reqs + 1 byte offsets
+    std::vector<int64_t> req_offset;  // num_reqs + 1 byte offsets (last = total_bytes)
+    std::vector<int64_t> req_tokens;  // num_reqs: n_r
+    std::vector<int64_t> req_stride;  // num_reqs: plane stride in tokens (dense: n_r)
     std::vector<int64_t> req_run_begin;  // num_reqs + 1: runs of request r are [begin[r], begin[r+1])
 };
 
@@ -63,6 +65,7 @@ int build_chunks(const HostPlan& hp, const RunDesc* runs, int64_t slot_bytes,
 
 // Validates and flattens.  Returns a lumen_kv_status.
 int build_host_plan(const lumen_kv_geom* geom, const lumen_kv_req* reqs,
+                    const lumen_kv_req_layout* layouts /* nullptr: dense */,
                     int32_t num_reqs, uint32_t flags, HostPlan* out);
 
 }  // namespace lumen

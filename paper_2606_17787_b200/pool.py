@@ -89,10 +89,10 @@ class Checkpointer:
         self.pool = pool
         self.flags = int(flags)
 
-    def plan(self, reqs: Sequence, *, unique_dst: bool = False, stream=None) -> B.Plan:
+    def plan(self, reqs: Sequence, *, unique_dst: bool = False, stream=None, layouts=None) -> B.Plan:
         s = stream if stream is not None else torch.cuda.current_stream(self.pool.device)
         f = self.flags | (B.LUMEN_KV_VALIDATE_UNIQUE_DST if unique_dst else 0)
-        return B.lumen_kv_plan_build(self.pool.geom, reqs, f, s.cuda_stream)
+        return B.lumen_kv_plan_build(self.pool.geom, reqs, f, s.cuda_stream, layouts)
 
     def pack(self, plan: B.Plan, buf: torch.Tensor, *, stream=None) -> None:
         s = stream if stream is not None else torch.cuda.current_stream(self.pool.device)

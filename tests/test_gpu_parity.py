@@ -406,3 +406,54 @@ def test_staged_commit_and_ready_flags(G):
     for t, ref in zip(pool_b.planes(), [x for kv in zip(K2, V2) for x in kv]):
         assert np.array_equal(G.plane_to_np(t), ref), "restore read a chunk before it was ready"
     plan.close(); rplan.close(); ring.close()
+
+
+# ---- explicit buffer layout (checkpoint store, f3) ------------------------------------------
+@pytest.mark.parametrize("kernel", ["warp", "warp_upload", "bulk"])
+def test_layout_parity(G, kernel):
+    """pack / unpack with per-request (offset, plane stride), one-shot (HBM, mapped host) and
+    staged: the whole buffer (gaps included) and the whole restored pool equal the oracle's."""
+    import torch
+    rng = substream(99, "gpu_layout")
+    done = 0
+    while done < 18:
+        w = random_tiny(rng) if done % 3 else cfg1_qwen14b(L=2, N=1024, n_reqs=12, grow_iters=8,
+                                                           median=150, hi=400, lo=20).advanced(16 * (done // 3 + 1))
+        L, H, D, S, N = w.geom
+        row = H * D * 2
+        if row % 16 or not w.tokens:
+            continue
+        lays, at = [], int(rng.integers(0, 4)) * row
+        for _, tb, te in w.reqs:
+            stride = (te - tb) + int(rng.integers(0, 4))
+            lays.append((at, stride))
+            at += 2 * L * stride * row + int(rng.integers(0, 3)) * row
+        size = at + row
+        seed = 200 + done
+        K, V = G.host_planes(w.geom, seed)
+        B_ref = np.full(size // 2, 0xA5A5, dtype=np.uint16)
+        oracle.pack_layout(w.geom, K, V, w.reqs, [(o // 2, s) for o, s in lays], B_ref)
+        K2, V2 = G.host_planes(w.geom, seed + 1)
+        oracle.unpack_layout(w.geom, K2, V2, w.restore_reqs, [(o // 2, s) for o, s in lays], B_ref)
+        pool_a, pool_b = G.make_pool(w.geom, seed), G.make_pool(w.geom, seed + 1)
+        ck_a, ck_b = G.Checkpointer(pool_a, G.KERNELS[kernel]), G.Checkpointer(pool_b, G.KERNELS[kernel])
+        plan = ck_a.plan(w.reqs, layouts=lays)
+        rplan = ck_b.plan(w.restore_reqs, unique_dst=True, layouts=lays)
+        assert plan.nbytes <= size
+        mode = ("device", "host", "staged")[done % 3 if done >= 3 else done]
+        whole, buf = G.alloc_buffer(size, "device" if mode == "device" else "host")
+        if mode == "staged":
+            max_run = max(plan.run(i).count for i in range(plan.num_runs)) * row
+            ring = G.StagingRing((max_run * int(rng.integers(1, 5)) + 15) // 16 * 16, 3)
+            ck_a.pack_staged(plan, buf, ring)
+            ck_b.unpack_staged(rplan, buf, ring)
+        else:
+            ck_a.pack(plan, buf)
+            ck_b.unpack(rplan, buf)
+        torch.cuda.synchronize()
+        assert np.array_equal(G.buf_to_np(buf, size), B_ref), f"layout pack mismatch ({mode})"
+        assert G.guards_intact(whole, size)
+        for t, ref in zip(pool_b.planes(), [x for kv in zip(K2, V2) for x in kv]):
+            assert np.array_equal(G.plane_to_np(t), ref), f"layout unpack mismatch ({mode})"
+        plan.close(); rplan.close()
+        done += 1

@@ -320,3 +320,80 @@ def test_chunks_of_the_big_configs(lk):
     ch = p.chunks(slot)
     assert len(ch) == 128 * 8 and all(c.run_end - c.run_begin == 16384 for c in ch)
     assert p.chunks(1 << 40)[0].byte_end == 32 << 30 and len(p.chunks(1 << 40)) == 1
+
+
+# ---- explicit buffer layout (checkpoint store, f3) ------------------------------------------
+def _random_layouts(rng, w):
+    """Non-overlapping blocks with random gaps and plane strides >= n (bytes, tokens)."""
+    L, H, D, S, N = w.geom
+    row = H * D * 2
+    lays, at = [], int(rng.integers(0, 4)) * row
+    for _, tb, te in w.reqs:
+        stride = (te - tb) + int(rng.integers(0, 4))
+        lays.append((at, stride))
+        at += 2 * L * stride * row + int(rng.integers(0, 3)) * row
+    return lays, at + row
+
+
+def test_layout_plan_addresses_equal_oracle(lk):
+    """Bytes addressed by (runs x planes) under a layout, and by the chunks of the staged path,
+    are exactly the words the layout oracle writes into a sentinel buffer."""
+    rng = substream(88, "layout_plan")
+    for _ in range(40):
+        w = random_tiny(rng)
+        L, H, D, S, N = w.geom
+        row = H * D * 2
+        if row % 16:
+            continue
+        lays, size = _random_layouts(rng, w)
+        plan = lk.lumen_kv_plan_build(geom_of(lk, w), w.reqs, lk.LUMEN_KV_HOST_ONLY, layouts=lays)
+        K = [np.ones(N * S * H * D, np.uint16) for _ in range(L)]
+        B = np.zeros(size // 2, dtype=np.uint16)
+        oracle.pack_layout(w.geom, K, K, w.reqs, [(o // 2, s) for o, s in lays], B)
+        want = np.repeat(B.astype(bool), 2)                       # byte mask of addressed bytes
+        got = np.zeros(size, dtype=bool)
+        runs = [plan.run(i) for i in range(plan.num_runs)]
+        for r in runs:
+            off, stride = lays[r.req]
+            for p in range(2 * L):
+                b0 = off + (p * stride + r.dst_token) * row
+                assert not got[b0:b0 + r.count * row].any()
+                got[b0:b0 + r.count * row] = True
+        assert np.array_equal(got, want)
+        extent = int(np.flatnonzero(want)[-1]) + 1 if want.any() else 0
+        assert plan.nbytes == extent
+        for i, (off, _) in enumerate(lays):
+            assert plan.req_offset(i) == off
+        max_run = max([r.count for r in runs] + [1]) * row
+        for slot in (max_run, 3 * max_run + 16, 1 << 20):
+            slot = (slot + 15) // 16 * 16
+            cov = np.zeros(size, dtype=bool)
+            for c in plan.chunks(slot):
+                assert 0 < c.byte_end - c.byte_begin <= slot
+                seg = np.zeros(size, dtype=bool)
+                for p in range(c.plane_begin, c.plane_end):
+                    for r in runs[c.run_begin:c.run_end]:
+                        off, stride = lays[r.req]
+                        b0 = off + (p * stride + r.dst_token) * row
+                        seg[b0:b0 + r.count * row] = True
+                assert seg[c.byte_begin:c.byte_end].all() and seg.sum() == c.byte_end - c.byte_begin
+                assert not (cov & seg).any()
+                cov |= seg
+            assert np.array_equal(cov, want)
+
+
+def test_layout_validation(lk):
+    g = lk.make_geom(2, 2, 8, 4, 16)                              # row = 32 B
+    pt = np.arange(4, dtype=np.int32)
+    ok = lk.lumen_kv_plan_build(g, [(pt, 2, 9)], lk.LUMEN_KV_HOST_ONLY, layouts=[(64, 7)])
+    assert ok.nbytes == 64 + (3 * 7 + 7) * 32 and ok.req_offset(0) == 64
+    for bad in ((48, 7), (-32, 7), (64, 6)):                      # not a row multiple / negative / stride < n
+        with pytest.raises(lk.LumenKVError) as e:
+            lk.lumen_kv_plan_build(g, [(pt, 2, 9)], lk.LUMEN_KV_HOST_ONLY, layouts=[bad])
+        assert e.value.status == lk.LUMEN_KV_EINVAL
+    # dense layout given explicitly == no layout
+    a = lk.lumen_kv_plan_build(g, [(pt, 2, 9), (pt, 0, 3)], lk.LUMEN_KV_HOST_ONLY,
+                               layouts=[(0, 7), (7 * 4 * 32, 3)])
+    b = lk.lumen_kv_plan_build(g, [(pt, 2, 9), (pt, 0, 3)], lk.LUMEN_KV_HOST_ONLY)
+    spans = lambda p: [(c.byte_begin, c.byte_end) for c in p.chunks(1 << 20)]
+    assert a.nbytes == b.nbytes and spans(a) == spans(b)
