@@ -67,7 +67,7 @@ typedef enum {
     LUMEN_KV_OK       =  0,
     LUMEN_KV_EINVAL   = -1,  /* null pointer, bad geometry, misaligned base, bad kind/flag   */
     LUMEN_KV_ERANGE   = -2,  /* page index outside [0, num_pages) or range outside the table */
-    LUMEN_KV_EOVERLAP = -3,  /* VALIDATE_UNIQUE_DST: a physical page is addressed twice      */
+    LUMEN_KV_EOVERLAP = -3,  /* VALIDATE_UNIQUE_DST: a pool token slot is addressed twice     */
     LUMEN_KV_ESIZE    = -4,  /* buffer smaller than lumen_kv_plan_bytes()                    */
     LUMEN_KV_ENOMEM   = -5,  /* host or device allocation of the descriptors failed          */
     LUMEN_KV_ECUDA    = -6   /* CUDA runtime error; see lumen_kv_last_cuda_error()           */
@@ -96,7 +96,7 @@ typedef struct {
 typedef struct lumen_kv_plan lumen_kv_plan;  /* opaque; library owns its descriptors */
 
 /* plan_build flags */
-#define LUMEN_KV_VALIDATE_UNIQUE_DST 0x1u /* reject plans that address a physical page twice  */
+#define LUMEN_KV_VALIDATE_UNIQUE_DST 0x1u /* reject plans that address a pool token slot twice  */
 #define LUMEN_KV_MERGE_ADJACENT      0x2u /* merge runs whose physical pages are adjacent     */
 #define LUMEN_KV_HOST_ONLY           0x4u /* build descriptors on the host only (no CUDA call);
                                              such a plan can be inspected but not executed   */
@@ -306,6 +306,62 @@ LUMEN_KV_API int lumen_kv_page_tags(const int32_t* token_ids, const int64_t* tok
  */
 LUMEN_KV_API int64_t lumen_kv_longest_prefix(const lumen_kv_tag* regen, int64_t n_regen,
                                              const lumen_kv_tag* stored, int64_t n_stored);
+
+/*
+ * Checkpoint store: the host-memory region of a worker that
+ * persists "incoming remote KV pages".  One checkpoint per request; a request's footprint
+ * is RESERVED at assignment from its maximum context length ("a conservative allocation
+ * derived from the maximum context length rather than the current dynamic KV size") and
+ * released at completion, so a holder can never run out of host memory; the per-worker
+ * limit is the arena size (80 / 160 GB in the paper's deployments).  Deltas are appended as
+ * they arrive, each with the page tags it carries, and become visible to lookups only when
+ * the append has completed ("pages become visible in the checkpoint store only upon complete
+ * reception").  Pure host code; thread-safe; the library allocates no payload memory:
+ *   arena : caller's host memory (pin it if the GPU is to restore from it), 16-byte aligned.
+ *   token_bytes = 2 * num_layers * row : bytes of one token over all planes.
+ * A delta is the dense pack buffer of one request's range [t_begin, t_end)
+ * ([plane][token][head][dim], what lumen_kv_checkpoint_pack writes for a 1-request plan);
+ * deltas of a request must arrive in order (t_begin == tokens stored so far).
+ * Status codes: EINVAL (unknown / duplicate request, out-of-order or oversized delta, bad
+ * tag), ENOMEM (no contiguous room for the reservation), ESIZE (delta_bytes mismatch).
+ */
+typedef struct lumen_kv_store lumen_kv_store;
+LUMEN_KV_API int lumen_kv_store_create(void* arena, int64_t arena_bytes, int64_t token_bytes,
+                                       int32_t page_size, int32_t copy_threads,
+                                       lumen_kv_store** out);
+LUMEN_KV_API void lumen_kv_store_destroy(lumen_kv_store* store);
+/* bytes not reserved: the "available checkpoint-store capacity" of the load table */
+LUMEN_KV_API int64_t lumen_kv_store_available(const lumen_kv_store* store);
+/* reserved footprint of all requests held, in bytes */
+LUMEN_KV_API int64_t lumen_kv_store_reserved(const lumen_kv_store* store);
+LUMEN_KV_API int lumen_kv_store_reserve(lumen_kv_store* store, uint64_t request_id,
+                                        int64_t max_tokens);
+LUMEN_KV_API int lumen_kv_store_release(lumen_kv_store* store, uint64_t request_id);
+/* tags: the tags of the pages this delta touches, any order; every end_pos must lie in
+ * (t_begin, t_end].  n_tags may be 0. */
+LUMEN_KV_API int lumen_kv_store_append(lumen_kv_store* store, uint64_t request_id,
+                                       int64_t t_begin, int64_t t_end, const void* delta,
+                                       int64_t delta_bytes, const lumen_kv_tag* tags,
+                                       int32_t n_tags);
+/* tokens stored for the request (its "actual checkpointed size"), or EINVAL */
+LUMEN_KV_API int64_t lumen_kv_store_tokens(const lumen_kv_store* store, uint64_t request_id);
+/* longest contiguous checkpointed prefix, in tokens, for the tags regenerated from the
+ * request's token history (lumen_kv_page_tags / lumen_kv_longest_prefix over the stored tags) */
+LUMEN_KV_API int64_t lumen_kv_store_lookup(const lumen_kv_store* store, uint64_t request_id,
+                                           const lumen_kv_tag* regen, int64_t n_regen);
+/* The stored deltas that cover [0, prefix_tokens), in order: segment i holds tokens
+ * [t_begin, t_end) at byte offset buf_offset of the arena with plane stride
+ * plane_stride_tokens -- exactly a lumen_kv_req range + lumen_kv_req_layout for
+ * lumen_kv_plan_build_layout, so the prefix is restored straight out of the arena.
+ * Writes at most cap entries; returns the number of segments or a status. */
+typedef struct {
+    int64_t t_begin, t_end;
+    int64_t buf_offset;
+    int64_t plane_stride_tokens;
+} lumen_kv_segment;
+LUMEN_KV_API int64_t lumen_kv_store_segments(const lumen_kv_store* store, uint64_t request_id,
+                                             int64_t prefix_tokens, lumen_kv_segment* out,
+                                             int64_t cap);
 
 /* Release a plan.  Safe to call while work using the plan is still in flight on a
  * stream: the descriptors are recycled only after that work has completed.       */

@@ -38,6 +38,10 @@ EXPORTS = (
     "lumen_kv_restore_unpack_staged", "lumen_kv_plan_num_chunks", "lumen_kv_plan_get_chunks",
     "lumen_kv_checkpoint_pack_staged_commit", "lumen_kv_restore_unpack_staged_ready",
     "lumen_kv_tags_num_pages", "lumen_kv_page_tags", "lumen_kv_longest_prefix",
+    "lumen_kv_store_create", "lumen_kv_store_destroy", "lumen_kv_store_available",
+    "lumen_kv_store_reserved", "lumen_kv_store_reserve", "lumen_kv_store_release",
+    "lumen_kv_store_append", "lumen_kv_store_tokens", "lumen_kv_store_lookup",
+    "lumen_kv_store_segments",
 )
 
 
@@ -128,6 +132,26 @@ def _lib() -> ctypes.CDLL:
     L.lumen_kv_page_tags.argtypes = [vp, vp, i32, i32, vp, i64, vp]
     L.lumen_kv_longest_prefix.restype = i64
     L.lumen_kv_longest_prefix.argtypes = [vp, i64, vp, i64]
+    u64 = ctypes.c_uint64
+    L.lumen_kv_store_create.restype = ctypes.c_int
+    L.lumen_kv_store_create.argtypes = [vp, i64, i64, i32, i32, ctypes.POINTER(vp)]
+    L.lumen_kv_store_destroy.restype = None
+    L.lumen_kv_store_destroy.argtypes = [vp]
+    for name in ("lumen_kv_store_available", "lumen_kv_store_reserved"):
+        getattr(L, name).restype = i64
+        getattr(L, name).argtypes = [vp]
+    L.lumen_kv_store_reserve.restype = ctypes.c_int
+    L.lumen_kv_store_reserve.argtypes = [vp, u64, i64]
+    L.lumen_kv_store_release.restype = ctypes.c_int
+    L.lumen_kv_store_release.argtypes = [vp, u64]
+    L.lumen_kv_store_append.restype = ctypes.c_int
+    L.lumen_kv_store_append.argtypes = [vp, u64, i64, i64, vp, i64, vp, i32]
+    L.lumen_kv_store_tokens.restype = i64
+    L.lumen_kv_store_tokens.argtypes = [vp, u64]
+    L.lumen_kv_store_lookup.restype = i64
+    L.lumen_kv_store_lookup.argtypes = [vp, u64, vp, i64]
+    L.lumen_kv_store_segments.restype = i64
+    L.lumen_kv_store_segments.argtypes = [vp, u64, i64, vp, i64]
     L.lumen_kv_plan_num_chunks.restype = i64
     L.lumen_kv_plan_num_chunks.argtypes = [vp, i64]
     L.lumen_kv_plan_get_chunks.restype = i64
@@ -427,6 +451,79 @@ def lumen_kv_longest_prefix(regen: np.ndarray, stored: np.ndarray) -> int:
     if n < 0:
         raise LumenKVError(n, "lumen_kv_longest_prefix")
     return n
+
+
+SEGMENT_DTYPE = np.dtype([("t_begin", np.int64), ("t_end", np.int64), ("buf_offset", np.int64),
+                          ("plane_stride_tokens", np.int64)])          # lumen_kv_segment
+
+
+class Store:
+    """Owner of a `lumen_kv_store*` over a caller-provided host arena (pointer + size)."""
+
+    def __init__(self, arena_ptr: int, arena_bytes: int, token_bytes: int, page_size: int,
+                 copy_threads: int = 1):
+        out = ctypes.c_void_p()
+        rc = _lib().lumen_kv_store_create(ctypes.c_void_p(int(arena_ptr)), int(arena_bytes),
+                                          int(token_bytes), int(page_size), int(copy_threads),
+                                          ctypes.byref(out))
+        if rc:
+            raise LumenKVError(rc, "lumen_kv_store_create")
+        self._h = out
+        self.token_bytes = int(token_bytes)
+
+    def _check(self, rc, where):
+        if rc < 0:
+            raise LumenKVError(int(rc), where)
+        return int(rc)
+
+    @property
+    def available(self) -> int:
+        return self._check(_lib().lumen_kv_store_available(self._h), "lumen_kv_store_available")
+
+    @property
+    def reserved(self) -> int:
+        return self._check(_lib().lumen_kv_store_reserved(self._h), "lumen_kv_store_reserved")
+
+    def reserve(self, request_id: int, max_tokens: int) -> None:
+        self._check(_lib().lumen_kv_store_reserve(self._h, int(request_id), int(max_tokens)),
+                    "lumen_kv_store_reserve")
+
+    def release(self, request_id: int) -> None:
+        self._check(_lib().lumen_kv_store_release(self._h, int(request_id)), "lumen_kv_store_release")
+
+    def append(self, request_id: int, t_begin: int, t_end: int, delta_ptr: int, delta_bytes: int,
+               tags: np.ndarray) -> None:
+        t = np.ascontiguousarray(tags, dtype=TAG_DTYPE)
+        self._check(_lib().lumen_kv_store_append(self._h, int(request_id), int(t_begin), int(t_end),
+                                                 ctypes.c_void_p(int(delta_ptr)), int(delta_bytes),
+                                                 t.ctypes.data, t.size), "lumen_kv_store_append")
+
+    def tokens(self, request_id: int) -> int:
+        return self._check(_lib().lumen_kv_store_tokens(self._h, int(request_id)), "lumen_kv_store_tokens")
+
+    def lookup(self, request_id: int, regen: np.ndarray) -> int:
+        t = np.ascontiguousarray(regen, dtype=TAG_DTYPE)
+        return self._check(_lib().lumen_kv_store_lookup(self._h, int(request_id), t.ctypes.data, t.size),
+                           "lumen_kv_store_lookup")
+
+    def segments(self, request_id: int, prefix_tokens: int) -> np.ndarray:
+        n = self._check(_lib().lumen_kv_store_segments(self._h, int(request_id), int(prefix_tokens),
+                                                       None, 0), "lumen_kv_store_segments")
+        out = np.zeros(n, dtype=SEGMENT_DTYPE)
+        self._check(_lib().lumen_kv_store_segments(self._h, int(request_id), int(prefix_tokens),
+                                                   out.ctypes.data, n), "lumen_kv_store_segments")
+        return out
+
+    def close(self) -> None:
+        if self._h:
+            _lib().lumen_kv_store_destroy(self._h)
+            self._h = ctypes.c_void_p(None)
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
 
 
 def lumen_kv_plan_free(plan: Plan) -> None:

@@ -590,7 +590,7 @@ const char* lumen_kv_strerror(int status) {
         case LUMEN_KV_OK: return "ok";
         case LUMEN_KV_EINVAL: return "invalid argument (null, misaligned, bad geometry, kind or flag)";
         case LUMEN_KV_ERANGE: return "page index or token range outside the page table / pool";
-        case LUMEN_KV_EOVERLAP: return "a physical page is addressed more than once";
+        case LUMEN_KV_EOVERLAP: return "a pool token slot is addressed more than once";
         case LUMEN_KV_ESIZE: return "buffer smaller than the plan's bytes";
         case LUMEN_KV_ENOMEM: return "out of host or device memory for descriptors";
         case LUMEN_KV_ECUDA: return "CUDA runtime error (see lumen_kv_last_cuda_error)";

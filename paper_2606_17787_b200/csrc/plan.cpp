@@ -123,9 +123,12 @@ int build_host_plan(const lumen_kv_geom* g, const lumen_kv_req* reqs,
     hp->total_bytes = layouts ? extent : tokens * planes * row;
     hp->req_offset[num_reqs] = hp->total_bytes;
 
-    // optional: every physical page addressed at most once across the whole plan (A5)
+    // optional: every pool token slot addressed at most once across the whole plan (A5).
+    // Pages are checked first (bitmap or sort); only pages that appear twice -- e.g. two
+    // consecutive deltas of one request meeting inside a page -- get the exact slot-interval test.
     if (unique && touched > 0) {
         const int64_t N = g->num_pages;
+        std::vector<int32_t> dup;
         if (N <= 64 * touched || N <= (int64_t{1} << 23)) {
             std::vector<uint64_t> bits(static_cast<size_t>((N + 63) / 64), 0);
             for (int32_t r = 0; r < num_reqs; ++r) {
@@ -135,7 +138,7 @@ int build_host_plan(const lumen_kv_geom* g, const lumen_kv_req* reqs,
                     const uint32_t p = static_cast<uint32_t>(q.page_table[lp]);
                     uint64_t& w = bits[p >> 6];
                     const uint64_t m = uint64_t{1} << (p & 63);
-                    if (w & m) return LUMEN_KV_EOVERLAP;
+                    if (w & m) dup.push_back(static_cast<int32_t>(p));
                     w |= m;
                 }
             }
@@ -149,8 +152,33 @@ int build_host_plan(const lumen_kv_geom* g, const lumen_kv_req* reqs,
                     all.push_back(q.page_table[lp]);
             }
             std::sort(all.begin(), all.end());
-            if (std::adjacent_find(all.begin(), all.end()) != all.end())
-                return LUMEN_KV_EOVERLAP;
+            for (size_t i = 1; i < all.size(); ++i)
+                if (all[i] == all[i - 1]) dup.push_back(all[i]);
+        }
+        if (!dup.empty()) {
+            std::sort(dup.begin(), dup.end());
+            dup.erase(std::unique(dup.begin(), dup.end()), dup.end());
+            struct Span { int32_t page; int32_t lo, hi; };
+            std::vector<Span> spans;
+            for (int32_t r = 0; r < num_reqs; ++r) {
+                const lumen_kv_req& q = reqs[r];
+                if (q.t_end == q.t_begin) continue;
+                for (int64_t lp = q.t_begin / S; lp <= (q.t_end - 1) / S; ++lp) {
+                    const int32_t p = q.page_table[lp];
+                    if (!std::binary_search(dup.begin(), dup.end(), p)) continue;
+                    const int64_t lo = std::max(q.t_begin, lp * S) - lp * S;
+                    const int64_t hi = std::min(q.t_end, (lp + 1) * S) - lp * S;
+                    spans.push_back(Span{p, static_cast<int32_t>(lo), static_cast<int32_t>(hi)});
+                }
+            }
+            std::sort(spans.begin(), spans.end(), [](const Span& a, const Span& b) {
+                return a.page != b.page ? a.page < b.page : a.lo < b.lo;
+            });
+            for (size_t i = 1; i < spans.size(); ++i)
+                if (spans[i].page == spans[i - 1].page && spans[i].lo < spans[i - 1].hi)
+                    return LUMEN_KV_EOVERLAP;
+            // (sorted by lo, so comparing with the predecessor's hi suffices once overlaps are
+            //  rejected: non-overlapping predecessors have increasing hi)
         }
     }
 

@@ -397,3 +397,20 @@ def test_layout_validation(lk):
     b = lk.lumen_kv_plan_build(g, [(pt, 2, 9), (pt, 0, 3)], lk.LUMEN_KV_HOST_ONLY)
     spans = lambda p: [(c.byte_begin, c.byte_end) for c in p.chunks(1 << 20)]
     assert a.nbytes == b.nbytes and spans(a) == spans(b)
+
+
+def test_unique_dst_is_slot_granular(lk):
+    """Consecutive deltas of one request meet inside a page: disjoint token slots are legal,
+    one shared slot is EOVERLAP (both the bitmap and the sort path)."""
+    U = lk.LUMEN_KV_VALIDATE_UNIQUE_DST | lk.LUMEN_KV_HOST_ONLY
+    pt = np.array([7, 3, 9], dtype=np.int32)
+    for N in (16, 1 << 24):                                   # small pool: bitmap; huge pool: sort
+        g = lk.make_geom(1, 1, 8, 4, N)
+        lk.lumen_kv_plan_build(g, [(pt, 0, 6), (pt, 6, 7), (pt, 7, 12)], U).close()
+        for bad in ([(pt, 0, 6), (pt, 5, 9)], [(pt, 0, 12), (pt, 7, 8)],
+                    [(pt, 2, 3), (np.array([7], np.int32), 2, 3)]):
+            with pytest.raises(lk.LumenKVError) as e:
+                lk.lumen_kv_plan_build(g, bad, U)
+            assert e.value.status == lk.LUMEN_KV_EOVERLAP
+        # another request using the other half of the same physical page
+        lk.lumen_kv_plan_build(g, [(pt, 0, 2), (np.array([7], np.int32), 2, 4)], U).close()

@@ -1,0 +1,222 @@
+"""Checkpoint store: reservation
+arithmetic, append-only deltas, visibility, tags and segments -- on the CPU against a plain
+Python model and the oracle; then the whole chain on the GPU: incremental packs -> store ->
+failure -> tag lookup -> restore of the longest checkpointed prefix straight out of the arena,
+equal to the oracle's restore of that prefix."""
+import threading
+
+import numpy as np
+import pytest
+
+import oracle
+from workloads import MASTER_SEED, cfg0_tiny, cfg1_qwen14b, substream
+
+
+@pytest.fixture(scope="module")
+def lk():
+    from paper_2606_17787_b200 import build
+    build.build()
+    import paper_2606_17787_b200 as lk
+    return lk
+
+
+def _arena(nbytes):
+    a = np.zeros(nbytes + 16, dtype=np.uint8)
+    off = (-a.ctypes.data) % 16
+    return a, a[off:off + nbytes]
+
+
+def test_reservation_arithmetic(lk):
+    """Footprint = max context length x bytes per token, reserved at assignment, released at
+    completion: closed forms, first fit, coalescing."""
+    tokb = 1024                                              # cfg 0: 2 layers x 2 x 256 B rows
+    keep, arena = _arena(100 * tokb)
+    st = lk.Store(arena.ctypes.data, arena.size, tokb, 16)
+    assert st.available == 100 * tokb and st.reserved == 0
+    st.reserve(1, 40); st.reserve(2, 30); st.reserve(3, 30)
+    assert st.available == 0 and st.reserved == 100 * tokb
+    with pytest.raises(lk.LumenKVError) as e:
+        st.reserve(4, 1)
+    assert e.value.status == lk.LUMEN_KV_ENOMEM               # a holder never over-commits
+    with pytest.raises(lk.LumenKVError) as e:
+        st.reserve(1, 1)                                      # exactly one checkpoint per request
+    assert e.value.status == lk.LUMEN_KV_EINVAL
+    st.release(2)
+    assert st.available == 30 * tokb
+    with pytest.raises(lk.LumenKVError):
+        st.reserve(5, 31)                                     # 30 free, contiguous
+    st.release(1)
+    st.reserve(6, 70)                                         # the two holes coalesced: 40 + 30
+    assert st.available == 0
+    st.release(3); st.release(6)
+    assert st.available == 100 * tokb
+    st.reserve(7, 100)
+    with pytest.raises(lk.LumenKVError):
+        st.release(99)
+
+
+def test_append_segments_and_lookup_against_model(lk):
+    rng = substream(5, "store")
+    w = cfg0_tiny(full_prefix=True)
+    L, H, D, S, N = w.geom
+    E, tokb = H * D, 2 * L * H * D * 2
+    from workloads import fill_plane_np
+    K = [fill_plane_np(3, 2 * l, N * S * E) for l in range(L)]
+    V = [fill_plane_np(3, 2 * l + 1, N * S * E) for l in range(L)]
+    keep, arena = _arena(400 * tokb)
+    st = lk.Store(arena.ctypes.data, arena.size, tokb, S, copy_threads=3)
+    model = {}
+    for rid, (pt, _, n) in enumerate(w.reqs):
+        st.reserve(rid, n + 20)
+        toks = rng.integers(0, 1000, size=n).astype(np.int32)
+        cuts = sorted(set(rng.integers(1, n, size=3).tolist())) if n > 2 else []
+        at, segs = 0, []
+        for te in cuts + [n]:
+            delta = oracle.pack(w.geom, K, V, [(pt, at, te)])
+            tags = oracle.page_tags(toks[:te], S)              # tags as of this delta
+            tags = tags[(tags["end_pos"] > at) & (tags["end_pos"] <= te)]
+            st.append(rid, at, te, delta.ctypes.data, delta.nbytes, tags)
+            segs.append((at, te, delta))
+            at = te
+        model[rid] = (toks, segs)
+        assert st.tokens(rid) == n
+    for rid, (toks, segs) in model.items():
+        n = toks.size
+        # history = exactly what was checkpointed: everything is reusable
+        assert st.lookup(rid, oracle.page_tags(toks, S)) == n
+        # history has grown: a partly filled last page no longer matches, the prefix is page aligned
+        longer = np.concatenate([toks, rng.integers(0, 1000, size=S).astype(np.int32)])
+        prefix = st.lookup(rid, oracle.page_tags(longer, S))
+        assert prefix == (n // S) * S
+        # a different token history shares no prefix beyond the common pages
+        other = toks.copy()
+        if n > S:
+            other[S] += 1
+            assert st.lookup(rid, oracle.page_tags(other, S)) == S
+        segs_got = st.segments(rid, prefix)
+        want = [(a, min(b, prefix), b - a) for a, b, _ in segs if a < prefix]
+        assert [(int(s["t_begin"]), int(s["t_end"]), int(s["plane_stride_tokens"])) for s in segs_got] == want
+        for s, (a, b, delta) in zip(segs_got, segs):           # bytes in the arena == the delta received
+            off = int(s["buf_offset"])
+            assert np.array_equal(arena[off:off + delta.nbytes].view(np.uint16), delta)
+    # out-of-order / oversized / wrong-size deltas and bad tags are refused
+    st.reserve(50, 10)
+    d = np.zeros(4 * tokb // 2, dtype=np.uint16)
+    none = np.zeros(0, dtype=lk.TAG_DTYPE)
+    for args, code in (((50, 1, 5, d.ctypes.data, d.nbytes, none), lk.LUMEN_KV_EINVAL),
+                       ((50, 0, 4, d.ctypes.data, d.nbytes - 2, none), lk.LUMEN_KV_ESIZE),
+                       ((51, 0, 4, d.ctypes.data, d.nbytes, none), lk.LUMEN_KV_EINVAL)):
+        with pytest.raises(lk.LumenKVError) as e:
+            st.append(*args)
+        assert e.value.status == code
+    bad = np.array([(1, 9)], dtype=lk.TAG_DTYPE)               # end position outside (0, 4]
+    with pytest.raises(lk.LumenKVError):
+        st.append(50, 0, 4, d.ctypes.data, d.nbytes, bad)
+    st.append(50, 0, 4, d.ctypes.data, d.nbytes, none)
+    big = np.zeros(7 * tokb // 2, dtype=np.uint16)
+    with pytest.raises(lk.LumenKVError):
+        st.append(50, 4, 11, big.ctypes.data, big.nbytes, none)   # beyond the reserved footprint
+
+
+def test_visibility_only_after_complete_reception(lk):
+    """A lookup running while a large delta is being copied in sees either nothing of it or
+    all of it."""
+    tokb, S, n = 1 << 20, 16, 64                               # 64 MiB delta, copied by 4 threads
+    keep, arena = _arena(n * tokb)
+    st = lk.Store(arena.ctypes.data, arena.size, tokb, S, copy_threads=4)
+    st.reserve(7, n)
+    toks = np.arange(n, dtype=np.int32)
+    tags = oracle.page_tags(toks, S)
+    delta = np.full(n * tokb, 0x5C, dtype=np.uint8)
+    seen, stop = set(), threading.Event()
+
+    def poll():
+        while not stop.is_set():
+            seen.add((st.tokens(7), st.lookup(7, tags)))
+
+    th = threading.Thread(target=poll)
+    th.start()
+    st.append(7, 0, n, delta.ctypes.data, delta.nbytes, tags)
+    seen.add((st.tokens(7), st.lookup(7, tags)))
+    stop.set(); th.join()
+    # the two reads of a sample are separate calls, so (0, n) can straddle the publication;
+    # a partial count or tags without their tokens ((n, 0), (k, .) with 0 < k < n) never appear
+    assert seen <= {(0, 0), (0, n), (n, n)} and (n, n) in seen
+    assert (arena[:n * tokb] == 0x5C).all()
+
+
+@pytest.mark.gpu
+def test_gpu_checkpoint_chain_end_to_end(lk):
+    """Worker A packs a delta per step into a pinned buffer (3), the bytes reach the holder's
+    store (4); A fails; the holder regenerates the tags from the token history, finds the
+    longest checkpointed prefix and restores it into fresh pages straight out of the pinned
+    arena (staged, explicit layout).  The restored pool equals the oracle's restore of that
+    prefix; tags come from the CUDA kernel."""
+    import torch
+    from tests import gpu_util as G
+    G.build_all()
+    w = cfg1_qwen14b(L=3, N=1024, n_reqs=6, grow_iters=8, median=150, hi=300, lo=40)
+    L, H, D, S, N = w.geom
+    E, tokb = H * D, 2 * L * H * D * 2
+    rng = substream(6, "chain")
+    lens = [te for _, _, te in w.reqs]
+    steps, delta_tok = 5, 16
+    hist = [rng.integers(0, 32000, size=n + steps * delta_tok).astype(np.int32) for n in lens]
+    pool_a = G.make_pool(w.geom, 21)
+    ck_a = G.Checkpointer(pool_a)
+    arena_t = G.pinned_buffer(sum(n + 8 * delta_tok for n in lens) * tokb)
+    st = lk.Store(arena_t.data_ptr(), arena_t.numel(), tokb, S, copy_threads=2)
+    for rid, n in enumerate(lens):
+        st.reserve(rid, n + 8 * delta_tok)
+    stage = G.pinned_buffer(max(lens) * tokb)                  # worker A's pinned staging buffer
+    ring = G.StagingRing(1 << 20, 3)
+    d_tags = torch.empty((4096, 2), dtype=torch.int64, device="cuda")
+
+    def tags_of(tokens):                                       # CUDA tag kernel
+        d_tok = torch.from_numpy(np.ascontiguousarray(tokens)).cuda()
+        n = lk.lumen_kv_tags_num_pages([0, tokens.size], S)
+        lk.lumen_kv_page_tags(d_tok.data_ptr(), [0, tokens.size], S, d_tags.data_ptr(), n, 0)
+        torch.cuda.synchronize()
+        return d_tags[:n].cpu().numpy().copy().view(lk.TAG_DTYPE).reshape(-1)
+
+    sent = [0] * len(lens)
+    for step in range(steps + 1):                              # step 0 = prefill-completion checkpoint
+        for rid, (pt, _, n) in enumerate(w.reqs):
+            te = n + step * delta_tok if step < steps else n + (steps - 1) * delta_tok + 5
+            if te <= sent[rid]:
+                continue
+            plan = ck_a.plan([(pt, sent[rid], te)])
+            ck_a.pack_staged(plan, stage, ring)
+            torch.cuda.synchronize()
+            tags = tags_of(hist[rid][:te])
+            tags = tags[(tags["end_pos"] > sent[rid]) & (tags["end_pos"] <= te)]
+            st.append(rid, sent[rid], te, stage.data_ptr(), plan.nbytes, tags)   # "network"
+            plan.close()
+            sent[rid] = te
+    # ---- failure of worker A; the holder restores into its own pool under fresh page tables ----
+    pool_b = G.make_pool(w.geom, 22)
+    ck_b = G.Checkpointer(pool_b)
+    K, V = G.host_planes(w.geom, 21)
+    K2, V2 = G.host_planes(w.geom, 22)
+    reqs, lays, total_prefix = [], [], 0
+    for rid, (pt_new, _, _) in enumerate(w.restore_reqs):
+        regen = tags_of(hist[rid])                             # full token history kept by the gateway
+        assert np.array_equal(regen, oracle.page_tags(hist[rid], S))
+        prefix = st.lookup(rid, regen)
+        assert prefix == (sent[rid] // S) * S                  # the 5-token tail page does not match
+        total_prefix += prefix
+        for s in st.segments(rid, prefix):
+            reqs.append((pt_new, int(s["t_begin"]), int(s["t_end"])))
+            lays.append((int(s["buf_offset"]), int(s["plane_stride_tokens"])))
+        # oracle: restore of exactly that prefix
+        oracle.unpack(w.geom, K2, V2, [(pt_new, 0, prefix)], oracle.pack(w.geom, K, V, [(w.reqs[rid][0], 0, prefix)]))
+    rplan = ck_b.plan(reqs, unique_dst=True, layouts=lays)
+    assert rplan.nbytes <= arena_t.numel()
+    ck_b.unpack_staged(rplan, arena_t, ring)
+    torch.cuda.synchronize()
+    for t, ref in zip(pool_b.planes(), [x for kv in zip(K2, V2) for x in kv]):
+        assert np.array_equal(G.plane_to_np(t), ref)
+    assert total_prefix > 0
+    for rid in range(len(lens)):                               # completion releases the footprint
+        st.release(rid)
+    assert st.reserved == 0
