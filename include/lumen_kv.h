@@ -363,6 +363,37 @@ LUMEN_KV_API int64_t lumen_kv_store_segments(const lumen_kv_store* store, uint64
                                              int64_t prefix_tokens, lumen_kv_segment* out,
                                              int64_t cap);
 
+/*
+ * Controller logic (host arithmetic only; section 4.2 Eq. (1), section 4.3).
+ *
+ * lumen_kv_choose_holder -- checkpoint placement, Eq. (1):
+ *     h(r) = argmin over w in F(r) of  q_w + lambda * p_w(r)
+ *   q[w]        : queueing delay of worker w;
+ *   p_w(r)      : mean reserved footprint of the checkpoints w would hold after assigning r
+ *                 (held[held_begin[w] .. held_begin[w+1]) plus footprint), divided by bandwidth;
+ *   F(r)        : workers other than `serving` with available[w] >= footprint.
+ *   Evaluated in double, in the order ((sum / count) / bandwidth) * lambda + q; ties go to
+ *   the lowest worker id (reading F1).  *holder = h(r), or -1 if F(r) is empty.
+ * lumen_kv_recover -- recovery dispatch + greedy load rebalancing:
+ *   load[w]     : queued + running requests of worker w (ignored where alive[w] == 0);
+ *   holder[i], ckpt_size[i] : checkpoint holder and checkpointed size of interrupted request i;
+ *   assign[i]   : worker that takes request i;  reuse[i] : 1 if it restores its checkpoint
+ *                 there, 0 if it recomputes;  final_load[w] : loads after rebalancing.
+ *   Interrupted requests go to their holder (reuse) or, if the holder is dead, to the
+ *   least-loaded survivor (recompute); then, while a survivor holding reusable requests has
+ *   load > ceil(average load after dispatch), the most loaded such worker sheds its
+ *   smallest checkpoint to the least-loaded other survivor (readings F2-F4).
+ * Errors: EINVAL (null, no worker alive, negative sizes, bad ids).
+ */
+LUMEN_KV_API int lumen_kv_choose_holder(const double* q, const int64_t* held,
+                                        const int32_t* held_begin, const int64_t* available,
+                                        int32_t num_workers, int32_t serving, int64_t footprint,
+                                        double lambda, double bandwidth, int32_t* holder);
+LUMEN_KV_API int lumen_kv_recover(const int64_t* load, const uint8_t* alive, int32_t num_workers,
+                                  const int32_t* holder, const int64_t* ckpt_size,
+                                  int32_t num_interrupted, int32_t* assign, uint8_t* reuse,
+                                  int64_t* final_load);
+
 /* Release a plan.  Safe to call while work using the plan is still in flight on a
  * stream: the descriptors are recycled only after that work has completed.       */
 LUMEN_KV_API void lumen_kv_plan_free(lumen_kv_plan* plan);

@@ -41,7 +41,7 @@ EXPORTS = (
     "lumen_kv_store_create", "lumen_kv_store_destroy", "lumen_kv_store_available",
     "lumen_kv_store_reserved", "lumen_kv_store_reserve", "lumen_kv_store_release",
     "lumen_kv_store_append", "lumen_kv_store_tokens", "lumen_kv_store_lookup",
-    "lumen_kv_store_segments",
+    "lumen_kv_store_segments", "lumen_kv_choose_holder", "lumen_kv_recover",
 )
 
 
@@ -152,6 +152,11 @@ def _lib() -> ctypes.CDLL:
     L.lumen_kv_store_lookup.argtypes = [vp, u64, vp, i64]
     L.lumen_kv_store_segments.restype = i64
     L.lumen_kv_store_segments.argtypes = [vp, u64, i64, vp, i64]
+    L.lumen_kv_choose_holder.restype = ctypes.c_int
+    L.lumen_kv_choose_holder.argtypes = [vp, vp, vp, vp, i32, i32, i64, ctypes.c_double,
+                                         ctypes.c_double, ctypes.POINTER(i32)]
+    L.lumen_kv_recover.restype = ctypes.c_int
+    L.lumen_kv_recover.argtypes = [vp, vp, i32, vp, vp, i32, vp, vp, vp]
     L.lumen_kv_plan_num_chunks.restype = i64
     L.lumen_kv_plan_num_chunks.argtypes = [vp, i64]
     L.lumen_kv_plan_get_chunks.restype = i64
@@ -524,6 +529,42 @@ class Store:
             self.close()
         except Exception:
             pass
+
+
+def lumen_kv_choose_holder(q, held, available, serving: int, footprint: int, lam: float,
+                           bandwidth: float) -> int:
+    """Eq. (1).  held: per worker, the reserved footprints of the checkpoints it holds.
+    Returns h(r), or -1 if no worker can hold the checkpoint."""
+    qa = np.ascontiguousarray(q, dtype=np.float64)
+    begin = np.zeros(len(held) + 1, dtype=np.int32)
+    begin[1:] = np.cumsum([len(h) for h in held])
+    flat = np.ascontiguousarray([x for h in held for x in h], dtype=np.int64)
+    av = np.ascontiguousarray(available, dtype=np.int64)
+    out = ctypes.c_int32(-1)
+    rc = _lib().lumen_kv_choose_holder(qa.ctypes.data, flat.ctypes.data if flat.size else None,
+                                       begin.ctypes.data, av.ctypes.data, qa.size, int(serving),
+                                       int(footprint), float(lam), float(bandwidth), ctypes.byref(out))
+    if rc:
+        raise LumenKVError(rc, "lumen_kv_choose_holder")
+    return int(out.value)
+
+
+def lumen_kv_recover(load, alive, interrupted):
+    """interrupted: (holder, checkpointed size) per request.  Returns (assign, reuse, final loads)."""
+    la = np.ascontiguousarray(load, dtype=np.int64)
+    al = np.ascontiguousarray(alive, dtype=np.uint8)
+    n = len(interrupted)
+    ho = np.ascontiguousarray([h for h, _ in interrupted], dtype=np.int32)
+    sz = np.ascontiguousarray([s for _, s in interrupted], dtype=np.int64)
+    assign, reuse = np.zeros(n, dtype=np.int32), np.zeros(n, dtype=np.uint8)
+    final = np.zeros(la.size, dtype=np.int64)
+    rc = _lib().lumen_kv_recover(la.ctypes.data, al.ctypes.data, la.size,
+                                 ho.ctypes.data if n else None, sz.ctypes.data if n else None, n,
+                                 assign.ctypes.data if n else None, reuse.ctypes.data if n else None,
+                                 final.ctypes.data)
+    if rc:
+        raise LumenKVError(rc, "lumen_kv_recover")
+    return assign.tolist(), [bool(x) for x in reuse], final.tolist()
 
 
 def lumen_kv_plan_free(plan: Plan) -> None:
