@@ -40,22 +40,31 @@ def _free():
 
 
 def run_wave(G, pool, ck, geom, wave_reqs, running, hbuf, nbytes, n_pack_iters, pack_bufs,
-             s_restore, s_pack, t0):
+             s_restore, s_pack, t0, rings=None):
     """Restore one wave on s_restore while s_pack packs `n_pack_iters` 1-token deltas.
-    Returns the per-iteration running-request lists that were packed."""
+    rings = (restore ring, pack ring): both directions go through the two-stage path, as in
+    bench.py --workload cfg3.  Returns the per-iteration running-request lists that were packed."""
     import torch
     lk = G.lk
     rplan = lk.lumen_kv_plan_build(pool.geom, wave_reqs, lk.LUMEN_KV_VALIDATE_UNIQUE_DST,
                                    s_restore.cuda_stream)
     assert rplan.nbytes == nbytes
     packed = []
-    lk.lumen_kv_restore_unpack(rplan, pool.k_ptrs, pool.v_ptrs, hbuf.data_ptr(), nbytes,
-                               lk.LUMEN_KV_MEM_HOST_MAPPED, s_restore.cuda_stream)
+    if rings:
+        lk.lumen_kv_restore_unpack_staged(rplan, pool.k_ptrs, pool.v_ptrs, hbuf.data_ptr(), nbytes,
+                                          rings[0].stager, s_restore.cuda_stream)
+    else:
+        lk.lumen_kv_restore_unpack(rplan, pool.k_ptrs, pool.v_ptrs, hbuf.data_ptr(), nbytes,
+                                   lk.LUMEN_KV_MEM_HOST_MAPPED, s_restore.cuda_stream)
     for it in range(n_pack_iters):                      # a2-a4 on the second stream, meanwhile
         reqs = [(pt, te + t0 + it - 1, te + t0 + it) for pt, _, te in running]
         p = lk.lumen_kv_plan_build(pool.geom, reqs, 0, s_pack.cuda_stream)
-        lk.lumen_kv_checkpoint_pack(p, pool.k_ptrs, pool.v_ptrs, pack_bufs[it].data_ptr(),
-                                    p.nbytes, lk.LUMEN_KV_MEM_HOST_MAPPED, s_pack.cuda_stream)
+        if rings:
+            lk.lumen_kv_checkpoint_pack_staged(p, pool.k_ptrs, pool.v_ptrs, pack_bufs[it].data_ptr(),
+                                               p.nbytes, rings[1].stager, s_pack.cuda_stream)
+        else:
+            lk.lumen_kv_checkpoint_pack(p, pool.k_ptrs, pool.v_ptrs, pack_bufs[it].data_ptr(),
+                                        p.nbytes, lk.LUMEN_KV_MEM_HOST_MAPPED, s_pack.cuda_stream)
         p.close()
         packed.append(reqs)
     s_restore.synchronize(); s_pack.synchronize()
@@ -63,10 +72,12 @@ def run_wave(G, pool, ck, geom, wave_reqs, running, hbuf, nbytes, n_pack_iters, 
     return packed
 
 
-def test_cfg3_mid_size_whole_pool(G):
+@pytest.mark.parametrize("staged", [False, True])
+def test_cfg3_mid_size_whole_pool(G, staged):
     """Burst shape at a size the full oracle finishes in seconds: every byte of the pool after
     all waves, and every concurrent pack buffer, equal the oracle's."""
     import torch
+    rings = (G.StagingRing(1 << 20, 3), G.StagingRing(1 << 20, 3)) if staged else None
     b = cfg3_burst(MASTER_SEED + 3, L=2, N=768, n_running=8, n_interrupted=7, p_lo=40, p_hi=2500,
                    grow_iters=16)
     assert b.meta["n_waves"] >= 2
@@ -84,7 +95,7 @@ def test_cfg3_mid_size_whole_pool(G):
         hbuf.numpy().view(np.uint16)[:] = ref_ck
         pbufs = [G.pinned_buffer(len(b.running) * tok_bytes) for _ in range(iters)]
         packed = run_wave(G, pool, ck, b.geom, wave, b.running, hbuf, nbytes, iters, pbufs, s1, s2,
-                          t0=(wv * iters) % 12)
+                          t0=(wv * iters) % 12, rings=rings)
         for reqs, pb in zip(packed, pbufs):             # packs read only the running requests' pages
             assert np.array_equal(pb.numpy().view(np.uint16), oracle.pack(b.geom, K, V, reqs))
         oracle.unpack(b.geom, K, V, wave, ref_ck, check_overlap=True)
@@ -92,12 +103,14 @@ def test_cfg3_mid_size_whole_pool(G):
             assert np.array_equal(G.plane_to_np(t), ref), f"pool mismatch after wave {wv}"
 
 
-def test_cfg3_full_size_waves(G):
+@pytest.mark.parametrize("staged", [False, True])
+def test_cfg3_full_size_waves(G, staged):
     """configs[3] at full size: Qwen3-32B shape, N = 30,720 pages (120 GiB), 40 % occupied by
     64 running requests, 48 interrupted prefixes U{1024..32768} restored in waves from
     pinned host into a seeded shuffled free list, 1-token delta packs on a second stream."""
     import torch
     _free()
+    rings = (G.StagingRing(32 << 20, 3), G.StagingRing(32 << 20, 3)) if staged else None
     b = cfg3_burst()
     L, H, D, S, N = b.geom
     E = H * D
@@ -133,7 +146,7 @@ def test_cfg3_full_size_waves(G):
         tails = [(int(pt[(te - 1) // S]), te % S) for pt, _, te in wave if te % S]
         snaps = [[t.view(torch.int16).view(N, S, E)[pg, a:].clone() for t in planes] for pg, a in tails]
         packed = run_wave(G, pool, ck, b.geom, wave, b.running, hbuf, nbytes, iters, pbufs, s1, s2,
-                          t0=(wv * iters) % 48)
+                          t0=(wv * iters) % 48, rings=rings)
         # concurrent packs: whole buffers against the C oracle
         for reqs, pb in zip(packed, pbufs):
             assert np.array_equal(pb.numpy().view(np.uint16), oracle.pack(b.geom, Kh, Vh, reqs))

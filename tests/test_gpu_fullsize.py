@@ -92,8 +92,9 @@ def all_checksums(G, pool):
     return torch.stack([G.wdev.page_checksums(t, g.num_pages, page_bytes) for t in pool.planes()])
 
 
-def restore_and_check(G, pool, ck, w, buf, whole, nbytes):
-    """unpack into the fresh pages of the same pool; check targets, non-targets and guards."""
+def restore_and_check(G, pool, ck, w, buf, whole, nbytes, ring=None):
+    """unpack into the fresh pages of the same pool; check targets, non-targets and guards.
+    ring: restore through the two-stage path (lumen_kv_restore_unpack_staged)."""
     import torch
     L, H, D, S, N = w.geom
     E = H * D
@@ -111,7 +112,10 @@ def restore_and_check(G, pool, ck, w, buf, whole, nbytes):
     snaps = [[t.view(torch.int16).view(N, S, E)[pg, a:b].clone() for (pg, a, b) in partial]
              for t in pool.planes()]
     rplan = ck.plan(w.restore_reqs, unique_dst=True)
-    ck.unpack(rplan, buf)
+    if ring is not None:
+        ck.unpack_staged(rplan, buf, ring)
+    else:
+        ck.unpack(rplan, buf)
     torch.cuda.synchronize()
     after = all_checksums(G, pool)
     changed = (before != after).any(dim=0)
@@ -125,7 +129,7 @@ def restore_and_check(G, pool, ck, w, buf, whole, nbytes):
     rplan.close()
 
 
-@pytest.mark.parametrize("where", ["device", "host"])
+@pytest.mark.parametrize("where", ["device", "host", "staged"])
 def test_cfg1_full_size(G, where):
     """configs[1] as bench.py runs it: 60,000-page pool (146.5 GiB), 64 requests, 16-token deltas."""
     import torch
@@ -137,12 +141,17 @@ def test_cfg1_full_size(G, where):
         pytest.skip("not enough free HBM for the 146.5 GiB pool")
     pool = G.make_pool(w.geom, MASTER_SEED)
     ck = G.Checkpointer(pool)                                   # AUTO kernel, as in bench.py
+    ring = G.StagingRing(32 << 20, 3) if where == "staged" else None   # bench.py's e2e ring
     rng = substream(1, "cfg1_samples")
     for it in range(3):                                         # three iterations: alignment mix varies
         plan = ck.plan(G.lk.ReqArray(w.reqs))
         assert plan.nbytes == 167_772_160
-        whole, buf = G.alloc_buffer(plan.nbytes, where)
-        ck.pack(plan, buf)
+        whole, buf = G.alloc_buffer(plan.nbytes, "host" if ring else where)
+        if ring:
+            assert len(plan.chunks(32 << 20)) == 6
+            ck.pack_staged(plan, buf, ring)
+        else:
+            ck.pack(plan, buf)
         torch.cuda.synchronize()
         assert G.guards_intact(whole, plan.nbytes)
         sampled_pack_check(G, w.geom, w.reqs, MASTER_SEED, buf, 1500, rng)
@@ -153,14 +162,14 @@ def test_cfg1_full_size(G, where):
             ref = oracle.pack(w.geom, K, V, w.reqs)
             assert np.array_equal(G.buf_to_np(buf, plan.nbytes), ref)
             del K, V, keep, ref
-        restore_and_check(G, pool, ck, w, buf, whole, plan.nbytes)
+        restore_and_check(G, pool, ck, w, buf, whole, plan.nbytes, ring)
         plan.close()
         w = w.advanced(16)
     del pool
     _free()
 
 
-@pytest.mark.parametrize("where", ["device", "host"])
+@pytest.mark.parametrize("where", ["device", "host", "staged"])
 def test_cfg2_full_size(G, where):
     """configs[2]: 16 x 8k-token full-prefix pack (32 GiB) then restore into fresh pages."""
     import torch
@@ -170,16 +179,21 @@ def test_cfg2_full_size(G, where):
     ck = G.Checkpointer(pool)
     plan = ck.plan(w.reqs)
     assert plan.nbytes == 32 * 2**30 and plan.num_runs == 8192
+    ring = G.StagingRing(32 << 20, 3) if where == "staged" else None
     try:
-        whole, buf = G.alloc_buffer(plan.nbytes, where)
+        whole, buf = G.alloc_buffer(plan.nbytes, "host" if ring else where)
     except RuntimeError as e:
         pytest.skip(f"cannot allocate the 32 GiB {where} buffer: {e}")
-    ck.pack(plan, buf)
+    if ring:
+        assert len(plan.chunks(32 << 20)) == 1024               # 2 planes of 16 MiB per chunk
+        ck.pack_staged(plan, buf, ring)
+    else:
+        ck.pack(plan, buf)
     torch.cuda.synchronize()
     assert G.guards_intact(whole, plan.nbytes)
     sampled_pack_check(G, w.geom, w.reqs, MASTER_SEED + 2, buf, 1500, substream(2, "cfg2_samples"))
     gather_check(G, pool, w.reqs, buf, "pack")
-    restore_and_check(G, pool, ck, w, buf, whole, plan.nbytes)
+    restore_and_check(G, pool, ck, w, buf, whole, plan.nbytes, ring)
     plan.close()
     G.release(whole)
     del pool, buf, whole
@@ -216,10 +230,13 @@ def test_cfg4_token_granular_wave(G):
     _free()
 
 
-def test_cfg4_host_path_one_request(G):
-    """configs[4] to pinned host and back: one 128k-token request (32 GiB over the host link)."""
+@pytest.mark.parametrize("staged", [False, True])
+def test_cfg4_host_path_one_request(G, staged):
+    """configs[4] to pinned host and back: one 128k-token request (32 GiB over the host link),
+    zero-copy and through the two-stage path (128 planes x 8 token-range chunks)."""
     import torch
     _free()
+    ring = G.StagingRing(32 << 20, 3) if staged else None
     w = cfg4_longctx(wave_reqs=1, wave=1)
     pool = G.make_pool(w.geom, MASTER_SEED + 5)
     ck = G.Checkpointer(pool)
@@ -228,12 +245,19 @@ def test_cfg4_host_path_one_request(G):
         whole, buf = G.alloc_buffer(plan.nbytes, "host")
     except RuntimeError as e:
         pytest.skip(f"cannot pin 32 GiB: {e}")
-    ck.pack(plan, buf)
+    if ring:
+        assert len(plan.chunks(32 << 20)) == 1024
+        ck.pack_staged(plan, buf, ring)
+    else:
+        ck.pack(plan, buf)
     torch.cuda.synchronize()
     sampled_pack_check(G, w.geom, w.reqs, MASTER_SEED + 5, buf, 1000, substream(5, "cfg4h"))
     gather_check(G, pool, w.reqs, buf, "pack")
     rplan = ck.plan(w.restore_reqs, unique_dst=True)
-    ck.unpack(rplan, buf)
+    if ring:
+        ck.unpack_staged(rplan, buf, ring)
+    else:
+        ck.unpack(rplan, buf)
     torch.cuda.synchronize()
     gather_check(G, pool, w.restore_reqs, buf, "restore")
     assert G.guards_intact(whole, plan.nbytes)
