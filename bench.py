@@ -44,7 +44,7 @@ def parse_args():
     ap.add_argument("--steps", type=int, default=300)
     ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
-    ap.add_argument("--workload", choices=["cfg1", "cfg2", "cfg3", "cfg4"], default="cfg1")
+    ap.add_argument("--workload", choices=["cfg1", "cfg2", "cfg3", "cfg4", "chain"], default="cfg1")
     ap.add_argument("--kernel", choices=["auto", "warp", "bulk"], default="auto")
     ap.add_argument("--upload-descriptors", action="store_true",
                     help="LUMEN_KV_NO_INLINE: upload small plans to device memory too (A/B evidence)")
@@ -156,6 +156,8 @@ def oracle_sample(workload: str, seed: int):
     """A bounded sample of the workload on a sparse host pool: one step's pack + restore
     for cfg1 (2 x 160 MiB); for the 32 GiB configs the first request's first 4096 tokens."""
     from workloads.hostpool import sparse_host_pool
+    if workload == "chain":
+        workload = "cfg2"                  # the chain restores a cfg 2-shaped prefix
     if workload == "cfg3":
         # burst sample: one 1-token delta pack of the 64 running requests + the restore of the
         # first interrupted request's first 4096 tokens into its free-list pages
@@ -727,12 +729,191 @@ def run_cfg3(args):
     wdev.unpin(hbuf)
 
 
+def run_chain(args):
+    """The rows built after the hot path, measured:
+    page tags (f1), checkpoint-store append (f3), restore of the longest checkpointed prefix
+    straight out of the store's pinned arena through an explicit-layout plan and the two-stage
+    path (f3 + f2), and the controller's decisions (f4).  `value` = that restore's payload GB/s."""
+    import torch
+    import paper_2606_17787_b200 as lk
+    from paper_2606_17787_b200.pool import Checkpointer, KVPool, StagingRing, pinned_buffer
+    from workloads import MASTER_SEED, cfg2_qwen32b, substream
+    from workloads import device as wdev
+
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: there is no CPU path for --impl ours")
+    torch.cuda.set_device(rank_env()[2])
+    wdev.build()
+    rng = substream(MASTER_SEED, "chain")
+    S = 16
+
+    def gpu_ms(fn, reps):
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        for _ in range(3):
+            fn()
+        torch.cuda.synchronize()
+        a.record()
+        for _ in range(reps):
+            fn()
+        b.record()
+        torch.cuda.synchronize()
+        return a.elapsed_time(b) / reps
+
+    # ---- f1: tags of 64 requests x 131,072 tokens (524,288 pages), and of one 8k prompt ----
+    off = np.arange(65, dtype=np.int64) * 131072
+    tok = torch.randint(0, 151936, (int(off[-1]),), dtype=torch.int32, device="cuda")
+    n_pages = lk.lumen_kv_tags_num_pages(off, S)
+    d_tags = torch.empty((n_pages, 2), dtype=torch.int64, device="cuda")
+    ms_big = gpu_ms(lambda: lk.lumen_kv_page_tags(tok.data_ptr(), off, S, d_tags.data_ptr(), n_pages,
+                                                  torch.cuda.current_stream().cuda_stream), 50)
+    ms_8k = gpu_ms(lambda: lk.lumen_kv_page_tags(tok.data_ptr(), [0, 8192], S, d_tags.data_ptr(), n_pages,
+                                                 torch.cuda.current_stream().cuda_stream), 200)
+    tag_bytes = int(off[-1]) * 4 + n_pages * 16
+    tags = {"pages": n_pages, "ms": ms_big, "pages_per_s": n_pages / ms_big * 1e3,
+            "GBps": tag_bytes / ms_big / 1e6, "one_8k_prompt_us": ms_8k * 1e3,
+            "note": "64 B of token IDs per page against 4 MiB of KV: launch-bound at request sizes"}
+
+    # ---- f3: store append (host memcpy into the arena), 2 GiB prefill checkpoint -----------
+    w = cfg2_qwen32b(MASTER_SEED, N=20000, n_reqs=4, prompt=8192)
+    L, H, D, _, N = w.geom
+    tokb = 2 * L * H * D * 2
+    n_tok, tail, n_delta = 8192, 16, 12
+    first = n_tok - tail * n_delta
+    arena = wdev.pinned_exact(4 * (n_tok + 64) * tokb)
+    src = torch.empty(first * tokb, dtype=torch.uint8).random_(0, 255)
+    no_tags = np.zeros(0, dtype=lk.TAG_DTYPE)
+    append = {}
+    for threads in (1, 4, 16):
+        st = lk.Store(arena.data_ptr(), arena.numel(), tokb, S, copy_threads=threads)
+        st.reserve(0, n_tok)
+        t0 = time.perf_counter()
+        st.append(0, 0, first, src.data_ptr(), src.numel(), no_tags)
+        append[f"{threads}_threads_GBps"] = src.numel() / (time.perf_counter() - t0) / 1e9
+        st.close()
+    del src
+
+    # ---- chain: incremental packs -> store -> lookup -> restore out of the arena ----------------
+    pool = KVPool(L, H, D, S, N)
+    for i, t in enumerate(pool.planes()):
+        wdev.fill_plane(t, MASTER_SEED, i)
+    ck = Checkpointer(pool)
+    ring, ring2 = StagingRing(32 << 20, 3), StagingRing(32 << 20, 3)
+    stage = pinned_buffer(first * tokb)
+    st = lk.Store(arena.data_ptr(), arena.numel(), tokb, S, copy_threads=16)
+    hist = [rng.integers(0, 151936, size=n_tok + 7).astype(np.int32) for _ in w.reqs]
+    h_tags = torch.empty((n_tok // S + 2, 2), dtype=torch.int64, device="cuda")
+
+    def tags_of(tokens):
+        d = torch.from_numpy(np.ascontiguousarray(tokens)).cuda()
+        n = lk.lumen_kv_tags_num_pages([0, tokens.size], S)
+        lk.lumen_kv_page_tags(d.data_ptr(), [0, tokens.size], S, h_tags.data_ptr(), n, 0)
+        torch.cuda.synchronize()
+        return h_tags[:n].cpu().numpy().copy().view(lk.TAG_DTYPE).reshape(-1)
+
+    t_pack = time.perf_counter()
+    for rid, (pt, _, _) in enumerate(w.reqs):
+        st.reserve(rid, n_tok + 64)
+        cuts = [0, first] + [first + tail * (i + 1) for i in range(n_delta)]
+        cuts[-1] -= 3                                          # the last delta ends inside a page
+        for tb, te in zip(cuts, cuts[1:]):
+            plan = ck.plan([(pt, tb, te)])
+            ck.pack_staged(plan, stage, ring)
+            torch.cuda.synchronize()
+            tg = tags_of(hist[rid][:te])
+            st.append(rid, tb, te, stage.data_ptr(), plan.nbytes, tg[(tg["end_pos"] > tb) & (tg["end_pos"] <= te)])
+            plan.close()
+    t_pack = time.perf_counter() - t_pack
+    t_look = time.perf_counter()
+    reqs, lays, restored = [], [], 0
+    for rid, (pt_new, _, _) in enumerate(w.restore_reqs):
+        prefix = st.lookup(rid, tags_of(hist[rid]))
+        restored += prefix
+        for s_ in st.segments(rid, prefix):
+            reqs.append((pt_new, int(s_["t_begin"]), int(s_["t_end"])))
+            lays.append((int(s_["buf_offset"]), int(s_["plane_stride_tokens"])))
+    t_look = time.perf_counter() - t_look
+    link = memcpy_peaks(torch)
+    sampler = ClockSampler(rank_env()[2])
+    stream = torch.cuda.Stream()
+    K, W = max(1, min(args.steps, 10)), max(3, min(args.warmup, 5))
+    payload = restored * tokb
+
+    def restore_once():
+        rplan = lk.lumen_kv_plan_build(pool.geom, reqs, lk.LUMEN_KV_VALIDATE_UNIQUE_DST,
+                                       stream.cuda_stream, layouts=lays)
+        lk.lumen_kv_restore_unpack_staged(rplan, pool.k_ptrs, pool.v_ptrs, arena.data_ptr(),
+                                          arena.numel(), ring2.stager, stream.cuda_stream)
+        n = len(rplan.chunks(32 << 20))
+        rplan.close()
+        return n
+
+    for _ in range(W):
+        n_chunks = restore_once()
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    sampler.start()
+    a.record(stream)
+    for _ in range(K):
+        restore_once()
+    b.record(stream)
+    torch.cuda.synchronize()
+    sampler.stop()
+    ms = a.elapsed_time(b) / K
+    value = payload / ms / 1e6
+
+    # ---- f4: controller decisions --------------------------------------------------------------
+    Wk = 64
+    q = rng.random(Wk).tolist()
+    held = [[int(x) for x in rng.integers(1, 80, size=int(rng.integers(0, 30)))] for _ in range(Wk)]
+    avail = [int(x) for x in rng.integers(0, 160, size=Wk)]
+    t0 = time.perf_counter()
+    for i in range(2000):
+        lk.lumen_kv_choose_holder(q, held, avail, i % Wk, 20, 1.0, 26.0)
+    t_choose = (time.perf_counter() - t0) / 2000
+    alive = [i % 8 != 0 for i in range(Wk)]
+    inter = [(int(rng.integers(0, Wk)), int(rng.integers(0, 32768))) for _ in range(2000)]
+    t0 = time.perf_counter()
+    lk.lumen_kv_recover([int(x) for x in rng.integers(0, 40, size=Wk)], alive, inter)
+    t_recover = time.perf_counter() - t0
+
+    line = {
+        "metric": "kv_pack_restore_payload_GBps", "value": value, "unit": "GB/s", "n_gpus": 1,
+        "steps": K, "warmup": W, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "u16", "data": "synthetic",
+        "config": {"workload": ("checkpoint chain (SURVEY.md 8(f)): Qwen3-32B shape, 4 requests x 8,192 tokens "
+                                "checkpointed as a prefill delta + 12 decode deltas of 16 tokens into a pinned "
+                                "store arena; restore of the longest checkpointed prefix (page aligned, ends "
+                                "inside the last delta) out of the arena via lumen_kv_plan_build_layout + "
+                                "lumen_kv_restore_unpack_staged"),
+                   "restored_tokens": restored, "segments": len(reqs), "chunks": n_chunks,
+                   "l2": "inputs larger than L2: 8 GiB read over the host link per step"},
+        "tokens_per_s": value * 1e9 / tokb,
+        "roofline": {"bound": "host_link", "kernel": "lumen_kv_restore_unpack_staged (copy engine H2D + kv_copy_warp)",
+                     "achieved": value, "peak": link["h2d"], "unit": "GB/s", "frac": value / link["h2d"],
+                     "traffic": None, "peak_source": "pinned cudaMemcpyAsync H2D, 1 GiB, best of 10, this run"},
+        "e2e": {"value": value, "unit": "GB/s", "h2d_bytes_per_step": payload, "d2h_bytes_per_step": 0,
+                "note": "the timed region is the H2D restore out of the pinned arena"},
+        "page_tags": tags, "store_append": append,
+        "checkpointing": {"s_total": t_pack, "deltas": 13 * len(w.reqs),
+                          "note": "staged pack -> pinned staging -> store.append, incl. tags, synchronous per delta"},
+        "lookup_s": t_look,
+        "controller": {"choose_holder_us": t_choose * 1e6, "workers": Wk,
+                       "recover_2000_interrupted_ms": t_recover * 1e3,
+                       "note": "through the ctypes binding (marshalling included)"},
+        "gpu_launches": K * n_chunks, "clocks": sampler.summary(),
+    }
+    print(json.dumps(line), flush=True)
+    wdev.unpin(arena)
+
+
 def main():
     args = parse_args()
     if args.impl == "reference":
         run_reference(args)
     elif args.workload == "cfg3":
         run_cfg3(args)
+    elif args.workload == "chain":
+        run_chain(args)
     else:
         run_ours(args)
 

@@ -592,7 +592,7 @@ const char* lumen_kv_strerror(int status) {
         case LUMEN_KV_ERANGE: return "page index or token range outside the page table / pool";
         case LUMEN_KV_EOVERLAP: return "a pool token slot is addressed more than once";
         case LUMEN_KV_ESIZE: return "buffer smaller than the plan's bytes";
-        case LUMEN_KV_ENOMEM: return "out of host or device memory for descriptors";
+        case LUMEN_KV_ENOMEM: return "out of memory (descriptors), or no room for the reservation in the store arena";
         case LUMEN_KV_ECUDA: return "CUDA runtime error (see lumen_kv_last_cuda_error)";
         default: return "unknown status";
     }
