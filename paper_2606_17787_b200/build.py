@@ -16,8 +16,8 @@ PKG = Path(__file__).resolve().parent
 ROOT = PKG.parent
 CSRC = PKG / "csrc"
 SO = PKG / "liblumen_kv.so"
-SOURCES = [CSRC / "lib.cu", CSRC / "kernels.cu", CSRC / "tags.cu", CSRC / "plan.cpp", CSRC / "store.cpp", CSRC / "placement.cpp"]
-HEADERS = [CSRC / "plan.hpp", CSRC / "kernels.hpp", ROOT / "include" / "lumen_kv.h"]
+SOURCES = [CSRC / "lib.cu", CSRC / "stager.cu", CSRC / "kernels.cu", CSRC / "tags.cu", CSRC / "plan.cpp", CSRC / "store.cpp", CSRC / "placement.cpp"]
+HEADERS = [CSRC / "plan.hpp", CSRC / "kernels.hpp", CSRC / "internal.hpp", ROOT / "include" / "lumen_kv.h"]
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",

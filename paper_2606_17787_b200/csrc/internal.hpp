@@ -1,0 +1,46 @@
+// Internals shared by the C entry points (lib.cu) and the two-stage host path (stager.cu).
+// Not part of the public ABI.
+#pragma once
+#include <cuda_runtime.h>
+
+#include <cstdint>
+#include <vector>
+
+#include "lumen_kv.h"
+#include "plan.hpp"
+
+namespace lumen {
+struct Blob;   // descriptor blob of the arena (lib.cu)
+
+// records the CUDA error for lumen_kv_last_cuda_error() and returns LUMEN_KV_ECUDA
+int cuda_fail(cudaError_t e);
+}  // namespace lumen
+
+struct lumen_kv_plan {
+    lumen::HostPlan hp;        // runs/reqs vectors are released after upload unless host-only
+    lumen::Blob* blob = nullptr;
+    const lumen::RunDesc* h_runs = nullptr;   // inside blob->host
+    const lumen::ReqDesc* h_reqs = nullptr;
+    const lumen::RunDesc* d_runs = nullptr;   // inside blob->dev
+    const lumen::ReqDesc* d_reqs = nullptr;
+    int64_t n_runs = 0;
+    int32_t n_reqs = 0;
+    uint32_t flags = 0;
+    bool inline_desc = false;  // small plan: descriptors stay in hp and travel as kernel parameters
+};
+
+namespace lumen {
+
+// validation shared by the one-shot and the staged calls: interleaves the plane pointers
+// (K0,V0,K1,V1,..) into `planes`
+int gather_planes(const lumen_kv_plan* plan, const void* const* k_planes,
+                  const void* const* v_planes, std::vector<const void*>* planes);
+
+// Enqueue runs [ra, rb) x planes [p0, p1) of the plan.  `buf` is the address that byte 0 of
+// the plan's checkpoint buffer would have (for a staging slot: slot base - chunk offset, so
+// it may lie outside any allocation; only bytes of the chunk are ever addressed).
+int launch_part(const lumen_kv_plan* plan, const std::vector<const void*>& planes, uintptr_t buf,
+                bool buf_is_host, cudaStream_t stream, bool pack, int64_t ra, int64_t rb,
+                int32_t p0, int32_t p1);
+
+}  // namespace lumen

@@ -457,3 +457,42 @@ def test_layout_parity(G, kernel):
             assert np.array_equal(G.plane_to_np(t), ref), f"layout unpack mismatch ({mode})"
         plan.close(); rplan.close()
         done += 1
+
+
+def test_host_threads_share_the_library(G):
+    """The library holds no per-call global state: four host threads build, pack, restore and
+    free their own plans on their own streams at once (uploaded descriptors, so the arena's
+    cache is shared); every thread's bytes equal the oracle's."""
+    import threading
+    import torch
+    lk = G.lk
+    w = cfg1_qwen14b(L=2, N=2048, n_reqs=16, grow_iters=8, median=150, hi=400, lo=20)
+    K, V = G.host_planes(w.geom, 77)
+    pool = G.make_pool(w.geom, 77)
+    errors = []
+
+    def worker(tid):
+        try:
+            torch.cuda.set_device(0)
+            stream = torch.cuda.Stream()
+            flags = lk.LUMEN_KV_NO_INLINE if tid % 2 else 0
+            for it in range(12):
+                ww = w.advanced(16 * (1 + (tid + it) % 6))
+                ref = oracle.pack(ww.geom, K, V, ww.reqs)
+                plan = lk.lumen_kv_plan_build(pool.geom, ww.reqs, flags, stream.cuda_stream)
+                buf = torch.empty(plan.nbytes, dtype=torch.uint8, device="cuda")
+                lk.lumen_kv_checkpoint_pack(plan, pool.k_ptrs, pool.v_ptrs, buf.data_ptr(), plan.nbytes,
+                                            lk.LUMEN_KV_MEM_DEVICE, stream.cuda_stream)
+                plan.close()                                # freed while the kernel may still run
+                stream.synchronize()
+                if not np.array_equal(G.buf_to_np(buf, ref.size * 2), ref):
+                    errors.append((tid, it))
+        except Exception as e:                              # noqa: BLE001
+            errors.append((tid, repr(e)))
+
+    threads = [threading.Thread(target=worker, args=(t,)) for t in range(4)]
+    for t in threads:
+        t.start()
+    for t in threads:
+        t.join(timeout=120)
+    assert not errors and not any(t.is_alive() for t in threads)
