@@ -496,3 +496,24 @@ def test_host_threads_share_the_library(G):
     for t in threads:
         t.join(timeout=120)
     assert not errors and not any(t.is_alive() for t in threads)
+
+
+@pytest.mark.parametrize("kernel", ["warp", "warp_upload", "bulk"])
+def test_many_planes_and_huge_rows(G, kernel):
+    """Edge geometries: 2L = 260 planes (more than the 256 plane pointers one launch carries, so
+    the plane base of the second launch matters) and a 64 KiB row (one row is larger than the
+    32 KiB run limit and than the TMA ring slot: the bulk kernel hands over to the SIMT one)."""
+    import workloads.gen as gen
+    rng = substream(7, "edge")
+    perm = rng.permutation(64)
+    reqs = [(perm[0:5].astype(np.int32), 3, 18), (perm[5:8].astype(np.int32), 0, 9)]
+    rreqs = [(perm[8:13].astype(np.int32), 3, 18), (perm[13:16].astype(np.int32), 0, 9)]
+    w = gen.Workload("many_planes", (130, 1, 8, 4, 64), reqs, rreqs)
+    run_case(G, w, kernel, "device")
+    run_case(G, w, kernel, "host")
+    assert run_staged_case(G, w, 4096, 3, kernel=kernel) >= 2
+    reqs = [(perm[0:3].astype(np.int32), 1, 5)]
+    rreqs = [(perm[3:6].astype(np.int32), 1, 5)]
+    w = gen.Workload("huge_rows", (1, 64, 512, 2, 8), reqs, rreqs)      # row = 64 KiB
+    run_case(G, w, kernel, "device")
+    run_staged_case(G, w, 1 << 16, 2, kernel=kernel)
