@@ -512,6 +512,7 @@ def test_many_planes_and_huge_rows(G, kernel):
     run_case(G, w, kernel, "device")
     run_case(G, w, kernel, "host")
     assert run_staged_case(G, w, 4096, 3, kernel=kernel) >= 2
+    perm = rng.permutation(8)
     reqs = [(perm[0:3].astype(np.int32), 1, 5)]
     rreqs = [(perm[3:6].astype(np.int32), 1, 5)]
     w = gen.Workload("huge_rows", (1, 64, 512, 2, 8), reqs, rreqs)      # row = 64 KiB
