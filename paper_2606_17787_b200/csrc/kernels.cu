@@ -148,6 +148,58 @@ kv_copy_warp(const __grid_constant__ PlaneTable planes, const __grid_constant__ 
         if (i + u * 32 < nvec) st_stream16(dst + u * 512, v[u]);
 }
 
+// 32-byte variant, the default whenever every address is a multiple of 32: sm_100 has 256-bit
+// global loads / stores (LDG.E.256 / STG.E.256).  A task is UNROLL * 1 KiB = 4 KiB per warp, so
+// half the CTAs and half the memory instructions per byte: +1.7 % on cfg 1, +2 % on cfg 4
+// (DESIGN.md section 6.1).  An L2::evict_first priority on both sides was measured too: no gain.
+struct V8 {
+    uint32_t a[8];
+};
+__device__ __forceinline__ V8 ld_stream32(const void* p) {
+    V8 v;
+    asm volatile("ld.global.L1::no_allocate.v8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                 : "=r"(v.a[0]), "=r"(v.a[1]), "=r"(v.a[2]), "=r"(v.a[3]), "=r"(v.a[4]),
+                   "=r"(v.a[5]), "=r"(v.a[6]), "=r"(v.a[7])
+                 : "l"(p)
+                 : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_stream32(void* p, const V8& v) {
+    asm volatile("st.global.L1::no_allocate.v8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"l"(p),
+                 "r"(v.a[0]), "r"(v.a[1]), "r"(v.a[2]), "r"(v.a[3]), "r"(v.a[4]), "r"(v.a[5]),
+                 "r"(v.a[6]), "r"(v.a[7])
+                 : "memory");
+}
+
+template <int UNROLL, class Desc>
+__global__ void __launch_bounds__(kWarpsPerCta * 32)
+kv_copy_warp32(const __grid_constant__ PlaneTable planes, const __grid_constant__ Desc desc,
+               int64_t n_runs, char* buf, uint32_t row_bytes, int32_t plane0, int sub_shift,
+               int pack) {
+    pdl_launch_dependents();
+    const int lane = threadIdx.x & 31;
+    const int64_t task = static_cast<int64_t>(blockIdx.x) * kWarpsPerCta + (threadIdx.x >> 5);
+    const int64_t run = task >> sub_shift;
+    if (run >= n_runs) return;
+    const uint32_t sub = static_cast<uint32_t>(task & ((int64_t{1} << sub_shift) - 1));
+    if (!Desc::kInline) pdl_wait();
+    const Item it = decode_item(desc, run, planes.p[blockIdx.y], plane0 + blockIdx.y, buf,
+                                row_bytes);
+    if (Desc::kInline) pdl_wait();
+    const uint32_t nvec = it.bytes >> 5;
+    const uint32_t i = sub * (UNROLL * 32) + lane;
+    if (sub * (UNROLL * 32) >= nvec) return;
+    const char* src = (pack ? it.pool : it.buf) + (static_cast<size_t>(i) << 5);
+    char* dst = (pack ? it.buf : it.pool) + (static_cast<size_t>(i) << 5);
+    V8 v[UNROLL];
+#pragma unroll
+    for (int u = 0; u < UNROLL; ++u)
+        if (i + u * 32 < nvec) v[u] = ld_stream32(src + u * 1024);
+#pragma unroll
+    for (int u = 0; u < UNROLL; ++u)
+        if (i + u * 32 < nvec) st_stream32(dst + u * 1024, v[u]);
+}
+
 // ---------------------------------------------------------------------------------
 // TMA kernel: persistent single-warp CTAs, 1-D bulk copies through a shared ring
 // ---------------------------------------------------------------------------------
@@ -351,6 +403,23 @@ struct WarpLaunch {
 };
 
 int g_pdl = 1;   // LUMEN_KV_PDL=0 launches without the programmatic attribute (A/B evidence)
+int g_wide = 1;   // LUMEN_KV_WIDE=0 keeps the 16-byte kernel even where 32-byte accesses are legal
+constexpr int kWideUnroll = 4;
+
+template <class Desc>
+cudaError_t launch_warp32(const PlaneTable& pt, const Desc& d, const WarpLaunch& w) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = w.grid;
+    cfg.blockDim = dim3(kWarpsPerCta * 32, 1, 1);
+    cfg.stream = w.stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = g_pdl ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, kv_copy_warp32<kWideUnroll, Desc>, pt, d, w.n_runs, w.buf,
+                              w.row_bytes, w.plane0, w.sub_shift, w.pack);
+}
 
 template <int UNROLL, class Desc>
 cudaError_t launch_warp(const PlaneTable& pt, const Desc& d, const WarpLaunch& w) {
@@ -391,6 +460,8 @@ cudaError_t preload_all() {
     if (e == cudaSuccess) e = preload(kv_copy_warp<4, InlineDesc>, false);
     if (e == cudaSuccess) e = preload(kv_copy_warp<8, GlobalDesc>, false);
     if (e == cudaSuccess) e = preload(kv_copy_warp<8, InlineDesc>, false);
+    if (e == cudaSuccess) e = preload(kv_copy_warp32<4, GlobalDesc>, false);
+    if (e == cudaSuccess) e = preload(kv_copy_warp32<4, InlineDesc>, false);
     if (e == cudaSuccess) e = preload_bulk<3>();
     if (e == cudaSuccess) e = preload_bulk<4>();
     if (e == cudaSuccess) e = preload_bulk<6>();
@@ -419,6 +490,7 @@ cudaError_t launch_kv_copy(const CopyArgs& a) {
     std::call_once(once, [] {
         if (const char* e = getenv("LUMEN_KV_WARP_UNROLL")) g_warp_unroll = (atoi(e) == 8) ? 8 : 4;
         if (const char* e = getenv("LUMEN_KV_PDL")) g_pdl = atoi(e) ? 1 : 0;
+        if (const char* e = getenv("LUMEN_KV_WIDE")) g_wide = atoi(e) ? 1 : 0;
         if (const char* e = getenv("LUMEN_KV_HOST_KERNEL"))
             g_host_kernel = (e[0] == 'w') ? kKernelWarp : kKernelBulk;
         if (const char* e = getenv("LUMEN_KV_HOST_CTAS")) g_host_ctas = atoi(e);
@@ -451,7 +523,13 @@ cudaError_t launch_kv_copy(const CopyArgs& a) {
             }
         } else {
             // sub-chunks per item: smallest power of two covering the longest run
-            const int64_t sub_bytes = int64_t{512} * g_warp_unroll;
+            // 32-byte accesses need every address to be a multiple of 32
+            bool wide = g_wide != 0 && a.pool_align32 &&
+                        (reinterpret_cast<uintptr_t>(a.buf) & 31) == 0;
+            for (int i = 0; wide && i < np; ++i)
+                wide = (reinterpret_cast<uintptr_t>(pt.p[i]) & 31) == 0;
+            const int64_t sub_bytes = wide ? int64_t{1024} * kWideUnroll
+                                           : int64_t{512} * g_warp_unroll;
             int sub_shift = 0;
             while ((sub_bytes << sub_shift) < item_max) ++sub_shift;
             const int64_t tasks = a.n_runs << sub_shift;
@@ -470,10 +548,12 @@ cudaError_t launch_kv_copy(const CopyArgs& a) {
                 InlineDesc d;   // unused tail entries are never indexed (run < n_runs)
                 std::memcpy(d.runs, a.runs, static_cast<size_t>(a.n_runs) * sizeof(RunDesc));
                 std::memcpy(d.reqs, a.reqs, static_cast<size_t>(a.n_reqs) * sizeof(ReqDesc));
-                e = (g_warp_unroll == 4) ? launch_warp<4>(pt, d, w) : launch_warp<8>(pt, d, w);
+                e = wide ? launch_warp32(pt, d, w)
+                         : (g_warp_unroll == 4) ? launch_warp<4>(pt, d, w) : launch_warp<8>(pt, d, w);
             } else {
                 const GlobalDesc d{a.runs, a.reqs};
-                e = (g_warp_unroll == 4) ? launch_warp<4>(pt, d, w) : launch_warp<8>(pt, d, w);
+                e = wide ? launch_warp32(pt, d, w)
+                         : (g_warp_unroll == 4) ? launch_warp<4>(pt, d, w) : launch_warp<8>(pt, d, w);
             }
         }
         if (e != cudaSuccess) return e;

@@ -26,6 +26,7 @@ struct CopyArgs {
     int64_t n_runs = 0;
     int64_t row_bytes = 0;
     int32_t max_count = 0;           // longest run in tokens
+    bool pool_align32 = false;       // row and page stride are multiples of 32 bytes
     const void* const* planes = nullptr;  // HOST array of n_planes device pointers (K0,V0,K1,V1,..)
     int32_t n_planes = 0;
     int32_t plane_base = 0;          // absolute index of planes[0] (a launch over a plane sub-range)

@@ -175,6 +175,7 @@ int launch_part(const lumen_kv_plan* plan, const std::vector<const void*>& plane
     a.n_reqs = plan->n_reqs;
     a.row_bytes = plan->hp.row_bytes;
     a.max_count = plan->hp.max_count;
+    a.pool_align32 = plan->hp.row_bytes % 32 == 0 && plan->hp.page_stride % 32 == 0;
     a.planes = planes.data() + p0;
     a.n_planes = p1 - p0;
     a.plane_base = p0;

@@ -518,3 +518,38 @@ def test_many_planes_and_huge_rows(G, kernel):
     w = gen.Workload("huge_rows", (1, 64, 512, 2, 8), reqs, rreqs)      # row = 64 KiB
     run_case(G, w, kernel, "device")
     run_staged_case(G, w, 1 << 16, 2, kernel=kernel)
+
+
+def test_alignment_falls_back_to_16_byte_accesses(G):
+    """The default SIMT kernel moves 32 bytes per access; a buffer, plane or page stride that is
+    only 16-byte aligned must take the 16-byte kernel and still be bit-exact."""
+    import torch
+    lk = G.lk
+    w = cfg1_qwen14b(L=2, N=512, n_reqs=8, grow_iters=2, median=100, hi=256, lo=20)
+    L, H, D, S, N = w.geom
+    K, V = G.host_planes(w.geom, 5)
+    ref = oracle.pack(w.geom, K, V, w.reqs)
+    pool = G.make_pool(w.geom, 5)
+    ck = G.Checkpointer(pool)
+    plan = ck.plan(w.reqs)
+    for shift in (16, 32, 48):                                # buffer base = 256-aligned + shift
+        raw = torch.full((plan.nbytes + 4096,), 0xA5, dtype=torch.uint8, device="cuda")
+        view = raw[shift: shift + plan.nbytes]
+        ck.pack(plan, view)
+        torch.cuda.synchronize()
+        assert np.array_equal(G.buf_to_np(view, plan.nbytes), ref)
+        assert bool((raw[:shift] == 0xA5).all()) and bool((raw[shift + plan.nbytes:] == 0xA5).all())
+    # page stride that is a multiple of 16 but not of 32: planes with 16 bytes of padding per page
+    row = H * D * 2
+    stride = S * row + 16
+    geom = lk.make_geom(L, H, D, S, N, page_stride_bytes=stride)
+    planes = [torch.zeros(N * stride, dtype=torch.uint8, device="cuda") for _ in range(2 * L)]
+    for p, src in zip(planes, pool.planes()):
+        p.view(N, stride)[:, : S * row] = src.view(torch.uint8).view(N, S * row)
+    kp = lk.plane_ptrs([planes[2 * l].data_ptr() for l in range(L)], L)
+    vp = lk.plane_ptrs([planes[2 * l + 1].data_ptr() for l in range(L)], L)
+    splan = lk.lumen_kv_plan_build(geom, w.reqs, 0, 0)
+    out = torch.empty(splan.nbytes, dtype=torch.uint8, device="cuda")
+    lk.lumen_kv_checkpoint_pack(splan, kp, vp, out.data_ptr(), splan.nbytes, lk.LUMEN_KV_MEM_DEVICE, 0)
+    torch.cuda.synchronize()
+    assert np.array_equal(G.buf_to_np(out, splan.nbytes), ref)
