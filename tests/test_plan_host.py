@@ -414,3 +414,28 @@ def test_unique_dst_is_slot_granular(lk):
             assert e.value.status == lk.LUMEN_KV_EOVERLAP
         # another request using the other half of the same physical page
         lk.lumen_kv_plan_build(g, [(pt, 0, 2), (np.array([7], np.int32), 2, 4)], U).close()
+
+
+def test_maximum_sizes_are_64_bit_clean(lk):
+    """Largest legal geometry: N = 2^31 - 1 pages of 32 KiB (a 64 TiB plane), page indices and
+    token positions near the top, 128k-token ranges: offsets never wrap (SURVEY 7.3 hard part 5)."""
+    N = (1 << 31) - 1
+    g = lk.make_geom(64, 8, 128, 16, N)
+    top = np.array([N - 1, 0, N - 2, 12345], dtype=np.int32)
+    p = lk.lumen_kv_plan_build(g, [(top, 5, 60)], lk.LUMEN_KV_HOST_ONLY | lk.LUMEN_KV_VALIDATE_UNIQUE_DST)
+    runs = [p.run(i) for i in range(p.num_runs)]
+    assert [(r.src_slot, r.dst_token, r.count) for r in runs] == [
+        ((N - 1) * 16 + 5, 0, 11), (0, 11, 16), ((N - 2) * 16, 27, 16), (12345 * 16, 43, 12)]
+    assert p.nbytes == 55 * 128 * 2048
+    # a 128k-token request in a token-granular pool of 2^31 - 1 slots, buffer offsets beyond 2^40
+    g1 = lk.make_geom(64, 8, 128, 1, N)
+    rng = substream(9, "max")
+    pt = rng.integers(0, N, size=131072, dtype=np.int64).astype(np.int32)
+    pt = np.unique(pt)[:100000].astype(np.int32)
+    big = lk.lumen_kv_plan_build(g1, [(pt, 0, pt.size)] * 1 + [(pt[::-1].copy(), 0, 7)],
+                                 lk.LUMEN_KV_HOST_ONLY, layouts=[(1 << 41, pt.size), (0, 7)])
+    assert big.req_offset(0) == 1 << 41 and big.nbytes == (1 << 41) + (127 * pt.size + pt.size) * 2048
+    r = big.run(99999)
+    assert r.src_slot == int(pt[99999]) and r.dst_token == 99999 and r.count == 1
+    with pytest.raises(lk.LumenKVError):                     # N = 2^31 is one too many
+        lk.lumen_kv_plan_build(lk.make_geom(1, 1, 8, 1, 1 << 31), [], lk.LUMEN_KV_HOST_ONLY)
