@@ -51,6 +51,7 @@ def build(force: bool = False, verbose: bool = False) -> Path:
         sys.stderr.write(res.stdout + res.stderr)
         raise RuntimeError("nvcc failed building liblumen_kv.so")
     log = (" ".join(cmd) + "\n" + res.stdout + res.stderr).replace(str(tmp), str(SO))
+    log = "\n".join(l for l in log.split("\n") if "Compile time" not in l)   # keep the log deterministic
     (PKG / "build_ptxas.log").write_text(log.replace(str(ROOT) + "/", ""))
     if verbose:
         print(res.stdout + res.stderr)
