@@ -68,3 +68,35 @@ def unpack(geom, k_planes, v_planes, reqs, B) -> None:
         for l in range(L):
             k_planes[l].reshape(N * S, E)[ids] = blk[l, 0]
             v_planes[l].reshape(N * S, E)[ids] = blk[l, 1]
+
+
+def pack_layout(geom, k_planes, v_planes, reqs, layouts, B: np.ndarray) -> None:
+    """Explicit buffer layout (checkpoint store), second restatement:
+    request r's plane p occupies B[off_r + p*stride_r*E : ... + n_r*E] as a strided 3-D view."""
+    L, H, D, S, N = (int(x) for x in geom)
+    E = H * D
+    for (pt, tb, te), (off, stride) in zip(reqs, layouts):
+        n = int(te) - int(tb)
+        if n == 0:
+            continue
+        ids = slot_ids(S, pt, tb, te)
+        view = np.lib.stride_tricks.as_strided(B[off:], shape=(2 * L, n, E),
+                                               strides=(stride * E * 2, E * 2, 2))
+        for l in range(L):
+            view[2 * l] = k_planes[l].reshape(N * S, E)[ids]
+            view[2 * l + 1] = v_planes[l].reshape(N * S, E)[ids]
+
+
+def unpack_layout(geom, k_planes, v_planes, reqs, layouts, B: np.ndarray) -> None:
+    L, H, D, S, N = (int(x) for x in geom)
+    E = H * D
+    for (pt, tb, te), (off, stride) in zip(reqs, layouts):
+        n = int(te) - int(tb)
+        if n == 0:
+            continue
+        ids = slot_ids(S, pt, tb, te)
+        view = np.lib.stride_tricks.as_strided(B[off:], shape=(2 * L, n, E),
+                                               strides=(stride * E * 2, E * 2, 2))
+        for l in range(L):
+            k_planes[l].reshape(N * S, E)[ids] = view[2 * l]
+            v_planes[l].reshape(N * S, E)[ids] = view[2 * l + 1]

@@ -553,3 +553,32 @@ def test_alignment_falls_back_to_16_byte_accesses(G):
     lk.lumen_kv_checkpoint_pack(splan, kp, vp, out.data_ptr(), splan.nbytes, lk.LUMEN_KV_MEM_DEVICE, 0)
     torch.cuda.synchronize()
     assert np.array_equal(G.buf_to_np(out, splan.nbytes), ref)
+
+
+@pytest.mark.parametrize("elem_bytes", [1, 4])
+def test_other_element_widths(G, elem_bytes):
+    """The payload is opaque: an fp8 KV cache (1-byte elements) or a 4-byte one is the same byte
+    permutation.  The library gets (H, D, elem_bytes); the oracle sees the same rows as 16-bit
+    words (E = H*D*elem_bytes/2) -- results must be identical bytes."""
+    import torch
+    lk = G.lk
+    L, H, D, S, N = 3, 4, 32, 16, 256
+    E16 = H * D * elem_bytes // 2
+    geom16 = (L, 1, E16, S, N)                                  # what the oracle is told
+    w = cfg1_qwen14b(L=L, H=1, D=E16, S=S, N=N, n_reqs=6, grow_iters=2, median=100, hi=200, lo=20)
+    K, V = G.host_planes(geom16, 31)
+    ref = oracle.pack(geom16, K, V, w.reqs)
+    K2, V2 = G.host_planes(geom16, 32)
+    oracle.unpack(geom16, K2, V2, w.restore_reqs, ref)
+    pool_a, pool_b = G.make_pool(geom16, 31), G.make_pool(geom16, 32)
+    g = lk.make_geom(L, H, D, S, N, elem_bytes=elem_bytes)      # what the library is told
+    plan = lk.lumen_kv_plan_build(g, w.reqs, 0, 0)
+    rplan = lk.lumen_kv_plan_build(g, w.restore_reqs, lk.LUMEN_KV_VALIDATE_UNIQUE_DST, 0)
+    assert plan.nbytes == ref.size * 2
+    buf = torch.empty(plan.nbytes, dtype=torch.uint8, device="cuda")
+    lk.lumen_kv_checkpoint_pack(plan, pool_a.k_ptrs, pool_a.v_ptrs, buf.data_ptr(), plan.nbytes, 0, 0)
+    lk.lumen_kv_restore_unpack(rplan, pool_b.k_ptrs, pool_b.v_ptrs, buf.data_ptr(), plan.nbytes, 0, 0)
+    torch.cuda.synchronize()
+    assert np.array_equal(G.buf_to_np(buf, plan.nbytes), ref)
+    for t, r in zip(pool_b.planes(), [x for kv in zip(K2, V2) for x in kv]):
+        assert np.array_equal(G.plane_to_np(t), r)

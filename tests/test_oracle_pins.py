@@ -422,3 +422,32 @@ def test_layout_delta_append_in_place_and_prefix_cut():
     assert all(np.array_equal(a, b) for a, b in zip(K2 + V2, K3 + V3))
     with pytest.raises(oracle.OracleError):                  # stride shorter than the range
         oracle.unpack_layout(w.geom, K2, V2, [(pt2, 37, 53)], [(0, 15)], seg)
+
+
+def test_layout_numpy_restatement_equals_c_loops():
+    """P2 for the explicit layout: strided-view NumPy restatement == the C loop nest."""
+    rng = substream(33, "layout3")
+    n = 0
+    while n < 60:
+        w = random_tiny(rng)
+        if not w.tokens:
+            continue
+        L, H, D, S, N = w.geom
+        E = H * D
+        K, V = make_pool(w.geom, 11)
+        lays, at = [], int(rng.integers(0, 9))
+        for _, tb, te in w.reqs:
+            stride = (te - tb) + int(rng.integers(0, 5))
+            lays.append((at, stride))
+            at += 2 * L * stride * E + int(rng.integers(0, 7))
+        B1 = np.full(at + 3, 0xDEAD, dtype=np.uint16)
+        B2 = B1.copy()
+        oracle.pack_layout(w.geom, K, V, w.reqs, lays, B1)
+        oracle_np.pack_layout(w.geom, K, V, w.reqs, lays, B2)
+        assert np.array_equal(B1, B2)
+        Ka, Va = make_pool(w.geom, 12)
+        Kb, Vb = clone(Ka), clone(Va)
+        oracle.unpack_layout(w.geom, Ka, Va, w.restore_reqs, lays, B1)
+        oracle_np.unpack_layout(w.geom, Kb, Vb, w.restore_reqs, lays, B1)
+        assert all(np.array_equal(a, b) for a, b in zip(Ka + Va, Kb + Vb))
+        n += 1
