@@ -220,3 +220,55 @@ def test_gpu_checkpoint_chain_end_to_end(lk):
     for rid in range(len(lens)):                               # completion releases the footprint
         st.release(rid)
     assert st.reserved == 0
+
+
+def test_concurrent_appends_and_churn(lk):
+    """Eight host threads (receivers of different workers' streams) append deltas to their own
+    requests while requests are reserved and released around them; every stored byte and every
+    count matches, and the arena is whole again at the end."""
+    tokb, S = 4096, 16
+    n_req, per_req = 8, 200
+    keep, arena = _arena((n_req * per_req + 300) * tokb)
+    st = lk.Store(arena.ctypes.data, arena.size, tokb, S, copy_threads=2)
+    for rid in range(n_req):
+        st.reserve(rid, per_req)
+    errors = []
+    none = np.zeros(0, dtype=lk.TAG_DTYPE)
+
+    def receiver(rid):
+        try:
+            rng = np.random.default_rng(rid)
+            at = 0
+            while at < per_req:
+                n = int(min(per_req - at, rng.integers(1, 40)))
+                delta = np.full(n * tokb, (rid * 37 + at) % 251, dtype=np.uint8)
+                st.append(rid, at, at + n, delta.ctypes.data, delta.nbytes, none)
+                at += n
+            segs = st.segments(rid, per_req)
+            for s in segs:
+                blk = arena[int(s["buf_offset"]): int(s["buf_offset"]) + int(s["t_end"] - s["t_begin"]) * tokb]
+                if not (blk == (rid * 37 + int(s["t_begin"])) % 251).all():
+                    errors.append(("bytes", rid, int(s["t_begin"])))
+        except Exception as e:                                   # noqa: BLE001
+            errors.append((rid, repr(e)))
+
+    def churn():
+        try:
+            for i in range(300):
+                st.reserve(1000 + i, 1 + i % 90)
+                st.release(1000 + i)
+        except Exception as e:                                   # noqa: BLE001
+            errors.append(("churn", repr(e)))
+
+    threads = [threading.Thread(target=receiver, args=(r,)) for r in range(n_req)] + [threading.Thread(target=churn)]
+    for t in threads:
+        t.start()
+    for t in threads:
+        t.join(timeout=120)
+    assert not errors and not any(t.is_alive() for t in threads)
+    assert all(st.tokens(r) == per_req for r in range(n_req))
+    assert st.reserved == n_req * per_req * tokb
+    for r in range(n_req):
+        st.release(r)
+    assert st.available == arena.size
+    st.reserve(9999, arena.size // tokb)                          # coalesced back into one hole
