@@ -364,6 +364,51 @@ LUMEN_KV_API int64_t lumen_kv_store_segments(const lumen_kv_store* store, uint64
                                              int64_t cap);
 
 /*
+ * Background checkpointer -- the worker side of the incremental checkpoint pipeline
+ * (PAPER.md:145): "workers track checkpoint progress and transmit only newly generated KV
+ * pages after each prefill or decode batch. A background thread copies these pages from GPU
+ * memory to the local pinned buffer (3), then streams them over the network to the designated
+ * checkpoint store (4). This two-stage pipeline completely overlaps with normal inference".
+ *
+ * One object = one worker's thread.  It keeps t_prev per tracked request (step a1), and for
+ * every notification builds ONE plan over all pending deltas [t_prev, t_cur) (a2), waits for
+ * the batch's ready event on its own stream (A10), packs through the two-stage path with
+ * per-chunk commit flags into the caller's pinned buffer (a3-a5) and hands each request's
+ * delta to `sink` as soon as the chunks that hold it have committed -- while later chunks are
+ * still in flight -- then advances t_prev.  The sink stands in for step (4); it runs on the
+ * checkpointer's thread, must not keep the pointer, and sees for each request exactly the
+ * dense pack buffer of its range: [plane][token][head][dim].
+ *   k_planes, v_planes : device pointers of the pool (copied).
+ *   staging / slot_bytes / n_slots : device staging ring as for lumen_kv_stager_create.
+ *   pinned / pinned_bytes : pinned host buffer, at least as large as the largest single
+ *                 request delta the caller will notify (deltas are batched up to its size).
+ * notify() copies the page tables and returns at once; deltas of one request are delivered
+ * in order; a later notify for a request supersedes an earlier one that has not started.
+ * ready_event: a cudaEvent_t recorded after the batch that produced the tokens (NULL: they
+ * already exist); it must stay valid until the delta has been delivered.
+ * flush() blocks until everything notified before the call has been delivered and returns
+ * the first error the thread met (0 if none).  Errors: EINVAL, ESIZE, ENOMEM, ECUDA.
+ */
+typedef struct lumen_kv_ckpt lumen_kv_ckpt;
+typedef void (*lumen_kv_sink_fn)(void* user, uint64_t request_id, int64_t t_begin, int64_t t_end,
+                                 const void* delta, int64_t delta_bytes);
+LUMEN_KV_API int lumen_kv_ckpt_create(const lumen_kv_geom* geom, const void* const* k_planes,
+                                      const void* const* v_planes, void* staging,
+                                      int64_t slot_bytes, int32_t n_slots, void* pinned,
+                                      int64_t pinned_bytes, lumen_kv_sink_fn sink, void* user,
+                                      lumen_kv_ckpt** out);
+LUMEN_KV_API void lumen_kv_ckpt_destroy(lumen_kv_ckpt* ckpt);          /* flushes, joins the thread */
+LUMEN_KV_API int lumen_kv_ckpt_track(lumen_kv_ckpt* ckpt, uint64_t request_id, int64_t t_prev);
+LUMEN_KV_API int lumen_kv_ckpt_untrack(lumen_kv_ckpt* ckpt, uint64_t request_id);
+/* reqs[i].page_table / page_table_len: request ids[i]'s current table; reqs[i].t_end = t_cur;
+ * reqs[i].t_begin is ignored (the checkpointer knows t_prev). */
+LUMEN_KV_API int lumen_kv_ckpt_notify(lumen_kv_ckpt* ckpt, const uint64_t* ids,
+                                      const lumen_kv_req* reqs, int32_t n, void* ready_event);
+LUMEN_KV_API int lumen_kv_ckpt_flush(lumen_kv_ckpt* ckpt);
+/* tokens of the request delivered to the sink so far (its t_prev), or EINVAL */
+LUMEN_KV_API int64_t lumen_kv_ckpt_progress(lumen_kv_ckpt* ckpt, uint64_t request_id);
+
+/*
  * Controller logic (host arithmetic only; section 4.2 Eq. (1), section 4.3).
  *
  * lumen_kv_choose_holder -- checkpoint placement, Eq. (1):

@@ -42,6 +42,8 @@ EXPORTS = (
     "lumen_kv_store_reserved", "lumen_kv_store_reserve", "lumen_kv_store_release",
     "lumen_kv_store_append", "lumen_kv_store_tokens", "lumen_kv_store_lookup",
     "lumen_kv_store_segments", "lumen_kv_choose_holder", "lumen_kv_recover",
+    "lumen_kv_ckpt_create", "lumen_kv_ckpt_destroy", "lumen_kv_ckpt_track", "lumen_kv_ckpt_untrack",
+    "lumen_kv_ckpt_notify", "lumen_kv_ckpt_flush", "lumen_kv_ckpt_progress",
 )
 
 
@@ -70,6 +72,11 @@ class lumen_kv_chunk_info(ctypes.Structure):
     _fields_ = [("run_begin", ctypes.c_int64), ("run_end", ctypes.c_int64),
                 ("plane_begin", ctypes.c_int32), ("plane_end", ctypes.c_int32),
                 ("byte_begin", ctypes.c_int64), ("byte_end", ctypes.c_int64)]
+
+
+# lumen_kv_sink_fn: (user, request_id, t_begin, t_end, delta pointer, delta_bytes)
+SINK_FN = ctypes.CFUNCTYPE(None, ctypes.c_void_p, ctypes.c_uint64, ctypes.c_int64, ctypes.c_int64,
+                           ctypes.c_void_p, ctypes.c_int64)
 
 
 class LumenKVError(RuntimeError):
@@ -157,6 +164,22 @@ def _lib() -> ctypes.CDLL:
                                          ctypes.c_double, ctypes.POINTER(i32)]
     L.lumen_kv_recover.restype = ctypes.c_int
     L.lumen_kv_recover.argtypes = [vp, vp, i32, vp, vp, i32, vp, vp, vp]
+    L.lumen_kv_ckpt_create.restype = ctypes.c_int
+    L.lumen_kv_ckpt_create.argtypes = [ctypes.POINTER(lumen_kv_geom), ctypes.POINTER(vp),
+                                       ctypes.POINTER(vp), vp, i64, i32, vp, i64, SINK_FN, vp,
+                                       ctypes.POINTER(vp)]
+    L.lumen_kv_ckpt_destroy.restype = None
+    L.lumen_kv_ckpt_destroy.argtypes = [vp]
+    L.lumen_kv_ckpt_track.restype = ctypes.c_int
+    L.lumen_kv_ckpt_track.argtypes = [vp, ctypes.c_uint64, i64]
+    L.lumen_kv_ckpt_untrack.restype = ctypes.c_int
+    L.lumen_kv_ckpt_untrack.argtypes = [vp, ctypes.c_uint64]
+    L.lumen_kv_ckpt_notify.restype = ctypes.c_int
+    L.lumen_kv_ckpt_notify.argtypes = [vp, vp, ctypes.POINTER(lumen_kv_req), i32, vp]
+    L.lumen_kv_ckpt_flush.restype = ctypes.c_int
+    L.lumen_kv_ckpt_flush.argtypes = [vp]
+    L.lumen_kv_ckpt_progress.restype = i64
+    L.lumen_kv_ckpt_progress.argtypes = [vp, ctypes.c_uint64]
     L.lumen_kv_plan_num_chunks.restype = i64
     L.lumen_kv_plan_num_chunks.argtypes = [vp, i64]
     L.lumen_kv_plan_get_chunks.restype = i64
@@ -565,6 +588,67 @@ def lumen_kv_recover(load, alive, interrupted):
     if rc:
         raise LumenKVError(rc, "lumen_kv_recover")
     return assign.tolist(), [bool(x) for x in reuse], final.tolist()
+
+
+class BackgroundCheckpointer:
+    """Owner of a `lumen_kv_ckpt*` (the worker's background checkpointing thread).
+    sink(request_id, t_begin, t_end, delta_ptr, delta_bytes) is called on that thread."""
+
+    def __init__(self, geom: lumen_kv_geom, k_planes, v_planes, staging_ptr: int, slot_bytes: int,
+                 n_slots: int, pinned_ptr: int, pinned_bytes: int, sink):
+        L = geom.num_layers
+        self._cb = SINK_FN(lambda _u, rid, tb, te, ptr, nb: sink(int(rid), int(tb), int(te), int(ptr), int(nb)))
+        out = ctypes.c_void_p()
+        rc = _lib().lumen_kv_ckpt_create(ctypes.byref(geom), _as_ptr_array(k_planes, L),
+                                         _as_ptr_array(v_planes, L), ctypes.c_void_p(int(staging_ptr)),
+                                         int(slot_bytes), int(n_slots), ctypes.c_void_p(int(pinned_ptr)),
+                                         int(pinned_bytes), self._cb, None, ctypes.byref(out))
+        if rc:
+            raise LumenKVError(rc, "lumen_kv_ckpt_create")
+        self._h = out
+
+    def _check(self, rc, where):
+        if rc < 0:
+            raise LumenKVError(int(rc), where)
+        return int(rc)
+
+    def track(self, request_id: int, t_prev: int = 0) -> None:
+        self._check(_lib().lumen_kv_ckpt_track(self._h, int(request_id), int(t_prev)), "lumen_kv_ckpt_track")
+
+    def untrack(self, request_id: int) -> None:
+        self._check(_lib().lumen_kv_ckpt_untrack(self._h, int(request_id)), "lumen_kv_ckpt_untrack")
+
+    def notify(self, ids, reqs, ready_event: int = 0) -> None:
+        """reqs: (page_table, _, t_cur) per id; ready_event: a cudaEvent_t handle or 0."""
+        n = len(ids)
+        ida = np.ascontiguousarray(ids, dtype=np.uint64)
+        arr = (lumen_kv_req * max(n, 1))()
+        keep = []
+        for i, (pt, _tb, te) in enumerate(reqs):
+            pt = np.ascontiguousarray(pt, dtype=np.int32)
+            keep.append(pt)
+            arr[i].page_table = pt.ctypes.data if pt.size else None
+            arr[i].page_table_len = pt.size
+            arr[i].t_begin, arr[i].t_end = 0, int(te)
+        self._check(_lib().lumen_kv_ckpt_notify(self._h, ida.ctypes.data, arr, n,
+                                                ctypes.c_void_p(int(ready_event))), "lumen_kv_ckpt_notify")
+
+    def flush(self) -> None:
+        self._check(_lib().lumen_kv_ckpt_flush(self._h), "lumen_kv_ckpt_flush")
+
+    def progress(self, request_id: int) -> int:
+        return self._check(_lib().lumen_kv_ckpt_progress(self._h, int(request_id)), "lumen_kv_ckpt_progress")
+
+    def close(self) -> None:
+        if self._h:
+            _lib().lumen_kv_ckpt_destroy(self._h)
+            self._h = ctypes.c_void_p(None)
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
 
 
 def lumen_kv_plan_free(plan: Plan) -> None:

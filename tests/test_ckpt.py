@@ -1,0 +1,122 @@
+"""The worker's background checkpointer (include/lumen_kv.h lumen_kv_ckpt_*):
+host-side argument checks on the CPU; on the GPU a decode loop notifies it after every batch
+without ever waiting, the sink (standing in for the network send) appends to a checkpoint
+store, and what arrives equals the oracle's pack of exactly the ranges delivered; after a
+"failure" the stored prefix is restored and equals the oracle's restore."""
+import threading
+
+import numpy as np
+import pytest
+
+import oracle
+from workloads import cfg1_qwen14b, substream
+
+
+@pytest.fixture(scope="module")
+def lk():
+    from paper_2606_17787_b200 import build
+    build.build()
+    import paper_2606_17787_b200 as lk
+    return lk
+
+
+def test_create_needs_a_device_and_valid_arguments(lk):
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("GPU present")
+    g = lk.make_geom(2, 2, 64, 16, 64)
+    host = np.zeros(1 << 16, dtype=np.uint8)
+    with pytest.raises(lk.LumenKVError) as e:               # the stager's copy stream needs CUDA
+        lk.BackgroundCheckpointer(g, [16, 16], [16, 16], 4096, 4096, 2, host.ctypes.data & ~15, 1 << 15,
+                                  lambda *a: None)
+    assert e.value.status == lk.LUMEN_KV_ECUDA
+    bad = lk.make_geom(2, 2, 3, 16, 64)                      # 12-byte rows
+    with pytest.raises(lk.LumenKVError) as e:
+        lk.BackgroundCheckpointer(bad, [16, 16], [16, 16], 4096, 4096, 2, host.ctypes.data & ~15, 1 << 15,
+                                  lambda *a: None)
+    assert e.value.status == lk.LUMEN_KV_EINVAL
+
+
+@pytest.mark.gpu
+def test_background_checkpointing_decode_loop(lk):
+    import torch
+    from tests import gpu_util as G
+    G.build_all()
+    w = cfg1_qwen14b(L=3, N=1024, n_reqs=6, grow_iters=10, median=150, hi=300, lo=40)
+    L, H, D, S, N = w.geom
+    tokb = 2 * L * H * D * 2
+    pool = G.make_pool(w.geom, 41)
+    K, V = G.host_planes(w.geom, 41)
+    lens = [te for _, _, te in w.reqs]
+    steps, dtok = 8, 16
+    ring_mem = torch.empty(3 << 20, dtype=torch.uint8, device="cuda")
+    pinned = G.pinned_buffer(64 * tokb)                      # smaller than every prefill delta: splits
+    arena = G.pinned_buffer(sum(n + steps * dtok for n in lens) * tokb)
+    st = lk.Store(arena.data_ptr(), arena.numel(), tokb, S)
+    for rid, n in enumerate(lens):
+        st.reserve(rid, n + steps * dtok)
+    delivered, errors = {rid: [] for rid in range(len(lens))}, []
+    none = np.zeros(0, dtype=lk.TAG_DTYPE)
+
+    def sink(rid, tb, te, ptr, nbytes):                      # runs on the checkpointer's thread
+        try:
+            got = np.ctypeslib.as_array((np.ctypeslib.ctypes.c_uint16 * (nbytes // 2)).from_address(ptr))
+            ref = oracle.pack(w.geom, K, V, [(w.reqs[rid][0], tb, te)])
+            if nbytes != (te - tb) * tokb or not np.array_equal(got, ref):
+                errors.append(("bytes", rid, tb, te))
+            st.append(rid, tb, te, ptr, nbytes, none)        # step (4): into the holder's store
+            delivered[rid].append((tb, te))
+        except Exception as e:                               # noqa: BLE001
+            errors.append((rid, repr(e)))
+
+    bg = lk.BackgroundCheckpointer(pool.geom, pool.k_ptrs, pool.v_ptrs, ring_mem.data_ptr(), 1 << 20, 3,
+                                   pinned.data_ptr(), pinned.numel(), sink)
+    for rid in range(len(lens)):
+        bg.track(rid, 0)
+    compute = torch.cuda.Stream()
+    scratch = torch.zeros(1 << 22, device="cuda")
+    events = []
+    ids = list(range(len(lens)))
+    for step in range(steps + 1):                            # step 0: prefill completion
+        with torch.cuda.stream(compute):
+            scratch.add_(1.0)                                # "the batch that produced the tokens"
+            ev = torch.cuda.Event()
+            ev.record(compute)
+        events.append(ev)
+        cur = [(pt, 0, n + step * dtok) for (pt, _, n) in w.reqs]
+        bg.notify(ids, cur, ev.cuda_event)                   # never waits for the checkpointer
+    with pytest.raises(lk.LumenKVError):                     # going backwards is refused
+        bg.notify([0], [(w.reqs[0][0], 0, 5)])
+    with pytest.raises(lk.LumenKVError):
+        bg.notify([99], [(w.reqs[0][0], 0, 5)])
+    bg.flush()
+    assert not errors
+    for rid, n in enumerate(lens):
+        final = n + steps * dtok
+        assert bg.progress(rid) == final and st.tokens(rid) == final
+        spans = delivered[rid]
+        assert spans[0][0] == 0 and spans[-1][1] == final
+        assert all(a[1] == b[0] for a, b in zip(spans, spans[1:]))        # in order, no gap
+        assert all(te - tb <= 64 for tb, te in spans)                      # never more than the pinned buffer
+    # ---- failure: restore every request's checkpoint out of the arena into fresh pages ----
+    pool_b = G.make_pool(w.geom, 42)
+    K2, V2 = G.host_planes(w.geom, 42)
+    reqs, lays = [], []
+    for rid, (pt_new, _, n) in enumerate(w.restore_reqs):
+        final = n + steps * dtok
+        for s in st.segments(rid, final):
+            reqs.append((pt_new, int(s["t_begin"]), int(s["t_end"])))
+            lays.append((int(s["buf_offset"]), int(s["plane_stride_tokens"])))
+        oracle.unpack(w.geom, K2, V2, [(pt_new, 0, final)],
+                      oracle.pack(w.geom, K, V, [(w.reqs[rid][0], 0, final)]))
+    ck_b = G.Checkpointer(pool_b)
+    rplan = ck_b.plan(reqs, unique_dst=True, layouts=lays)
+    ring = G.StagingRing(1 << 20, 3)
+    ck_b.unpack_staged(rplan, arena, ring)
+    torch.cuda.synchronize()
+    for t, ref in zip(pool_b.planes(), [x for kv in zip(K2, V2) for x in kv]):
+        assert np.array_equal(G.plane_to_np(t), ref)
+    bg.untrack(0)
+    with pytest.raises(lk.LumenKVError):
+        bg.progress(0)
+    bg.close()
