@@ -359,6 +359,12 @@ typedef struct {
     int64_t buf_offset;
     int64_t plane_stride_tokens;
 } lumen_kv_segment;
+/* A ready-made sink for lumen_kv_ckpt_create (user = the lumen_kv_store*): appends the delta
+ * as it is, without tags -- a holder on the same host, or the receiving end of the transport in
+ * tests.  A sink cannot return a status, so failed appends are counted instead. */
+LUMEN_KV_API void lumen_kv_store_sink(void* store, uint64_t request_id, int64_t t_begin,
+                                      int64_t t_end, const void* delta, int64_t delta_bytes);
+LUMEN_KV_API int64_t lumen_kv_store_sink_errors(const lumen_kv_store* store);
 LUMEN_KV_API int64_t lumen_kv_store_segments(const lumen_kv_store* store, uint64_t request_id,
                                              int64_t prefix_tokens, lumen_kv_segment* out,
                                              int64_t cap);

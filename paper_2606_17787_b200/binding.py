@@ -41,7 +41,8 @@ EXPORTS = (
     "lumen_kv_store_create", "lumen_kv_store_destroy", "lumen_kv_store_available",
     "lumen_kv_store_reserved", "lumen_kv_store_reserve", "lumen_kv_store_release",
     "lumen_kv_store_append", "lumen_kv_store_tokens", "lumen_kv_store_lookup",
-    "lumen_kv_store_segments", "lumen_kv_choose_holder", "lumen_kv_recover",
+    "lumen_kv_store_segments", "lumen_kv_store_sink", "lumen_kv_store_sink_errors",
+    "lumen_kv_choose_holder", "lumen_kv_recover",
     "lumen_kv_ckpt_create", "lumen_kv_ckpt_destroy", "lumen_kv_ckpt_track", "lumen_kv_ckpt_untrack",
     "lumen_kv_ckpt_notify", "lumen_kv_ckpt_flush", "lumen_kv_ckpt_progress",
 )
@@ -157,6 +158,8 @@ def _lib() -> ctypes.CDLL:
     L.lumen_kv_store_tokens.argtypes = [vp, u64]
     L.lumen_kv_store_lookup.restype = i64
     L.lumen_kv_store_lookup.argtypes = [vp, u64, vp, i64]
+    L.lumen_kv_store_sink_errors.restype = i64
+    L.lumen_kv_store_sink_errors.argtypes = [vp]
     L.lumen_kv_store_segments.restype = i64
     L.lumen_kv_store_segments.argtypes = [vp, u64, i64, vp, i64]
     L.lumen_kv_choose_holder.restype = ctypes.c_int
@@ -534,6 +537,10 @@ class Store:
         return self._check(_lib().lumen_kv_store_lookup(self._h, int(request_id), t.ctypes.data, t.size),
                            "lumen_kv_store_lookup")
 
+    @property
+    def sink_errors(self) -> int:
+        return self._check(_lib().lumen_kv_store_sink_errors(self._h), "lumen_kv_store_sink_errors")
+
     def segments(self, request_id: int, prefix_tokens: int) -> np.ndarray:
         n = self._check(_lib().lumen_kv_store_segments(self._h, int(request_id), int(prefix_tokens),
                                                        None, 0), "lumen_kv_store_segments")
@@ -597,12 +604,18 @@ class BackgroundCheckpointer:
     def __init__(self, geom: lumen_kv_geom, k_planes, v_planes, staging_ptr: int, slot_bytes: int,
                  n_slots: int, pinned_ptr: int, pinned_bytes: int, sink):
         L = geom.num_layers
-        self._cb = SINK_FN(lambda _u, rid, tb, te, ptr, nb: sink(int(rid), int(tb), int(te), int(ptr), int(nb)))
+        if isinstance(sink, Store):      # native sink: deltas go straight into the store, no Python
+            self._keep = sink
+            self._cb = ctypes.cast(_lib().lumen_kv_store_sink, SINK_FN)
+            user = sink._h
+        else:
+            self._cb = SINK_FN(lambda _u, rid, tb, te, ptr, nb: sink(int(rid), int(tb), int(te), int(ptr), int(nb)))
+            user = None
         out = ctypes.c_void_p()
         rc = _lib().lumen_kv_ckpt_create(ctypes.byref(geom), _as_ptr_array(k_planes, L),
                                          _as_ptr_array(v_planes, L), ctypes.c_void_p(int(staging_ptr)),
                                          int(slot_bytes), int(n_slots), ctypes.c_void_p(int(pinned_ptr)),
-                                         int(pinned_bytes), self._cb, None, ctypes.byref(out))
+                                         int(pinned_bytes), self._cb, user, ctypes.byref(out))
         if rc:
             raise LumenKVError(rc, "lumen_kv_ckpt_create")
         self._h = out

@@ -43,6 +43,7 @@ struct lumen_kv_store {
     std::map<int64_t, int64_t> free_;                    // offset -> bytes, coalesced
     std::unordered_map<uint64_t, Entry> reqs;
     int64_t reserved = 0;
+    int64_t sink_errors = 0;
 };
 
 namespace {
@@ -199,6 +200,22 @@ int64_t lumen_kv_store_lookup(const lumen_kv_store* s, uint64_t id, const lumen_
     }
     return lumen_kv_longest_prefix(regen, n_regen, stored.data(),
                                    static_cast<int64_t>(stored.size()));
+}
+
+void lumen_kv_store_sink(void* store, uint64_t id, int64_t t_begin, int64_t t_end,
+                         const void* delta, int64_t delta_bytes) {
+    lumen_kv_store* s = static_cast<lumen_kv_store*>(store);
+    if (!s) return;
+    if (lumen_kv_store_append(s, id, t_begin, t_end, delta, delta_bytes, nullptr, 0) != LUMEN_KV_OK) {
+        std::lock_guard<std::mutex> g(s->mu);
+        ++s->sink_errors;
+    }
+}
+
+int64_t lumen_kv_store_sink_errors(const lumen_kv_store* s) {
+    if (!s) return LUMEN_KV_EINVAL;
+    std::lock_guard<std::mutex> g(s->mu);
+    return s->sink_errors;
 }
 
 int64_t lumen_kv_store_segments(const lumen_kv_store* s, uint64_t id, int64_t prefix_tokens,
