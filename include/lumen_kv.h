@@ -386,8 +386,9 @@ LUMEN_KV_API int64_t lumen_kv_store_segments(const lumen_kv_store* store, uint64
  * dense pack buffer of its range: [plane][token][head][dim].
  *   k_planes, v_planes : device pointers of the pool (copied).
  *   staging / slot_bytes / n_slots : device staging ring as for lumen_kv_stager_create.
- *   pinned / pinned_bytes : pinned host buffer, at least as large as the largest single
- *                 request delta the caller will notify (deltas are batched up to its size).
+ *   pinned / pinned_bytes : pinned host buffer (a multiple of 32 bytes), used as two halves:
+ *                 while the sink drains one, the copy engine fills the other.  Deltas are
+ *                 batched up to one half; a delta larger than a half is delivered in pieces.
  * notify() copies the page tables and returns at once; deltas of one request are delivered
  * in order; a later notify for a request supersedes an earlier one that has not started.
  * ready_event: a cudaEvent_t recorded after the batch that produced the tokens (NULL: they

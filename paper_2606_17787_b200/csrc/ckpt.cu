@@ -25,8 +25,9 @@ struct Pending {
 
 struct Tracked {
     int64_t t_prev = 0;        // tokens delivered to the sink
+    int64_t t_sent = 0;        // tokens handed to a pack that has been enqueued (>= t_prev)
     bool has_pending = false;
-    bool in_flight = false;
+    int in_flight = 0;         // batches enqueued but not yet delivered that contain this request
     bool zombie = false;       // untracked while in flight: erased after delivery
     Pending p;
 };
@@ -36,6 +37,16 @@ struct Job {
     std::vector<int32_t> pt;
     int64_t tb, te;
     cudaEvent_t ev;
+};
+
+// One enqueued pack: it owns one half of the pinned buffer until it has been delivered.
+struct Batch {
+    std::vector<Job> jobs;
+    lumen_kv_plan* plan = nullptr;
+    std::vector<lumen_kv_chunk_info> chunks;
+    uint64_t epoch = 0;
+    int half = 0;
+    int rc = LUMEN_KV_OK;
 };
 
 }  // namespace
@@ -50,8 +61,8 @@ struct lumen_kv_ckpt {
     int device = 0;
     lumen_kv_stager* stager = nullptr;
     cudaStream_t stream = nullptr;
-    uint64_t* flags = nullptr;   // pinned, one word per chunk of the plan in flight
-    int64_t flags_cap = 0;
+    uint64_t* flags[2] = {nullptr, nullptr};   // pinned, one word per chunk, per buffer half
+    int64_t flags_cap[2] = {0, 0};
     uint64_t epoch = 0;
 
     std::mutex mu;
@@ -70,17 +81,12 @@ bool any_pending(const lumen_kv_ckpt* c) {
     return false;
 }
 
-void set_error(lumen_kv_ckpt* c, int rc) {
-    std::lock_guard<std::mutex> g(c->mu);
-    if (c->first_error == 0) c->first_error = rc;
-}
-
 // Waits until flags[idx] == epoch; false if the stream died or finished without the flag.
-bool wait_flag(lumen_kv_ckpt* c, int64_t idx) {
-    volatile uint64_t* f = c->flags + idx;
+bool wait_flag(lumen_kv_ckpt* c, const Batch& b, int64_t idx) {
+    volatile uint64_t* f = c->flags[b.half] + idx;
     int spins = 0;
     for (;;) {
-        if (*f == c->epoch) {
+        if (*f == b.epoch) {
             std::atomic_thread_fence(std::memory_order_acquire);
             return true;
         }
@@ -88,7 +94,7 @@ bool wait_flag(lumen_kv_ckpt* c, int64_t idx) {
             const cudaError_t e = cudaStreamQuery(c->stream);
             if (e == cudaSuccess) {                 // everything ran: the flag must be there now
                 std::atomic_thread_fence(std::memory_order_acquire);
-                return *f == c->epoch;
+                return *f == b.epoch;
             }
             if (e != cudaErrorNotReady) {
                 (void)cudaGetLastError();
@@ -99,129 +105,161 @@ bool wait_flag(lumen_kv_ckpt* c, int64_t idx) {
     }
 }
 
-int process(lumen_kv_ckpt* c, std::vector<Job>& jobs) {
-    const int32_t n = static_cast<int32_t>(jobs.size());
+// Stage 1: build the plan of the batch and enqueue its pack into one half of the pinned buffer.
+void submit(lumen_kv_ckpt* c, Batch& b) {
+    const int32_t n = static_cast<int32_t>(b.jobs.size());
+    const int64_t half_bytes = c->pinned_bytes / 2;
     std::vector<lumen_kv_req> reqs(static_cast<size_t>(n));
     for (int32_t i = 0; i < n; ++i) {
-        reqs[i].page_table = jobs[i].pt.data();
-        reqs[i].page_table_len = static_cast<int64_t>(jobs[i].pt.size());
-        reqs[i].t_begin = jobs[i].tb;
-        reqs[i].t_end = jobs[i].te;
+        reqs[i].page_table = b.jobs[i].pt.data();
+        reqs[i].page_table_len = static_cast<int64_t>(b.jobs[i].pt.size());
+        reqs[i].t_begin = b.jobs[i].tb;
+        reqs[i].t_end = b.jobs[i].te;
     }
-    lumen_kv_plan* plan = nullptr;
-    int rc = lumen_kv_plan_build(&c->geom, reqs.data(), n, 0, c->stream, &plan);
-    if (rc != LUMEN_KV_OK) return rc;
-    const int64_t n_chunks = lumen_kv_plan_num_chunks(plan, c->slot_bytes);
+    b.rc = lumen_kv_plan_build(&c->geom, reqs.data(), n, 0, c->stream, &b.plan);
+    if (b.rc != LUMEN_KV_OK) return;
+    const int64_t n_chunks = lumen_kv_plan_num_chunks(b.plan, c->slot_bytes);
     if (n_chunks < 0) {
-        lumen_kv_plan_free(plan);
-        return static_cast<int>(n_chunks);
+        b.rc = static_cast<int>(n_chunks);
+        return;
     }
-    if (n_chunks > c->flags_cap) {                  // control memory, grown rarely
-        if (c->flags) cudaFreeHost(c->flags);
-        c->flags = nullptr;
-        c->flags_cap = 0;
+    if (n_chunks > c->flags_cap[b.half]) {          // control memory, grown rarely
+        if (c->flags[b.half]) cudaFreeHost(c->flags[b.half]);
+        c->flags[b.half] = nullptr;
+        c->flags_cap[b.half] = 0;
         int64_t cap = 256;
         while (cap < n_chunks) cap <<= 1;
-        if (cudaHostAlloc(reinterpret_cast<void**>(&c->flags), static_cast<size_t>(cap) * 8,
+        if (cudaHostAlloc(reinterpret_cast<void**>(&c->flags[b.half]), static_cast<size_t>(cap) * 8,
                           cudaHostAllocDefault) != cudaSuccess) {
             (void)cudaGetLastError();
-            lumen_kv_plan_free(plan);
-            return LUMEN_KV_ENOMEM;
+            b.rc = LUMEN_KV_ENOMEM;
+            return;
         }
-        for (int64_t i = 0; i < cap; ++i) c->flags[i] = 0;
-        c->flags_cap = cap;
+        for (int64_t i = 0; i < cap; ++i) c->flags[b.half][i] = 0;
+        c->flags_cap[b.half] = cap;
     }
-    std::vector<lumen_kv_chunk_info> chunks(static_cast<size_t>(n_chunks));
-    lumen_kv_plan_get_chunks(plan, c->slot_bytes, chunks.data(), n_chunks);
+    b.chunks.resize(static_cast<size_t>(n_chunks));
+    lumen_kv_plan_get_chunks(b.plan, c->slot_bytes, b.chunks.data(), n_chunks);
     cudaEvent_t last = nullptr;
-    for (const Job& j : jobs)                       // A10: stream order behind the producing batch
+    for (const Job& j : b.jobs)                     // A10: stream order behind the producing batch
         if (j.ev && j.ev != last) {
             if (cudaStreamWaitEvent(c->stream, j.ev, 0) != cudaSuccess) {
                 (void)cudaGetLastError();
-                lumen_kv_plan_free(plan);
-                return LUMEN_KV_ECUDA;
+                b.rc = LUMEN_KV_ECUDA;
+                return;
             }
             last = j.ev;
         }
-    ++c->epoch;
-    rc = lumen_kv_checkpoint_pack_staged_commit(plan, c->k.data(), c->v.data(), c->pinned,
-                                                c->pinned_bytes, c->stager, c->stream, c->flags,
-                                                c->epoch);
-    if (rc == LUMEN_KV_OK) {
-        int64_t ci = 0;
-        for (int32_t i = 0; i < n && rc == LUMEN_KV_OK; ++i) {
-            const int64_t off = lumen_kv_plan_req_offset(plan, i);
-            const int64_t end = lumen_kv_plan_req_offset(plan, i + 1);
-            if (end > off) {
-                while (ci < n_chunks && chunks[static_cast<size_t>(ci)].byte_end < end) ++ci;
-                if (ci >= n_chunks || !wait_flag(c, ci)) {   // the chunk that completes request i
-                    rc = LUMEN_KV_ECUDA;
-                    break;
-                }
-                c->sink(c->user, jobs[i].id, jobs[i].tb, jobs[i].te, c->pinned + off, end - off);
-            }
-            std::lock_guard<std::mutex> g(c->mu);
-            auto it = c->reqs.find(jobs[i].id);
-            if (it != c->reqs.end()) it->second.t_prev = jobs[i].te;   // progress (a1)
-        }
-    }
-    if (rc != LUMEN_KV_OK) cudaStreamSynchronize(c->stream);
-    lumen_kv_plan_free(plan);
-    return rc;
+    b.epoch = ++c->epoch;
+    b.rc = lumen_kv_checkpoint_pack_staged_commit(b.plan, c->k.data(), c->v.data(),
+                                                  c->pinned + b.half * half_bytes, half_bytes,
+                                                  c->stager, c->stream, c->flags[b.half], b.epoch);
 }
 
+// Stage 2: hand every request's delta to the sink as soon as the chunks that hold it have
+// committed (later chunks, and the next batch's pack into the other half, are still in flight).
+void deliver(lumen_kv_ckpt* c, Batch& b) {
+    const int32_t n = static_cast<int32_t>(b.jobs.size());
+    const char* base = c->pinned + b.half * (c->pinned_bytes / 2);
+    const int64_t n_chunks = static_cast<int64_t>(b.chunks.size());
+    int64_t ci = 0;
+    for (int32_t i = 0; i < n && b.rc == LUMEN_KV_OK; ++i) {
+        const int64_t off = lumen_kv_plan_req_offset(b.plan, i);
+        const int64_t end = lumen_kv_plan_req_offset(b.plan, i + 1);
+        if (end > off) {
+            while (ci < n_chunks && b.chunks[static_cast<size_t>(ci)].byte_end < end) ++ci;
+            if (ci >= n_chunks || !wait_flag(c, b, ci)) {   // the chunk that completes request i
+                b.rc = LUMEN_KV_ECUDA;
+                break;
+            }
+            c->sink(c->user, b.jobs[i].id, b.jobs[i].tb, b.jobs[i].te, base + off, end - off);
+        }
+        std::lock_guard<std::mutex> g(c->mu);
+        auto it = c->reqs.find(b.jobs[i].id);
+        if (it != c->reqs.end()) it->second.t_prev = b.jobs[i].te;   // progress (a1)
+    }
+    if (b.rc != LUMEN_KV_OK) cudaStreamSynchronize(c->stream);
+    if (b.plan) lumen_kv_plan_free(b.plan);
+    b.plan = nullptr;
+    std::lock_guard<std::mutex> g(c->mu);
+    if (b.rc != LUMEN_KV_OK && c->first_error == 0) c->first_error = b.rc;
+    for (const Job& j : b.jobs) {
+        auto it = c->reqs.find(j.id);
+        if (it == c->reqs.end()) continue;
+        Tracked& t = it->second;
+        --t.in_flight;
+        if (b.rc != LUMEN_KV_OK) {                  // do not retry for ever
+            t.has_pending = false;
+            t.t_sent = t.t_prev;
+        }
+        if (t.zombie && t.in_flight == 0) c->reqs.erase(it);
+    }
+}
+
+// Under the lock: move pending deltas into a batch, at most `room` bytes (one buffer half).
+void take_jobs(lumen_kv_ckpt* c, Batch& b, int64_t room) {
+    for (auto& kv : c->reqs) {
+        Tracked& t = kv.second;
+        if (!t.has_pending) continue;
+        if (t.p.t_cur <= t.t_sent) {                // nothing beyond what is already on its way
+            t.has_pending = false;
+            continue;
+        }
+        const int64_t want = (t.p.t_cur - t.t_sent) * c->token_bytes;
+        if (want <= room) {
+            b.jobs.push_back(Job{kv.first, std::move(t.p.pt), t.t_sent, t.p.t_cur, t.p.ev});
+            t.has_pending = false;
+            t.t_sent = t.p.t_cur;
+            room -= want;
+        } else if (b.jobs.empty()) {                // larger than a whole half: take a prefix
+            const int64_t fit = room / c->token_bytes;
+            if (fit < 1) {
+                if (c->first_error == 0) c->first_error = LUMEN_KV_ESIZE;
+                t.has_pending = false;
+                continue;
+            }
+            b.jobs.push_back(Job{kv.first, t.p.pt, t.t_sent, t.t_sent + fit, t.p.ev});
+            t.t_sent += fit;                        // the rest stays pending
+            room = 0;
+        } else {
+            break;                                  // next batch
+        }
+        ++t.in_flight;
+        if (room == 0) break;
+    }
+}
+
+// The thread: a two-deep software pipeline over the two halves of the pinned buffer.  The pack
+// of batch k+1 is enqueued before batch k is delivered, so the copy engine fills one half while
+// the sink drains the other.
 void run(lumen_kv_ckpt* c) {
     cudaSetDevice(c->device);
+    const int64_t half_bytes = c->pinned_bytes / 2;
+    Batch cur;
+    bool have_cur = false;
+    int half = 0;
     for (;;) {
-        std::vector<Job> jobs;
+        Batch nxt;
         {
             std::unique_lock<std::mutex> lk(c->mu);
-            c->busy = false;
-            c->idle_cv.notify_all();
-            c->work_cv.wait(lk, [&] { return c->stop || any_pending(c); });
-            if (!any_pending(c)) break;             // stop requested and nothing left
-            c->busy = true;
-            int64_t room = c->pinned_bytes;
-            for (auto& kv : c->reqs) {
-                Tracked& t = kv.second;
-                if (!t.has_pending) continue;
-                if (t.p.t_cur <= t.t_prev) {        // already delivered by the job that was in flight
-                    t.has_pending = false;
-                    continue;
-                }
-                const int64_t want = (t.p.t_cur - t.t_prev) * c->token_bytes;
-                if (want <= room) {
-                    jobs.push_back(Job{kv.first, std::move(t.p.pt), t.t_prev, t.p.t_cur, t.p.ev});
-                    t.has_pending = false;
-                    room -= want;
-                } else if (jobs.empty()) {          // larger than the whole buffer: take a prefix
-                    const int64_t fit = room / c->token_bytes;
-                    if (fit < 1) {
-                        if (c->first_error == 0) c->first_error = LUMEN_KV_ESIZE;
-                        t.has_pending = false;
-                        continue;
-                    }
-                    jobs.push_back(Job{kv.first, t.p.pt, t.t_prev, t.t_prev + fit, t.p.ev});
-                    room = 0;                       // the rest stays pending
-                } else {
-                    break;                          // next round
-                }
-                t.in_flight = true;
-                if (room == 0) break;
+            if (!have_cur) {
+                c->busy = false;
+                c->idle_cv.notify_all();
+                c->work_cv.wait(lk, [&] { return c->stop || any_pending(c); });
+                if (!any_pending(c)) break;         // stop requested and nothing left
+                c->busy = true;
             }
+            nxt.half = half;
+            take_jobs(c, nxt, half_bytes);
         }
-        if (!jobs.empty()) {
-            const int rc = process(c, jobs);
-            if (rc != LUMEN_KV_OK) set_error(c, rc);
-            std::lock_guard<std::mutex> g(c->mu);
-            for (const Job& j : jobs) {
-                auto it = c->reqs.find(j.id);
-                if (it == c->reqs.end()) continue;
-                it->second.in_flight = false;
-                if (rc != LUMEN_KV_OK) it->second.has_pending = false;   // do not retry for ever
-                if (it->second.zombie) c->reqs.erase(it);
-            }
+        const bool have_nxt = !nxt.jobs.empty();
+        if (have_nxt) {
+            half ^= 1;
+            submit(c, nxt);
         }
+        if (have_cur) deliver(c, cur);
+        have_cur = have_nxt;
+        if (have_nxt) cur = std::move(nxt);
     }
     std::lock_guard<std::mutex> g(c->mu);
     c->busy = false;
@@ -238,7 +276,8 @@ int lumen_kv_ckpt_create(const lumen_kv_geom* geom, const void* const* k_planes,
                          lumen_kv_sink_fn sink, void* user, lumen_kv_ckpt** out) {
     if (!out) return LUMEN_KV_EINVAL;
     *out = nullptr;
-    if (!geom || !k_planes || !v_planes || !pinned || !sink || pinned_bytes < 16 ||
+    if (!geom || !k_planes || !v_planes || !pinned || !sink || pinned_bytes < 64 ||
+        pinned_bytes % 32 != 0 ||
         (reinterpret_cast<uintptr_t>(pinned) & 15) || geom->num_layers < 1)
         return LUMEN_KV_EINVAL;
     lumen_kv_plan* probe = nullptr;                 // validates the geometry, host only
@@ -284,7 +323,8 @@ void lumen_kv_ckpt_destroy(lumen_kv_ckpt* c) {
     cudaStreamSynchronize(c->stream);
     lumen_kv_stager_destroy(c->stager);
     cudaStreamDestroy(c->stream);
-    if (c->flags) cudaFreeHost(c->flags);
+    for (int h = 0; h < 2; ++h)
+        if (c->flags[h]) cudaFreeHost(c->flags[h]);
     (void)cudaGetLastError();
     delete c;
 }
@@ -293,7 +333,7 @@ int lumen_kv_ckpt_track(lumen_kv_ckpt* c, uint64_t id, int64_t t_prev) {
     if (!c || t_prev < 0) return LUMEN_KV_EINVAL;
     std::lock_guard<std::mutex> g(c->mu);
     if (c->reqs.count(id)) return LUMEN_KV_EINVAL;
-    c->reqs[id].t_prev = t_prev;
+    c->reqs[id].t_prev = c->reqs[id].t_sent = t_prev;
     return LUMEN_KV_OK;
 }
 
@@ -320,7 +360,7 @@ int lumen_kv_ckpt_notify(lumen_kv_ckpt* c, const uint64_t* ids, const lumen_kv_r
             auto it = c->reqs.find(ids[i]);
             if (it == c->reqs.end() || it->second.zombie) return LUMEN_KV_EINVAL;
             const Tracked& t = it->second;
-            const int64_t floor_ = t.has_pending ? t.p.t_cur : t.t_prev;
+            const int64_t floor_ = t.has_pending ? t.p.t_cur : t.t_sent;
             if (reqs[i].t_end < floor_ || reqs[i].page_table_len < 0 ||
                 (reqs[i].t_end > 0 && (!reqs[i].page_table ||
                                        (reqs[i].t_end + S - 1) / S > reqs[i].page_table_len)))
@@ -328,7 +368,7 @@ int lumen_kv_ckpt_notify(lumen_kv_ckpt* c, const uint64_t* ids, const lumen_kv_r
         }
         for (int32_t i = 0; i < n; ++i) {
             Tracked& t = c->reqs[ids[i]];
-            if (reqs[i].t_end == t.t_prev && !t.in_flight && !t.has_pending) continue;   // nothing new
+            if (reqs[i].t_end == t.t_sent && !t.has_pending) continue;   // nothing new
             t.p.pt.assign(reqs[i].page_table, reqs[i].page_table + reqs[i].page_table_len);
             t.p.t_cur = reqs[i].t_end;
             t.p.ev = static_cast<cudaEvent_t>(ready_event);
