@@ -44,7 +44,7 @@ def parse_args():
     ap.add_argument("--steps", type=int, default=300)
     ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
-    ap.add_argument("--workload", choices=["cfg1", "cfg2", "cfg3", "cfg4", "chain", "interference", "overhead"],
+    ap.add_argument("--workload", choices=["cfg0", "cfg1", "cfg2", "cfg3", "cfg4", "chain", "interference", "overhead"],
                     default="cfg1")
     ap.add_argument("--kernel", choices=["auto", "warp", "bulk"], default="auto")
     ap.add_argument("--upload-descriptors", action="store_true",
@@ -59,8 +59,14 @@ def parse_args():
 # workload construction (structure only; see workloads/gen.py)
 # ------------------------------------------------------------------------------------
 def make_workload(name: str, seed: int, pages_cap=None):
-    from workloads import cfg1_qwen14b, cfg2_qwen32b, cfg4_longctx
-    if name == "cfg1":
+    from workloads import cfg0_tiny, cfg1_qwen14b, cfg2_qwen32b, cfg4_longctx
+    if name == "cfg0":
+        w = cfg0_tiny(seed)
+        label = ("BASELINE.json configs[0]: tiny pool, 2 layers x [64 pages, 16, 2 kv_heads, 64], 4 requests "
+                 "37/100/5/64 tokens, deltas [t_prev, len) -- a correctness config: it fits in L2, its GB/s "
+                 "is launch latency, not a roofline claim")
+        delta = 0
+    elif name == "cfg1":
         N = 60000 if pages_cap is None else min(60000, pages_cap)
         w = cfg1_qwen14b(seed, N=N, grow_iters=CYCLE)
         label = (f"BASELINE.json configs[1]: Qwen3-14B-shaped KV (40 layers, 8 kv_heads, head_dim 128, "
@@ -173,8 +179,9 @@ def oracle_sample(workload: str, seed: int):
         return (w, "BASELINE.json configs[3] (recovery burst, Qwen3-32B shape)", w.reqs, w.restore_reqs,
                 K, V, keep, f"1-token pack of 64 running requests + restore of {n} tokens of one request")
     w, label, delta = make_workload(workload, seed)
-    if workload == "cfg1":
-        reqs, rreqs, what = w.reqs, w.restore_reqs, "one full step (64 requests x 16 tokens, pack + restore)"
+    if workload in ("cfg0", "cfg1"):
+        reqs, rreqs = w.reqs, w.restore_reqs
+        what = f"one full step ({len(w.reqs)} requests, {w.tokens} tokens, pack + restore)"
     else:
         n = 4096
         reqs = [(w.reqs[0][0], 0, n)]
@@ -207,7 +214,10 @@ def cpu_baseline(workload: str, seed: int, budget_s: float = 12.0):
     for _ in range(reps):
         oracle_step(w.geom, K, V, reqs, rreqs)
     dt = time.perf_counter() - t0
-    out = {"value": nbytes * reps / dt / 1e9, "unit": "GB/s", "cores": 1, "kind": "oracle",
+    cpu_model = next((l.split(":", 1)[1].strip() for l in open("/proc/cpuinfo") if l.startswith("model name")),
+                     "unknown")
+    out = {"value": nbytes * reps / dt / 1e9, "unit": "GB/s", "cores": 1, "kind": "oracle", "cpu": cpu_model,
+           "cores_available": len(os.sched_getaffinity(0)),
            "sample": f"{what}, {reps} repetitions, plain single-thread C oracle as it stands"}
     # context only: the OpenMP/memcpy timing variant (asserted equal to the plain one in tests)
     threads = oracle.omp_threads()
@@ -404,6 +414,8 @@ def run_ours(args):
         if r is not None:
             r.close()
 
+    single_stats = {}
+
     def timed_loop(K, W, bufs, kind, lag_, sampler=None, per_launch=False, only=None):
         """W warm-up steps, then exactly K steps between one event pair.  per_launch=True adds
         an event between the launches of every step (kernel durations); those records sit
@@ -432,8 +444,11 @@ def run_ours(args):
         ms = max_over_ranks(e_start.elapsed_time(e_end), dist, "cuda")
         pack_ms = unpack_ms = None
         if per_launch:
-            pack_ms = float(np.mean([e[0].elapsed_time(e[1]) for e in evs]))
-            unpack_ms = float(np.mean([e[1].elapsed_time(e[2]) for e in evs]))
+            pk = [e[0].elapsed_time(e[1]) for e in evs]
+            up = [e[1].elapsed_time(e[2]) for e in evs]
+            single_stats["pack"] = {"mean": float(np.mean(pk)), "median": float(np.median(pk)), "best": float(np.min(pk))}
+            single_stats["unpack"] = {"mean": float(np.mean(up)), "median": float(np.median(up)), "best": float(np.min(up))}
+            pack_ms, unpack_ms = single_stats["pack"]["mean"], single_stats["unpack"]["mean"]
         return ms, pack_ms, unpack_ms, t_wall * 1e3, t_host * 1e3
 
     K, W = max(1, args.steps), max(3, args.warmup)
@@ -442,10 +457,21 @@ def run_ours(args):
     with torch.cuda.stream(stream):
         ms, _, _, wall_ms, host_ms = timed_loop(K, W, dbufs, DEV, lag, sampler)
         ms_k, pack_1, unpack_1, _, _ = timed_loop(Kk, 3, dbufs, DEV, lag, per_launch=True)
+        single = {k: dict(v) for k, v in single_stats.items()}      # single-launch latency: mean/median/best
         pack_ms = timed_loop(Kk, 3, dbufs, DEV, lag, only="pack")[0] / Kk
         unpack_ms = timed_loop(Kk, 3, dbufs, DEV, lag, only="unpack")[0] / Kk
     value = job_payload_gbps(world, K, P, ms)
     token_bytes = 2 * L * H * D * 2
+    n_pb = 200 if P <= (1 << 30) else 10                 # a2 alone, on the host clock
+    t0 = time.perf_counter()
+    for i in range(n_pb):
+        tb, te = ranges[i % len(ranges)]
+        ra_p.set_ranges(tb, te)
+        pl = lk.lumen_kv_plan_build(geom, ra_p, kflag, sh)
+        runs_per_plan = pl.num_runs
+        pl.close()
+    plan_build_us = (time.perf_counter() - t0) / n_pb * 1e6
+    stream.synchronize()
 
     # ---- roofline of the dominant kernel ------------------------------------------------
     peak, peak_src = measured_peaks()
@@ -465,7 +491,7 @@ def run_ours(args):
                            f"whole steps ({ms_k / Kk:.4f} ms/step: the records between the launches cost a "
                            "few us each and prevent the overlap of consecutive launches)"),
                 "pack_ms": pack_ms, "unpack_ms": unpack_ms,
-                "pack_single_ms": pack_1, "unpack_single_ms": unpack_1,
+                "pack_single_ms": pack_1, "unpack_single_ms": unpack_1, "single_launch_ms": single,
                 "pack_traffic_GBps": 2 * P / pack_ms / 1e6, "unpack_traffic_GBps": 2 * P / unpack_ms / 1e6}
 
     # ---- e2e: same step, host buffers, bytes cross the host link inside the timed region --
@@ -575,8 +601,9 @@ def run_ours(args):
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "u16", "data": "synthetic",
         "config": {"workload": label, "payload_bytes_per_direction_per_step": P,
-                   "tokens_per_step": w.tokens, "runs_per_plan": None,
-                   "l2": (f"inputs larger than L2: steps rotate over {n_stage} staging buffers of "
+                   "tokens_per_step": w.tokens, "runs_per_plan": runs_per_plan,
+                   "l2": ("fits in L2 (latency config, no roofline claim)" if args.workload == "cfg0" else
+                          f"inputs larger than L2: steps rotate over {n_stage} staging buffers of "
                           f"{P / 2**20:.0f} MiB and {len(ranges)} distinct delta sets; the restore reads "
                           f"the buffer packed {lag} steps earlier"),
                    "kernel": args.kernel, "replicas": world,
@@ -584,6 +611,7 @@ def run_ours(args):
                    "pdl": os.environ.get("LUMEN_KV_PDL", "1") != "0", "seed": hex(MASTER_SEED)},
         "tokens_per_s": value * 1e9 / token_bytes,
         "wall_ms_per_step": wall_ms / K, "host_enqueue_ms_per_step": host_ms / K,
+        "plan_build_us": plan_build_us,
         "roofline": roofline, "e2e": e2e, "gpu_launches": 2 * K, "clocks": sampler.summary(),
     }
     if rank == 0:
