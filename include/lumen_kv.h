@@ -299,6 +299,16 @@ LUMEN_KV_API int lumen_kv_page_tags(const int32_t* token_ids, const int64_t* tok
                                     int32_t num_reqs, int32_t page_size, lumen_kv_tag* tags_out,
                                     int64_t tags_cap, void* stream);
 /*
+ * lumen_kv_page_tags_host -- the same tags on the host, for the sender of a delta: the tags of
+ * the pages touched by [t_begin, t_end) as of a history of t_end tokens (so the last page's end
+ * position is min(page end, t_end)).  token_ids points at token `first_token`, which must be
+ * a multiple of page_size and <= t_begin rounded down to a page.  Writes at most cap tags;
+ * returns their number ((t_end-1)/S - t_begin/S + 1, or 0 for an empty range) or EINVAL.
+ */
+LUMEN_KV_API int64_t lumen_kv_page_tags_host(const int32_t* token_ids, int64_t first_token,
+                                             int64_t t_begin, int64_t t_end, int32_t page_size,
+                                             lumen_kv_tag* out, int64_t cap);
+/*
  * lumen_kv_longest_prefix -- host lookup: walk the regenerated tags of one request in page
  * order and halt at the first that is not among `stored` (any order, duplicates allowed);
  * returns the end position of the last tag found = tokens of the longest contiguous
@@ -360,10 +370,11 @@ typedef struct {
     int64_t plane_stride_tokens;
 } lumen_kv_segment;
 /* A ready-made sink for lumen_kv_ckpt_create (user = the lumen_kv_store*): appends the delta
- * as it is, without tags -- a holder on the same host, or the receiving end of the transport in
- * tests.  A sink cannot return a status, so failed appends are counted instead. */
+ * with the tags it carries -- a holder on the same host, or the receiving end of the
+ * transport in tests.  A sink cannot return a status, so failed appends are counted instead. */
 LUMEN_KV_API void lumen_kv_store_sink(void* store, uint64_t request_id, int64_t t_begin,
-                                      int64_t t_end, const void* delta, int64_t delta_bytes);
+                                      int64_t t_end, const void* delta, int64_t delta_bytes,
+                                      const lumen_kv_tag* tags, int32_t n_tags);
 LUMEN_KV_API int64_t lumen_kv_store_sink_errors(const lumen_kv_store* store);
 LUMEN_KV_API int64_t lumen_kv_store_segments(const lumen_kv_store* store, uint64_t request_id,
                                              int64_t prefix_tokens, lumen_kv_segment* out,
@@ -383,7 +394,8 @@ LUMEN_KV_API int64_t lumen_kv_store_segments(const lumen_kv_store* store, uint64
  * delta to `sink` as soon as the chunks that hold it have committed -- while later chunks are
  * still in flight -- then advances t_prev.  The sink stands in for step (4); it runs on the
  * checkpointer's thread, must not keep the pointer, and sees for each request exactly the
- * dense pack buffer of its range: [plane][token][head][dim].
+ * dense pack buffer of its range: [plane][token][head][dim], with the tags of the pages it
+ * touches when the caller supplied token IDs.
  *   k_planes, v_planes : device pointers of the pool (copied).
  *   staging / slot_bytes / n_slots : device staging ring as for lumen_kv_stager_create.
  *   pinned / pinned_bytes : pinned host buffer (a multiple of 32 bytes), used as two halves:
@@ -398,7 +410,8 @@ LUMEN_KV_API int64_t lumen_kv_store_segments(const lumen_kv_store* store, uint64
  */
 typedef struct lumen_kv_ckpt lumen_kv_ckpt;
 typedef void (*lumen_kv_sink_fn)(void* user, uint64_t request_id, int64_t t_begin, int64_t t_end,
-                                 const void* delta, int64_t delta_bytes);
+                                 const void* delta, int64_t delta_bytes,
+                                 const lumen_kv_tag* tags, int32_t n_tags);
 LUMEN_KV_API int lumen_kv_ckpt_create(const lumen_kv_geom* geom, const void* const* k_planes,
                                       const void* const* v_planes, void* staging,
                                       int64_t slot_bytes, int32_t n_slots, void* pinned,
@@ -408,9 +421,14 @@ LUMEN_KV_API void lumen_kv_ckpt_destroy(lumen_kv_ckpt* ckpt);          /* flushe
 LUMEN_KV_API int lumen_kv_ckpt_track(lumen_kv_ckpt* ckpt, uint64_t request_id, int64_t t_prev);
 LUMEN_KV_API int lumen_kv_ckpt_untrack(lumen_kv_ckpt* ckpt, uint64_t request_id);
 /* reqs[i].page_table / page_table_len: request ids[i]'s current table; reqs[i].t_end = t_cur;
- * reqs[i].t_begin is ignored (the checkpointer knows t_prev). */
+ * reqs[i].t_begin is ignored (the checkpointer knows t_prev).
+ * token_ids: NULL, or for each request a HOST pointer to its token history [0, t_cur) (entries
+ * may be NULL); the part the new delta needs is copied, and the sink then receives the page
+ * tags of the pages each delta touches ("each transferred page carries a page tag",
+ * PAPER.md:147), computed by lumen_kv_page_tags_host.  Without tokens n_tags is 0. */
 LUMEN_KV_API int lumen_kv_ckpt_notify(lumen_kv_ckpt* ckpt, const uint64_t* ids,
-                                      const lumen_kv_req* reqs, int32_t n, void* ready_event);
+                                      const lumen_kv_req* reqs, const int32_t* const* token_ids,
+                                      int32_t n, void* ready_event);
 LUMEN_KV_API int lumen_kv_ckpt_flush(lumen_kv_ckpt* ckpt);
 /* tokens of the request delivered to the sink so far (its t_prev), or EINVAL */
 LUMEN_KV_API int64_t lumen_kv_ckpt_progress(lumen_kv_ckpt* ckpt, uint64_t request_id);

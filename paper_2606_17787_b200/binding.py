@@ -37,7 +37,7 @@ EXPORTS = (
     "lumen_kv_stager_create", "lumen_kv_stager_destroy", "lumen_kv_checkpoint_pack_staged",
     "lumen_kv_restore_unpack_staged", "lumen_kv_plan_num_chunks", "lumen_kv_plan_get_chunks",
     "lumen_kv_checkpoint_pack_staged_commit", "lumen_kv_restore_unpack_staged_ready",
-    "lumen_kv_tags_num_pages", "lumen_kv_page_tags", "lumen_kv_longest_prefix",
+    "lumen_kv_tags_num_pages", "lumen_kv_page_tags", "lumen_kv_page_tags_host", "lumen_kv_longest_prefix",
     "lumen_kv_store_create", "lumen_kv_store_destroy", "lumen_kv_store_available",
     "lumen_kv_store_reserved", "lumen_kv_store_reserve", "lumen_kv_store_release",
     "lumen_kv_store_append", "lumen_kv_store_tokens", "lumen_kv_store_lookup",
@@ -75,9 +75,9 @@ class lumen_kv_chunk_info(ctypes.Structure):
                 ("byte_begin", ctypes.c_int64), ("byte_end", ctypes.c_int64)]
 
 
-# lumen_kv_sink_fn: (user, request_id, t_begin, t_end, delta pointer, delta_bytes)
+# lumen_kv_sink_fn: (user, request_id, t_begin, t_end, delta pointer, delta_bytes, tags, n_tags)
 SINK_FN = ctypes.CFUNCTYPE(None, ctypes.c_void_p, ctypes.c_uint64, ctypes.c_int64, ctypes.c_int64,
-                           ctypes.c_void_p, ctypes.c_int64)
+                           ctypes.c_void_p, ctypes.c_int64, ctypes.c_void_p, ctypes.c_int32)
 
 
 class LumenKVError(RuntimeError):
@@ -178,7 +178,9 @@ def _lib() -> ctypes.CDLL:
     L.lumen_kv_ckpt_untrack.restype = ctypes.c_int
     L.lumen_kv_ckpt_untrack.argtypes = [vp, ctypes.c_uint64]
     L.lumen_kv_ckpt_notify.restype = ctypes.c_int
-    L.lumen_kv_ckpt_notify.argtypes = [vp, vp, ctypes.POINTER(lumen_kv_req), i32, vp]
+    L.lumen_kv_ckpt_notify.argtypes = [vp, vp, ctypes.POINTER(lumen_kv_req), ctypes.POINTER(vp), i32, vp]
+    L.lumen_kv_page_tags_host.restype = i64
+    L.lumen_kv_page_tags_host.argtypes = [vp, i64, i64, i64, i32, vp, i64]
     L.lumen_kv_ckpt_flush.restype = ctypes.c_int
     L.lumen_kv_ckpt_flush.argtypes = [vp]
     L.lumen_kv_ckpt_progress.restype = i64
@@ -474,6 +476,18 @@ def lumen_kv_page_tags(token_ids_dev: int, tok_offset, page_size: int, tags_out_
         raise LumenKVError(rc, "lumen_kv_page_tags")
 
 
+def lumen_kv_page_tags_host(token_ids, first_token: int, t_begin: int, t_end: int, page_size: int) -> np.ndarray:
+    """Tags of the pages [t_begin, t_end) touches; token_ids[0] is token `first_token`."""
+    tok = np.ascontiguousarray(token_ids, dtype=np.int32)
+    cap = max(0, (int(t_end) - 1) // int(page_size) - int(t_begin) // int(page_size) + 1) if t_end > t_begin else 0
+    out = np.zeros(cap, dtype=TAG_DTYPE)
+    n = int(_lib().lumen_kv_page_tags_host(tok.ctypes.data, int(first_token), int(t_begin), int(t_end),
+                                           int(page_size), out.ctypes.data, cap))
+    if n < 0:
+        raise LumenKVError(n, "lumen_kv_page_tags_host")
+    return out[:n]
+
+
 def lumen_kv_longest_prefix(regen: np.ndarray, stored: np.ndarray) -> int:
     """regen, stored: host arrays of TAG_DTYPE.  Returns tokens of the longest contiguous prefix."""
     a = np.ascontiguousarray(regen, dtype=TAG_DTYPE)
@@ -599,7 +613,8 @@ def lumen_kv_recover(load, alive, interrupted):
 
 class BackgroundCheckpointer:
     """Owner of a `lumen_kv_ckpt*` (the worker's background checkpointing thread).
-    sink(request_id, t_begin, t_end, delta_ptr, delta_bytes) is called on that thread."""
+    sink(request_id, t_begin, t_end, delta_ptr, delta_bytes, tags) is called on that thread
+    (tags: a TAG_DTYPE array, empty unless notify() was given token IDs); or pass a Store."""
 
     def __init__(self, geom: lumen_kv_geom, k_planes, v_planes, staging_ptr: int, slot_bytes: int,
                  n_slots: int, pinned_ptr: int, pinned_bytes: int, sink):
@@ -609,7 +624,11 @@ class BackgroundCheckpointer:
             self._cb = ctypes.cast(_lib().lumen_kv_store_sink, SINK_FN)
             user = sink._h
         else:
-            self._cb = SINK_FN(lambda _u, rid, tb, te, ptr, nb: sink(int(rid), int(tb), int(te), int(ptr), int(nb)))
+            def _call(_u, rid, tb, te, ptr, nb, tags, n_tags):
+                t = (np.ctypeslib.as_array((ctypes.c_uint8 * (16 * n_tags)).from_address(tags)).view(TAG_DTYPE).copy()
+                     if n_tags else np.zeros(0, dtype=TAG_DTYPE))
+                sink(int(rid), int(tb), int(te), int(ptr), int(nb), t)
+            self._cb = SINK_FN(_call)
             user = None
         out = ctypes.c_void_p()
         rc = _lib().lumen_kv_ckpt_create(ctypes.byref(geom), _as_ptr_array(k_planes, L),
@@ -631,9 +650,14 @@ class BackgroundCheckpointer:
     def untrack(self, request_id: int) -> None:
         self._check(_lib().lumen_kv_ckpt_untrack(self._h, int(request_id)), "lumen_kv_ckpt_untrack")
 
-    def notify(self, ids, reqs, ready_event: int = 0) -> None:
-        """reqs: (page_table, _, t_cur) per id; ready_event: a cudaEvent_t handle or 0."""
+    def notify(self, ids, reqs, ready_event: int = 0, token_ids=None) -> None:
+        """reqs: (page_table, _, t_cur) per id; ready_event: a cudaEvent_t handle or 0;
+        token_ids: None or one int32 array (the request's token history [0, t_cur)) per id."""
         n = len(ids)
+        toks = None
+        if token_ids is not None:
+            tk = [np.ascontiguousarray(t, dtype=np.int32) for t in token_ids]
+            toks = (ctypes.c_void_p * max(n, 1))(*[t.ctypes.data for t in tk])
         ida = np.ascontiguousarray(ids, dtype=np.uint64)
         arr = (lumen_kv_req * max(n, 1))()
         keep = []
@@ -643,7 +667,7 @@ class BackgroundCheckpointer:
             arr[i].page_table = pt.ctypes.data if pt.size else None
             arr[i].page_table_len = pt.size
             arr[i].t_begin, arr[i].t_end = 0, int(te)
-        self._check(_lib().lumen_kv_ckpt_notify(self._h, ida.ctypes.data, arr, n,
+        self._check(_lib().lumen_kv_ckpt_notify(self._h, ida.ctypes.data, arr, toks, n,
                                                 ctypes.c_void_p(int(ready_event))), "lumen_kv_ckpt_notify")
 
     def flush(self) -> None:

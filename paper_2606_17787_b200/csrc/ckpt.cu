@@ -21,6 +21,8 @@ struct Pending {
     std::vector<int32_t> pt;   // page table as of the notification
     int64_t t_cur = 0;
     cudaEvent_t ev = nullptr;  // fires when tokens [.., t_cur) exist
+    std::vector<int32_t> toks; // token IDs [tok_base, t_cur), empty if the caller gave none
+    int64_t tok_base = 0;      // multiple of the page size, <= the page of the delta's first token
 };
 
 struct Tracked {
@@ -37,7 +39,19 @@ struct Job {
     std::vector<int32_t> pt;
     int64_t tb, te;
     cudaEvent_t ev;
+    std::vector<lumen_kv_tag> tags;   // tags of the pages [tb, te) touches
 };
+
+// tags of a job, from the token IDs the notification carried
+std::vector<lumen_kv_tag> tags_of(const Pending& p, int64_t tb, int64_t te, int32_t S) {
+    std::vector<lumen_kv_tag> out;
+    if (p.toks.empty() || te <= tb) return out;
+    out.resize(static_cast<size_t>((te - 1) / S - tb / S + 1));
+    if (lumen_kv_page_tags_host(p.toks.data(), p.tok_base, tb, te, S, out.data(),
+                                static_cast<int64_t>(out.size())) < 0)
+        out.clear();
+    return out;
+}
 
 // One enqueued pack: it owns one half of the pinned buffer until it has been delivered.
 struct Batch {
@@ -172,7 +186,8 @@ void deliver(lumen_kv_ckpt* c, Batch& b) {
                 b.rc = LUMEN_KV_ECUDA;
                 break;
             }
-            c->sink(c->user, b.jobs[i].id, b.jobs[i].tb, b.jobs[i].te, base + off, end - off);
+            c->sink(c->user, b.jobs[i].id, b.jobs[i].tb, b.jobs[i].te, base + off, end - off,
+                    b.jobs[i].tags.data(), static_cast<int32_t>(b.jobs[i].tags.size()));
         }
         std::lock_guard<std::mutex> g(c->mu);
         auto it = c->reqs.find(b.jobs[i].id);
@@ -207,7 +222,8 @@ void take_jobs(lumen_kv_ckpt* c, Batch& b, int64_t room) {
         }
         const int64_t want = (t.p.t_cur - t.t_sent) * c->token_bytes;
         if (want <= room) {
-            b.jobs.push_back(Job{kv.first, std::move(t.p.pt), t.t_sent, t.p.t_cur, t.p.ev});
+            b.jobs.push_back(Job{kv.first, std::move(t.p.pt), t.t_sent, t.p.t_cur, t.p.ev,
+                                 tags_of(t.p, t.t_sent, t.p.t_cur, c->geom.page_size)});
             t.has_pending = false;
             t.t_sent = t.p.t_cur;
             room -= want;
@@ -218,7 +234,8 @@ void take_jobs(lumen_kv_ckpt* c, Batch& b, int64_t room) {
                 t.has_pending = false;
                 continue;
             }
-            b.jobs.push_back(Job{kv.first, t.p.pt, t.t_sent, t.t_sent + fit, t.p.ev});
+            b.jobs.push_back(Job{kv.first, t.p.pt, t.t_sent, t.t_sent + fit, t.p.ev,
+                                 tags_of(t.p, t.t_sent, t.t_sent + fit, c->geom.page_size)});
             t.t_sent += fit;                        // the rest stays pending
             room = 0;
         } else {
@@ -350,8 +367,8 @@ int lumen_kv_ckpt_untrack(lumen_kv_ckpt* c, uint64_t id) {
     return LUMEN_KV_OK;
 }
 
-int lumen_kv_ckpt_notify(lumen_kv_ckpt* c, const uint64_t* ids, const lumen_kv_req* reqs, int32_t n,
-                         void* ready_event) {
+int lumen_kv_ckpt_notify(lumen_kv_ckpt* c, const uint64_t* ids, const lumen_kv_req* reqs,
+                         const int32_t* const* token_ids, int32_t n, void* ready_event) {
     if (!c || n < 0 || (n > 0 && (!ids || !reqs))) return LUMEN_KV_EINVAL;
     {
         std::lock_guard<std::mutex> g(c->mu);
@@ -372,6 +389,11 @@ int lumen_kv_ckpt_notify(lumen_kv_ckpt* c, const uint64_t* ids, const lumen_kv_r
             t.p.pt.assign(reqs[i].page_table, reqs[i].page_table + reqs[i].page_table_len);
             t.p.t_cur = reqs[i].t_end;
             t.p.ev = static_cast<cudaEvent_t>(ready_event);
+            t.p.toks.clear();
+            if (token_ids && token_ids[i]) {        // the tokens of the pages the delta touches
+                t.p.tok_base = (t.t_sent / S) * S;
+                t.p.toks.assign(token_ids[i] + t.p.tok_base, token_ids[i] + reqs[i].t_end);
+            }
             t.has_pending = true;
         }
     }

@@ -103,6 +103,30 @@ int lumen_kv_page_tags(const int32_t* token_ids, const int64_t* tok_offset, int3
     return LUMEN_KV_OK;
 }
 
+int64_t lumen_kv_page_tags_host(const int32_t* token_ids, int64_t first_token, int64_t t_begin,
+                                int64_t t_end, int32_t S, lumen_kv_tag* out, int64_t cap) {
+    if (S < 1 || t_begin < 0 || t_end < t_begin || cap < 0 || first_token < 0 ||
+        first_token % S != 0)
+        return LUMEN_KV_EINVAL;
+    if (t_end == t_begin) return 0;
+    const int64_t p0 = t_begin / S, p1 = (t_end - 1) / S;
+    if (!token_ids || first_token > p0 * S || (cap > 0 && !out)) return LUMEN_KV_EINVAL;
+    for (int64_t p = p0; p <= p1 && p - p0 < cap; ++p) {
+        const int64_t end = (p + 1) * S < t_end ? (p + 1) * S : t_end;
+        uint64_t h = 0xcbf29ce484222325ull;
+        for (int64_t t = p * S; t < end; ++t) {
+            const uint32_t v = static_cast<uint32_t>(token_ids[t - first_token]);
+            for (int b = 0; b < 4; ++b) {             // little-endian bytes of the token ID
+                h ^= (v >> (8 * b)) & 0xffu;
+                h *= 0x100000001b3ull;
+            }
+        }
+        out[p - p0].hash = h;
+        out[p - p0].end_pos = end;
+    }
+    return p1 - p0 + 1;
+}
+
 int64_t lumen_kv_longest_prefix(const lumen_kv_tag* regen, int64_t n_regen,
                                 const lumen_kv_tag* stored, int64_t n_stored) {
     if (n_regen < 0 || n_stored < 0 || (n_regen > 0 && !regen) || (n_stored > 0 && !stored))

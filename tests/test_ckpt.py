@@ -56,15 +56,19 @@ def test_background_checkpointing_decode_loop(lk):
     for rid, n in enumerate(lens):
         st.reserve(rid, n + steps * dtok)
     delivered, errors = {rid: [] for rid in range(len(lens))}, []
-    none = np.zeros(0, dtype=lk.TAG_DTYPE)
+    rng = substream(8, "ckpt_tokens")
+    hist = [rng.integers(0, 151936, size=n + steps * dtok + 9).astype(np.int32) for n in lens]
 
-    def sink(rid, tb, te, ptr, nbytes):                      # runs on the checkpointer's thread
+    def sink(rid, tb, te, ptr, nbytes, tags):                # runs on the checkpointer's thread
         try:
             got = np.ctypeslib.as_array((np.ctypeslib.ctypes.c_uint16 * (nbytes // 2)).from_address(ptr))
             ref = oracle.pack(w.geom, K, V, [(w.reqs[rid][0], tb, te)])
             if nbytes != (te - tb) * tokb or not np.array_equal(got, ref):
                 errors.append(("bytes", rid, tb, te))
-            st.append(rid, tb, te, ptr, nbytes, none)        # step (4): into the holder's store
+            want = oracle.page_tags(hist[rid][:te], S)       # "each transferred page carries a page tag"
+            if not np.array_equal(tags, want[want["end_pos"] > tb]):
+                errors.append(("tags", rid, tb, te))
+            st.append(rid, tb, te, ptr, nbytes, tags)        # step (4): into the holder's store
             delivered[rid].append((tb, te))
         except Exception as e:                               # noqa: BLE001
             errors.append((rid, repr(e)))
@@ -84,7 +88,7 @@ def test_background_checkpointing_decode_loop(lk):
             ev.record(compute)
         events.append(ev)
         cur = [(pt, 0, n + step * dtok) for (pt, _, n) in w.reqs]
-        bg.notify(ids, cur, ev.cuda_event)                   # never waits for the checkpointer
+        bg.notify(ids, cur, ev.cuda_event, token_ids=hist)   # never waits for the checkpointer
     with pytest.raises(lk.LumenKVError):                     # going backwards is refused
         bg.notify([0], [(w.reqs[0][0], 0, 5)])
     with pytest.raises(lk.LumenKVError):
@@ -104,6 +108,14 @@ def test_background_checkpointing_decode_loop(lk):
     reqs, lays = [], []
     for rid, (pt_new, _, n) in enumerate(w.restore_reqs):
         final = n + steps * dtok
+        # the holder regenerates the tags from the token history (CUDA kernel) and finds the prefix
+        d_tok = torch.from_numpy(hist[rid]).cuda()
+        n_pg = lk.lumen_kv_tags_num_pages([0, hist[rid].size], S)
+        d_tags = torch.empty((n_pg, 2), dtype=torch.int64, device="cuda")
+        lk.lumen_kv_page_tags(d_tok.data_ptr(), [0, hist[rid].size], S, d_tags.data_ptr(), n_pg, 0)
+        torch.cuda.synchronize()
+        regen = d_tags.cpu().numpy().copy().view(lk.TAG_DTYPE).reshape(-1)
+        assert st.lookup(rid, regen) == (final // S) * S      # history is 9 tokens longer: page aligned
         for s in st.segments(rid, final):
             reqs.append((pt_new, int(s["t_begin"]), int(s["t_end"])))
             lays.append((int(s["buf_offset"]), int(s["plane_stride_tokens"])))

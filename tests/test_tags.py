@@ -112,6 +112,27 @@ def test_library_lookup_equals_oracle(lk):
         lk.lumen_kv_tags_num_pages([0, 5, 3], 16)
 
 
+def test_host_tags_equal_oracle(lk):
+    """lumen_kv_page_tags_host: the tags a sender attaches to a delta [tb, te) == the oracle's tags
+    of a history of te tokens, restricted to the pages the delta touches."""
+    rng = substream(4, "tags_host")
+    for _ in range(200):
+        S = int(rng.choice([1, 3, 16, 32]))
+        te = int(rng.integers(1, 20 * S))
+        tb = int(rng.integers(0, te))
+        tok = rng.integers(-2**31, 2**31, size=te + 5, dtype=np.int64).astype(np.int32)
+        ref = oracle.page_tags(tok[:te], S)
+        ref = ref[ref["end_pos"] > tb]
+        first = (tb // S) * S - S * int(rng.integers(0, 2)) * (tb // S > 0)      # any earlier page start
+        got = lk.lumen_kv_page_tags_host(tok[first:], first, tb, te, S)
+        assert np.array_equal(got, ref)
+    assert lk.lumen_kv_page_tags_host(np.zeros(4, np.int32), 0, 3, 3, 16).size == 0
+    with pytest.raises(lk.LumenKVError):                              # first_token not a page start
+        lk.lumen_kv_page_tags_host(np.zeros(40, np.int32), 5, 6, 20, 16)
+    with pytest.raises(lk.LumenKVError):                              # tokens start after the delta's page
+        lk.lumen_kv_page_tags_host(np.zeros(40, np.int32), 16, 6, 20, 16)
+
+
 # ---- CUDA kernel vs oracle -------------------------------------------------------------------
 @pytest.mark.gpu
 def test_gpu_page_tags_equal_oracle(lk):
