@@ -434,6 +434,28 @@ LUMEN_KV_API int lumen_kv_ckpt_flush(lumen_kv_ckpt* ckpt);
 LUMEN_KV_API int64_t lumen_kv_ckpt_progress(lumen_kv_ckpt* ckpt, uint64_t request_id);
 
 /*
+ * lumen_kv_store_restore -- KV-reuse recovery of one request on its checkpoint holder
+ * (PAPER.md:157): "From the request's token history, the holder deterministically regenerates
+ * page tags to locate the longest contiguous checkpointed prefix within its local store,
+ * subsequently loading the matching KV pages into GPU memory."  One call: regenerate the tags
+ * of token_ids[0, n_tokens) (host), look the prefix up in the store, build an explicit-layout
+ * plan over the stored deltas that cover it (lumen_kv_store_segments) with the fresh
+ * page_table, and restore it out of the store's arena through the two-stage path.
+ *   arena must be pinned (it is the source of the H2D copies); page_table must cover the
+ *   prefix; k_planes / v_planes / stager / stream as for lumen_kv_restore_unpack_staged.
+ *   *restored_tokens receives the prefix length P; the suffix [P, n_tokens) is the caller's to
+ *   recompute ("partial prefill on the uncheckpointed suffix").
+ * Asynchronous on `stream` like the restore itself.  Errors: EINVAL (unknown request, table too
+ * short), ERANGE, EOVERLAP, ESIZE, ENOMEM, ECUDA.
+ */
+LUMEN_KV_API int lumen_kv_store_restore(const lumen_kv_store* store, uint64_t request_id,
+                                        const int32_t* token_ids, int64_t n_tokens,
+                                        const lumen_kv_geom* geom, const int32_t* page_table,
+                                        int64_t page_table_len, void* const* k_planes,
+                                        void* const* v_planes, lumen_kv_stager* stager,
+                                        void* stream, int64_t* restored_tokens);
+
+/*
  * Controller logic (host arithmetic only; section 4.2 Eq. (1), section 4.3).
  *
  * lumen_kv_choose_holder -- checkpoint placement, Eq. (1):

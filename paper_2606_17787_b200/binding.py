@@ -42,6 +42,7 @@ EXPORTS = (
     "lumen_kv_store_reserved", "lumen_kv_store_reserve", "lumen_kv_store_release",
     "lumen_kv_store_append", "lumen_kv_store_tokens", "lumen_kv_store_lookup",
     "lumen_kv_store_segments", "lumen_kv_store_sink", "lumen_kv_store_sink_errors",
+    "lumen_kv_store_restore",
     "lumen_kv_choose_holder", "lumen_kv_recover",
     "lumen_kv_ckpt_create", "lumen_kv_ckpt_destroy", "lumen_kv_ckpt_track", "lumen_kv_ckpt_untrack",
     "lumen_kv_ckpt_notify", "lumen_kv_ckpt_flush", "lumen_kv_ckpt_progress",
@@ -158,6 +159,10 @@ def _lib() -> ctypes.CDLL:
     L.lumen_kv_store_tokens.argtypes = [vp, u64]
     L.lumen_kv_store_lookup.restype = i64
     L.lumen_kv_store_lookup.argtypes = [vp, u64, vp, i64]
+    L.lumen_kv_store_restore.restype = ctypes.c_int
+    L.lumen_kv_store_restore.argtypes = [vp, u64, vp, i64, ctypes.POINTER(lumen_kv_geom), vp, i64,
+                                         ctypes.POINTER(vp), ctypes.POINTER(vp), vp, vp,
+                                         ctypes.POINTER(i64)]
     L.lumen_kv_store_sink_errors.restype = i64
     L.lumen_kv_store_sink_errors.argtypes = [vp]
     L.lumen_kv_store_segments.restype = i64
@@ -550,6 +555,21 @@ class Store:
         t = np.ascontiguousarray(regen, dtype=TAG_DTYPE)
         return self._check(_lib().lumen_kv_store_lookup(self._h, int(request_id), t.ctypes.data, t.size),
                            "lumen_kv_store_lookup")
+
+    def restore(self, request_id: int, token_ids, geom: lumen_kv_geom, page_table, k_planes, v_planes,
+                stager: "Stager", stream: int = 0) -> int:
+        """KV-reuse recovery of one request (lumen_kv_store_restore); returns the restored prefix."""
+        tok = np.ascontiguousarray(token_ids, dtype=np.int32)
+        pt = np.ascontiguousarray(page_table, dtype=np.int32)
+        L = geom.num_layers
+        out = ctypes.c_int64(0)
+        rc = _lib().lumen_kv_store_restore(self._h, int(request_id), tok.ctypes.data, tok.size,
+                                           ctypes.byref(geom), pt.ctypes.data, pt.size,
+                                           _as_ptr_array(k_planes, L), _as_ptr_array(v_planes, L),
+                                           stager.handle, ctypes.c_void_p(int(stream)), ctypes.byref(out))
+        if rc:
+            raise LumenKVError(rc, "lumen_kv_store_restore")
+        return int(out.value)
 
     @property
     def sink_errors(self) -> int:

@@ -213,6 +213,12 @@ void lumen_kv_store_sink(void* store, uint64_t id, int64_t t_begin, int64_t t_en
     }
 }
 
+// internal (recover.cu): the arena the segments' offsets refer to; not exported
+const void* lumen_kv_store_arena_(const lumen_kv_store* s, int64_t* bytes) {
+    if (bytes) *bytes = s ? s->arena_bytes : 0;
+    return s ? s->arena : nullptr;
+}
+
 int64_t lumen_kv_store_sink_errors(const lumen_kv_store* s) {
     if (!s) return LUMEN_KV_EINVAL;
     std::lock_guard<std::mutex> g(s->mu);

@@ -102,32 +102,33 @@ def test_background_checkpointing_decode_loop(lk):
         assert spans[0][0] == 0 and spans[-1][1] == final
         assert all(a[1] == b[0] for a, b in zip(spans, spans[1:]))        # in order, no gap
         assert all(te - tb <= 32 for tb, te in spans)                      # never more than half the pinned buffer
-    # ---- failure: restore every request's checkpoint out of the arena into fresh pages ----
+    # ---- failure: KV-reuse recovery of every request on the holder, one call each ----
     pool_b = G.make_pool(w.geom, 42)
     K2, V2 = G.host_planes(w.geom, 42)
-    reqs, lays = [], []
+    ring = G.StagingRing(1 << 20, 3)
+    side = torch.cuda.Stream()
     for rid, (pt_new, _, n) in enumerate(w.restore_reqs):
         final = n + steps * dtok
-        # the holder regenerates the tags from the token history (CUDA kernel) and finds the prefix
+        # cross-check the host-regenerated tags the call uses with the CUDA kernel's
         d_tok = torch.from_numpy(hist[rid]).cuda()
         n_pg = lk.lumen_kv_tags_num_pages([0, hist[rid].size], S)
         d_tags = torch.empty((n_pg, 2), dtype=torch.int64, device="cuda")
         lk.lumen_kv_page_tags(d_tok.data_ptr(), [0, hist[rid].size], S, d_tags.data_ptr(), n_pg, 0)
         torch.cuda.synchronize()
         regen = d_tags.cpu().numpy().copy().view(lk.TAG_DTYPE).reshape(-1)
-        assert st.lookup(rid, regen) == (final // S) * S      # history is 9 tokens longer: page aligned
-        for s in st.segments(rid, final):
-            reqs.append((pt_new, int(s["t_begin"]), int(s["t_end"])))
-            lays.append((int(s["buf_offset"]), int(s["plane_stride_tokens"])))
-        oracle.unpack(w.geom, K2, V2, [(pt_new, 0, final)],
-                      oracle.pack(w.geom, K, V, [(w.reqs[rid][0], 0, final)]))
-    ck_b = G.Checkpointer(pool_b)
-    rplan = ck_b.plan(reqs, unique_dst=True, layouts=lays)
-    ring = G.StagingRing(1 << 20, 3)
-    ck_b.unpack_staged(rplan, arena, ring)
-    torch.cuda.synchronize()
+        assert np.array_equal(regen, lk.lumen_kv_page_tags_host(hist[rid], 0, 0, hist[rid].size, S))
+        prefix = st.restore(rid, hist[rid], pool_b.geom, pt_new, pool_b.k_ptrs, pool_b.v_ptrs,
+                            ring.stager, side.cuda_stream)
+        assert prefix == st.lookup(rid, regen) == (final // S) * S   # the history is 9 tokens longer
+        oracle.unpack(w.geom, K2, V2, [(pt_new, 0, prefix)],
+                      oracle.pack(w.geom, K, V, [(w.reqs[rid][0], 0, prefix)]))
+    side.synchronize()
     for t, ref in zip(pool_b.planes(), [x for kv in zip(K2, V2) for x in kv]):
         assert np.array_equal(G.plane_to_np(t), ref)
+    assert st.restore(0, hist[0][::-1].copy(), pool_b.geom, w.restore_reqs[0][0], pool_b.k_ptrs,
+                      pool_b.v_ptrs, ring.stager, 0) == 0               # another history: nothing to reuse
+    with pytest.raises(lk.LumenKVError):
+        st.restore(77, hist[0], pool_b.geom, w.restore_reqs[0][0], pool_b.k_ptrs, pool_b.v_ptrs, ring.stager, 0)
     bg.untrack(0)
     with pytest.raises(lk.LumenKVError):
         bg.progress(0)
