@@ -1059,6 +1059,9 @@ def run_overhead(args):
     pinned = pinned_buffer(1 << 30)
     lens = [te for _, _, te in w.reqs]
     ids = list(range(len(lens)))
+    from paper_2606_17787_b200.pool import StagingRing
+    rng = np.random.default_rng(MASTER_SEED)
+    hist = [rng.integers(0, 151936, size=n + iters * 16).astype(np.int32) for n in lens]   # token IDs
 
     # the GPU side of the pipeline alone: prefill-completion checkpoint of all prompts into a sink
     # that drops the bytes (pack -> staging ring -> copy engine -> pinned halves -> nothing)
@@ -1087,7 +1090,7 @@ def run_overhead(args):
                 st.reserve(rid, n + iters * delta_tokens)
                 bg.track(rid, 0)
             t0 = time.perf_counter()                         # prefill-completion checkpoint, untimed part
-            bg.notify(ids, [(pt, 0, n) for (pt, _, n) in w.reqs])
+            bg.notify(ids, [(pt, 0, n) for (pt, _, n) in w.reqs], token_ids=hist)
             bg.flush()
             dt = time.perf_counter() - t0
             prefill = {"GiB": sum(lens) * tokb / 2**30, "s": dt, "GBps": sum(lens) * tokb / dt / 1e9}
@@ -1105,7 +1108,7 @@ def run_overhead(args):
                 evs.append(ev)
                 if bg is not None:
                     bg.notify(ids, [(pt, 0, n + (it + 1) * delta_tokens) for (pt, _, n) in w.reqs],
-                              ev.cuda_event)
+                              ev.cuda_event, token_ids=hist)
             e1.record(compute)
         compute.synchronize()
         t_loop = time.perf_counter() - t0
@@ -1118,6 +1121,25 @@ def run_overhead(args):
             assert st.sink_errors == 0 and all(st.tokens(r) == n + iters * delta_tokens for r, n in enumerate(lens))
             out["checkpointed_MiB_per_iteration"] = len(lens) * delta_tokens * tokb / 2**20
             out["prefill_checkpoint"] = prefill
+            # the worker "fails": every request is recovered on the holder, one call each
+            # (tags from the token history -> prefix -> layout plan -> staged restore into fresh pages)
+            rs = torch.cuda.Stream()
+            ringr = StagingRing(32 << 20, 3)
+            r0, r1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize()
+            t1 = time.perf_counter()
+            r0.record(rs)
+            restored = 0
+            for rid, (pt_new, _, n) in enumerate(w.restore_reqs):
+                restored += st.restore(rid, hist[rid][: n + iters * delta_tokens], pool.geom, pt_new,
+                                       pool.k_ptrs, pool.v_ptrs, ringr.stager, rs.cuda_stream)
+            r1.record(rs)
+            rs.synchronize()
+            assert restored == sum(n + iters * delta_tokens for n in lens)   # history == what was checkpointed
+            out["recovery"] = {"requests": len(lens), "tokens": restored, "GiB": restored * tokb / 2**30,
+                               "device_ms": r0.elapsed_time(r1), "host_s": time.perf_counter() - t1,
+                               "GBps": restored * tokb / r0.elapsed_time(r1) / 1e6}
+            ringr.close()
             bg.close()
             st.close()
             wdev.unpin(arena)
