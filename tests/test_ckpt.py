@@ -133,3 +133,77 @@ def test_background_checkpointing_decode_loop(lk):
     with pytest.raises(lk.LumenKVError):
         bg.progress(0)
     bg.close()
+
+
+@pytest.mark.gpu
+def test_background_checkpointer_stress(lk):
+    """Three producer threads notify their requests at random paces (tiny pinned buffer, so deltas
+    are batched, split and superseded in every combination), some requests are untracked in
+    mid-flight: every delivered delta is the oracle's, each request's deltas tile a prefix of its
+    tokens in order, and what was not untracked is delivered completely."""
+    import random
+    import time
+    import torch
+    from tests import gpu_util as G
+    G.build_all()
+    w = cfg1_qwen14b(L=2, N=2048, n_reqs=12, grow_iters=20, median=120, hi=260, lo=30)
+    L, H, D, S, N = w.geom
+    tokb = 2 * L * H * D * 2
+    pool = G.make_pool(w.geom, 51)
+    K, V = G.host_planes(w.geom, 51)
+    lens = [te for _, _, te in w.reqs]
+    final = [n + 20 * 16 for n in lens]
+    ring_mem = torch.empty(2 * (256 << 10), dtype=torch.uint8, device="cuda")
+    pinned = G.pinned_buffer(48 * tokb)
+    spans, errors, lock = {r: [] for r in range(len(lens))}, [], threading.Lock()
+
+    def sink(rid, tb, te, ptr, nbytes, tags):
+        got = np.ctypeslib.as_array((np.ctypeslib.ctypes.c_uint16 * (nbytes // 2)).from_address(ptr))
+        if not np.array_equal(got, oracle.pack(w.geom, K, V, [(w.reqs[rid][0], tb, te)])):
+            errors.append(("bytes", rid, tb, te))
+        with lock:
+            spans[rid].append((tb, te))
+
+    bg = lk.BackgroundCheckpointer(pool.geom, pool.k_ptrs, pool.v_ptrs, ring_mem.data_ptr(), 256 << 10, 2,
+                                   pinned.data_ptr(), pinned.numel(), sink)
+    for rid in range(len(lens)):
+        bg.track(rid, 0)
+    dropped = {}
+
+    def producer(tid):
+        rnd = random.Random(tid)
+        mine = [r for r in range(len(lens)) if r % 3 == tid]
+        cur = {r: 0 for r in mine}
+        try:
+            while mine:
+                batch = rnd.sample(mine, rnd.randint(1, len(mine)))
+                for r in batch:
+                    cur[r] = min(final[r], cur[r] + rnd.choice([1, 1, 16, 40, lens[r]]))
+                bg.notify(batch, [(w.reqs[r][0], 0, cur[r]) for r in batch])
+                if rnd.random() < 0.3:
+                    time.sleep(rnd.random() * 0.002)
+                if rnd.random() < 0.04 and len(mine) > 1:       # a request completes / is cancelled
+                    r = mine.pop(rnd.randrange(len(mine)))
+                    bg.untrack(r)
+                    dropped[r] = cur[r]
+                mine = [r for r in mine if cur[r] < final[r]]
+        except Exception as e:                                   # noqa: BLE001
+            errors.append((tid, repr(e)))
+
+    threads = [threading.Thread(target=producer, args=(t,)) for t in range(3)]
+    for t in threads:
+        t.start()
+    for t in threads:
+        t.join(timeout=120)
+    bg.flush()
+    assert not errors and not any(t.is_alive() for t in threads)
+    for rid in range(len(lens)):
+        sp = spans[rid]
+        assert all(a[1] == b[0] for a, b in zip(sp, sp[1:])) and (not sp or sp[0][0] == 0)
+        assert all(te - tb <= 24 for tb, te in sp)               # half of the 48-token pinned buffer
+        end = sp[-1][1] if sp else 0
+        if rid in dropped:
+            assert end <= dropped[rid]                           # a prefix of what had been notified
+        else:
+            assert end == final[rid] and bg.progress(rid) == final[rid]
+    bg.close()
