@@ -345,7 +345,7 @@ def run_ours(args):
         raise RuntimeError("bench.py needs a CUDA device: there is no CPU path for --impl ours")
     torch.cuda.set_device(local)
     dist = None
-    if world > 1:
+    if world > 1 or os.environ.get("LUMEN_BENCH_FORCE_DIST"):   # the switch exercises the N > 1 code on 1 GPU
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     wdev.build()
