@@ -39,6 +39,8 @@
  *     complete (and, for host destinations, host-visible) once an event recorded
  *     on that stream after the call has fired (nothing is promised
  *     earlier).
+ *   - pack/unpack may be captured into a CUDA graph (stream capture); the plan must then
+ *     stay alive for as long as the graph can be replayed.
  *   - A plan is immutable and direction-agnostic: the same plan drives pack and
  *     unpack.  The caller owns pools, buffers, streams and page tables (page
  *     tables are copied at build time).  Plans may be used concurrently from

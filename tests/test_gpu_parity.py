@@ -582,3 +582,36 @@ def test_other_element_widths(G, elem_bytes):
     assert np.array_equal(G.buf_to_np(buf, plan.nbytes), ref)
     for t, r in zip(pool_b.planes(), [x for kv in zip(K2, V2) for x in kv]):
         assert np.array_equal(G.plane_to_np(t), r)
+
+
+@pytest.mark.parametrize("kernel", ["warp", "warp_upload", "bulk"])
+def test_cuda_graph_capture(G, kernel):
+    """pack + restore captured into a CUDA graph (with the programmatic-launch attribute on the
+    SIMT kernel) and replayed: same bytes as the oracle, every replay."""
+    import torch
+    lk = G.lk
+    w = cfg1_qwen14b(L=2, N=1024, n_reqs=8, grow_iters=2, median=100, hi=256, lo=20)
+    K, V = G.host_planes(w.geom, 3)
+    ref = oracle.pack(w.geom, K, V, w.reqs)
+    K2, V2 = G.host_planes(w.geom, 4)
+    oracle.unpack(w.geom, K2, V2, w.restore_reqs, ref)
+    pool, pool_b = G.make_pool(w.geom, 3), G.make_pool(w.geom, 4)
+    s = torch.cuda.Stream()
+    plan = lk.lumen_kv_plan_build(pool.geom, w.reqs, G.KERNELS[kernel], s.cuda_stream)
+    rplan = lk.lumen_kv_plan_build(pool.geom, w.restore_reqs, G.KERNELS[kernel], s.cuda_stream)
+    buf = torch.zeros(plan.nbytes, dtype=torch.uint8, device="cuda")
+    s.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g, stream=s):
+        lk.lumen_kv_checkpoint_pack(plan, pool.k_ptrs, pool.v_ptrs, buf.data_ptr(), plan.nbytes, 0, s.cuda_stream)
+        lk.lumen_kv_restore_unpack(rplan, pool_b.k_ptrs, pool_b.v_ptrs, buf.data_ptr(), plan.nbytes, 0,
+                                   s.cuda_stream)
+    for _ in range(3):
+        buf.zero_()
+        g.replay()
+        torch.cuda.synchronize()
+        assert np.array_equal(G.buf_to_np(buf, plan.nbytes), ref)
+    for t, r in zip(pool_b.planes(), [x for kv in zip(K2, V2) for x in kv]):
+        assert np.array_equal(G.plane_to_np(t), r)
+    del g
+    plan.close(); rplan.close()
