@@ -430,6 +430,10 @@ def run_ours(args):
         barrier(); torch.cuda.synchronize()
         if sampler:
             sampler.start()
+        # the W warm-up steps again, untimed, right in front of the timed ones: the device is
+        # busy (clocks up, pipeline full) when the start event fires, whatever K is
+        for i in range(W):
+            step(i, bufs, kind, lag_, None, only)
         t_wall = time.perf_counter()
         e_start.record(stream)
         for i in range(K):
