@@ -11,6 +11,7 @@
 #include <new>
 #include <vector>
 
+#include "internal.hpp"
 #include "lumen_kv.h"
 
 namespace {
@@ -96,7 +97,8 @@ int lumen_kv_page_tags(const int32_t* token_ids, const int64_t* tok_offset, int3
             dim3 grid(static_cast<unsigned>(gx), static_cast<unsigned>(nr), 1);
             page_tags_kernel<<<grid, 128, 0, static_cast<cudaStream_t>(stream)>>>(
                 p, token_ids, tags_out + tag_base, page_size);
-            if (cudaGetLastError() != cudaSuccess) return LUMEN_KV_ECUDA;
+            const cudaError_t e = cudaGetLastError();
+            if (e != cudaSuccess) return lumen::cuda_fail(e);
         }
         tag_base += p.page_off[nr];
     }
