@@ -2,6 +2,7 @@
 // caller-provided host arena, append-only deltas with their page tags, lookups that only see
 // completely received deltas.  Pure host C++: no CUDA in here.
 #include <algorithm>
+#include <condition_variable>
 #include <cstring>
 #include <map>
 #include <mutex>
@@ -29,7 +30,80 @@ struct Entry {
     std::vector<lumen_kv_tag> tags;
 };
 
-constexpr int64_t kParallelCopyMin = 8 << 20;   // below this one memcpy beats starting threads
+constexpr int64_t kParallelCopyMin = 1 << 20;   // below this one memcpy beats waking the pool
+
+// Persistent copy threads: an append is cut into slices that the pool's threads and the caller
+// copy together.  Waking sleeping threads costs microseconds, starting new ones per append
+// (the first version) cost tens -- too much for the 2.5 MiB deltas of a decode step.
+class CopyPool {
+public:
+    explicit CopyPool(int threads) {
+        for (int i = 1; i < threads; ++i) workers_.emplace_back([this] { loop(); });
+    }
+    ~CopyPool() {
+        {
+            std::lock_guard<std::mutex> g(mu_);
+            stop_ = true;
+        }
+        cv_.notify_all();
+        for (auto& t : workers_) t.join();
+    }
+    // One copy at a time (appends of different requests queue up here: the memory bus is shared).
+    void copy(char* dst, const char* src, int64_t bytes) {
+        const int64_t parts = static_cast<int64_t>(workers_.size()) + 1;
+        if (parts == 1 || bytes < kParallelCopyMin) {
+            std::memcpy(dst, src, static_cast<size_t>(bytes));
+            return;
+        }
+        std::lock_guard<std::mutex> one(job_mu_);
+        const int64_t slice = ((bytes / parts) + 4095) & ~int64_t{4095};
+        {
+            std::lock_guard<std::mutex> g(mu_);
+            dst_ = dst;
+            src_ = src;
+            bytes_ = bytes;
+            slice_ = slice;
+            next_ = slice;          // slice 0 is the caller's
+            pending_ = 0;
+            for (int64_t at = slice; at < bytes; at += slice) ++pending_;
+            ++generation_;
+        }
+        cv_.notify_all();
+        std::memcpy(dst, src, static_cast<size_t>(std::min(slice, bytes)));
+        std::unique_lock<std::mutex> lk(mu_);
+        done_cv_.wait(lk, [&] { return pending_ == 0; });
+    }
+
+private:
+    void loop() {
+        uint64_t seen = 0;
+        std::unique_lock<std::mutex> lk(mu_);
+        for (;;) {
+            cv_.wait(lk, [&] { return stop_ || (generation_ != seen && next_ < bytes_); });
+            if (stop_) return;
+            while (next_ < bytes_) {
+                const int64_t at = next_;
+                next_ += slice_;
+                const int64_t n = std::min(slice_, bytes_ - at);
+                char* d = dst_ + at;
+                const char* s = src_ + at;
+                lk.unlock();
+                std::memcpy(d, s, static_cast<size_t>(n));
+                lk.lock();
+                if (--pending_ == 0) done_cv_.notify_all();
+            }
+            seen = generation_;
+        }
+    }
+    std::vector<std::thread> workers_;
+    std::mutex mu_, job_mu_;
+    std::condition_variable cv_, done_cv_;
+    char* dst_ = nullptr;
+    const char* src_ = nullptr;
+    int64_t bytes_ = 0, slice_ = 0, next_ = 0, pending_ = 0;
+    uint64_t generation_ = 0;
+    bool stop_ = false;
+};
 
 }  // namespace
 
@@ -44,26 +118,9 @@ struct lumen_kv_store {
     std::unordered_map<uint64_t, Entry> reqs;
     int64_t reserved = 0;
     int64_t sink_errors = 0;
+    CopyPool* pool = nullptr;
+    ~lumen_kv_store() { delete pool; }
 };
-
-namespace {
-
-void parallel_copy(char* dst, const char* src, int64_t bytes, int threads) {
-    if (threads <= 1 || bytes < kParallelCopyMin) {
-        std::memcpy(dst, src, static_cast<size_t>(bytes));
-        return;
-    }
-    const int64_t slice = ((bytes / threads) + 4095) & ~int64_t{4095};
-    std::vector<std::thread> pool;
-    for (int64_t at = slice; at < bytes; at += slice) {
-        const int64_t n = std::min(slice, bytes - at);
-        pool.emplace_back([=] { std::memcpy(dst + at, src + at, static_cast<size_t>(n)); });
-    }
-    std::memcpy(dst, src, static_cast<size_t>(std::min(slice, bytes)));
-    for (auto& t : pool) t.join();
-}
-
-}  // namespace
 
 extern "C" {
 
@@ -82,6 +139,11 @@ int lumen_kv_store_create(void* arena, int64_t arena_bytes, int64_t token_bytes,
     s->token_bytes = token_bytes;
     s->page_size = page_size;
     s->copy_threads = copy_threads;
+    s->pool = new (std::nothrow) CopyPool(copy_threads);
+    if (!s->pool) {
+        delete s;
+        return LUMEN_KV_ENOMEM;
+    }
     if (arena_bytes > 0) s->free_[0] = arena_bytes;
     *out = s;
     return LUMEN_KV_OK;
@@ -168,7 +230,7 @@ int lumen_kv_store_append(lumen_kv_store* s, uint64_t id, int64_t t_begin, int64
         e.receiving = n;                                   // claims the region's tail
         dst = s->arena + e.region_off + e.tokens * s->token_bytes;
     }
-    parallel_copy(dst, static_cast<const char*>(delta), delta_bytes, s->copy_threads);
+    s->pool->copy(dst, static_cast<const char*>(delta), delta_bytes);
     {
         // publication: the delta and its tags become visible together, after the last byte
         std::lock_guard<std::mutex> g(s->mu);
