@@ -404,7 +404,9 @@ LUMEN_KV_API int64_t lumen_kv_store_segments(const lumen_kv_store* store, uint64
  *                 while the sink drains one, the copy engine fills the other.  Deltas are
  *                 batched up to one half; a delta larger than a half is delivered in pieces.
  * notify() copies the page tables and returns at once; deltas of one request are delivered
- * in order; a later notify for a request supersedes an earlier one that has not started.
+ * in order; a later notification for a request extends an earlier one that has not started, and
+ * each keeps its own ready event: the checkpointer packs what is ready now, up to the newest
+ * notification whose event has fired.
  * ready_event: a cudaEvent_t recorded after the batch that produced the tokens (NULL: they
  * already exist); it must stay valid until the delta has been delivered.
  * flush() blocks until everything notified before the call has been delivered and returns

@@ -19,8 +19,10 @@ namespace {
 
 struct Pending {
     std::vector<int32_t> pt;   // page table as of the notification
-    int64_t t_cur = 0;
-    cudaEvent_t ev = nullptr;  // fires when tokens [.., t_cur) exist
+    int64_t t_cur = 0;         // = marks.back().first
+    // (t, event): tokens [.., t) exist once the event has fired; ascending in t.  A later
+    // notification does not replace an earlier one's event: what is ready now is packed now.
+    std::vector<std::pair<int64_t, cudaEvent_t>> marks;
     std::vector<int32_t> toks; // token IDs [tok_base, t_cur), empty if the caller gave none
     int64_t tok_base = 0;      // multiple of the page size, <= the page of the delta's first token
 };
@@ -205,10 +207,26 @@ void deliver(lumen_kv_ckpt* c, Batch& b) {
         --t.in_flight;
         if (b.rc != LUMEN_KV_OK) {                  // do not retry for ever
             t.has_pending = false;
+            t.p.marks.clear();
             t.t_sent = t.t_prev;
         }
         if (t.zombie && t.in_flight == 0) c->reqs.erase(it);
     }
+}
+
+// The newest mark whose event has fired (readiness is monotonic in t); the oldest one if none has.
+size_t ready_mark(const Pending& p) {
+    size_t k = 0;
+    for (size_t i = 0; i < p.marks.size(); ++i) {
+        const cudaEvent_t ev = p.marks[i].second;
+        if (ev != nullptr && cudaEventQuery(ev) == cudaErrorNotReady) {
+            (void)cudaGetLastError();
+            break;
+        }
+        (void)cudaGetLastError();
+        k = i;
+    }
+    return k;
 }
 
 // Under the lock: move pending deltas into a batch, at most `room` bytes (one buffer half).
@@ -216,25 +234,33 @@ void take_jobs(lumen_kv_ckpt* c, Batch& b, int64_t room) {
     for (auto& kv : c->reqs) {
         Tracked& t = kv.second;
         if (!t.has_pending) continue;
-        if (t.p.t_cur <= t.t_sent) {                // nothing beyond what is already on its way
+        while (!t.p.marks.empty() && t.p.marks.front().first <= t.t_sent)
+            t.p.marks.erase(t.p.marks.begin());     // already on its way
+        if (t.p.marks.empty()) {
             t.has_pending = false;
             continue;
         }
-        const int64_t want = (t.p.t_cur - t.t_sent) * c->token_bytes;
+        const size_t k = ready_mark(t.p);
+        const int64_t te = t.p.marks[k].first;
+        const cudaEvent_t ev = t.p.marks[k].second;
+        const int64_t want = (te - t.t_sent) * c->token_bytes;
         if (want <= room) {
-            b.jobs.push_back(Job{kv.first, std::move(t.p.pt), t.t_sent, t.p.t_cur, t.p.ev,
-                                 tags_of(t.p, t.t_sent, t.p.t_cur, c->geom.page_size)});
-            t.has_pending = false;
-            t.t_sent = t.p.t_cur;
+            const bool last = (k + 1 == t.p.marks.size());
+            b.jobs.push_back(Job{kv.first, last ? std::move(t.p.pt) : t.p.pt, t.t_sent, te, ev,
+                                 tags_of(t.p, t.t_sent, te, c->geom.page_size)});
+            t.p.marks.erase(t.p.marks.begin(), t.p.marks.begin() + static_cast<long>(k) + 1);
+            t.has_pending = !last;
+            t.t_sent = te;
             room -= want;
         } else if (b.jobs.empty()) {                // larger than a whole half: take a prefix
             const int64_t fit = room / c->token_bytes;
             if (fit < 1) {
                 if (c->first_error == 0) c->first_error = LUMEN_KV_ESIZE;
                 t.has_pending = false;
+                t.p.marks.clear();
                 continue;
             }
-            b.jobs.push_back(Job{kv.first, t.p.pt, t.t_sent, t.t_sent + fit, t.p.ev,
+            b.jobs.push_back(Job{kv.first, t.p.pt, t.t_sent, t.t_sent + fit, ev,
                                  tags_of(t.p, t.t_sent, t.t_sent + fit, c->geom.page_size)});
             t.t_sent += fit;                        // the rest stays pending
             room = 0;
@@ -360,6 +386,7 @@ int lumen_kv_ckpt_untrack(lumen_kv_ckpt* c, uint64_t id) {
     auto it = c->reqs.find(id);
     if (it == c->reqs.end() || it->second.zombie) return LUMEN_KV_EINVAL;
     it->second.has_pending = false;
+    it->second.p.marks.clear();
     if (it->second.in_flight)
         it->second.zombie = true;
     else
@@ -388,7 +415,13 @@ int lumen_kv_ckpt_notify(lumen_kv_ckpt* c, const uint64_t* ids, const lumen_kv_r
             if (reqs[i].t_end == t.t_sent && !t.has_pending) continue;   // nothing new
             t.p.pt.assign(reqs[i].page_table, reqs[i].page_table + reqs[i].page_table_len);
             t.p.t_cur = reqs[i].t_end;
-            t.p.ev = static_cast<cudaEvent_t>(ready_event);
+            if (!t.has_pending) t.p.marks.clear();
+            const cudaEvent_t ev = static_cast<cudaEvent_t>(ready_event);
+            if (!t.p.marks.empty() && t.p.marks.back().second == ev)
+                t.p.marks.back().first = reqs[i].t_end;
+            else
+                t.p.marks.emplace_back(reqs[i].t_end, ev);
+            if (t.p.marks.size() > 256) t.p.marks.erase(t.p.marks.begin());   // covered by its successor
             t.p.toks.clear();
             if (token_ids && token_ids[i]) {        // the tokens of the pages the delta touches
                 t.p.tok_base = (t.t_sent / S) * S;
