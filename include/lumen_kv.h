@@ -111,7 +111,7 @@ typedef struct lumen_kv_plan lumen_kv_plan;  /* opaque; library owns its descrip
 #define LUMEN_KV_KERNEL_SHIFT        8
 #define LUMEN_KV_KERNEL_MASK         0xF00u
 #define LUMEN_KV_KERNEL_AUTO         0x000u
-#define LUMEN_KV_KERNEL_WARP         0x100u /* SIMT: warp per (run, plane), 16 B ld/st        */
+#define LUMEN_KV_KERNEL_WARP         0x100u /* SIMT: warp per (run, plane, sub-chunk), 32 B ld/st */
 #define LUMEN_KV_KERNEL_BULK         0x200u /* TMA 1-D bulk copies through a shared-memory ring */
 
 /* where the checkpoint buffer lives */

@@ -6,10 +6,13 @@
 // buffer side.  Pure data movement: no tensor cores, no arithmetic on the payload,
 // the 16-bit words are never interpreted (they include NaN encodings).
 //
-// Two kernels, chosen per launch:
-//   kv_copy_warp : SIMT.  One warp per item, 16-byte ld/st per lane, UNROLL
-//                  independent loads in flight per lane before the first store.
-//   kv_copy_bulk : TMA.   Persistent single-warp CTAs; one elected lane moves
+// Kernels, chosen per launch:
+//   kv_copy_warp32 / kv_copy_warp : SIMT, the HBM <-> HBM path.  One warp per (run, plane,
+//                  sub-chunk), 32-byte (LDG/STG.E.256) or 16-byte accesses per lane, UNROLL
+//                  independent loads in flight per lane before the first store; descriptors
+//                  in global memory or in the kernel parameters; programmatic dependent launch.
+//   kv_copy_bulk : TMA, the zero-copy host path (small grid).  Persistent single-warp CTAs;
+//                  one elected lane moves
 //                  whole items global -> shared ring -> global with 1-D
 //                  cp.async.bulk (UBLKCP), completion tracked by mbarriers (loads)
 //                  and bulk groups (stores).  The other lanes only prefetch and
