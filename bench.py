@@ -1013,17 +1013,32 @@ def run_interference(args):
                 else:
                     ck.pack(plan, host)
 
-        pack(); torch.cuda.synchronize()
-        p0, p1 = ev(), ev()
-        p0.record(s1); pack(); p1.record(s1)
-        torch.cuda.synchronize()
-        gbps_alone = P / p0.elapsed_time(p1) / 1e6
-        n = int(P / 50e9 * 1e3 / alone) + 8                    # copies outlast the pack
-        x, y = copies(n)
-        p0.record(s1); pack(); p1.record(s1)
-        torch.cuda.synchronize()
-        out[name] = {"pack_GBps_alone": gbps_alone, "pack_GBps_beside_copy": P / p0.elapsed_time(p1) / 1e6,
-                     "hbm_copy_ms": x.elapsed_time(y) / n, "hbm_copy_slowdown": x.elapsed_time(y) / n / alone}
+        rplan = ck.plan(w.restore_reqs, unique_dst=True)
+
+        def restore():
+            with torch.cuda.stream(s1):
+                if mode == "staged":
+                    ck.unpack_staged(rplan, host, ring)
+                else:
+                    ck.unpack(rplan, host)
+
+        res = {}
+        for what, fn in (("pack", pack), ("restore", restore)):
+            fn(); torch.cuda.synchronize()
+            p0, p1 = ev(), ev()
+            p0.record(s1); fn(); p1.record(s1)
+            torch.cuda.synchronize()
+            gbps_alone = P / p0.elapsed_time(p1) / 1e6
+            n = int(P / 50e9 * 1e3 / alone) + 8                # copies outlast the transfer
+            x, y = copies(n)
+            p0.record(s1); fn(); p1.record(s1)
+            torch.cuda.synchronize()
+            res.update({f"{what}_GBps_alone": gbps_alone,
+                        f"{what}_GBps_beside_copy": P / p0.elapsed_time(p1) / 1e6,
+                        f"hbm_copy_slowdown_during_{what}": x.elapsed_time(y) / n / alone})
+        res["hbm_copy_slowdown"] = res["hbm_copy_slowdown_during_pack"]
+        out[name] = res
+        rplan.close()
         plan.close()
     best = out["staged (kernel -> HBM ring -> copy engine)"]
     link = memcpy_peaks(torch)
