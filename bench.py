@@ -51,6 +51,8 @@ def parse_args():
                     help="LUMEN_KV_NO_INLINE: upload small plans to device memory too (A/B evidence)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-large", action="store_true",
+                    help="default run only: skip the large_configs block (cfg2 + cfg4 wave 0)")
     ap.add_argument("--e2e-steps", type=int, default=0, help="default: min(steps, 100)")
     return ap.parse_args()
 
@@ -96,73 +98,158 @@ def iteration_ranges(w, delta: int, cycle: int):
 
 
 # ------------------------------------------------------------------------------------
-# clocks during the timed region (NVML polled from a thread)
+# clocks during the timed region: NVML polled by a HELPER PROCESS (its own interpreter, so it can
+# neither take this process's GIL nor sit between the two event records of a timed region)
 # ------------------------------------------------------------------------------------
+_CLOCK_HELPER = r"""
+import signal, sys, time
+import pynvml as nv
+uuid, index, path = sys.argv[1], int(sys.argv[2]), sys.argv[3]
+nv.nvmlInit()
+try:
+    h = nv.nvmlDeviceGetHandleByUUID(uuid)
+except Exception:
+    h = nv.nvmlDeviceGetHandleByIndex(index)
+state = {"stop": False, "period": None}          # period None: idle (no NVML traffic at all)
+signal.signal(signal.SIGTERM, lambda *a: state.update(stop=True))
+signal.signal(signal.SIGUSR1, lambda *a: state.update(period=0.0002))   # short kernel regions
+signal.signal(signal.SIGHUP, lambda *a: state.update(period=0.05))      # seconds-long host-link regions
+signal.signal(signal.SIGUSR2, lambda *a: state.update(period=None))
+f = open(path, "w")
+f.write("max %d\n" % nv.nvmlDeviceGetMaxClockInfo(h, nv.NVML_CLOCK_SM)); f.flush()
+while not state["stop"]:
+    if state["period"] is None:
+        time.sleep(0.001)
+        continue
+    t = time.monotonic_ns()
+    mhz = nv.nvmlDeviceGetClockInfo(h, nv.NVML_CLOCK_SM)
+    try:
+        mask = nv.nvmlDeviceGetCurrentClocksEventReasons(h)
+    except Exception:
+        mask = nv.nvmlDeviceGetCurrentClocksThrottleReasons(h)
+    f.write("%d %d %d\n" % (t, mhz, mask)); f.flush()
+    time.sleep(state["period"] or 0.0002)
+f.close()
+"""
+
+
 class ClockSampler:
+    """SM clock and throttle reasons DURING timed regions.  A helper process polls NVML while a
+    window is open and stamps each sample with CLOCK_MONOTONIC; start() / stop() signal the helper
+    and note the window's two timestamps, summary() keeps the samples inside the windows.  Outside
+    windows the helper makes no NVML call: polling at kHz rate for the whole run was measured to
+    cost the copy engines a quarter of their D2H rate (pinned memcpy 41 instead of 57 GB/s), so
+    seconds-long host-link regions are sampled at 20 Hz (start(slow=True)).
+    poll() takes one sample from the calling thread: call it only where the host has nothing
+    left to enqueue (after the end event has been recorded, while the device is still busy)."""
     REASONS = {0x1: "gpu_idle", 0x2: "applications_clocks_setting", 0x4: "sw_power_cap",
                0x8: "hw_slowdown", 0x10: "sync_boost", 0x20: "sw_thermal_slowdown",
                0x40: "hw_thermal_slowdown", 0x80: "hw_power_brake_slowdown",
                0x100: "display_clock_setting"}
 
-    def __init__(self, index: int):
-        self.samples, self.reasons, self._stop, self._th = [], set(), threading.Event(), None
-        self.max_mhz = None
+    def __init__(self, index: int, uuid: str = ""):
+        import subprocess
+        import tempfile
+        self.windows, self._open, self.own = [], None, []
+        self.max_mhz, self.proc, self.nv, self.h = None, None, None, None
+        fd, self.path = tempfile.mkstemp(prefix="lumen_clocks_", suffix=".txt")
+        os.close(fd)
+        try:
+            self.proc = subprocess.Popen([sys.executable, "-c", _CLOCK_HELPER, uuid, str(index), self.path],
+                                         stdout=subprocess.DEVNULL, stderr=subprocess.DEVNULL)
+        except Exception:
+            self.proc = None
         try:
             import pynvml
             pynvml.nvmlInit()
             self.nv = pynvml
-            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            try:
+                self.h = pynvml.nvmlDeviceGetHandleByUUID(uuid)
+            except Exception:
+                self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
             self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
         except Exception:
             self.nv = None
 
-    def _poll_once(self):
-        nv = self.nv
-        self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
-        try:
-            mask = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
-        except Exception:
-            mask = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
-        for bit, name in self.REASONS.items():
-            if mask & bit and name != "gpu_idle":
-                self.reasons.add(name)
-
-    def _run(self):
-        while not self._stop.is_set():
+    def _signal(self, sig):
+        if self.proc is not None and self.proc.poll() is None:
             try:
-                self._poll_once()
-            except Exception:
-                break
-            time.sleep(0.0005)
-
-    def poll(self):
-        """One sample from the calling thread (the timed loop takes a few itself, so the record
-        never depends on how the polling thread was scheduled)."""
-        if self.nv is not None:
-            try:
-                self._poll_once()
-            except Exception:
+                os.kill(self.proc.pid, sig)
+            except OSError:
                 pass
 
-    def start(self):
-        if self.nv is None:
-            return
-        self._stop.clear()
-        self._th = threading.Thread(target=self._run, daemon=True)
-        self._th.start()
+    def start(self, slow: bool = False):
+        import signal
+        self._signal(signal.SIGHUP if slow else signal.SIGUSR1)
+        self._open = time.monotonic_ns()
 
     def stop(self):
-        if self._th is not None:
-            self._stop.set()
-            self._th.join()
-            self._th = None
+        import signal
+        if self._open is not None:
+            self.windows.append((self._open, time.monotonic_ns()))
+            self._open = None
+        self._signal(signal.SIGUSR2)
 
-    def summary(self):
-        if not self.samples:
-            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
-                    "samples": 0}
-        return {"sm_mhz": float(np.median(self.samples)), "sm_max_mhz": self.max_mhz,
-                "reasons": sorted(self.reasons), "samples": len(self.samples)}
+    def poll(self):
+        if self.nv is None:
+            return
+        try:
+            mhz = self.nv.nvmlDeviceGetClockInfo(self.h, self.nv.NVML_CLOCK_SM)
+            try:
+                mask = self.nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+            except Exception:
+                mask = self.nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+            self.own.append((mhz, mask))
+        except Exception:
+            pass
+
+    def _helper_samples(self):
+        out = []
+        try:
+            for line in open(self.path):
+                p = line.split()
+                if len(p) == 3:
+                    out.append((int(p[0]), int(p[1]), int(p[2])))
+        except Exception:
+            pass
+        return out
+
+    def summary(self, reset: bool = False):
+        """Median SM MHz and the union of throttle reasons over the windows noted so far."""
+        hs = [(m, k) for t, m, k in self._helper_samples()
+              if any(a <= t <= b for a, b in self.windows)]
+        allp = hs + self.own
+        reasons = sorted({name for _, mask in allp for bit, name in self.REASONS.items()
+                          if mask & bit and name != "gpu_idle"})
+        out = {"sm_mhz": float(np.median([m for m, _ in allp])) if allp else None,
+               "sm_max_mhz": self.max_mhz, "reasons": reasons, "samples": len(allp),
+               "sampler": "NVML polled by a helper process during the timed regions"
+                          + (f" ({len(hs)} samples)" if hs else " (none fell inside)")
+                          + (f" + {len(self.own)} from this process after the end event was recorded, "
+                             "device still busy" if self.own else "")}
+        if reset:
+            self.windows, self.own = [], []
+        return out
+
+    def close(self):
+        if self.proc is not None:
+            self.proc.terminate()
+            try:
+                self.proc.wait(timeout=5)
+            except Exception:
+                self.proc.kill()
+            self.proc = None
+        try:
+            os.unlink(self.path)
+        except OSError:
+            pass
+
+
+def gpu_uuid(torch, local: int) -> str:
+    try:
+        return "GPU-" + str(torch.cuda.get_device_properties(local).uuid)
+    except Exception:
+        return ""
 
 
 # ------------------------------------------------------------------------------------
@@ -188,16 +275,36 @@ def oracle_sample(workload: str, seed: int):
         return (w, "BASELINE.json configs[3] (recovery burst, Qwen3-32B shape)", w.reqs, w.restore_reqs,
                 K, V, keep, f"1-token pack of 64 running requests + restore of {n} tokens of one request")
     w, label, delta = make_workload(workload, seed)
+    content = "g"
     if workload in ("cfg0", "cfg1"):
         reqs, rreqs = w.reqs, w.restore_reqs
         what = f"one full step ({len(w.reqs)} requests, {w.tokens} tokens, pack + restore)"
+    elif workload == "cfg2" and mem_available_gib() >= 40:
+        # "cfg 2 whole if host RAM allows a 32 GiB pool + 32 GiB buffer, else the first
+        # 4 requests (8 GiB) and say so".  The sparse pool holds source pages + fresh pages + buffer
+        # = 3 x 8 GiB for 4 requests; the whole config would need 96 GiB of host RAM.
+        reqs, rreqs = w.reqs[:4], w.restore_reqs[:4]
+        content = "tiled"
+        what = ("the first 4 of the 16 requests, 8,192 tokens each (8 GiB packed + 8 GiB restored per "
+                f"step; the whole config needs 96 GiB of host RAM, {mem_available_gib():.0f} GiB available; "
+                "touched pages hold tiled seeded random page images, see workloads/hostpool.py)")
     else:
         n = 4096
         reqs = [(w.reqs[0][0], 0, n)]
         rreqs = [(w.restore_reqs[0][0], 0, n)]
-        what = f"first request, first {n} tokens (pack + restore)"
-    K, V, keep = sparse_host_pool(w.geom, seed, list(reqs) + list(rreqs))
+        what = f"first request, first {n} tokens (pack + restore; 1 GiB each way)"
+    K, V, keep = sparse_host_pool(w.geom, seed, list(reqs) + list(rreqs), content=content)
     return w, label, reqs, rreqs, K, V, keep, what
+
+
+def mem_available_gib() -> float:
+    try:
+        for l in open("/proc/meminfo"):
+            if l.startswith("MemAvailable:"):
+                return int(l.split()[1]) / 2**20
+    except Exception:
+        pass
+    return 0.0
 
 
 def oracle_step(geom, K, V, reqs, rreqs, omp=False):
@@ -311,20 +418,23 @@ def measured_peaks():
 
 
 def ncu_traffic(workload: str, kernel: str, direction: str):
-    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the
-    committed ncu --set full capture (profiles/traffic.csv, see profiles/README.md), else None."""
+    """(dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, source):
+    NOT measured in this run -- read from the committed ncu --set full capture that
+    profiles/traffic.csv indexes (profiles/README.md names the commands); (None, None) if absent."""
     import csv
     p = ROOT / "profiles" / "traffic.csv"
     if not p.exists():
-        return None
+        return None, None
     try:
-        with open(p, newline="") as f:
-            for r in csv.DictReader(f):
-                if (r["workload"], r["kernel"], r["direction"]) == (workload, kernel, direction):
-                    return int(r["dram_bytes_read"]) + int(r["dram_bytes_write"])
+        rows = [r for r in csv.DictReader(open(p, newline=""))
+                if (r["workload"], r["kernel"], r["direction"]) == (workload, kernel, direction)]
     except Exception:
-        return None
-    return None
+        return None, None
+    if not rows:
+        return None, None
+    r = rows[-1]                                        # the newest capture is appended last
+    return (int(r["dram_bytes_read"]) + int(r["dram_bytes_write"]),
+            f"profiles/{r['source']} (committed ncu --set full capture, not measured in this run)")
 
 
 def memcpy_peaks(torch, nbytes=1 << 30):
@@ -339,6 +449,227 @@ def memcpy_peaks(torch, nbytes=1 << 30):
             a.record(); dst.copy_(src, non_blocking=True); b.record(); torch.cuda.synchronize()
             best = min(best, a.elapsed_time(b))
         out[name] = nbytes / best / 1e6
+    return out
+
+
+class HbmPath:
+    """One pool + one workload: the step of DESIGN.md section 7 (a1, a2 x 2, a3, a7, plan_free x 2)
+    and the loops that time it.  Nothing between the two event records of a timed region but the
+    calls of the path itself."""
+
+    def __init__(self, torch, lk, pool, w, delta, kflag, stream, dist):
+        self.torch, self.lk, self.pool, self.w, self.dist = torch, lk, pool, w, dist
+        self.P = w.payload_bytes
+        self.ranges = iteration_ranges(w, delta, CYCLE)
+        self.kflag, self.stream, self.sh = kflag, stream, stream.cuda_stream
+        self.ra_p, self.ra_r = lk.ReqArray(w.reqs), lk.ReqArray(w.restore_reqs)
+        self.single_stats = {}
+
+    def barrier(self):
+        if self.dist is not None:
+            self.dist.barrier()
+
+    def step(self, i, bufs, kind, lag_, evs=None, only=None):
+        """only=None: the whole step.  only="pack"/"unpack": that direction alone (same plans,
+        same rotation), used to time one kernel as a back-to-back batch of launches."""
+        lk, pool, ranges, P, sh, stream = self.lk, self.pool, self.ranges, self.P, self.sh, self.stream
+        nb = len(bufs)
+        p = r = None
+        if only != "unpack":
+            tb, te = ranges[i % len(ranges)]
+            self.ra_p.set_ranges(tb, te)                                                    # a1
+            p = lk.lumen_kv_plan_build(pool.geom, self.ra_p, self.kflag, sh)                # a2
+        if only != "pack":
+            tb, te = ranges[(i - lag_) % len(ranges)]
+            self.ra_r.set_ranges(tb, te)
+            r = lk.lumen_kv_plan_build(pool.geom, self.ra_r,
+                                       self.kflag | lk.LUMEN_KV_VALIDATE_UNIQUE_DST, sh)
+        if evs is not None:
+            evs[0].record(stream)
+        if p is not None:
+            lk.lumen_kv_checkpoint_pack(p, pool.k_ptrs, pool.v_ptrs, bufs[i % nb].data_ptr(), P, kind, sh)  # a3 / a4
+        if evs is not None:
+            evs[1].record(stream)
+        if r is not None:
+            lk.lumen_kv_restore_unpack(r, pool.k_ptrs, pool.v_ptrs, bufs[(i - lag_) % nb].data_ptr(), P,
+                                       kind, sh)                                            # a7
+        if evs is not None:
+            evs[2].record(stream)
+        if p is not None:
+            p.close()
+        if r is not None:
+            r.close()
+
+    def timed_loop(self, K, W, bufs, kind, lag_, sampler=None, per_launch=False, only=None):
+        """W warm-up steps, then exactly K steps between one event pair.  per_launch=True adds
+        an event between the launches of every step (kernel durations); those records sit
+        between the kernels, so that variant is never the one `value` comes from.
+        Returns (ms, pack_ms, unpack_ms, wall_ms, host_enqueue_ms)."""
+        torch, stream, ranges = self.torch, self.stream, self.ranges
+        for i in range(-lag_, 0):                      # fill the buffers the first restores read
+            self.step(i + len(ranges) * len(bufs), bufs, kind, 0)
+        for i in range(W):
+            self.step(i, bufs, kind, lag_, only=only)
+        evs = ([[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(K)]
+               if per_launch else None)
+        e_start, e_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        self.barrier(); torch.cuda.synchronize()
+        if sampler:
+            sampler.start()                            # one signal to the helper + a timestamp
+        # the W warm-up steps again, untimed, right in front of the timed ones: the device is
+        # busy (clocks up, pipeline full) when the start event fires, whatever K is
+        for i in range(W):
+            self.step(i, bufs, kind, lag_, None, only)
+        t_wall = time.perf_counter()
+        e_start.record(stream)
+        for i in range(K):                             # nothing in here but the path's own calls
+            self.step(W + i, bufs, kind, lag_, evs[i] if per_launch else None, only)
+        e_end.record(stream)
+        t_host = time.perf_counter() - t_wall          # host time to enqueue K steps
+        if sampler:
+            sampler.poll()                             # everything is enqueued, the device still runs it
+        stream.synchronize(); torch.cuda.synchronize()
+        t_wall = time.perf_counter() - t_wall
+        if sampler:
+            sampler.stop()
+        self.barrier()
+        ms = max_over_ranks(e_start.elapsed_time(e_end), self.dist, "cuda")
+        pack_ms = unpack_ms = None
+        if per_launch:
+            pk = [e[0].elapsed_time(e[1]) for e in evs]
+            up = [e[1].elapsed_time(e[2]) for e in evs]
+            for name, xs in (("pack", pk), ("unpack", up)):
+                self.single_stats[name] = {"mean": float(np.mean(xs)), "median": float(np.median(xs)),
+                                           "best": float(np.min(xs))}
+            pack_ms, unpack_ms = self.single_stats["pack"]["mean"], self.single_stats["unpack"]["mean"]
+        return ms, pack_ms, unpack_ms, t_wall * 1e3, t_host * 1e3
+
+    def idle_single_launch(self, bufs, kind, idle_s=0.012, n=12):
+        """A decode loop issues one pack per 13-58 ms iteration: every launch meets an idle device.
+        One event pair per launch around nothing but the call (plan built beforehand), `idle_s` of
+        host sleep with the device idle before each."""
+        torch, stream, lk, pool = self.torch, self.stream, self.lk, self.pool
+        out = {}
+        for only in ("pack", "unpack"):
+            ts = []
+            for i in range(n):
+                tb, te = self.ranges[i % len(self.ranges)]
+                ra = self.ra_p if only == "pack" else self.ra_r
+                ra.set_ranges(tb, te)
+                plan = lk.lumen_kv_plan_build(pool.geom, ra, self.kflag, self.sh)
+                fn = lk.lumen_kv_checkpoint_pack if only == "pack" else lk.lumen_kv_restore_unpack
+                torch.cuda.synchronize(); time.sleep(idle_s)
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record(stream)
+                fn(plan, pool.k_ptrs, pool.v_ptrs, bufs[i % len(bufs)].data_ptr(), self.P, kind, self.sh)
+                b.record(stream)
+                stream.synchronize()
+                plan.close()
+                ts.append(a.elapsed_time(b))
+            out[only] = {"median": float(np.median(ts)), "best": float(np.min(ts)), "mean": float(np.mean(ts))}
+        return out
+
+
+def fill_pool(pool, seed, wdev):
+    for i, t in enumerate(pool.planes()):
+        wdev.fill_plane(t, seed, i)
+
+
+def staged_host_once(torch, lk, path, hb, ring, direction, async_call=False):
+    """One staged call on a HOST buffer, device-timed; also the host time spent inside the call."""
+    pool, P, s = path.pool, path.P, path.stream
+    reqs, flag = ((path.ra_p, 0) if direction == "pack" else (path.ra_r, lk.LUMEN_KV_VALIDATE_UNIQUE_DST))
+    tb, te = path.ranges[0]
+    reqs.set_ranges(tb, te)
+    plan = lk.lumen_kv_plan_build(pool.geom, reqs, path.kflag | flag, s.cuda_stream)
+    fn = lk.lumen_kv_checkpoint_pack_staged if direction == "pack" else lk.lumen_kv_restore_unpack_staged
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    a.record(s)
+    t0 = time.perf_counter()
+    fn(plan, pool.k_ptrs, pool.v_ptrs, hb.data_ptr(), P, ring.stager, s.cuda_stream)
+    call_ms = (time.perf_counter() - t0) * 1e3
+    b.record(s)
+    s.synchronize()
+    n_chunks = len(plan.chunks(ring.stager.slot_bytes))
+    plan.close()
+    return a.elapsed_time(b), call_ms, n_chunks
+
+
+def large_config(torch, lk, name, seed, kflag, stream, sampler, peak, link, with_host, waves=(0,)):
+    """One of the large configs (BASELINE.json configs[2], configs[4]) inside the default line:
+    HBM pack + restore (3 warm-up + 3 timed steps, then 3 launches of each direction alone), and
+    for cfg2 the staged host path once in each direction.  Every `frac` is recomputable from the
+    `*_ms` beside it."""
+    from paper_2606_17787_b200.pool import KVPool, StagingRing
+    from workloads import cfg4_longctx
+    from workloads import device as wdev
+    DEV = lk.LUMEN_KV_MEM_DEVICE
+    out, pool, dbuf = {}, None, None
+    agg_bytes = agg_ms = 0.0
+    per_wave = []
+    for wave in waves:
+        if name == "cfg4":
+            w = cfg4_longctx(seed, wave_reqs=2, wave=wave)
+        else:
+            w, _, _ = make_workload(name, seed)
+        L, H, D, S, N = w.geom
+        if pool is None:
+            pool = KVPool(L, H, D, S, N)
+            dbuf = torch.empty(w.payload_bytes, dtype=torch.uint8, device="cuda")
+        fill_pool(pool, seed + wave, wdev)
+        torch.cuda.synchronize()
+        path = HbmPath(torch, lk, pool, w, 0, kflag, stream, None)
+        P = path.P
+        with torch.cuda.stream(stream):
+            ms, _, _, _, host_ms = path.timed_loop(3, 3, [dbuf], DEV, 0, sampler)
+            pack_ms = path.timed_loop(3, 3, [dbuf], DEV, 0, sampler, only="pack")[0] / 3
+            unpack_ms = path.timed_loop(3, 3, [dbuf], DEV, 0, sampler, only="unpack")[0] / 3
+        per_wave.append({"wave": wave, "ms_per_step": ms / 3, "pack_ms": pack_ms, "unpack_ms": unpack_ms,
+                         "payload_GBps": 2 * P / (ms / 3) / 1e6})
+        agg_bytes += 2 * P
+        agg_ms += ms / 3
+    dom_ms = max(pack_ms, unpack_ms)
+    out = {"payload_bytes_per_direction": P, "pool_pages": N, "page_size": S,
+           "ms_per_step": ms / 3, "payload_GBps": 2 * P / (ms / 3) / 1e6,
+           "pack_ms": pack_ms, "unpack_ms": unpack_ms,
+           "achieved_GBps": 2 * P / dom_ms / 1e6, "peak_GBps": peak, "frac": 2 * P / dom_ms / 1e6 / peak,
+           "frac_formula": "2 * payload_bytes_per_direction / max(pack_ms, unpack_ms) / peak_GBps",
+           "host_enqueue_ms_per_step": host_ms / 3,
+           "timing": "3 warm-up + 3 timed steps between one event pair; pack_ms / unpack_ms = 3 launches of "
+                     "that direction alone between one event pair; inputs larger than L2 (tens of GiB per launch)"}
+    if len(waves) > 1:
+        out["waves"] = per_wave
+        out["all_waves_payload_GBps"] = agg_bytes / agg_ms / 1e6
+    traffic, tsrc = ncu_traffic(name, "warp", "pack" if pack_ms >= unpack_ms else "unpack")
+    out["traffic"], out["traffic_source"] = traffic, tsrc
+    avail = wdev.host_mem_available()
+    if with_host and avail is not None and P > avail - (8 << 30):
+        out["host_staged"] = {"skipped": f"pinning {P >> 30} GiB needs more host memory than this box has "
+                                         f"available ({avail >> 30} GiB); see --workload cfg2 on a larger host"}
+        with_host = False
+    if with_host:
+        hb = wdev.pinned_exact(P)
+        ring = StagingRing(32 << 20, 3)
+        staged_host_once(torch, lk, path, hb, ring, "pack")        # warm-up
+        sampler.start(slow=True)
+        p_ms, p_call, n_chunks = staged_host_once(torch, lk, path, hb, ring, "pack")
+        r_ms, r_call, _ = staged_host_once(torch, lk, path, hb, ring, "restore")
+        sampler.stop()
+        out["host_staged"] = {"pack_GBps": P / p_ms / 1e6, "restore_GBps": P / r_ms / 1e6,
+                              "pack_ms": p_ms, "restore_ms": r_ms, "chunks_per_call": n_chunks,
+                              "pack_frac_of_d2h_memcpy": P / p_ms / 1e6 / link["d2h"],
+                              "restore_frac_of_h2d_memcpy": P / r_ms / 1e6 / link["h2d"],
+                              "memcpy_peak_d2h_GBps": link["d2h"], "memcpy_peak_h2d_GBps": link["h2d"],
+                              "staged_call_host_ms": {"pack": p_call, "restore": r_call}}
+        ring.close()
+        wdev.unpin(hb)
+        del hb
+    out["clocks"] = sampler.summary(reset=True)
+    del pool, dbuf, path
+    import gc
+    gc.collect()
+    torch.cuda.empty_cache()
     return out
 
 
@@ -358,6 +689,7 @@ def run_ours(args):
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     wdev.build()
+    sampler = ClockSampler(local, gpu_uuid(torch, local))
 
     def barrier():
         if dist is not None:
@@ -375,11 +707,9 @@ def run_ours(args):
     w, label, delta = make_workload(args.workload, seed, pages_cap)
     L, H, D, S, N = w.geom
     pool = KVPool(L, H, D, S, N)
-    for i, t in enumerate(pool.planes()):
-        wdev.fill_plane(t, seed, i)
+    fill_pool(pool, seed, wdev)
     torch.cuda.synchronize()
     P = w.payload_bytes
-    ranges = iteration_ranges(w, delta, CYCLE)
     n_stage = N_STAGE if P <= (1 << 30) else 1
     lag = 2 if n_stage > 1 else 0
     dbufs = [torch.empty(P, dtype=torch.uint8, device="cuda") for _ in range(n_stage)]
@@ -388,97 +718,28 @@ def run_ours(args):
              "bulk": lk.LUMEN_KV_KERNEL_BULK}[args.kernel]
     if args.upload_descriptors:
         kflag |= lk.LUMEN_KV_NO_INLINE
-    ra_p, ra_r = lk.ReqArray(w.reqs), lk.ReqArray(w.restore_reqs)
     stream = torch.cuda.Stream()
     sh = stream.cuda_stream
+    path = HbmPath(torch, lk, pool, w, delta, kflag, stream, dist)
+    ranges, ra_p, ra_r = path.ranges, path.ra_p, path.ra_r
     geom, kp, vp = pool.geom, pool.k_ptrs, pool.v_ptrs
     DEV, HOST = lk.LUMEN_KV_MEM_DEVICE, lk.LUMEN_KV_MEM_HOST_MAPPED
     UNIQUE = lk.LUMEN_KV_VALIDATE_UNIQUE_DST
 
-    def step(i, bufs, kind, lag_, evs=None, only=None):
-        """only=None: the whole step.  only="pack"/"unpack": that direction alone (same plans,
-        same rotation), used to time one kernel as a back-to-back batch of launches."""
-        nb = len(bufs)
-        p = r = None
-        if only != "unpack":
-            tb, te = ranges[i % len(ranges)]
-            ra_p.set_ranges(tb, te)                                           # a1
-            p = lk.lumen_kv_plan_build(geom, ra_p, kflag, sh)                 # a2
-        if only != "pack":
-            tb, te = ranges[(i - lag_) % len(ranges)]
-            ra_r.set_ranges(tb, te)
-            r = lk.lumen_kv_plan_build(geom, ra_r, kflag | UNIQUE, sh)
-        if evs is not None:
-            evs[0].record(stream)
-        if p is not None:
-            lk.lumen_kv_checkpoint_pack(p, kp, vp, bufs[i % nb].data_ptr(), P, kind, sh)          # a3 / a4
-        if evs is not None:
-            evs[1].record(stream)
-        if r is not None:
-            lk.lumen_kv_restore_unpack(r, kp, vp, bufs[(i - lag_) % nb].data_ptr(), P, kind, sh)  # a7
-        if evs is not None:
-            evs[2].record(stream)
-        if p is not None:
-            p.close()
-        if r is not None:
-            r.close()
-
-    single_stats = {}
-
-    def timed_loop(K, W, bufs, kind, lag_, sampler=None, per_launch=False, only=None):
-        """W warm-up steps, then exactly K steps between one event pair.  per_launch=True adds
-        an event between the launches of every step (kernel durations); those records sit
-        between the kernels, so that variant is never the one `value` comes from."""
-        for i in range(-lag_, 0):                      # fill the buffers the first restores read
-            step(i + len(ranges) * len(bufs), bufs, kind, 0)
-        for i in range(W):
-            step(i, bufs, kind, lag_, only=only)
-        evs = ([[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(K)]
-               if per_launch else None)
-        e_start, e_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        barrier(); torch.cuda.synchronize()
-        if sampler:
-            sampler.start()
-        # the W warm-up steps again, untimed, right in front of the timed ones: the device is
-        # busy (clocks up, pipeline full) when the start event fires, whatever K is
-        for i in range(W):
-            step(i, bufs, kind, lag_, None, only)
-        t_wall = time.perf_counter()
-        e_start.record(stream)
-        marks = {K // 4, K // 2, (3 * K) // 4} if sampler else ()
-        for i in range(K):
-            step(W + i, bufs, kind, lag_, evs[i] if per_launch else None, only)
-            if i in marks:
-                sampler.poll()                         # the device is mid-region: clocks under load
-        e_end.record(stream)
-        t_host = time.perf_counter() - t_wall          # host time to enqueue K steps
-        stream.synchronize(); torch.cuda.synchronize()
-        t_wall = time.perf_counter() - t_wall
-        if sampler:
-            sampler.stop()
-        barrier()
-        ms = max_over_ranks(e_start.elapsed_time(e_end), dist, "cuda")
-        pack_ms = unpack_ms = None
-        if per_launch:
-            pk = [e[0].elapsed_time(e[1]) for e in evs]
-            up = [e[1].elapsed_time(e[2]) for e in evs]
-            single_stats["pack"] = {"mean": float(np.mean(pk)), "median": float(np.median(pk)), "best": float(np.min(pk))}
-            single_stats["unpack"] = {"mean": float(np.mean(up)), "median": float(np.median(up)), "best": float(np.min(up))}
-            pack_ms, unpack_ms = single_stats["pack"]["mean"], single_stats["unpack"]["mean"]
-        return ms, pack_ms, unpack_ms, t_wall * 1e3, t_host * 1e3
-
     K, W = max(1, args.steps), max(3, args.warmup)
-    sampler = ClockSampler(local)
-    Kk = min(K, 200)                                   # per-launch pass: same steps, instrumented
+    big = P > (1 << 30)
+    Kk = min(K, 200) if not big else min(K, 3)         # per-launch pass: same steps, instrumented
     with torch.cuda.stream(stream):
-        ms, _, _, wall_ms, host_ms = timed_loop(K, W, dbufs, DEV, lag, sampler)
-        ms_k, pack_1, unpack_1, _, _ = timed_loop(Kk, 3, dbufs, DEV, lag, per_launch=True)
-        single = {k: dict(v) for k, v in single_stats.items()}      # single-launch latency: mean/median/best
-        pack_ms = timed_loop(Kk, 3, dbufs, DEV, lag, only="pack")[0] / Kk
-        unpack_ms = timed_loop(Kk, 3, dbufs, DEV, lag, only="unpack")[0] / Kk
+        ms, _, _, wall_ms, host_ms = path.timed_loop(K, W, dbufs, DEV, lag, sampler)
+        clocks = sampler.summary(reset=True)
+        ms_k, pack_1, unpack_1, _, _ = path.timed_loop(Kk, 3, dbufs, DEV, lag, per_launch=True)
+        single = {k: dict(v) for k, v in path.single_stats.items()}   # single-launch latency: mean/median/best
+        pack_ms = path.timed_loop(Kk, 3, dbufs, DEV, lag, only="pack")[0] / Kk
+        unpack_ms = path.timed_loop(Kk, 3, dbufs, DEV, lag, only="unpack")[0] / Kk
+        idle = path.idle_single_launch(dbufs, DEV) if not big else None
     value = job_payload_gbps(world, K, P, ms)
     token_bytes = 2 * L * H * D * 2
-    n_pb = 200 if P <= (1 << 30) else 10                 # a2 alone, on the host clock
+    n_pb = 200 if not big else 10                        # a2 alone, on the host clock
     t0 = time.perf_counter()
     for i in range(n_pb):
         tb, te = ranges[i % len(ranges)]
@@ -488,6 +749,7 @@ def run_ours(args):
         pl.close()
     plan_build_us = (time.perf_counter() - t0) / n_pb * 1e6
     stream.synchronize()
+    host_bound = host_ms / K > pack_ms + unpack_ms
 
     # ---- roofline of the dominant kernel ------------------------------------------------
     peak, peak_src = measured_peaks()
@@ -496,30 +758,49 @@ def run_ours(args):
     achieved = 2 * P / (dom_ms * 1e-3) / 1e9
     resolved = args.kernel if args.kernel != "auto" else "warp"
     kname = "kv_copy_warp32 (256-bit accesses)" if resolved == "warp" else "kv_copy_" + resolved
+    traffic, traffic_src = ncu_traffic(args.workload, resolved, "pack" if dom.endswith("pack") else "unpack")
     roofline = {"bound": "hbm", "kernel": f"{dom} ({kname})", "achieved": achieved,
                 "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": ncu_traffic(args.workload, resolved,
-                                       "pack" if dom.endswith("pack") else "unpack"),
+                "traffic": traffic, "traffic_source": traffic_src,
                 "algorithmic_bytes_per_launch": 2 * P, "peak_source": peak_src,
                 "timing": (f"average launch duration = one CUDA-event pair around {Kk} back-to-back launches "
                            "of that direction alone (same plans and buffer rotation as the step), on the "
                            "launching stream, in this run; *_single_ms = one event pair per launch inside "
                            f"whole steps ({ms_k / Kk:.4f} ms/step: the records between the launches cost a "
-                           "few us each and prevent the overlap of consecutive launches)"),
+                           "few us each and prevent the overlap of consecutive launches); "
+                           "single_launch_after_idle_ms = one event pair per launch after 12 ms of idle device"),
                 "pack_ms": pack_ms, "unpack_ms": unpack_ms,
                 "pack_single_ms": pack_1, "unpack_single_ms": unpack_1, "single_launch_ms": single,
+                "single_launch_after_idle_ms": idle,
                 "pack_traffic_GBps": 2 * P / pack_ms / 1e6, "unpack_traffic_GBps": 2 * P / unpack_ms / 1e6}
+
+    # ---- A16: the page-aligned delta variant of cfg 1 (1 run per request instead of 1-2) ---
+    aligned = None
+    if args.workload == "cfg1":
+        from workloads import cfg1_qwen14b
+        w_al = cfg1_qwen14b(seed, N=N, grow_iters=CYCLE, aligned=True)
+        path_al = HbmPath(torch, lk, pool, w_al, delta, kflag, stream, dist)
+        with torch.cuda.stream(stream):
+            ms_al = path_al.timed_loop(K, W, dbufs, DEV, lag)[0]
+        path_al.ra_p.set_ranges(*path_al.ranges[0])
+        pl = lk.lumen_kv_plan_build(geom, path_al.ra_p, kflag, sh)
+        aligned = {"value": job_payload_gbps(world, K, P, ms_al), "unit": "GB/s", "ms_per_step": ms_al / K,
+                   "runs_per_plan": pl.num_runs,
+                   "note": "SURVEY A16: t_begin = 16*floor((len-16)/16), t_end = t_begin + 16 (page-aligned deltas)"}
+        pl.close()
+        del path_al
 
     # ---- e2e: same step, host buffers, bytes cross the host link inside the timed region --
     e2e = None
+    link = None
     if not args.no_e2e:
         est = 2 * P / 50e9
         Ke = args.e2e_steps or int(max(3, min(K, 100, 20.0 / est)))
-        hb = [pinned_buffer(P) for _ in range(2 if P <= (1 << 30) else 1)]
+        hb = [pinned_buffer(P) for _ in range(2 if not big else 1)]
         link = memcpy_peaks(torch)
         with torch.cuda.stream(stream):
-            ms_e, pack_e, unpack_e, _, _ = timed_loop(Ke, 3, hb, HOST, 1 if len(hb) > 1 else 0,
-                                                      per_launch=True)
+            ms_e, pack_e, unpack_e, _, _ = path.timed_loop(Ke, 3, hb, HOST, 1 if len(hb) > 1 else 0,
+                                                           per_launch=True)
         e2e = {"value": job_payload_gbps(world, Ke, P, ms_e), "unit": "GB/s",
                "h2d_bytes_per_step": P, "d2h_bytes_per_step": P, "steps": Ke,
                "ms_per_step": ms_e / Ke, "gpu_launches": 2 * Ke,
@@ -627,15 +908,57 @@ def run_ours(args):
                    "pdl": os.environ.get("LUMEN_KV_PDL", "1") != "0", "seed": hex(MASTER_SEED)},
         "tokens_per_s": value * 1e9 / token_bytes,
         "wall_ms_per_step": wall_ms / K, "host_enqueue_ms_per_step": host_ms / K,
+        "host_bound": bool(host_bound),
+        "step_over_kernels": (ms / K) / (pack_ms + unpack_ms),
         "plan_build_us": plan_build_us,
-        "roofline": roofline, "e2e": e2e, "gpu_launches": 2 * K, "clocks": sampler.summary(),
+        "roofline": roofline, "e2e": e2e, "gpu_launches": 2 * K, "clocks": clocks,
     }
+    if aligned is not None:
+        line["aligned_delta_variant"] = aligned
+
+    # ---- the large configs the north_star target is worded on, in the same driver-run line ----
+    if args.workload == "cfg1" and world == 1 and not args.no_large:
+        del path, pool, dbufs
+        import gc
+        gc.collect()
+        torch.cuda.empty_cache()
+        if link is None:
+            link = memcpy_peaks(torch)
+        t_large = time.perf_counter()
+        line["large_configs"] = {
+            "cfg2": large_config(torch, lk, "cfg2", MASTER_SEED, kflag, stream, sampler, peak, link, True),
+            "cfg4_wave0": large_config(torch, lk, "cfg4", MASTER_SEED, kflag, stream, sampler, peak, link, False),
+        }
+        line["large_configs"]["wall_s"] = time.perf_counter() - t_large
+        line["large_configs"]["what"] = (
+            "BASELINE.json configs[2] (16 x 8k tokens, Qwen3-32B shape, 32 GiB per direction, pool 20000 pages) "
+            "and one wave of configs[4] (2 of the 8 requests x 128k tokens, page_size 1, 64 GiB per direction; "
+            "the as-written 256 GiB does not fit one GPU -- all four waves: --workload cfg4), HBM pack + restore; "
+            "cfg2 also once through the staged host path (32 GiB each way over the host link)")
+    if args.workload == "cfg4" and world == 1:
+        # BASELINE.json configs[4] is 8 requests: all four waves of 2, fresh seeds per wave
+        del path, pool, dbufs
+        import gc
+        gc.collect()
+        torch.cuda.empty_cache()
+        aw = large_config(torch, lk, "cfg4", MASTER_SEED, kflag, stream, sampler, peak, link, False,
+                          waves=(0, 1, 2, 3))
+        line["all_waves"] = {"requests": 8, "waves": aw["waves"],
+                             "payload_GBps": aw["all_waves_payload_GBps"],
+                             "payload_bytes_total": 8 * aw["payload_bytes_per_direction"],
+                             "note": "4 waves x 2 requests x 128k tokens, page tables and pool content reseeded "
+                                     "per wave; payload_GBps = sum of bytes packed + restored / sum of step times",
+                             "clocks": aw["clocks"]}
+    sampler.close()
     if rank == 0:
         if world == 1 and not args.no_cpu_baseline:
             line["cpu_baseline"] = cpu_baseline(args.workload, MASTER_SEED)
         print(json.dumps(line), flush=True)
     if dist is not None:
         dist.destroy_process_group()
+    if host_bound and args.workload == "cfg1":
+        sys.exit(f"bench.py: the step is HOST-bound (enqueue {host_ms / K:.4f} ms/step > kernels "
+                 f"{pack_ms + unpack_ms:.4f} ms/step): the headline does not measure the kernels")
 
 
 def run_cfg3(args):
@@ -674,7 +997,7 @@ def run_cfg3(args):
     geom, kp, vp, HOST = pool.geom, pool.k_ptrs, pool.v_ptrs, lk.LUMEN_KV_MEM_HOST_MAPPED
     ra = lk.ReqArray(b.running)
     te0 = np.array([te for _, _, te in b.running], dtype=np.int64)
-    sampler = ClockSampler(local)
+    sampler = ClockSampler(local, gpu_uuid(torch, local))
 
     from paper_2606_17787_b200.pool import StagingRing
     ringR, ringP = StagingRing(32 << 20, 3), StagingRing(32 << 20, 3)
@@ -732,7 +1055,7 @@ def run_cfg3(args):
     restore(b.waves[-1], wave_bytes[-1], True, None)
     modes = {"mapped_alone": all_waves(False, None), "staged_alone": all_waves(True, None),
              "mapped_paced_packs": all_waves(False, PACE)}
-    sampler.start()
+    sampler.start(slow=True)
     modes["staged_paced_packs"] = all_waves(True, PACE)
     sampler.stop()
     modes["staged_saturating_packs"] = all_waves(True, 0)
@@ -773,6 +1096,7 @@ def run_cfg3(args):
                 "note": "this workload is the host path: the timed region is the H2D restore itself"},
         "gpu_launches": launches, "clocks": sampler.summary(),
     }
+    sampler.close()
     print(json.dumps(line), flush=True)
     wdev.unpin(hbuf)
 
@@ -881,7 +1205,7 @@ def run_chain(args):
             lays.append((int(s_["buf_offset"]), int(s_["plane_stride_tokens"])))
     t_look = time.perf_counter() - t_look
     link = memcpy_peaks(torch)
-    sampler = ClockSampler(rank_env()[2])
+    sampler = ClockSampler(rank_env()[2], gpu_uuid(torch, rank_env()[2]))
     stream = torch.cuda.Stream()
     K, W = max(1, min(args.steps, 10)), max(3, min(args.warmup, 5))
     payload = restored * tokb
@@ -899,7 +1223,7 @@ def run_chain(args):
         n_chunks = restore_once()
     a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     torch.cuda.synchronize()
-    sampler.start()
+    sampler.start(slow=True)
     a.record(stream)
     for _ in range(K):
         restore_once()
@@ -950,6 +1274,7 @@ def run_chain(args):
                        "note": "through the ctypes binding (marshalling included)"},
         "gpu_launches": K * n_chunks, "clocks": sampler.summary(),
     }
+    sampler.close()
     print(json.dumps(line), flush=True)
     wdev.unpin(arena)
 

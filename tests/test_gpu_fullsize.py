@@ -200,32 +200,44 @@ def test_cfg2_full_size(G, where):
     _free()
 
 
-def test_cfg4_token_granular_wave(G):
-    """configs[4], one wave of 2 requests x 128k tokens, page_size 1, fully shuffled slots:
-    64 GiB pool + 64 GiB HBM buffer (the as-written 256 GiB + 256 GiB cannot exist on one GPU)."""
+def test_cfg4_token_granular_all_waves(G):
+    """configs[4]: 8 requests x 128k tokens, page_size 1, fully shuffled slots, as four waves of
+    2 requests (64 GiB pool + 64 GiB HBM buffer per wave; the as-written 256 GiB + 256 GiB cannot
+    exist on one GPU).  Page tables and pool content are reseeded per wave (SURVEY 8(d):
+    "All 8 requests are covered in 8/W waves with fresh seeds")."""
     import torch
     _free()
-    w = cfg4_longctx(wave_reqs=2)
+    w0 = cfg4_longctx(wave_reqs=2)
     free_b, _ = torch.cuda.mem_get_info()
-    if free_b < 2 * w.payload_bytes + (8 << 30):
+    if free_b < 2 * w0.payload_bytes + (8 << 30):
         pytest.skip("not enough free HBM for a 2-request wave")
-    pool = G.make_pool(w.geom, MASTER_SEED + 4)
+    L, H, D, S, N = w0.geom
+    pool = G.KVPool(L, H, D, S, N)
     ck = G.Checkpointer(pool)
-    plan = ck.plan(w.reqs)
-    assert plan.num_runs == 2 * 131072 and plan.nbytes == 64 * 2**30
-    whole, buf = G.alloc_buffer(plan.nbytes, "device")
-    ck.pack(plan, buf)
-    torch.cuda.synchronize()
-    sampled_pack_check(G, w.geom, w.reqs, MASTER_SEED + 4, buf, 1500, substream(4, "cfg4_samples"))
-    gather_check(G, pool, w.reqs, buf, "pack")
-    # restore under the new shuffle: with S = 1 and a full shuffle every slot is a target, so
-    # "untouched" reduces to the guard bands; P3 closes the loop: re-pack under the new table
-    rplan = ck.plan(w.restore_reqs, unique_dst=True)
-    ck.unpack(rplan, buf)
-    torch.cuda.synchronize()
-    gather_check(G, pool, w.restore_reqs, buf, "restore")
-    assert G.guards_intact(whole, plan.nbytes)
-    plan.close(); rplan.close()
+    whole, buf = G.alloc_buffer(w0.payload_bytes, "device")
+    seen = set()
+    for wave in range(4):
+        w = cfg4_longctx(wave_reqs=2, wave=wave)
+        key = tuple(int(x) for x in w.reqs[0][0][:8])
+        assert key not in seen                   # every wave has its own shuffle
+        seen.add(key)
+        seed = MASTER_SEED + 40 + wave
+        for i, t in enumerate(pool.planes()):
+            G.wdev.fill_plane(t, seed, i)
+        plan = ck.plan(w.reqs)
+        assert plan.num_runs == 2 * 131072 and plan.nbytes == 64 * 2**30
+        ck.pack(plan, buf)
+        torch.cuda.synchronize()
+        sampled_pack_check(G, w.geom, w.reqs, seed, buf, 1500, substream(4 + wave, "cfg4_samples"))
+        gather_check(G, pool, w.reqs, buf, "pack")
+        # restore under the new shuffle: with S = 1 and a full shuffle every slot is a target, so
+        # "untouched" reduces to the guard bands; P3 closes the loop: re-pack under the new table
+        rplan = ck.plan(w.restore_reqs, unique_dst=True)
+        ck.unpack(rplan, buf)
+        torch.cuda.synchronize()
+        gather_check(G, pool, w.restore_reqs, buf, "restore")
+        assert G.guards_intact(whole, plan.nbytes)
+        plan.close(); rplan.close()
     del pool, buf, whole
     _free()
 

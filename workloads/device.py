@@ -85,11 +85,26 @@ def page_checksums(t, n_pages: int, page_bytes: int, stream: int = 0):
 _registered = {}
 
 
+def host_mem_available():
+    """MemAvailable of /proc/meminfo in bytes (None if unreadable)."""
+    try:
+        for line in open("/proc/meminfo"):
+            if line.startswith("MemAvailable:"):
+                return int(line.split()[1]) * 1024
+    except OSError:
+        pass
+    return None
+
+
 def pinned_exact(nbytes: int):
     """Page-locked host tensor of exactly nbytes (torch's pinned allocator rounds sizes up
     to a power of two, which doubles a 32 GiB + guard-band buffer).  Registers a pageable
     tensor with cudaHostRegister; call unpin(t) when done."""
     import torch
+    avail = host_mem_available()
+    if avail is not None and int(nbytes) > avail - (4 << 30):
+        # page-locking more than the box has would get the process (or the box) killed
+        raise RuntimeError(f"pinned_exact({nbytes}): only {avail} bytes of host memory available")
     t = torch.empty(int(nbytes), dtype=torch.uint8)
     rc = torch.cuda.cudart().cudaHostRegister(t.data_ptr(), t.numel(), 0)
     if int(rc) != 0:
