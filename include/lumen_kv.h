@@ -35,12 +35,26 @@
  *   - All validation happens in lumen_kv_plan_build on the host, before any
  *     launch; pack/unpack never read or write out of bounds for a plan that built.
  *   - pack/unpack are asynchronous on the caller's cudaStream_t (passed as
- *     void*), perform no synchronisation and no allocation.  Results are
- *     complete (and, for host destinations, host-visible) once an event recorded
- *     on that stream after the call has fired (nothing is promised
- *     earlier).
+ *     void*): they enqueue one kernel launch per 256 planes and return.  They never
+ *     synchronise the device or a stream and never allocate device or pinned memory;
+ *     the only CUDA calls besides the launch are cudaGetDevice, for a host buffer one
+ *     cudaHostGetDevicePointer (a table lookup), and for a plan with uploaded
+ *     descriptors one cudaEventRecord.  After a thread's first call they do not touch
+ *     the heap either.  Results are complete (and, for host destinations,
+ *     host-visible) once an event recorded on that stream after the call has fired
+ *     (nothing is promised earlier).
+ *   - One-time cost: the first launch on a device loads every kernel variant and sets
+ *     its shared-memory limit (about twenty cudaFuncGetAttributes / cudaFuncSetAttribute
+ *     calls; a lazily loaded kernel can otherwise wait for kernels that are already
+ *     running).  Call lumen_kv_init() at start-up to take that outside the first pack.
+ *   - Devices: plans, stagers, checkpointers and the library's cached descriptor memory
+ *     belong to the device that was current when they were created; every call must be
+ *     made with that device current (a stream of another device makes the call fail with
+ *     LUMEN_KV_ECUDA).  A process may drive several devices; each is initialised at its
+ *     first launch.
  *   - pack/unpack may be captured into a CUDA graph (stream capture); the plan must then
- *     stay alive for as long as the graph can be replayed.
+ *     stay alive for as long as the graph can be replayed (its descriptor memory is kept
+ *     until lumen_kv_trim()).
  *   - A plan is immutable and direction-agnostic: the same plan drives pack and
  *     unpack.  The caller owns pools, buffers, streams and page tables (page
  *     tables are copied at build time).  Plans may be used concurrently from
@@ -72,7 +86,8 @@ typedef enum {
     LUMEN_KV_EOVERLAP = -3,  /* VALIDATE_UNIQUE_DST: a pool token slot is addressed twice     */
     LUMEN_KV_ESIZE    = -4,  /* buffer smaller than lumen_kv_plan_bytes()                    */
     LUMEN_KV_ENOMEM   = -5,  /* host or device allocation of the descriptors failed          */
-    LUMEN_KV_ECUDA    = -6   /* CUDA runtime error; see lumen_kv_last_cuda_error()           */
+    LUMEN_KV_ECUDA    = -6,  /* CUDA runtime error; see lumen_kv_last_cuda_error()           */
+    LUMEN_KV_ESINK    = -7   /* background checkpointer: the sink rejected a delta           */
 } lumen_kv_status;
 
 /* Geometry of the caller's paged pool (host struct, read during plan_build only). */
@@ -207,8 +222,8 @@ LUMEN_KV_API int lumen_kv_restore_unpack(const lumen_kv_plan* plan,
  * chunk is being packed; restore runs the mirror image (H2D copy, then unpack).  The
  * bytes that arrive are identical to the one-shot call's.
  *
- * A stager owns one non-blocking copy stream and 2*n_slots events; it holds no payload
- * memory.  staging: device pointer, 16-byte aligned, n_slots*slot_bytes bytes, owned by
+ * A stager owns two non-blocking streams (copies; kernels of asynchronous calls), 2*n_slots+1
+ * events and, once an _async call has been made, one thread; it holds no payload memory.  staging: device pointer, 16-byte aligned, n_slots*slot_bytes bytes, owned by
  * the caller and not touched by anything else while a staged call is in flight.
  * slot_bytes must be a multiple of 16 and at least as large as the longest run of every
  * plan used with it (32 KiB unless a single row is larger), else ESIZE.  2 <= n_slots <= 16.
@@ -224,7 +239,7 @@ LUMEN_KV_API int lumen_kv_restore_unpack(const lumen_kv_plan* plan,
 typedef struct lumen_kv_stager lumen_kv_stager;
 LUMEN_KV_API int lumen_kv_stager_create(void* staging, int64_t slot_bytes, int32_t n_slots,
                                         lumen_kv_stager** out);
-LUMEN_KV_API void lumen_kv_stager_destroy(lumen_kv_stager* stager);   /* synchronises its copy stream */
+LUMEN_KV_API void lumen_kv_stager_destroy(lumen_kv_stager* stager);   /* issues what is queued, synchronises its streams */
 LUMEN_KV_API int lumen_kv_checkpoint_pack_staged(const lumen_kv_plan* plan,
                              const void* const* k_planes, const void* const* v_planes,
                              void* dst_host, int64_t dst_bytes, lumen_kv_stager* stager,
@@ -256,6 +271,45 @@ LUMEN_KV_API int lumen_kv_restore_unpack_staged_ready(const lumen_kv_plan* plan,
                              void* const* k_planes, void* const* v_planes,
                              const void* src_host, int64_t src_bytes, lumen_kv_stager* stager,
                              void* stream, const uint64_t* flags, uint64_t epoch);
+
+/*
+ * Asynchronous submission of a staged call.
+ *
+ * The calls above issue six stream operations per chunk from the calling thread: a decode
+ * step's delta (1-6 chunks) costs 10-40 us of host time, but a 32 GiB prefix is 1,024 chunks
+ * and a 70 GiB recovery wave 2,300 -- more operations than a CUDA stream queues, so the calling
+ * thread is held for most of the transfer.  The _async forms return at once: they validate,
+ * record one event on `stream`, and hand the call to a thread owned by the stager, which issues
+ * the same per-chunk pipeline on the stager's own streams.
+ *   ordering : the transfer starts after everything enqueued on `stream` before the call and
+ *              after every earlier call on the same stager.  Nothing enqueued on `stream`
+ *              AFTER the call is ordered behind it (CUDA cannot wait for an event that has not
+ *              been recorded yet); use lumen_kv_stager_wait for that.
+ *   flags, epoch : as in the _commit / _ready forms; NULL = none.
+ *   *ticket  : identifies the call (tickets of one stager increase and complete in order).
+ *   The plan may be freed and the plane-pointer arrays reused as soon as the call returns; the
+ *   host buffer, the pool, the staging ring and (for restore) the flag array must stay valid
+ *   until the ticket is complete.  Errors that validation can find (EINVAL, ESIZE) are returned
+ *   by the call; errors met while issuing are returned by query / wait / sync.
+ * lumen_kv_stager_query : 1 = complete (results visible as after a stream event), 0 = not yet,
+ *                         negative = the call failed with that status.  Never blocks.
+ * lumen_kv_stager_wait  : makes `stream` wait for the ticket's completion.  Blocks the calling
+ *                         thread only until the stager's thread has finished ISSUING the ticket.
+ * lumen_kv_stager_sync  : blocks the calling thread until the ticket is complete.
+ * Synchronous and asynchronous calls may be mixed on one stager; they are issued one at a time.
+ */
+LUMEN_KV_API int lumen_kv_checkpoint_pack_staged_async(const lumen_kv_plan* plan,
+                             const void* const* k_planes, const void* const* v_planes,
+                             void* dst_host, int64_t dst_bytes, lumen_kv_stager* stager,
+                             void* stream, uint64_t* flags, uint64_t epoch, uint64_t* ticket);
+LUMEN_KV_API int lumen_kv_restore_unpack_staged_async(const lumen_kv_plan* plan,
+                             void* const* k_planes, void* const* v_planes,
+                             const void* src_host, int64_t src_bytes, lumen_kv_stager* stager,
+                             void* stream, const uint64_t* flags, uint64_t epoch,
+                             uint64_t* ticket);
+LUMEN_KV_API int lumen_kv_stager_query(lumen_kv_stager* stager, uint64_t ticket);
+LUMEN_KV_API int lumen_kv_stager_wait(lumen_kv_stager* stager, uint64_t ticket, void* stream);
+LUMEN_KV_API int lumen_kv_stager_sync(lumen_kv_stager* stager, uint64_t ticket);
 
 /* number of chunks a staged call on this plan would be cut into for the given slot size
  * (host arithmetic only; ESIZE if a run does not fit a slot) */
@@ -373,8 +427,8 @@ typedef struct {
 } lumen_kv_segment;
 /* A ready-made sink for lumen_kv_ckpt_create (user = the lumen_kv_store*): appends the delta
  * with the tags it carries -- a holder on the same host, or the receiving end of the
- * transport in tests.  A sink cannot return a status, so failed appends are counted instead. */
-LUMEN_KV_API void lumen_kv_store_sink(void* store, uint64_t request_id, int64_t t_begin,
+ * transport in tests.  Returns the append's status; failed appends are counted as well. */
+LUMEN_KV_API int lumen_kv_store_sink(void* store, uint64_t request_id, int64_t t_begin,
                                       int64_t t_end, const void* delta, int64_t delta_bytes,
                                       const lumen_kv_tag* tags, int32_t n_tags);
 LUMEN_KV_API int64_t lumen_kv_store_sink_errors(const lumen_kv_store* store);
@@ -397,7 +451,10 @@ LUMEN_KV_API int64_t lumen_kv_store_segments(const lumen_kv_store* store, uint64
  * still in flight -- then advances t_prev.  The sink stands in for step (4); it runs on the
  * checkpointer's thread, must not keep the pointer, and sees for each request exactly the
  * dense pack buffer of its range: [plane][token][head][dim], with the tags of the pages it
- * touches when the caller supplied token IDs.
+ * touches when the caller supplied token IDs.  The sink returns 0 if it took the delta; on
+ * any other value the request's progress stays where it was (lumen_kv_ckpt_progress does not
+ * advance), what is pending or already in flight for that request is dropped, flush() reports
+ * LUMEN_KV_ESINK, and the request's next notification packs again from its last delivered token.
  *   k_planes, v_planes : device pointers of the pool (copied).
  *   staging / slot_bytes / n_slots : device staging ring as for lumen_kv_stager_create.
  *   pinned / pinned_bytes : pinned host buffer (a multiple of 32 bytes), used as two halves:
@@ -413,7 +470,7 @@ LUMEN_KV_API int64_t lumen_kv_store_segments(const lumen_kv_store* store, uint64
  * the first error the thread met (0 if none).  Errors: EINVAL, ESIZE, ENOMEM, ECUDA.
  */
 typedef struct lumen_kv_ckpt lumen_kv_ckpt;
-typedef void (*lumen_kv_sink_fn)(void* user, uint64_t request_id, int64_t t_begin, int64_t t_end,
+typedef int (*lumen_kv_sink_fn)(void* user, uint64_t request_id, int64_t t_begin, int64_t t_end,
                                  const void* delta, int64_t delta_bytes,
                                  const lumen_kv_tag* tags, int32_t n_tags);
 LUMEN_KV_API int lumen_kv_ckpt_create(const lumen_kv_geom* geom, const void* const* k_planes,
@@ -429,7 +486,9 @@ LUMEN_KV_API int lumen_kv_ckpt_untrack(lumen_kv_ckpt* ckpt, uint64_t request_id)
  * token_ids: NULL, or for each request a HOST pointer to its token history [0, t_cur) (entries
  * may be NULL); the part the new delta needs is copied, and the sink then receives the page
  * tags of the pages each delta touches ("each transferred page carries a page tag",
- * PAPER.md:147), computed by lumen_kv_page_tags_host.  Without tokens n_tags is 0. */
+ * PAPER.md:147), computed by lumen_kv_page_tags_host.  Without tokens n_tags is 0.  A request
+ * whose pending delta carries token IDs must keep passing them (EINVAL otherwise: the tags of
+ * the pending pages would be lost). */
 LUMEN_KV_API int lumen_kv_ckpt_notify(lumen_kv_ckpt* ckpt, const uint64_t* ids,
                                       const lumen_kv_req* reqs, const int32_t* const* token_ids,
                                       int32_t n, void* ready_event);
@@ -491,11 +550,18 @@ LUMEN_KV_API int lumen_kv_recover(const int64_t* load, const uint8_t* alive, int
                                   int64_t* final_load);
 
 /* Release a plan.  Safe to call while work using the plan is still in flight on a
- * stream: the descriptors are recycled only after that work has completed.       */
+ * stream, or still queued in a stager's thread: the descriptors are recycled only after
+ * that work has completed.  Never frees device or pinned memory (no implicit device
+ * synchronisation on the caller's thread): descriptor memory goes back to a cache that
+ * only lumen_kv_trim() empties.                                                      */
 LUMEN_KV_API void lumen_kv_plan_free(lumen_kv_plan* plan);
 
 /* Release cached descriptor memory held by the library (synchronises the device). */
 LUMEN_KV_API void lumen_kv_trim(void);
+
+/* One-time initialisation of the current device (SM count, load of every kernel variant);
+ * done implicitly by the first launch on a device.  Errors: ECUDA.                     */
+LUMEN_KV_API int lumen_kv_init(void);
 
 LUMEN_KV_API const char* lumen_kv_strerror(int status);
 /* last cudaError_t seen by the calling thread inside the library (0 if none) */

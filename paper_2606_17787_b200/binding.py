@@ -21,7 +21,7 @@ _SO = Path(__file__).resolve().parent / "liblumen_kv.so"
 
 # ---- constants mirrored from include/lumen_kv.h -----------------------------------
 LUMEN_KV_OK, LUMEN_KV_EINVAL, LUMEN_KV_ERANGE = 0, -1, -2
-LUMEN_KV_EOVERLAP, LUMEN_KV_ESIZE, LUMEN_KV_ENOMEM, LUMEN_KV_ECUDA = -3, -4, -5, -6
+LUMEN_KV_EOVERLAP, LUMEN_KV_ESIZE, LUMEN_KV_ENOMEM, LUMEN_KV_ECUDA, LUMEN_KV_ESINK = -3, -4, -5, -6, -7
 LUMEN_KV_VALIDATE_UNIQUE_DST = 0x1
 LUMEN_KV_MERGE_ADJACENT = 0x2
 LUMEN_KV_HOST_ONLY = 0x4
@@ -32,7 +32,9 @@ LUMEN_KV_MEM_DEVICE, LUMEN_KV_MEM_HOST_MAPPED = 0, 1
 EXPORTS = (
     "lumen_kv_plan_build", "lumen_kv_plan_build_layout", "lumen_kv_plan_bytes", "lumen_kv_plan_req_offset",
     "lumen_kv_plan_num_runs", "lumen_kv_plan_get_run", "lumen_kv_checkpoint_pack",
-    "lumen_kv_restore_unpack", "lumen_kv_plan_free", "lumen_kv_trim",
+    "lumen_kv_restore_unpack", "lumen_kv_plan_free", "lumen_kv_trim", "lumen_kv_init",
+    "lumen_kv_checkpoint_pack_staged_async", "lumen_kv_restore_unpack_staged_async",
+    "lumen_kv_stager_query", "lumen_kv_stager_wait", "lumen_kv_stager_sync",
     "lumen_kv_strerror", "lumen_kv_last_cuda_error", "lumen_kv_version",
     "lumen_kv_stager_create", "lumen_kv_stager_destroy", "lumen_kv_checkpoint_pack_staged",
     "lumen_kv_restore_unpack_staged", "lumen_kv_plan_num_chunks", "lumen_kv_plan_get_chunks",
@@ -77,7 +79,7 @@ class lumen_kv_chunk_info(ctypes.Structure):
 
 
 # lumen_kv_sink_fn: (user, request_id, t_begin, t_end, delta pointer, delta_bytes, tags, n_tags)
-SINK_FN = ctypes.CFUNCTYPE(None, ctypes.c_void_p, ctypes.c_uint64, ctypes.c_int64, ctypes.c_int64,
+SINK_FN = ctypes.CFUNCTYPE(ctypes.c_int, ctypes.c_void_p, ctypes.c_uint64, ctypes.c_int64, ctypes.c_int64,
                            ctypes.c_void_p, ctypes.c_int64, ctypes.c_void_p, ctypes.c_int32)
 
 
@@ -135,6 +137,19 @@ def _lib() -> ctypes.CDLL:
         f = getattr(L, name)
         f.restype = ctypes.c_int
         f.argtypes = [vp, ctypes.POINTER(vp), ctypes.POINTER(vp), vp, i64, vp, vp, vp, ctypes.c_uint64]
+    for name in ("lumen_kv_checkpoint_pack_staged_async", "lumen_kv_restore_unpack_staged_async"):
+        f = getattr(L, name)
+        f.restype = ctypes.c_int
+        f.argtypes = [vp, ctypes.POINTER(vp), ctypes.POINTER(vp), vp, i64, vp, vp, vp, ctypes.c_uint64,
+                      ctypes.POINTER(ctypes.c_uint64)]
+    L.lumen_kv_stager_query.restype = ctypes.c_int
+    L.lumen_kv_stager_query.argtypes = [vp, ctypes.c_uint64]
+    L.lumen_kv_stager_wait.restype = ctypes.c_int
+    L.lumen_kv_stager_wait.argtypes = [vp, ctypes.c_uint64, vp]
+    L.lumen_kv_stager_sync.restype = ctypes.c_int
+    L.lumen_kv_stager_sync.argtypes = [vp, ctypes.c_uint64]
+    L.lumen_kv_init.restype = ctypes.c_int
+    L.lumen_kv_init.argtypes = []
     L.lumen_kv_tags_num_pages.restype = i64
     L.lumen_kv_tags_num_pages.argtypes = [vp, i32, i32]
     L.lumen_kv_page_tags.restype = ctypes.c_int
@@ -402,6 +417,24 @@ class Stager:
             raise ValueError("stager already destroyed")
         return self._h
 
+    def query(self, ticket: int) -> bool:
+        """True once the asynchronous call `ticket` is complete; raises if it failed."""
+        rc = int(_lib().lumen_kv_stager_query(self.handle, int(ticket)))
+        if rc < 0:
+            raise LumenKVError(rc, "lumen_kv_stager_query")
+        return rc == 1
+
+    def wait(self, ticket: int, stream: int = 0) -> None:
+        """Make `stream` wait for the ticket (blocks the host only until it has been issued)."""
+        rc = int(_lib().lumen_kv_stager_wait(self.handle, int(ticket), ctypes.c_void_p(int(stream))))
+        if rc:
+            raise LumenKVError(rc, "lumen_kv_stager_wait")
+
+    def sync(self, ticket: int) -> None:
+        rc = int(_lib().lumen_kv_stager_sync(self.handle, int(ticket)))
+        if rc:
+            raise LumenKVError(rc, "lumen_kv_stager_sync")
+
     def close(self) -> None:
         if self._h:
             _lib().lumen_kv_stager_destroy(self._h)
@@ -457,6 +490,40 @@ def lumen_kv_restore_unpack_staged_ready(plan: Plan, k_planes, v_planes, src_hos
         ctypes.c_void_p(int(flags_host)), int(epoch))
     if rc:
         raise LumenKVError(rc, "lumen_kv_restore_unpack_staged_ready")
+
+
+def _staged_async(name, plan, k_planes, v_planes, host, nbytes, stager, stream, flags_host, epoch) -> int:
+    L = plan.geom.num_layers
+    ticket = ctypes.c_uint64(0)
+    rc = getattr(_lib(), name)(
+        plan.handle, _as_ptr_array(k_planes, L), _as_ptr_array(v_planes, L), ctypes.c_void_p(int(host)),
+        int(nbytes), stager.handle, ctypes.c_void_p(int(stream)),
+        ctypes.c_void_p(int(flags_host)) if flags_host else None, int(epoch), ctypes.byref(ticket))
+    if rc:
+        raise LumenKVError(rc, name)
+    return int(ticket.value)
+
+
+def lumen_kv_checkpoint_pack_staged_async(plan: Plan, k_planes, v_planes, dst_host: int, dst_bytes: int,
+                                          stager: Stager, stream: int = 0, flags_host: int = 0,
+                                          epoch: int = 0) -> int:
+    """Returns at once with a ticket; the stager's thread issues the chunk pipeline
+    (Stager.query / wait / sync)."""
+    return _staged_async("lumen_kv_checkpoint_pack_staged_async", plan, k_planes, v_planes, dst_host,
+                         dst_bytes, stager, stream, flags_host, epoch)
+
+
+def lumen_kv_restore_unpack_staged_async(plan: Plan, k_planes, v_planes, src_host: int, src_bytes: int,
+                                         stager: Stager, stream: int = 0, flags_host: int = 0,
+                                         epoch: int = 0) -> int:
+    return _staged_async("lumen_kv_restore_unpack_staged_async", plan, k_planes, v_planes, src_host,
+                         src_bytes, stager, stream, flags_host, epoch)
+
+
+def lumen_kv_init() -> None:
+    rc = _lib().lumen_kv_init()
+    if rc:
+        raise LumenKVError(rc, "lumen_kv_init")
 
 
 TAG_DTYPE = np.dtype([("hash", np.uint64), ("end_pos", np.int64)])   # lumen_kv_tag
@@ -634,7 +701,8 @@ def lumen_kv_recover(load, alive, interrupted):
 class BackgroundCheckpointer:
     """Owner of a `lumen_kv_ckpt*` (the worker's background checkpointing thread).
     sink(request_id, t_begin, t_end, delta_ptr, delta_bytes, tags) is called on that thread
-    (tags: a TAG_DTYPE array, empty unless notify() was given token IDs); or pass a Store."""
+    (tags: a TAG_DTYPE array, empty unless notify() was given token IDs) and returns None / 0
+    when it took the delta, another int to reject it; or pass a Store."""
 
     def __init__(self, geom: lumen_kv_geom, k_planes, v_planes, staging_ptr: int, slot_bytes: int,
                  n_slots: int, pinned_ptr: int, pinned_bytes: int, sink):
@@ -647,7 +715,8 @@ class BackgroundCheckpointer:
             def _call(_u, rid, tb, te, ptr, nb, tags, n_tags):
                 t = (np.ctypeslib.as_array((ctypes.c_uint8 * (16 * n_tags)).from_address(tags)).view(TAG_DTYPE).copy()
                      if n_tags else np.zeros(0, dtype=TAG_DTYPE))
-                sink(int(rid), int(tb), int(te), int(ptr), int(nb), t)
+                rc = sink(int(rid), int(tb), int(te), int(ptr), int(nb), t)
+                return int(rc) if rc else 0          # None / 0: taken; anything else: rejected
             self._cb = SINK_FN(_call)
             user = None
         out = ctypes.c_void_p()

@@ -33,6 +33,7 @@ struct Tracked {
     bool has_pending = false;
     int in_flight = 0;         // batches enqueued but not yet delivered that contain this request
     bool zombie = false;       // untracked while in flight: erased after delivery
+    uint64_t gen = 0;          // bumped when a delivery fails: jobs taken before that are void
     Pending p;
 };
 
@@ -42,6 +43,7 @@ struct Job {
     int64_t tb, te;
     cudaEvent_t ev;
     std::vector<lumen_kv_tag> tags;   // tags of the pages [tb, te) touches
+    uint64_t gen = 0;                 // the request's generation when the job was taken
 };
 
 // tags of a job, from the token IDs the notification carried
@@ -174,42 +176,64 @@ void submit(lumen_kv_ckpt* c, Batch& b) {
 
 // Stage 2: hand every request's delta to the sink as soon as the chunks that hold it have
 // committed (later chunks, and the next batch's pack into the other half, are still in flight).
+// Under the lock: request `t` lost a delta (sink rejection or batch failure).  Its progress stays
+// at t_prev, nothing of it remains pending, and jobs of it that are already in the next batch are
+// void (their generation is stale): they would reach the sink with a gap in front of them.
+void fail_request(Tracked& t) {
+    ++t.gen;
+    t.has_pending = false;
+    t.p.marks.clear();
+    t.p.toks.clear();
+    t.t_sent = t.t_prev;
+}
+
 void deliver(lumen_kv_ckpt* c, Batch& b) {
     const int32_t n = static_cast<int32_t>(b.jobs.size());
     const char* base = c->pinned + b.half * (c->pinned_bytes / 2);
     const int64_t n_chunks = static_cast<int64_t>(b.chunks.size());
     int64_t ci = 0;
+    int sink_rc = LUMEN_KV_OK;
     for (int32_t i = 0; i < n && b.rc == LUMEN_KV_OK; ++i) {
+        const Job& j = b.jobs[i];
         const int64_t off = lumen_kv_plan_req_offset(b.plan, i);
         const int64_t end = lumen_kv_plan_req_offset(b.plan, i + 1);
+        {
+            std::lock_guard<std::mutex> g(c->mu);
+            auto it = c->reqs.find(j.id);
+            if (it == c->reqs.end() || it->second.gen != j.gen) continue;   // void: see fail_request
+        }
+        bool taken = true;
         if (end > off) {
             while (ci < n_chunks && b.chunks[static_cast<size_t>(ci)].byte_end < end) ++ci;
             if (ci >= n_chunks || !wait_flag(c, b, ci)) {   // the chunk that completes request i
                 b.rc = LUMEN_KV_ECUDA;
                 break;
             }
-            c->sink(c->user, b.jobs[i].id, b.jobs[i].tb, b.jobs[i].te, base + off, end - off,
-                    b.jobs[i].tags.data(), static_cast<int32_t>(b.jobs[i].tags.size()));
+            taken = c->sink(c->user, j.id, j.tb, j.te, base + off, end - off, j.tags.data(),
+                            static_cast<int32_t>(j.tags.size())) == 0;
         }
         std::lock_guard<std::mutex> g(c->mu);
-        auto it = c->reqs.find(b.jobs[i].id);
-        if (it != c->reqs.end()) it->second.t_prev = b.jobs[i].te;   // progress (a1)
+        auto it = c->reqs.find(j.id);
+        if (it == c->reqs.end()) continue;
+        if (taken) {
+            it->second.t_prev = j.te;                       // progress (a1)
+        } else {
+            fail_request(it->second);
+            sink_rc = LUMEN_KV_ESINK;
+        }
     }
     if (b.rc != LUMEN_KV_OK) cudaStreamSynchronize(c->stream);
     if (b.plan) lumen_kv_plan_free(b.plan);
     b.plan = nullptr;
     std::lock_guard<std::mutex> g(c->mu);
-    if (b.rc != LUMEN_KV_OK && c->first_error == 0) c->first_error = b.rc;
+    if (c->first_error == 0) c->first_error = b.rc != LUMEN_KV_OK ? b.rc : sink_rc;
     for (const Job& j : b.jobs) {
         auto it = c->reqs.find(j.id);
         if (it == c->reqs.end()) continue;
         Tracked& t = it->second;
         --t.in_flight;
-        if (b.rc != LUMEN_KV_OK) {                  // do not retry for ever
-            t.has_pending = false;
-            t.p.marks.clear();
-            t.t_sent = t.t_prev;
-        }
+        if (b.rc != LUMEN_KV_OK && t.gen == j.gen && t.t_prev < j.te)   // do not retry for ever
+            fail_request(t);
         if (t.zombie && t.in_flight == 0) c->reqs.erase(it);
     }
 }
@@ -247,7 +271,7 @@ void take_jobs(lumen_kv_ckpt* c, Batch& b, int64_t room) {
         if (want <= room) {
             const bool last = (k + 1 == t.p.marks.size());
             b.jobs.push_back(Job{kv.first, last ? std::move(t.p.pt) : t.p.pt, t.t_sent, te, ev,
-                                 tags_of(t.p, t.t_sent, te, c->geom.page_size)});
+                                 tags_of(t.p, t.t_sent, te, c->geom.page_size), t.gen});
             t.p.marks.erase(t.p.marks.begin(), t.p.marks.begin() + static_cast<long>(k) + 1);
             t.has_pending = !last;
             t.t_sent = te;
@@ -261,7 +285,7 @@ void take_jobs(lumen_kv_ckpt* c, Batch& b, int64_t room) {
                 continue;
             }
             b.jobs.push_back(Job{kv.first, t.p.pt, t.t_sent, t.t_sent + fit, ev,
-                                 tags_of(t.p, t.t_sent, t.t_sent + fit, c->geom.page_size)});
+                                 tags_of(t.p, t.t_sent, t.t_sent + fit, c->geom.page_size), t.gen});
             t.t_sent += fit;                        // the rest stays pending
             room = 0;
         } else {
@@ -408,6 +432,10 @@ int lumen_kv_ckpt_notify(lumen_kv_ckpt* c, const uint64_t* ids, const lumen_kv_r
             if (reqs[i].t_end < floor_ || reqs[i].page_table_len < 0 ||
                 (reqs[i].t_end > 0 && (!reqs[i].page_table ||
                                        (reqs[i].t_end + S - 1) / S > reqs[i].page_table_len)))
+                return LUMEN_KV_EINVAL;
+            // the pending delta carries token IDs: a notification without them would lose the
+            // tags of pages that are still to be sent
+            if (t.has_pending && !t.p.toks.empty() && !(token_ids && token_ids[i]))
                 return LUMEN_KV_EINVAL;
         }
         for (int32_t i = 0; i < n; ++i) {

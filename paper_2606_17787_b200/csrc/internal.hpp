@@ -3,7 +3,10 @@
 #pragma once
 #include <cuda_runtime.h>
 
+#include <atomic>
 #include <cstdint>
+#include <memory>
+#include <mutex>
 #include <vector>
 
 #include "lumen_kv.h"
@@ -27,9 +30,24 @@ struct lumen_kv_plan {
     int32_t n_reqs = 0;
     uint32_t flags = 0;
     bool inline_desc = false;  // small plan: descriptors stay in hp and travel as kernel parameters
+    // lumen_kv_plan_free drops the caller's reference; an asynchronous staged call holds one of
+    // its own until the stager's thread has issued it
+    std::atomic<int> refs{1};
+    // the chunk list of the two-stage path, built once per slot size and shared with whoever
+    // is still issuing from it
+    std::mutex chunk_mu;
+    int64_t chunk_slot_bytes = 0;
+    std::shared_ptr<const std::vector<lumen::Chunk>> chunk_list;
 };
 
 namespace lumen {
+
+void plan_retain(const lumen_kv_plan* plan);
+void plan_release(const lumen_kv_plan* plan);   // frees the plan with the last reference
+
+// The plan's chunks for this slot size (build_chunks, cached on the plan); a lumen_kv_status.
+int plan_chunks(const lumen_kv_plan* plan, int64_t slot_bytes,
+                std::shared_ptr<const std::vector<Chunk>>* out);
 
 // validation shared by the one-shot and the staged calls: interleaves the plane pointers
 // (K0,V0,K1,V1,..) into `planes`

@@ -24,6 +24,9 @@
 #include <mutex>
 
 namespace lumen {
+
+int g_host_kernel = kKernelBulk;   // LUMEN_KV_HOST_KERNEL=warp|bulk: what AUTO picks for host buffers
+
 namespace {
 
 struct PlaneTable {
@@ -360,17 +363,16 @@ BulkCfg bulk_config(int64_t item_bytes_max) {
     return c;
 }
 
-int g_num_sms = 0;
 int g_warp_unroll = 4;   // LUMEN_KV_WARP_UNROLL=4|8 (tuning knob, read once; 4 measured best)
 
 int g_host_ctas = 0;   // grid of the bulk kernel when the buffer is host memory (0: default)
 
 template <int STAGES, class Desc>
 cudaError_t launch_bulk_desc(const PlaneTable& pt, const Desc& d, const CopyArgs& a, int32_t plane0,
-                             int32_t np, const BulkCfg& c) {
+                             int32_t np, const BulkCfg& c, int num_sms) {
     auto kern = kv_copy_bulk<STAGES, Desc>;   // dynamic shared memory limit set by preload_all()
     const int64_t total = a.n_runs * np;
-    int64_t grid = static_cast<int64_t>(g_num_sms) * c.ctas_per_sm;
+    int64_t grid = static_cast<int64_t>(num_sms) * c.ctas_per_sm;
     // A host-memory buffer is bound by the host link (~55 GB/s): a few dozen single-warp
     // CTAs keep it full, and the SMs stay free for whatever else the device is running
     // (checkpointing must stay off the GPU critical path).
@@ -384,14 +386,14 @@ cudaError_t launch_bulk_desc(const PlaneTable& pt, const Desc& d, const CopyArgs
 
 template <int STAGES>
 cudaError_t launch_bulk(const PlaneTable& pt, const CopyArgs& a, int32_t plane0, int32_t np,
-                        const BulkCfg& c) {
+                        const BulkCfg& c, int num_sms) {
     if (a.inline_desc) {
         InlineDesc d;
         std::memcpy(d.runs, a.runs, static_cast<size_t>(a.n_runs) * sizeof(RunDesc));
         std::memcpy(d.reqs, a.reqs, static_cast<size_t>(a.n_reqs) * sizeof(ReqDesc));
-        return launch_bulk_desc<STAGES>(pt, d, a, plane0, np, c);
+        return launch_bulk_desc<STAGES>(pt, d, a, plane0, np, c, num_sms);
     }
-    return launch_bulk_desc<STAGES>(pt, GlobalDesc{a.runs, a.reqs}, a, plane0, np, c);
+    return launch_bulk_desc<STAGES>(pt, GlobalDesc{a.runs, a.reqs}, a, plane0, np, c, num_sms);
 }
 
 struct WarpLaunch {
@@ -475,8 +477,6 @@ cudaError_t preload_all() {
 
 }  // namespace
 
-int g_host_kernel = kKernelBulk;   // LUMEN_KV_HOST_KERNEL=warp|bulk: what AUTO picks for host buffers
-
 int resolve_kernel(const CopyArgs& a) {
     int k = a.kernel;
     const int64_t item_max = static_cast<int64_t>(a.max_count) * a.row_bytes;
@@ -485,11 +485,19 @@ int resolve_kernel(const CopyArgs& a) {
     return k;
 }
 
-cudaError_t launch_kv_copy(const CopyArgs& a) {
-    if (a.n_runs == 0 || a.n_planes == 0) return cudaSuccess;
-    // one-time, thread-safe: tuning knobs, SM count, kernel preload
+// Per-device state: the SM count, and the one-time load of every kernel variant together with
+// its dynamic shared memory limit (cudaFuncSetAttribute is per device).  A process that drives
+// several GPUs initialises each device at its first launch there.
+struct DeviceState {
+    std::once_flag once;
+    cudaError_t err = cudaSuccess;
+    int num_sms = 0;
+};
+constexpr int kMaxDevices = 64;
+DeviceState g_dev[kMaxDevices];
+
+void read_env_once() {
     static std::once_flag once;
-    static cudaError_t init_err = cudaSuccess;
     std::call_once(once, [] {
         if (const char* e = getenv("LUMEN_KV_WARP_UNROLL")) g_warp_unroll = (atoi(e) == 8) ? 8 : 4;
         if (const char* e = getenv("LUMEN_KV_PDL")) g_pdl = atoi(e) ? 1 : 0;
@@ -497,12 +505,33 @@ cudaError_t launch_kv_copy(const CopyArgs& a) {
         if (const char* e = getenv("LUMEN_KV_HOST_KERNEL"))
             g_host_kernel = (e[0] == 'w') ? kKernelWarp : kKernelBulk;
         if (const char* e = getenv("LUMEN_KV_HOST_CTAS")) g_host_ctas = atoi(e);
-        int dev = 0;
-        init_err = cudaGetDevice(&dev);
-        if (init_err == cudaSuccess)
-            init_err = cudaDeviceGetAttribute(&g_num_sms, cudaDevAttrMultiProcessorCount, dev);
-        if (init_err == cudaSuccess) init_err = preload_all();
     });
+}
+
+cudaError_t device_state(DeviceState** out) {
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= kMaxDevices) return cudaErrorInvalidDevice;
+    DeviceState& st = g_dev[dev];
+    std::call_once(st.once, [&st, dev] {
+        read_env_once();
+        st.err = cudaDeviceGetAttribute(&st.num_sms, cudaDevAttrMultiProcessorCount, dev);
+        if (st.err == cudaSuccess) st.err = preload_all();
+    });
+    *out = &st;
+    return st.err;
+}
+
+cudaError_t init_current_device() {
+    DeviceState* st = nullptr;
+    return device_state(&st);
+}
+
+cudaError_t launch_kv_copy(const CopyArgs& a) {
+    if (a.n_runs == 0 || a.n_planes == 0) return cudaSuccess;
+    DeviceState* dev = nullptr;
+    const cudaError_t init_err = device_state(&dev);   // thread-safe; a table lookup after the first call
     if (init_err != cudaSuccess) return init_err;
     const int kernel = resolve_kernel(a);
     const int64_t item_max = static_cast<int64_t>(a.max_count) * a.row_bytes;
@@ -518,11 +547,11 @@ cudaError_t launch_kv_copy(const CopyArgs& a) {
         if (kernel == kKernelBulk) {
             const BulkCfg c = bulk_config(item_max);
             switch (c.stages) {
-                case 3:  e = launch_bulk<3>(pt, a, plane0, np, c); break;
-                case 4:  e = launch_bulk<4>(pt, a, plane0, np, c); break;
-                case 6:  e = launch_bulk<6>(pt, a, plane0, np, c); break;
-                case 8:  e = launch_bulk<8>(pt, a, plane0, np, c); break;
-                default: e = launch_bulk<16>(pt, a, plane0, np, c); break;
+                case 3:  e = launch_bulk<3>(pt, a, plane0, np, c, dev->num_sms); break;
+                case 4:  e = launch_bulk<4>(pt, a, plane0, np, c, dev->num_sms); break;
+                case 6:  e = launch_bulk<6>(pt, a, plane0, np, c, dev->num_sms); break;
+                case 8:  e = launch_bulk<8>(pt, a, plane0, np, c, dev->num_sms); break;
+                default: e = launch_bulk<16>(pt, a, plane0, np, c, dev->num_sms); break;
             }
         } else {
             // sub-chunks per item: smallest power of two covering the longest run

@@ -40,6 +40,10 @@ struct CopyArgs {
 // Enqueues the copy.  No synchronisation, no allocation.
 cudaError_t launch_kv_copy(const CopyArgs& a);
 
+// One-time initialisation of the CURRENT device (SM count, load of every kernel variant and its
+// shared-memory limit); launch_kv_copy does it by itself at the first launch on a device.
+cudaError_t init_current_device();
+
 // Which kernel AUTO resolves to for these arguments (exposed for tests / bench notes).
 int resolve_kernel(const CopyArgs& a);
 

@@ -4,8 +4,11 @@
 
 #include <cstdlib>
 #include <cstring>
+#include <map>
+#include <memory>
 #include <mutex>
 #include <new>
+#include <stdexcept>
 #include <vector>
 
 #include "internal.hpp"
@@ -27,9 +30,11 @@ int cuda_fail(cudaError_t e) {
 // the device copy is no longer read by enqueued work.
 struct Blob {
     void* host = nullptr;   // cudaHostAlloc (or malloc for HOST_ONLY)
-    void* dev = nullptr;    // cudaMalloc
+    void* dev = nullptr;    // cudaMalloc, on `device`
     size_t cap = 0;
+    int device = -1;        // the device `dev` and the events belong to
     bool host_only = false;
+    bool captured = false;  // used under stream capture: a graph may replay it at any time
     std::vector<std::pair<cudaStream_t, cudaEvent_t>> uses;  // last use per stream
 };
 
@@ -37,17 +42,25 @@ namespace {
 
 // Recycles blobs so that a build -> pack -> free loop per decode iteration performs
 // no cudaMalloc / cudaHostAlloc in steady state (SURVEY.md section 7.3 hard part 2).
+// Free lists are kept per (device, size class): a blob is only ever reused on the device that
+// owns its memory and events, and acquire() looks at blobs of the wanted size only.
+// Nothing is ever freed here -- cudaFree synchronises the device, and release() runs on the
+// decode loop's thread; lumen_kv_trim() is the one place that gives memory back.
 class Arena {
 public:
     int acquire(size_t bytes, Blob** out) {
         size_t cap = 4096;
         while (cap < bytes) cap <<= 1;
+        int dev = 0;
+        cudaError_t e = cudaGetDevice(&dev);
+        if (e != cudaSuccess) return cuda_fail(e);
         {
             std::lock_guard<std::mutex> g(mu_);
-            for (size_t i = 0; i < free_.size(); ++i) {
-                Blob* b = free_[i];
-                if (b->cap != cap || !idle(b)) continue;
-                free_.erase(free_.begin() + static_cast<long>(i));
+            std::vector<Blob*>& fl = free_[std::make_pair(dev, cap)];
+            for (size_t i = 0; i < fl.size(); ++i) {
+                Blob* b = fl[i];
+                if (!idle(b)) continue;
+                fl.erase(fl.begin() + static_cast<long>(i));
                 *out = b;
                 return LUMEN_KV_OK;
             }
@@ -55,7 +68,8 @@ public:
         Blob* b = new (std::nothrow) Blob();
         if (!b) return LUMEN_KV_ENOMEM;
         b->cap = cap;
-        cudaError_t e = cudaHostAlloc(&b->host, cap, cudaHostAllocDefault);
+        b->device = dev;
+        e = cudaHostAlloc(&b->host, cap, cudaHostAllocDefault);
         if (e == cudaSuccess) e = cudaMalloc(&b->dev, cap);
         if (e != cudaSuccess) {
             if (b->host) cudaFreeHost(b->host);
@@ -77,21 +91,20 @@ public:
             return;
         }
         std::lock_guard<std::mutex> g(mu_);
-        free_.push_back(b);
-        // bound the cache: drop the oldest idle blobs beyond 64 entries
-        while (free_.size() > 64) {
-            Blob* old = free_.front();
-            if (!idle(old)) break;
-            free_.erase(free_.begin());
-            destroy(old);
-        }
+        if (b->captured)
+            retired_.push_back(b);   // an instantiated graph may still read it: kept until trim()
+        else
+            free_[std::make_pair(b->device, b->cap)].push_back(b);
     }
 
     void trim() {
         cudaDeviceSynchronize();
         std::lock_guard<std::mutex> g(mu_);
-        for (Blob* b : free_) destroy(b);
+        for (auto& kv : free_)
+            for (Blob* b : kv.second) destroy(b);
         free_.clear();
+        for (Blob* b : retired_) destroy(b);
+        retired_.clear();
     }
 
 private:
@@ -107,10 +120,12 @@ private:
         for (auto& u : b->uses) cudaEventDestroy(u.second);
         if (b->host) cudaFreeHost(b->host);
         if (b->dev) cudaFree(b->dev);
+        (void)cudaGetLastError();
         delete b;
     }
     std::mutex mu_;
-    std::vector<Blob*> free_;
+    std::map<std::pair<int, size_t>, std::vector<Blob*>> free_;
+    std::vector<Blob*> retired_;
 };
 
 Arena& arena() {
@@ -127,6 +142,15 @@ namespace {
 // record "plan still in use on `stream`" so the arena does not recycle the blob early
 int note_use(lumen_kv_plan* p, cudaStream_t stream) {
     Blob* b = p->blob;
+    // Under stream capture an event record would become a graph node and could never be
+    // queried; the plan must outlive the graph anyway (lumen_kv.h), so the blob is simply
+    // never recycled.
+    cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+    if (cudaStreamIsCapturing(stream, &cs) != cudaSuccess) (void)cudaGetLastError();
+    if (cs != cudaStreamCaptureStatusNone) {
+        b->captured = true;
+        return LUMEN_KV_OK;
+    }
     for (auto& u : b->uses)
         if (u.first == stream) {
             cudaError_t e = cudaEventRecord(u.second, stream);
@@ -190,6 +214,32 @@ int launch_part(const lumen_kv_plan* plan, const std::vector<const void*>& plane
     return note_use(const_cast<lumen_kv_plan*>(plan), stream);
 }
 
+void plan_retain(const lumen_kv_plan* plan) {
+    const_cast<lumen_kv_plan*>(plan)->refs.fetch_add(1, std::memory_order_relaxed);
+}
+
+void plan_release(const lumen_kv_plan* plan_) {
+    lumen_kv_plan* plan = const_cast<lumen_kv_plan*>(plan_);
+    if (plan->refs.fetch_sub(1, std::memory_order_acq_rel) != 1) return;
+    if (plan->blob) arena().release(plan->blob);
+    delete plan;
+}
+
+int plan_chunks(const lumen_kv_plan* plan_, int64_t slot_bytes,
+                std::shared_ptr<const std::vector<Chunk>>* out) {
+    lumen_kv_plan* plan = const_cast<lumen_kv_plan*>(plan_);
+    std::lock_guard<std::mutex> g(plan->chunk_mu);
+    if (!plan->chunk_list || plan->chunk_slot_bytes != slot_bytes) {
+        auto v = std::make_shared<std::vector<Chunk>>();
+        const int rc = build_chunks(plan->hp, plan->h_runs, slot_bytes, v.get());
+        if (rc != LUMEN_KV_OK) return rc;
+        plan->chunk_list = std::move(v);
+        plan->chunk_slot_bytes = slot_bytes;
+    }
+    *out = plan->chunk_list;
+    return LUMEN_KV_OK;
+}
+
 namespace {
 
 int run_copy(const lumen_kv_plan* plan, const void* const* k_planes, const void* const* v_planes,
@@ -200,7 +250,8 @@ int run_copy(const lumen_kv_plan* plan, const void* const* k_planes, const void*
     if (buf_bytes < plan->hp.total_bytes) return LUMEN_KV_ESIZE;
     if (plan->hp.total_bytes == 0) return LUMEN_KV_OK;  // A4: empty plan launches nothing
     if (!buf) return LUMEN_KV_EINVAL;
-    std::vector<const void*> planes;
+    // reused across calls: after a thread's first call this allocates nothing
+    static thread_local std::vector<const void*> planes;
     int rc = gather_planes(plan, k_planes, v_planes, &planes);
     if (rc != LUMEN_KV_OK) return rc;
     void* dev_buf = buf;
@@ -243,6 +294,8 @@ int lumen_kv_plan_build_layout(const lumen_kv_geom* geom, const lumen_kv_req* re
     try {
         rc = build_host_plan(geom, reqs, layouts, num_reqs, flags, &p->hp);
     } catch (const std::bad_alloc&) {
+        rc = LUMEN_KV_ENOMEM;
+    } catch (const std::exception&) {   // e.g. length_error: nothing may cross the C boundary
         rc = LUMEN_KV_ENOMEM;
     }
     if (rc != LUMEN_KV_OK) {
@@ -348,12 +401,15 @@ int lumen_kv_restore_unpack(const lumen_kv_plan* plan, void* const* k_planes,
 }
 
 void lumen_kv_plan_free(lumen_kv_plan* plan) {
-    if (!plan) return;
-    if (plan->blob) lumen::arena().release(plan->blob);
-    delete plan;
+    if (plan) lumen::plan_release(plan);
 }
 
 void lumen_kv_trim(void) { lumen::arena().trim(); }
+
+int lumen_kv_init(void) {
+    const cudaError_t e = lumen::init_current_device();
+    return e == cudaSuccess ? LUMEN_KV_OK : lumen::cuda_fail(e);
+}
 
 const char* lumen_kv_strerror(int status) {
     switch (status) {
@@ -364,6 +420,7 @@ const char* lumen_kv_strerror(int status) {
         case LUMEN_KV_ESIZE: return "buffer smaller than the plan's bytes";
         case LUMEN_KV_ENOMEM: return "out of memory (descriptors), or no room for the reservation in the store arena";
         case LUMEN_KV_ECUDA: return "CUDA runtime error (see lumen_kv_last_cuda_error)";
+        case LUMEN_KV_ESINK: return "the checkpointer's sink rejected a delta";
         default: return "unknown status";
     }
 }

@@ -98,9 +98,19 @@ int build_host_plan(const lumen_kv_geom* g, const lumen_kv_req* reqs,
             hp->reqs[r].n = ly.plane_stride_tokens;
             hp->req_offset[r] = ly.buf_offset;
             hp->req_stride[r] = ly.plane_stride_tokens;
-            if (n > 0)
-                extent = std::max(extent, ly.buf_offset +
-                                              ((planes - 1) * ly.plane_stride_tokens + n) * row);
+            if (n > 0) {
+                // largest byte addressed + 1 = buf_offset + ((planes-1)*stride + n)*row, every
+                // step checked: stride < 2^40, row <= 2^30 and planes <= 65534 alone do not
+                // keep the product inside 63 bits
+                int64_t rows = 0, ext = 0;
+                if (__builtin_mul_overflow(planes - 1, ly.plane_stride_tokens, &rows) ||
+                    __builtin_add_overflow(rows, n, &rows) ||
+                    __builtin_mul_overflow(rows, row, &ext) ||
+                    __builtin_add_overflow(ext, ly.buf_offset, &ext) ||
+                    ext > (std::numeric_limits<int64_t>::max() / 4))
+                    return LUMEN_KV_EINVAL;
+                extent = std::max(extent, ext);
+            }
         } else {
             hp->reqs[r].row_base = tokens * planes;
             hp->reqs[r].n = n;
@@ -183,7 +193,8 @@ int build_host_plan(const lumen_kv_geom* g, const lumen_kv_req* reqs,
     }
 
     // pass 2: flatten into runs
-    hp->runs.reserve(static_cast<size_t>(touched * std::max<int64_t>(1, (dense + kChunkBytes - 1) / kChunkBytes)));
+    // a page span of k tokens yields ceil(k / chunk_tokens) <= k / chunk_tokens + 1 runs
+    hp->runs.reserve(static_cast<size_t>(tokens / chunk_tokens + touched));
     hp->req_run_begin.assign(static_cast<size_t>(num_reqs) + 1, 0);
     for (int32_t r = 0; r < num_reqs; ++r) {
         const lumen_kv_req& q = reqs[r];

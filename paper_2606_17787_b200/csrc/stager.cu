@@ -1,24 +1,64 @@
 // Two-stage host path (include/lumen_kv.h): device staging ring + copy-engine transfers,
-// per-chunk commit / ready flags.
+// per-chunk commit / ready flags, and the asynchronous form in which a stager-owned thread
+// issues the per-chunk stream operations.
 #include <cuda_runtime.h>
 
+#include <condition_variable>
+#include <deque>
+#include <memory>
 #include <mutex>
 #include <new>
+#include <thread>
 #include <vector>
 
 #include "internal.hpp"
 #include "lumen_kv.h"
 #include "plan.hpp"
 
+namespace {
+
+// One asynchronous call waiting for (or being issued by) the stager's thread.
+struct Job {
+    uint64_t ticket = 0;
+    const lumen_kv_plan* plan = nullptr;                        // holds a reference
+    std::shared_ptr<const std::vector<lumen::Chunk>> chunks;
+    std::vector<const void*> planes;                            // K0,V0,K1,V1,..
+    char* host = nullptr;
+    unsigned long long flags_dev = 0;
+    uint64_t epoch = 0;
+    bool pack = true;
+    cudaEvent_t begin = nullptr;   // recorded on the caller's stream at the call
+};
+
+struct TicketRec {
+    uint64_t id = 0;
+    cudaEvent_t done = nullptr;    // recorded behind the call's last operation once issued
+    int status = LUMEN_KV_OK;
+    bool issued = false;
+};
+
+}  // namespace
+
 struct lumen_kv_stager {
     char* base = nullptr;          // caller's device staging memory
     int64_t slot_bytes = 0;
     int32_t n_slots = 0;
+    int device = 0;                // the device its streams and events belong to
     int64_t next = 0;              // chunks issued so far: chunk i uses slot i % n_slots
     cudaStream_t copy = nullptr;   // the stager's copy stream (non-blocking)
+    cudaStream_t work = nullptr;   // kernels of asynchronous calls (non-blocking)
     cudaEvent_t full[16];          // slot holds a complete chunk (producer done)
     cudaEvent_t free_[16];         // slot may be overwritten (consumer done)
     cudaEvent_t join = nullptr;
+    std::mutex issue_mu;           // one call is issued at a time (calling threads and the worker)
+
+    std::mutex mu;                 // everything below
+    std::condition_variable cv;
+    std::deque<Job> queue;
+    std::deque<TicketRec> tickets; // ascending id; the front is pruned once complete
+    uint64_t next_ticket = 1;
+    bool worker_started = false, stop = false;
+    std::thread worker;
 };
 
 namespace lumen {
@@ -56,26 +96,29 @@ int load_stream_memops() {
     return err == cudaSuccess ? LUMEN_KV_OK : cuda_fail(err);
 }
 
-int run_staged(const lumen_kv_plan* plan, const void* const* k_planes, const void* const* v_planes,
-               void* host, int64_t host_bytes, lumen_kv_stager* st, void* stream_, bool pack,
-               const uint64_t* flags = nullptr, uint64_t epoch = 0) {
+// Everything a staged call checks before anything is enqueued; fills the job.
+int prepare(const lumen_kv_plan* plan, const void* const* k_planes, const void* const* v_planes,
+            void* host, int64_t host_bytes, lumen_kv_stager* st, bool pack, const uint64_t* flags,
+            uint64_t epoch, Job* job, bool* empty) {
+    *empty = false;
     if (!plan || !st) return LUMEN_KV_EINVAL;
     if (plan->flags & LUMEN_KV_HOST_ONLY) return LUMEN_KV_EINVAL;
     if (host_bytes < plan->hp.total_bytes) return LUMEN_KV_ESIZE;
-    if (plan->hp.total_bytes == 0) return LUMEN_KV_OK;
+    if (plan->hp.total_bytes == 0) {
+        *empty = true;
+        return LUMEN_KV_OK;
+    }
     if (!host || (reinterpret_cast<uintptr_t>(host) & 15)) return LUMEN_KV_EINVAL;
-    std::vector<const void*> planes;
-    int rc = gather_planes(plan, k_planes, v_planes, &planes);
+    int rc = gather_planes(plan, k_planes, v_planes, &job->planes);
     if (rc != LUMEN_KV_OK) return rc;
     void* alias = nullptr;         // only to reject pageable memory: the copies must be asynchronous
     if (cudaHostGetDevicePointer(&alias, host, 0) != cudaSuccess) {
         (void)cudaGetLastError();
         return LUMEN_KV_EINVAL;
     }
-    std::vector<Chunk> chunks;
-    rc = build_chunks(plan->hp, plan->h_runs, st->slot_bytes, &chunks);
+    rc = plan_chunks(plan, st->slot_bytes, &job->chunks);   // cached on the plan
     if (rc != LUMEN_KV_OK) return rc;
-    unsigned long long flags_dev = 0;   // device alias of the caller's pinned flag array
+    job->flags_dev = 0;            // device alias of the caller's pinned flag array
     if (flags) {
         if (reinterpret_cast<uintptr_t>(flags) & 7) return LUMEN_KV_EINVAL;
         void* fa = nullptr;
@@ -83,42 +126,53 @@ int run_staged(const lumen_kv_plan* plan, const void* const* k_planes, const voi
             (void)cudaGetLastError();
             return LUMEN_KV_EINVAL;
         }
-        flags_dev = reinterpret_cast<unsigned long long>(fa);
+        job->flags_dev = reinterpret_cast<unsigned long long>(fa);
         rc = load_stream_memops();
         if (rc != LUMEN_KV_OK) return rc;
     }
+    job->plan = plan;
+    job->host = static_cast<char*>(host);
+    job->epoch = epoch;
+    job->pack = pack;
+    return LUMEN_KV_OK;
+}
 
-    cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+// The per-chunk pipeline of one call, kernels on `stream`, transfers on the stager's copy
+// stream.  Called with st->issue_mu held.
+int issue(lumen_kv_stager* st, const Job& j, cudaStream_t stream) {
+    const lumen_kv_plan* plan = j.plan;
+    const bool pack = j.pack;
     int64_t ci = 0;                     // chunk index = entry of lumen_kv_plan_get_chunks
-    char* h = static_cast<char*>(host);
+    char* h = j.host;
     if (!pack) {   // the host buffer may have been produced by earlier work on `stream`
         LUMEN_CUDA(cudaEventRecord(st->join, stream));
         LUMEN_CUDA(cudaStreamWaitEvent(st->copy, st->join, 0));
     }
-    for (const Chunk& c : chunks) {
+    for (const Chunk& c : *j.chunks) {
         const int slot = static_cast<int>(st->next++ % st->n_slots);
         char* sbase = st->base + int64_t{slot} * st->slot_bytes;
         // the address byte 0 of the checkpoint buffer would have if the chunk sat in this slot
         const uintptr_t shifted = reinterpret_cast<uintptr_t>(sbase) - static_cast<uintptr_t>(c.b0);
         const size_t bytes = static_cast<size_t>(c.b1 - c.b0);
+        int rc;
         if (pack) {
             LUMEN_CUDA(cudaStreamWaitEvent(stream, st->free_[slot], 0));
-            rc = launch_part(plan, planes, shifted, false, stream, true, c.ra, c.rb, c.p0, c.p1);
+            rc = launch_part(plan, j.planes, shifted, false, stream, true, c.ra, c.rb, c.p0, c.p1);
             if (rc != LUMEN_KV_OK) return rc;
             LUMEN_CUDA(cudaEventRecord(st->full[slot], stream));
             LUMEN_CUDA(cudaStreamWaitEvent(st->copy, st->full[slot], 0));
             LUMEN_CUDA(cudaMemcpyAsync(h + c.b0, sbase, bytes, cudaMemcpyDeviceToHost, st->copy));
             LUMEN_CUDA(cudaEventRecord(st->free_[slot], st->copy));
-            if (flags && g_write64(st->copy, flags_dev + 8ull * ci, epoch, 0) != 0)
+            if (j.flags_dev && g_write64(st->copy, j.flags_dev + 8ull * ci, j.epoch, 0) != 0)
                 return cuda_fail(cudaErrorUnknown);
         } else {
             LUMEN_CUDA(cudaStreamWaitEvent(st->copy, st->free_[slot], 0));
-            if (flags && g_wait64(st->copy, flags_dev + 8ull * ci, epoch, 0 /* >= */) != 0)
+            if (j.flags_dev && g_wait64(st->copy, j.flags_dev + 8ull * ci, j.epoch, 0 /* >= */) != 0)
                 return cuda_fail(cudaErrorUnknown);
             LUMEN_CUDA(cudaMemcpyAsync(sbase, h + c.b0, bytes, cudaMemcpyHostToDevice, st->copy));
             LUMEN_CUDA(cudaEventRecord(st->full[slot], st->copy));
             LUMEN_CUDA(cudaStreamWaitEvent(stream, st->full[slot], 0));
-            rc = launch_part(plan, planes, shifted, false, stream, false, c.ra, c.rb, c.p0, c.p1);
+            rc = launch_part(plan, j.planes, shifted, false, stream, false, c.ra, c.rb, c.p0, c.p1);
             if (rc != LUMEN_KV_OK) return rc;
             LUMEN_CUDA(cudaEventRecord(st->free_[slot], stream));
         }
@@ -129,6 +183,125 @@ int run_staged(const lumen_kv_plan* plan, const void* const* k_planes, const voi
         LUMEN_CUDA(cudaStreamWaitEvent(stream, st->join, 0));
     }
     return LUMEN_KV_OK;
+}
+
+int run_staged(const lumen_kv_plan* plan, const void* const* k_planes, const void* const* v_planes,
+               void* host, int64_t host_bytes, lumen_kv_stager* st, void* stream_, bool pack,
+               const uint64_t* flags = nullptr, uint64_t epoch = 0) {
+    static thread_local Job job;   // its vectors are reused: no allocation in steady state
+    bool empty = false;
+    const int rc = prepare(plan, k_planes, v_planes, host, host_bytes, st, pack, flags, epoch, &job,
+                           &empty);
+    if (rc != LUMEN_KV_OK || empty) return rc;
+    std::lock_guard<std::mutex> g(st->issue_mu);
+    const int out = issue(st, job, static_cast<cudaStream_t>(stream_));
+    job.chunks.reset();
+    return out;
+}
+
+// The stager's thread: issues queued asynchronous calls in order.
+void worker_main(lumen_kv_stager* st) {
+    cudaSetDevice(st->device);
+    for (;;) {
+        Job job;
+        {
+            std::unique_lock<std::mutex> lk(st->mu);
+            st->cv.wait(lk, [&] { return st->stop || !st->queue.empty(); });
+            if (st->queue.empty()) return;          // stop requested and nothing left
+            job = std::move(st->queue.front());
+            st->queue.pop_front();
+        }
+        int rc = LUMEN_KV_OK;
+        cudaEvent_t done = nullptr;
+        {
+            std::lock_guard<std::mutex> g(st->issue_mu);
+            cudaError_t e = cudaStreamWaitEvent(st->work, job.begin, 0);
+            if (e != cudaSuccess) rc = cuda_fail(e);
+            if (rc == LUMEN_KV_OK) rc = issue(st, job, st->work);
+            if (rc == LUMEN_KV_OK) {
+                e = cudaEventCreateWithFlags(&done, cudaEventDisableTiming);
+                if (e == cudaSuccess) e = cudaEventRecord(done, st->work);
+                if (e != cudaSuccess) rc = cuda_fail(e);
+            }
+        }
+        cudaEventDestroy(job.begin);
+        plan_release(job.plan);
+        {
+            std::lock_guard<std::mutex> g(st->mu);
+            for (TicketRec& t : st->tickets)
+                if (t.id == job.ticket) {
+                    t.done = done;
+                    t.status = rc;
+                    t.issued = true;
+                }
+        }
+        st->cv.notify_all();
+    }
+}
+
+int run_staged_async(const lumen_kv_plan* plan, const void* const* k_planes,
+                     const void* const* v_planes, void* host, int64_t host_bytes,
+                     lumen_kv_stager* st, void* stream_, bool pack, const uint64_t* flags,
+                     uint64_t epoch, uint64_t* ticket) {
+    if (!ticket) return LUMEN_KV_EINVAL;
+    *ticket = 0;
+    Job job;
+    bool empty = false;
+    int rc = prepare(plan, k_planes, v_planes, host, host_bytes, st, pack, flags, epoch, &job, &empty);
+    if (rc != LUMEN_KV_OK) return rc;
+    if (!empty) {
+        LUMEN_CUDA(cudaEventCreateWithFlags(&job.begin, cudaEventDisableTiming));
+        const cudaError_t e = cudaEventRecord(job.begin, static_cast<cudaStream_t>(stream_));
+        if (e != cudaSuccess) {
+            cudaEventDestroy(job.begin);
+            return cuda_fail(e);
+        }
+        plan_retain(plan);
+    }
+    {
+        std::lock_guard<std::mutex> g(st->mu);
+        // completed tickets leave at the front (calls complete in submission order)
+        while (st->tickets.size() > 64 && st->tickets.front().issued &&
+               (!st->tickets.front().done ||
+                cudaEventQuery(st->tickets.front().done) == cudaSuccess)) {
+            if (st->tickets.front().done) cudaEventDestroy(st->tickets.front().done);
+            st->tickets.pop_front();
+        }
+        (void)cudaGetLastError();
+        TicketRec t;
+        t.id = job.ticket = st->next_ticket++;
+        t.issued = empty;          // an empty plan has nothing to issue: complete at once
+        st->tickets.push_back(t);
+        *ticket = t.id;
+        if (!empty) {
+            st->queue.push_back(std::move(job));
+            if (!st->worker_started) {
+                st->worker_started = true;
+                st->worker = std::thread(worker_main, st);
+            }
+        }
+    }
+    if (!empty) st->cv.notify_all();
+    return LUMEN_KV_OK;
+}
+
+// Blocks until the ticket has been issued; *done receives its completion event (nullptr: nothing
+// to wait for).  Returns the call's status.
+int wait_issued(lumen_kv_stager* st, uint64_t ticket, cudaEvent_t* done) {
+    *done = nullptr;
+    std::unique_lock<std::mutex> lk(st->mu);
+    if (ticket == 0 || ticket >= st->next_ticket) return LUMEN_KV_EINVAL;
+    for (;;) {
+        TicketRec* rec = nullptr;
+        for (TicketRec& t : st->tickets)
+            if (t.id == ticket) rec = &t;
+        if (!rec) return LUMEN_KV_OK;              // pruned: complete long ago
+        if (rec->issued) {
+            *done = rec->done;
+            return rec->status;
+        }
+        st->cv.wait(lk);
+    }
 }
 
 }  // namespace
@@ -150,7 +323,9 @@ int lumen_kv_stager_create(void* staging, int64_t slot_bytes, int32_t n_slots,
     st->slot_bytes = slot_bytes;
     st->n_slots = n_slots;
     for (int i = 0; i < 16; ++i) st->full[i] = st->free_[i] = nullptr;
-    cudaError_t e = cudaStreamCreateWithFlags(&st->copy, cudaStreamNonBlocking);
+    cudaError_t e = cudaGetDevice(&st->device);
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&st->copy, cudaStreamNonBlocking);
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&st->work, cudaStreamNonBlocking);
     for (int i = 0; i < n_slots && e == cudaSuccess; ++i) {
         e = cudaEventCreateWithFlags(&st->full[i], cudaEventDisableTiming);
         if (e == cudaSuccess) e = cudaEventCreateWithFlags(&st->free_[i], cudaEventDisableTiming);
@@ -166,6 +341,18 @@ int lumen_kv_stager_create(void* staging, int64_t slot_bytes, int32_t n_slots,
 
 void lumen_kv_stager_destroy(lumen_kv_stager* st) {
     if (!st) return;
+    if (st->worker_started) {          // queued calls are issued before the thread leaves
+        {
+            std::lock_guard<std::mutex> g(st->mu);
+            st->stop = true;
+        }
+        st->cv.notify_all();
+        st->worker.join();
+    }
+    if (st->work) {
+        cudaStreamSynchronize(st->work);
+        cudaStreamDestroy(st->work);
+    }
     if (st->copy) {
         cudaStreamSynchronize(st->copy);
         cudaStreamDestroy(st->copy);
@@ -174,6 +361,8 @@ void lumen_kv_stager_destroy(lumen_kv_stager* st) {
         if (st->full[i]) cudaEventDestroy(st->full[i]);
         if (st->free_[i]) cudaEventDestroy(st->free_[i]);
     }
+    for (auto& t : st->tickets)
+        if (t.done) cudaEventDestroy(t.done);
     if (st->join) cudaEventDestroy(st->join);
     (void)cudaGetLastError();
     delete st;
@@ -211,15 +400,68 @@ int lumen_kv_restore_unpack_staged_ready(const lumen_kv_plan* plan, void* const*
                              epoch);
 }
 
+int lumen_kv_checkpoint_pack_staged_async(const lumen_kv_plan* plan, const void* const* k_planes,
+                                          const void* const* v_planes, void* dst_host,
+                                          int64_t dst_bytes, lumen_kv_stager* stager, void* stream,
+                                          uint64_t* flags, uint64_t epoch, uint64_t* ticket) {
+    return lumen::run_staged_async(plan, k_planes, v_planes, dst_host, dst_bytes, stager, stream,
+                                   true, flags, epoch, ticket);
+}
+
+int lumen_kv_restore_unpack_staged_async(const lumen_kv_plan* plan, void* const* k_planes,
+                                         void* const* v_planes, const void* src_host,
+                                         int64_t src_bytes, lumen_kv_stager* stager, void* stream,
+                                         const uint64_t* flags, uint64_t epoch, uint64_t* ticket) {
+    return lumen::run_staged_async(plan, const_cast<const void* const*>(k_planes),
+                                   const_cast<const void* const*>(v_planes),
+                                   const_cast<void*>(src_host), src_bytes, stager, stream, false,
+                                   flags, epoch, ticket);
+}
+
+int lumen_kv_stager_query(lumen_kv_stager* st, uint64_t ticket) {
+    if (!st) return LUMEN_KV_EINVAL;
+    std::lock_guard<std::mutex> g(st->mu);
+    if (ticket == 0 || ticket >= st->next_ticket) return LUMEN_KV_EINVAL;
+    for (const TicketRec& t : st->tickets)
+        if (t.id == ticket) {
+            if (!t.issued) return 0;
+            if (t.status != LUMEN_KV_OK) return t.status;
+            if (!t.done) return 1;
+            const cudaError_t e = cudaEventQuery(t.done);
+            if (e == cudaSuccess) return 1;
+            (void)cudaGetLastError();
+            return e == cudaErrorNotReady ? 0 : lumen::cuda_fail(e);
+        }
+    return 1;                                       // pruned: complete long ago
+}
+
+int lumen_kv_stager_wait(lumen_kv_stager* st, uint64_t ticket, void* stream) {
+    if (!st) return LUMEN_KV_EINVAL;
+    cudaEvent_t done = nullptr;
+    const int rc = lumen::wait_issued(st, ticket, &done);
+    if (rc != LUMEN_KV_OK || !done) return rc;
+    const cudaError_t e = cudaStreamWaitEvent(static_cast<cudaStream_t>(stream), done, 0);
+    return e == cudaSuccess ? LUMEN_KV_OK : lumen::cuda_fail(e);
+}
+
+int lumen_kv_stager_sync(lumen_kv_stager* st, uint64_t ticket) {
+    if (!st) return LUMEN_KV_EINVAL;
+    cudaEvent_t done = nullptr;
+    const int rc = lumen::wait_issued(st, ticket, &done);
+    if (rc != LUMEN_KV_OK || !done) return rc;
+    const cudaError_t e = cudaEventSynchronize(done);
+    return e == cudaSuccess ? LUMEN_KV_OK : lumen::cuda_fail(e);
+}
+
 int64_t lumen_kv_plan_get_chunks(const lumen_kv_plan* plan, int64_t slot_bytes,
                                  lumen_kv_chunk_info* out, int64_t cap) {
     if (!plan || cap < 0 || (cap > 0 && !out)) return LUMEN_KV_EINVAL;
-    std::vector<lumen::Chunk> chunks;
-    const int rc = lumen::build_chunks(plan->hp, plan->h_runs, slot_bytes, &chunks);
+    std::shared_ptr<const std::vector<lumen::Chunk>> chunks;
+    const int rc = lumen::plan_chunks(plan, slot_bytes, &chunks);
     if (rc != LUMEN_KV_OK) return rc;
-    const int64_t n = static_cast<int64_t>(chunks.size());
+    const int64_t n = static_cast<int64_t>(chunks->size());
     for (int64_t i = 0; i < n && i < cap; ++i) {
-        const lumen::Chunk& c = chunks[static_cast<size_t>(i)];
+        const lumen::Chunk& c = (*chunks)[static_cast<size_t>(i)];
         out[i] = lumen_kv_chunk_info{c.ra, c.rb, c.p0, c.p1, c.b0, c.b1};
     }
     return n;

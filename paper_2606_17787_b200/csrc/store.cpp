@@ -264,15 +264,17 @@ int64_t lumen_kv_store_lookup(const lumen_kv_store* s, uint64_t id, const lumen_
                                    static_cast<int64_t>(stored.size()));
 }
 
-void lumen_kv_store_sink(void* store, uint64_t id, int64_t t_begin, int64_t t_end,
-                         const void* delta, int64_t delta_bytes, const lumen_kv_tag* tags,
-                         int32_t n_tags) {
+int lumen_kv_store_sink(void* store, uint64_t id, int64_t t_begin, int64_t t_end,
+                        const void* delta, int64_t delta_bytes, const lumen_kv_tag* tags,
+                        int32_t n_tags) {
     lumen_kv_store* s = static_cast<lumen_kv_store*>(store);
-    if (!s) return;
-    if (lumen_kv_store_append(s, id, t_begin, t_end, delta, delta_bytes, tags, n_tags) != LUMEN_KV_OK) {
+    if (!s) return LUMEN_KV_EINVAL;
+    const int rc = lumen_kv_store_append(s, id, t_begin, t_end, delta, delta_bytes, tags, n_tags);
+    if (rc != LUMEN_KV_OK) {
         std::lock_guard<std::mutex> g(s->mu);
         ++s->sink_errors;
     }
+    return rc;
 }
 
 // internal (recover.cu): the arena the segments' offsets refer to; not exported

@@ -207,3 +207,60 @@ def test_background_checkpointer_stress(lk):
         else:
             assert end == final[rid] and bg.progress(rid) == final[rid]
     bg.close()
+
+
+@pytest.mark.gpu
+def test_sink_rejection_keeps_progress_and_surfaces(lk):
+    """a sink that rejects a delta must not advance the request's progress; the
+    rest of that request (pending, and already in the next batch) is dropped, flush() reports
+    LUMEN_KV_ESINK, other requests are unaffected, and the next notification packs again from
+    the last delivered token so that the sink never sees a gap."""
+    import ctypes
+    import torch
+    from tests import gpu_util as G
+    G.build_all()
+    w = cfg1_qwen14b(L=2, N=512, n_reqs=3, grow_iters=6, median=100, hi=120, lo=90)
+    L, H, D, S, N = w.geom
+    tokb = 2 * L * H * D * 2
+    pool = G.make_pool(w.geom, 77)
+    K, V = G.host_planes(w.geom, 77)
+    lens = [te for _, _, te in w.reqs]
+    ring_mem = torch.empty(3 << 20, dtype=torch.uint8, device="cuda")
+    pinned = G.pinned_buffer(64 * tokb)                      # halves of 32 tokens: prefill deltas come in pieces
+    got = {r: [] for r in range(3)}
+    reject = {"on": True}
+
+    def sink(rid, tb, te, ptr, nb, tags):
+        if rid == 1 and reject["on"] and tb >= 32:           # request 1: second piece onwards
+            return -1
+        data = np.ctypeslib.as_array((ctypes.c_uint16 * (nb // 2)).from_address(ptr)).copy()
+        got[rid].append((tb, te, data))
+        return 0
+
+    bg = lk.BackgroundCheckpointer(pool.geom, pool.k_ptrs, pool.v_ptrs, ring_mem.data_ptr(), 1 << 20, 3,
+                                   pinned.data_ptr(), pinned.numel(), sink)
+    for rid in range(3):
+        bg.track(rid, 0)
+    bg.notify([0, 1, 2], [(pt, 0, n) for (pt, _, n) in w.reqs])
+    with pytest.raises(lk.LumenKVError) as e:
+        bg.flush()
+    assert e.value.status == lk.LUMEN_KV_ESINK
+    assert bg.progress(0) == lens[0] and bg.progress(2) == lens[2]
+    assert bg.progress(1) == 32                               # only the first piece was taken
+    assert [(tb, te) for tb, te, _ in got[1]] == [(0, 32)]
+    reject["on"] = False
+    bg.notify([1], [(w.reqs[1][0], 0, lens[1] + 5)])          # the retry starts at token 32
+    try:
+        bg.flush()
+    except lk.LumenKVError as e2:                             # first_error is sticky by design
+        assert e2.status == lk.LUMEN_KV_ESINK
+    assert bg.progress(1) == lens[1] + 5
+    for rid in range(3):
+        at = 0
+        for tb, te, data in got[rid]:
+            assert tb == at                                   # deltas tile [0, t) in order: no gap, no repeat
+            at = te
+            ref = oracle.pack(w.geom, K, V, [(w.reqs[rid][0], tb, te)])
+            assert np.array_equal(data, ref)
+        assert at == bg.progress(rid)
+    bg.close()

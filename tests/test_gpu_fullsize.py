@@ -186,7 +186,26 @@ def test_cfg2_full_size(G, where):
         pytest.skip(f"cannot allocate the 32 GiB {where} buffer: {e}")
     if ring:
         assert len(plan.chunks(32 << 20)) == 1024               # 2 planes of 16 MiB per chunk
-        ck.pack_staged(plan, buf, ring)
+        # asynchronous submission: 1,024 chunks x 6 stream operations are issued by the stager's
+        # thread; the call itself must come back in well under a millisecond, long before the
+        # 0.6 s transfer is over
+        import time
+        G.lk.lumen_kv_init()
+        st = torch.cuda.current_stream().cuda_stream
+        warm = ck.plan(w.reqs[:1])                              # starts the stager's thread
+        ring.stager.sync(G.lk.lumen_kv_checkpoint_pack_staged_async(
+            warm, pool.k_ptrs, pool.v_ptrs, buf.data_ptr(), warm.nbytes, ring.stager, st))
+        warm.close()
+        t0 = time.perf_counter()
+        ticket = G.lk.lumen_kv_checkpoint_pack_staged_async(plan, pool.k_ptrs, pool.v_ptrs, buf.data_ptr(),
+                                                           plan.nbytes, ring.stager, st)
+        call_ms = (time.perf_counter() - t0) * 1e3
+        in_flight = not ring.stager.query(ticket)
+        ring.stager.sync(ticket)
+        total_ms = (time.perf_counter() - t0) * 1e3
+        assert call_ms < 1.0, f"async staged call took {call_ms:.3f} ms on the calling thread"
+        assert in_flight and total_ms > 300, (in_flight, total_ms)
+        assert ring.stager.query(ticket)
     else:
         ck.pack(plan, buf)
     torch.cuda.synchronize()

@@ -408,6 +408,132 @@ def test_staged_commit_and_ready_flags(G):
     plan.close(); rplan.close(); ring.close()
 
 
+# ---- asynchronous staged calls (a stager-owned thread issues the chunk pipeline) -------------
+def test_staged_async_parity_and_ordering(G):
+    """_async returns a ticket at once; the plan is freed immediately, the pool of the producing
+    stream is filled by work enqueued BEFORE the call (begin ordering), stager_wait makes a
+    consumer stream see the result, query flips to True, sync blocks; bytes equal the oracle's.
+    All three chunk kinds, with slots reused many times per call."""
+    import torch
+    lk = G.lk
+    cases = [(cfg1_qwen14b(L=3, N=2048, n_reqs=24, grow_iters=2, median=200, hi=512, lo=20), 1 << 20, 3),
+             (cfg2_qwen32b(L=2, N=1200, n_reqs=3, prompt=1000), 5 << 20, 2),
+             (cfg4_longctx(L=2, tokens=3001, wave_reqs=2), 1 << 20, 4),
+             (cfg0_tiny(), 4096, 2)]
+    for n, (w, slot, nslots) in enumerate(cases):
+        seed = 300 + 2 * n
+        K, V = G.host_planes(w.geom, seed)
+        B_ref = oracle.pack(w.geom, K, V, w.reqs)
+        K2, V2 = G.host_planes(w.geom, seed + 1)
+        oracle.unpack(w.geom, K2, V2, w.restore_reqs, B_ref)
+        L, H, D, S, N = w.geom
+        pool_a = G.KVPool(L, H, D, S, N)
+        pool_b = G.make_pool(w.geom, seed + 1)
+        ring = G.StagingRing(slot, nslots)
+        whole, buf = G.alloc_buffer(w.payload_bytes, "host")
+        prod, cons = torch.cuda.Stream(), torch.cuda.Stream()
+        with torch.cuda.stream(prod):                       # the pool is produced on `prod` ...
+            for i, t in enumerate(pool_a.planes()):
+                G.wdev.fill_plane(t, seed, i, prod.cuda_stream)
+        plan = lk.lumen_kv_plan_build(pool_a.geom, w.reqs, 0, prod.cuda_stream)
+        n_chunks = len(plan.chunks(slot))
+        t1 = lk.lumen_kv_checkpoint_pack_staged_async(plan, pool_a.k_ptrs, pool_a.v_ptrs, buf.data_ptr(),
+                                                      plan.nbytes, ring.stager, prod.cuda_stream)
+        plan.close()                                        # ... and the plan is gone before it is issued
+        rplan = lk.lumen_kv_plan_build(pool_b.geom, w.restore_reqs, lk.LUMEN_KV_VALIDATE_UNIQUE_DST,
+                                       cons.cuda_stream)
+        # the restore reads what ticket t1 writes: same stager, so it is ordered behind it
+        t2 = lk.lumen_kv_restore_unpack_staged_async(rplan, pool_b.k_ptrs, pool_b.v_ptrs, buf.data_ptr(),
+                                                     rplan.nbytes, ring.stager, cons.cuda_stream)
+        rplan.close()
+        assert t2 == t1 + 1
+        ring.stager.wait(t2, cons.cuda_stream)              # consumer stream sees the restored pool
+        with torch.cuda.stream(cons):
+            snap = [t.clone() for t in pool_b.planes()]
+        cons.synchronize()
+        assert ring.stager.query(t1) and ring.stager.query(t2)
+        ring.stager.sync(t2)
+        assert np.array_equal(G.buf_to_np(buf, w.payload_bytes), B_ref), f"async pack mismatch, case {n}"
+        assert G.guards_intact(whole, w.payload_bytes)
+        for t, ref in zip(snap, [x for kv in zip(K2, V2) for x in kv]):
+            assert np.array_equal(G.plane_to_np(t), ref), f"async unpack mismatch, case {n}"
+        assert n_chunks >= 1
+        ring.close()
+        G.release(whole)
+
+
+def test_staged_async_mixed_with_sync_errors_and_flags(G):
+    import threading
+    import torch
+    lk = G.lk
+    w = cfg2_qwen32b(L=3, N=1500, n_reqs=4, prompt=1200)               # 4 x 14 MiB
+    slot = 1 << 20
+    K, V = G.host_planes(w.geom, 21)
+    B_ref = oracle.pack(w.geom, K, V, w.reqs)
+    ref_bytes = B_ref.view(np.uint8)
+    pool = G.make_pool(w.geom, 21)
+    ring = G.StagingRing(slot, 3)
+    plan = lk.lumen_kv_plan_build(pool.geom, w.reqs, 0, 0)
+    chunks = plan.chunks(slot)
+    whole, buf = G.alloc_buffer(plan.nbytes, "host")
+    whole2, buf2 = G.alloc_buffer(plan.nbytes, "host")
+    s = torch.cuda.Stream()
+    # validation errors come back from the call itself, and hand out no ticket
+    with pytest.raises(lk.LumenKVError) as e:
+        lk.lumen_kv_checkpoint_pack_staged_async(plan, pool.k_ptrs, pool.v_ptrs, buf.data_ptr(),
+                                                 plan.nbytes - 16, ring.stager, s.cuda_stream)
+    assert e.value.status == lk.LUMEN_KV_ESIZE
+    small = G.StagingRing(1024, 2)
+    with pytest.raises(lk.LumenKVError) as e:
+        lk.lumen_kv_checkpoint_pack_staged_async(plan, pool.k_ptrs, pool.v_ptrs, buf.data_ptr(),
+                                                 plan.nbytes, small.stager, s.cuda_stream)
+    assert e.value.status == lk.LUMEN_KV_ESIZE
+    with pytest.raises(lk.LumenKVError):
+        ring.stager.query(1)                               # no such ticket yet
+    empty = lk.lumen_kv_plan_build(pool.geom, [], 0, 0)
+    t0 = lk.lumen_kv_checkpoint_pack_staged_async(empty, pool.k_ptrs, pool.v_ptrs, buf.data_ptr(),
+                                                  plan.nbytes, ring.stager, s.cuda_stream)
+    assert ring.stager.query(t0)                           # A4: nothing to do, complete at once
+    ring.stager.wait(t0, s.cuda_stream); ring.stager.sync(t0)
+    # async with commit flags + a host consumer, then a synchronous call on the same stager
+    flags_t = torch.zeros(len(chunks), dtype=torch.int64, pin_memory=True)
+    flags, host = flags_t.numpy(), buf.numpy()
+    bad, seen = [], []
+
+    def consumer():
+        for i, c in enumerate(chunks):
+            while flags[i] != 5:
+                pass
+            if not np.array_equal(host[c.byte_begin:c.byte_end], ref_bytes[c.byte_begin:c.byte_end]):
+                bad.append(i)
+            seen.append(i)
+
+    th = threading.Thread(target=consumer)
+    th.start()
+    t1 = lk.lumen_kv_checkpoint_pack_staged_async(plan, pool.k_ptrs, pool.v_ptrs, buf.data_ptr(),
+                                                  plan.nbytes, ring.stager, s.cuda_stream,
+                                                  flags_t.data_ptr(), 5)
+    lk.lumen_kv_checkpoint_pack_staged(plan, pool.k_ptrs, pool.v_ptrs, buf2.data_ptr(), plan.nbytes,
+                                       ring.stager, s.cuda_stream)        # issued after t1, same slots
+    s.synchronize()
+    ring.stager.sync(t1)
+    th.join(timeout=60)
+    assert not th.is_alive() and len(seen) == len(chunks) and not bad
+    assert np.array_equal(G.buf_to_np(buf, plan.nbytes), B_ref)
+    assert np.array_equal(G.buf_to_np(buf2, plan.nbytes), B_ref)
+    assert G.guards_intact(whole, plan.nbytes) and G.guards_intact(whole2, plan.nbytes)
+    # a stager destroyed with calls still queued issues them first
+    ring3 = G.StagingRing(slot, 2)
+    buf.fill_(0)
+    for _ in range(3):
+        lk.lumen_kv_checkpoint_pack_staged_async(plan, pool.k_ptrs, pool.v_ptrs, buf.data_ptr(),
+                                                 plan.nbytes, ring3.stager, s.cuda_stream)
+    ring3.close()
+    torch.cuda.synchronize()
+    assert np.array_equal(G.buf_to_np(buf, plan.nbytes), B_ref)
+    plan.close(); empty.close(); ring.close(); small.close()
+
+
 # ---- explicit buffer layout (checkpoint store, f3) ------------------------------------------
 @pytest.mark.parametrize("kernel", ["warp", "warp_upload", "bulk"])
 def test_layout_parity(G, kernel):

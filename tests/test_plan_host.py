@@ -439,3 +439,57 @@ def test_maximum_sizes_are_64_bit_clean(lk):
     assert r.src_slot == int(pt[99999]) and r.dst_token == 99999 and r.count == 1
     with pytest.raises(lk.LumenKVError):                     # N = 2^31 is one too many
         lk.lumen_kv_plan_build(lk.make_geom(1, 1, 8, 1, 1 << 31), [], lk.LUMEN_KV_HOST_ONLY)
+
+
+def test_layout_extent_overflow_is_rejected(lk):
+    """buf_offset + ((planes-1)*stride + n)*row was evaluated without overflow
+    checks, so a layout whose true extent is about 2^70 built and reported 1 GiB.  Every step is
+    checked now and such a layout is EINVAL (it can never fit a real buffer)."""
+    H = lk.LUMEN_KV_HOST_ONLY
+    pt = np.zeros(1, dtype=np.int32)
+    # probe 1: L = 1, row = 2^30, stride = 2^40 - 1, n = 2
+    g = lk.make_geom(1, 1 << 15, 1 << 14, 2, 4)                 # row = 2^15 * 2^14 * 2 = 2^30
+    with pytest.raises(lk.LumenKVError) as e:
+        lk.lumen_kv_plan_build(g, [(pt, 0, 2)], H, layouts=[(0, (1 << 40) - 1)])
+    assert e.value.status == lk.LUMEN_KV_EINVAL
+    # probe 2: row = 16, L = 32767 (65,534 planes), stride = 2^40 - 1: about 2^60 bytes, which
+    # 64 bits hold -- it builds, and the extent it reports is the true one (so a real buffer is ESIZE)
+    g2 = lk.make_geom(32767, 1, 8, 4, 4)                        # row = 16
+    big = lk.lumen_kv_plan_build(g2, [(pt, 0, 2)], H, layouts=[(16, (1 << 40) - 1)])
+    assert big.nbytes == 16 + ((2 * 32767 - 1) * ((1 << 40) - 1) + 2) * 16
+    # row = 2^20 with the same stride and planes does wrap 63 bits: EINVAL
+    g3 = lk.make_geom(32767, 1 << 10, 1 << 9, 2, 4)             # row = 2^20
+    with pytest.raises(lk.LumenKVError) as e:
+        lk.lumen_kv_plan_build(g3, [(pt, 0, 2)], H, layouts=[(0, (1 << 40) - 1)])
+    assert e.value.status == lk.LUMEN_KV_EINVAL
+
+
+def test_run_reserve_is_exact_for_large_pages(lk):
+    """the run list was reserved as if every touched page were used in full:
+    S = 2^20, row = 16 KiB, 1-token deltas asked for 8 MiB of descriptors per page (false ENOMEM
+    for many requests, std::length_error across the C boundary for extreme ones)."""
+    g = lk.make_geom(1, 64, 128, 1 << 20, 4096)                 # row = 16 KiB, page = 16 GiB
+    reqs = [(np.array([i], dtype=np.int32), 5, 6) for i in range(4096)]
+    p = lk.lumen_kv_plan_build(g, reqs, lk.LUMEN_KV_HOST_ONLY)
+    assert p.num_runs == 4096 and p.nbytes == 4096 * 2 * 16384
+
+
+def test_async_staged_calls_validate_before_queueing(lk):
+    """The asynchronous staged entry points reject what can be checked on the host without ever
+    touching a device or starting the stager's thread (no GPU here: no stager can exist, so the
+    NULL-stager / NULL-ticket paths are what is reachable)."""
+    import ctypes
+    L = lk.binding._lib()
+    g = lk.make_geom(2, 2, 64, 16, 64)
+    p = lk.lumen_kv_plan_build(g, [(np.arange(4, dtype=np.int32), 0, 40)], lk.LUMEN_KV_HOST_ONLY)
+    t = ctypes.c_uint64(7)
+    kv = (ctypes.c_void_p * 2)(16, 16)
+    buf = np.zeros(1 << 16, dtype=np.uint8)
+    for fn in (L.lumen_kv_checkpoint_pack_staged_async, L.lumen_kv_restore_unpack_staged_async):
+        assert fn(p.handle, kv, kv, buf.ctypes.data, buf.size, None, None, None, 0, ctypes.byref(t)) == lk.LUMEN_KV_EINVAL
+        assert t.value == 0                                     # no ticket was handed out
+        assert fn(p.handle, kv, kv, buf.ctypes.data, buf.size, None, None, None, 0, None) == lk.LUMEN_KV_EINVAL
+    assert L.lumen_kv_stager_query(None, 1) == lk.LUMEN_KV_EINVAL
+    assert L.lumen_kv_stager_wait(None, 1, None) == lk.LUMEN_KV_EINVAL
+    assert L.lumen_kv_stager_sync(None, 1) == lk.LUMEN_KV_EINVAL
+    assert lk.lumen_kv_strerror(lk.LUMEN_KV_ESINK).startswith("the checkpointer's sink")
