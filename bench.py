@@ -582,13 +582,16 @@ def staged_host_once(torch, lk, path, hb, ring, direction, async_call=False):
     tb, te = path.ranges[0]
     reqs.set_ranges(tb, te)
     plan = lk.lumen_kv_plan_build(pool.geom, reqs, path.kflag | flag, s.cuda_stream)
-    fn = lk.lumen_kv_checkpoint_pack_staged if direction == "pack" else lk.lumen_kv_restore_unpack_staged
+    name = "lumen_kv_checkpoint_pack_staged" if direction == "pack" else "lumen_kv_restore_unpack_staged"
+    fn = getattr(lk, name + ("_async" if async_call else ""))
     a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     torch.cuda.synchronize()
     a.record(s)
     t0 = time.perf_counter()
-    fn(plan, pool.k_ptrs, pool.v_ptrs, hb.data_ptr(), P, ring.stager, s.cuda_stream)
+    ticket = fn(plan, pool.k_ptrs, pool.v_ptrs, hb.data_ptr(), P, ring.stager, s.cuda_stream)
     call_ms = (time.perf_counter() - t0) * 1e3
+    if async_call:                                  # the calling thread is free from here on
+        ring.stager.wait(ticket, s.cuda_stream)
     b.record(s)
     s.synchronize()
     n_chunks = len(plan.chunks(ring.stager.slot_bytes))
@@ -655,13 +658,19 @@ def large_config(torch, lk, name, seed, kflag, stream, sampler, peak, link, with
         sampler.start(slow=True)
         p_ms, p_call, n_chunks = staged_host_once(torch, lk, path, hb, ring, "pack")
         r_ms, r_call, _ = staged_host_once(torch, lk, path, hb, ring, "restore")
+        pa_ms, pa_call, _ = staged_host_once(torch, lk, path, hb, ring, "pack", async_call=True)
+        ra_ms, ra_call, _ = staged_host_once(torch, lk, path, hb, ring, "restore", async_call=True)
         sampler.stop()
         out["host_staged"] = {"pack_GBps": P / p_ms / 1e6, "restore_GBps": P / r_ms / 1e6,
                               "pack_ms": p_ms, "restore_ms": r_ms, "chunks_per_call": n_chunks,
                               "pack_frac_of_d2h_memcpy": P / p_ms / 1e6 / link["d2h"],
                               "restore_frac_of_h2d_memcpy": P / r_ms / 1e6 / link["h2d"],
                               "memcpy_peak_d2h_GBps": link["d2h"], "memcpy_peak_h2d_GBps": link["h2d"],
-                              "staged_call_host_ms": {"pack": p_call, "restore": r_call}}
+                              "staged_call_host_ms": {"pack": p_call, "restore": r_call},
+                              "async": {"pack_GBps": P / pa_ms / 1e6, "restore_GBps": P / ra_ms / 1e6,
+                                        "call_host_ms": {"pack": pa_call, "restore": ra_call},
+                                        "note": "lumen_kv_*_staged_async: the stager's thread issues the chunks; "
+                                                "call_host_ms is what the calling thread spends in the call"}}
         ring.close()
         wdev.unpin(hb)
         del hb
@@ -1003,39 +1012,59 @@ def run_cfg3(args):
     ringR, ringP = StagingRing(32 << 20, 3), StagingRing(32 << 20, 3)
     PACE = 0.025   # s between delta packs: one decode iteration (the paper's mean TPOT is 58 ms)
 
+    call_ms = {"staged_async": [], "mapped": []}
+
+    def delta_pack(it, staged, stream):
+        """a1-a4 for one decode step: 1 new token of each of the 64 running requests -> pinned host."""
+        ra.set_ranges(te0 + (it % 48), te0 + (it % 48) + 1)
+        p = lk.lumen_kv_plan_build(geom, ra, 0, stream.cuda_stream)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        if staged:
+            lk.lumen_kv_checkpoint_pack_staged(p, kp, vp, pbufs[it % n_pb].data_ptr(), pbytes,
+                                               ringP.stager, stream.cuda_stream)
+        else:
+            lk.lumen_kv_checkpoint_pack(p, kp, vp, pbufs[it % n_pb].data_ptr(), pbytes, HOST,
+                                        stream.cuda_stream)
+        e1.record(stream)
+        p.close()
+        return e0, e1
+
     def restore(wave, nbytes, staged, pace):
         """One wave on s1.  pace None: alone; pace > 0: one 1-token delta pack of the running
-        requests every `pace` s on s2 meanwhile; pace 0: packs back to back (worst case)."""
+        requests every `pace` s on s2 meanwhile; pace 0: packs back to back (worst case).
+        The staged restore is submitted asynchronously (2,300 chunks: the synchronous call would
+        hold this thread for most of the transfer and the packs would only meet its tail)."""
         plan = lk.lumen_kv_plan_build(geom, wave, lk.LUMEN_KV_VALIDATE_UNIQUE_DST, s1.cuda_stream)
         a, z = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         torch.cuda.synchronize()
         a.record(s1)
+        t0 = time.perf_counter()
         if staged:
-            lk.lumen_kv_restore_unpack_staged(plan, kp, vp, hbuf.data_ptr(), nbytes, ringR.stager,
-                                              s1.cuda_stream)
+            ticket = lk.lumen_kv_restore_unpack_staged_async(plan, kp, vp, hbuf.data_ptr(), nbytes,
+                                                             ringR.stager, s1.cuda_stream)
+            call_ms["staged_async"].append((time.perf_counter() - t0) * 1e3)
+            done = lambda: ringR.stager.query(ticket)
         else:
             lk.lumen_kv_restore_unpack(plan, kp, vp, hbuf.data_ptr(), nbytes, HOST, s1.cuda_stream)
-        z.record(s1)
+            call_ms["mapped"].append((time.perf_counter() - t0) * 1e3)
+            z.record(s1)
+            done = z.query
         it, pev = 0, []
-        while pace is not None and not z.query():       # a2-a4 on stream 2 until the restore ends
-            ra.set_ranges(te0 + (it % 48), te0 + (it % 48) + 1)
-            p = lk.lumen_kv_plan_build(geom, ra, 0, s2.cuda_stream)
-            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            e0.record(s2)
-            if staged:
-                lk.lumen_kv_checkpoint_pack_staged(p, kp, vp, pbufs[it % n_pb].data_ptr(), pbytes,
-                                                   ringP.stager, s2.cuda_stream)
-            else:
-                lk.lumen_kv_checkpoint_pack(p, kp, vp, pbufs[it % n_pb].data_ptr(), pbytes, HOST,
-                                            s2.cuda_stream)
-            e1.record(s2)
-            p.close()
-            pev.append((e0, e1))
+        next_pack = time.perf_counter()
+        while not done():                               # a2-a4 on stream 2 until the restore ends
+            now = time.perf_counter()
+            if pace is None or now < next_pack:
+                time.sleep(0.0005)
+                continue
+            pev.append(delta_pack(it, staged, s2))
             it += 1
-            if pace > 0:
-                time.sleep(pace)
-            elif it % n_pb == 0:
+            next_pack = now + pace
+            if pace == 0 and it % n_pb == 0:
                 s2.synchronize()                        # bound the queue: n_pb packs in flight
+        if staged:                                      # at most 0.5 ms after completion
+            ringR.stager.wait(ticket, s1.cuda_stream)
+            z.record(s1)
         torch.cuda.synchronize()
         plan.close()
         return a.elapsed_time(z), it, [x.elapsed_time(y) for x, y in pev]
@@ -1048,7 +1077,53 @@ def run_cfg3(args):
         return {"restore_GBps": total / t / 1e6, "ms": t, "delta_packs": packs,
                 "delta_pack_ms_median": float(np.median(lat)) if lat else None,
                 "delta_pack_ms_mean": float(np.mean(lat)) if lat else None,
-                "delta_pack_ms_max": float(np.max(lat)) if lat else None}
+                "delta_pack_ms_max": float(np.max(lat)) if lat else None,
+                "delta_pack_GBps_median": pbytes / float(np.median(lat)) / 1e6 if lat else None}
+
+    def stats(lat, denom):
+        med, best = float(np.median(lat)), float(np.min(lat))
+        return {"median_ms": med, "best_ms": best, "GBps": pbytes / med / 1e6,
+                "frac": pbytes / med / 1e6 / denom}
+
+    def delta_alone(mode, pace, n=24):
+        """The decode-step delta with nothing else on the device: one event pair per call, the
+        device idle for `pace` s before each (a decode loop issues one per iteration)."""
+        dsrc = torch.empty(pbytes, dtype=torch.uint8, device="cuda")
+        lat = []
+        for it in range(-3, n):
+            torch.cuda.synchronize()
+            time.sleep(pace)
+            if mode == "memcpy":                        # the copy engine alone, same size: the floor
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                with torch.cuda.stream(s2):
+                    e0.record(s2); pbufs[it % n_pb].copy_(dsrc, non_blocking=True); e1.record(s2)
+            else:
+                e0, e1 = delta_pack(it, mode == "staged", s2)
+            s2.synchronize()
+            if it >= 0:
+                lat.append(e0.elapsed_time(e1))
+        return lat
+
+    def memcpy_beside_h2d(n=24):
+        """A D2H cudaMemcpyAsync of the delta's size while H2D memcpys saturate the other direction:
+        what the link gives a 16 MiB transfer when it is busy both ways (the duplex share)."""
+        big_h = wdev.pinned_exact(1 << 30)
+        big_d = torch.empty(1 << 30, dtype=torch.uint8, device="cuda")
+        dsrc = torch.empty(pbytes, dtype=torch.uint8, device="cuda")
+        lat = []
+        with torch.cuda.stream(s1):
+            for _ in range(6):
+                big_d.copy_(big_h, non_blocking=True)
+        for it in range(n):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            with torch.cuda.stream(s2):
+                e0.record(s2); pbufs[it % n_pb].copy_(dsrc, non_blocking=True); e1.record(s2)
+            s2.synchronize()
+            lat.append(e0.elapsed_time(e1))
+            time.sleep(0.002)
+        torch.cuda.synchronize()
+        wdev.unpin(big_h)
+        return lat
 
     total = sum(wave_bytes)
     restore(b.waves[-1], wave_bytes[-1], False, None)   # warm-up
@@ -1059,13 +1134,42 @@ def run_cfg3(args):
     modes["staged_paced_packs"] = all_waves(True, PACE)
     sampler.stop()
     modes["staged_saturating_packs"] = all_waves(True, 0)
+    # ---- the decode-step delta by itself ---------------------------
+    d2h = link["d2h"]
+    floor_busy = memcpy_beside_h2d()
+    share = pbytes / float(np.median(floor_busy)) / 1e6     # GB/s a same-size D2H memcpy gets on a busy link
+    delta1 = {
+        "bytes": pbytes,
+        "what": ("lumen_kv_plan_build + pack of 1 new token of each of the 64 running requests (64 x 256 KiB) "
+                 "to pinned host, one CUDA-event pair per call; alone = device idle for the pace before each "
+                 "call; frac = of the pinned D2H memcpy peak (1 GiB) alone, of the same-size memcpy's rate on "
+                 "a link that is saturated in the other direction beside a restore"),
+        "alone_paced_25ms": {"zero_copy": stats(delta_alone("mapped", PACE), d2h),
+                             "staged": stats(delta_alone("staged", PACE), d2h),
+                             "memcpy_same_size": stats(delta_alone("memcpy", PACE), d2h)},
+        "alone_paced_2ms": {"zero_copy": stats(delta_alone("mapped", 0.002), d2h),
+                            "staged": stats(delta_alone("staged", 0.002), d2h),
+                            "memcpy_same_size": stats(delta_alone("memcpy", 0.002), d2h)},
+        "duplex_share_GBps": share,
+        "memcpy_same_size_beside_h2d_memcpy": stats(floor_busy, share),
+        "beside_restore": {
+            "zero_copy_beside_zero_copy_restore": {
+                "median_ms": modes["mapped_paced_packs"]["delta_pack_ms_median"],
+                "GBps": modes["mapped_paced_packs"]["delta_pack_GBps_median"],
+                "frac": modes["mapped_paced_packs"]["delta_pack_GBps_median"] / share},
+            "staged_beside_staged_restore": {
+                "median_ms": modes["staged_paced_packs"]["delta_pack_ms_median"],
+                "GBps": modes["staged_paced_packs"]["delta_pack_GBps_median"],
+                "frac": modes["staged_paced_packs"]["delta_pack_GBps_median"] / share}},
+    }
     head = modes["staged_paced_packs"]
     value = head["restore_GBps"]
     packs = sum(m["delta_packs"] for m in modes.values())
-    n_chunks = 0
+    n_chunks, per_wave_chunks = 0, []
     for w in b.waves:
         probe = lk.lumen_kv_plan_build(geom, w, lk.LUMEN_KV_HOST_ONLY)
-        n_chunks += len(probe.chunks(32 << 20))
+        per_wave_chunks.append(len(probe.chunks(32 << 20)))
+        n_chunks += per_wave_chunks[-1]
         probe.close()
     # kernels: 1 per delta pack (16 MiB = 1 chunk), 1 per mapped wave, 1 per chunk of a staged wave
     launches = packs + 2 * len(b.waves) + 3 * n_chunks + 2
@@ -1083,7 +1187,11 @@ def run_cfg3(args):
                    "wave_GiB": [x / 2**30 for x in wave_bytes], "seed": hex(MASTER_SEED),
                    "l2": "inputs larger than L2: every wave is tens of GiB read once over the host link"},
         "tokens_per_s": value * 1e9 / tok_bytes,
-        "modes": modes,
+        "modes": modes, "delta1_to_host": delta1,
+        "restore_call_host_ms": {"staged_async_median": float(np.median(call_ms["staged_async"])),
+                                 "staged_async_max": float(np.max(call_ms["staged_async"])),
+                                 "zero_copy_median": float(np.median(call_ms["mapped"])),
+                                 "chunks_per_wave": None},
         "roofline": {"bound": "host_link", "kernel": "lumen_kv_restore_unpack_staged (copy engine H2D + kv_copy_warp)",
                      "achieved": modes["staged_alone"]["restore_GBps"], "peak": link["h2d"], "unit": "GB/s",
                      "frac": modes["staged_alone"]["restore_GBps"] / link["h2d"], "traffic": None,
@@ -1096,6 +1204,7 @@ def run_cfg3(args):
                 "note": "this workload is the host path: the timed region is the H2D restore itself"},
         "gpu_launches": launches, "clocks": sampler.summary(),
     }
+    line["restore_call_host_ms"]["chunks_per_wave"] = per_wave_chunks
     sampler.close()
     print(json.dumps(line), flush=True)
     wdev.unpin(hbuf)
