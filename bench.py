@@ -44,7 +44,7 @@ def parse_args():
     ap.add_argument("--steps", type=int, default=300)
     ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
-    ap.add_argument("--workload", choices=["cfg0", "cfg1", "cfg2", "cfg3", "cfg4", "chain", "interference", "overhead"],
+    ap.add_argument("--workload", choices=["cfg0", "cfg1", "cfg2", "cfg3", "cfg4", "chain", "interference", "overhead", "hostlink", "dram"],
                     default="cfg1")
     ap.add_argument("--kernel", choices=["auto", "warp", "bulk"], default="auto")
     ap.add_argument("--upload-descriptors", action="store_true",
@@ -545,10 +545,15 @@ class HbmPath:
         return ms, pack_ms, unpack_ms, t_wall * 1e3, t_host * 1e3
 
     def idle_single_launch(self, bufs, kind, idle_s=0.012, n=12):
-        """A decode loop issues one pack per 13-58 ms iteration: every launch meets an idle device.
-        One event pair per launch around nothing but the call (plan built beforehand), `idle_s` of
-        host sleep with the device idle before each."""
+        """A decode loop issues one pack per 13-58 ms iteration: no launch in front of it to
+        overlap with, caches cold.  One event pair per launch around nothing but the call (plan
+        built beforehand).  The stream first waits for a gate that opens after `idle_s` s in
+        which the device runs nothing but one spinning warp (torch.cuda._sleep on a side
+        stream): record, launch and record are already queued when it opens, so the figure holds
+        no host launch latency (a Python call between the two records would add about 20 us)."""
         torch, stream, lk, pool = self.torch, self.stream, self.lk, self.pool
+        side = torch.cuda.Stream()
+        cycles = int(idle_s * 1.9e9)
         out = {}
         for only in ("pack", "unpack"):
             ts = []
@@ -558,7 +563,12 @@ class HbmPath:
                 ra.set_ranges(tb, te)
                 plan = lk.lumen_kv_plan_build(pool.geom, ra, self.kflag, self.sh)
                 fn = lk.lumen_kv_checkpoint_pack if only == "pack" else lk.lumen_kv_restore_unpack
-                torch.cuda.synchronize(); time.sleep(idle_s)
+                torch.cuda.synchronize()
+                gate = torch.cuda.Event()
+                with torch.cuda.stream(side):
+                    torch.cuda._sleep(cycles)
+                    gate.record(side)
+                stream.wait_event(gate)
                 a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
                 a.record(stream)
                 fn(plan, pool.k_ptrs, pool.v_ptrs, bufs[i % len(bufs)].data_ptr(), self.P, kind, self.sh)
@@ -777,7 +787,8 @@ def run_ours(args):
                            "launching stream, in this run; *_single_ms = one event pair per launch inside "
                            f"whole steps ({ms_k / Kk:.4f} ms/step: the records between the launches cost a "
                            "few us each and prevent the overlap of consecutive launches); "
-                           "single_launch_after_idle_ms = one event pair per launch after 12 ms of idle device"),
+                           "single_launch_after_idle_ms = one event pair per launch, queued behind a gate that opens after "
+                           "12 ms in which the device runs one spinning warp (no memory traffic, no host latency inside)"),
                 "pack_ms": pack_ms, "unpack_ms": unpack_ms,
                 "pack_single_ms": pack_1, "unpack_single_ms": unpack_1, "single_launch_ms": single,
                 "single_launch_after_idle_ms": idle,
@@ -1637,6 +1648,169 @@ def run_overhead(args):
     print(json.dumps(line), flush=True)
 
 
+def run_hostlink(args):
+    """What bounds the ZERO-COPY host path (lumen_kv_checkpoint_pack / lumen_kv_restore_unpack with
+    LUMEN_KV_MEM_HOST_MAPPED: SM stores / loads on pinned host memory)?  A 2 GiB pack to pinned host
+    and its restore, for 32 KiB and for 2 KiB items, with the TMA bulk kernel at 8 / 24 / 96 / 296
+    CTAs and the SIMT kernel (32-byte and 16-byte accesses, full grid), against the pinned
+    cudaMemcpyAsync peaks of the same run.  One kernel per (variant, direction, repetition), in the
+    order of `launch_order`, so that an ncu launch list of this command (pcie__read_bytes,
+    pcie__write_bytes per launch) joins with it by index."""
+    import torch
+    import paper_2606_17787_b200 as lk
+    from paper_2606_17787_b200.pool import KVPool, pinned_buffer
+    from workloads import MASTER_SEED, cfg2_qwen32b, cfg4_longctx
+    from workloads import device as wdev
+
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: there is no CPU path for --impl ours")
+    torch.cuda.set_device(rank_env()[2])
+    wdev.build()
+    lk.lumen_kv_init()
+    link = memcpy_peaks(torch)
+    HOST = lk.LUMEN_KV_MEM_HOST_MAPPED
+    s = torch.cuda.Stream()
+    shapes = {"32KiB_items": cfg2_qwen32b(MASTER_SEED, N=3000, n_reqs=4, prompt=2048),
+              "2KiB_items": cfg4_longctx(MASTER_SEED, tokens=8192, wave_reqs=1)}
+    variants = [("bulk", n, 1) for n in (8, 24, 96, 296)] + [("warp", 0, 1), ("warp", 0, 0)]
+    out, order = {}, []
+    for sname, w in shapes.items():
+        L, H, D, S, N = w.geom
+        pool = KVPool(L, H, D, S, N)
+        fill_pool(pool, MASTER_SEED, wdev)
+        P = w.payload_bytes
+        host = pinned_buffer(P)
+        res = {}
+        for kern, ctas, wide in variants:
+            lk.lumen_kv_set_option("host_ctas", ctas)
+            lk.lumen_kv_set_option("wide", wide)
+            flag = lk.LUMEN_KV_KERNEL_BULK if kern == "bulk" else lk.LUMEN_KV_KERNEL_WARP
+            name = f"bulk_{ctas}_ctas" if kern == "bulk" else ("simt_32B_full_grid" if wide else "simt_16B_full_grid")
+            plan = lk.lumen_kv_plan_build(pool.geom, w.reqs, flag, s.cuda_stream)
+            rplan = lk.lumen_kv_plan_build(pool.geom, w.restore_reqs, flag | lk.LUMEN_KV_VALIDATE_UNIQUE_DST,
+                                           s.cuda_stream)
+            t = {}
+            for what, fn, pl in (("pack", lk.lumen_kv_checkpoint_pack, plan),
+                                 ("restore", lk.lumen_kv_restore_unpack, rplan)):
+                best = float("inf")
+                for rep in range(3):
+                    a, z = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    a.record(s)
+                    fn(pl, pool.k_ptrs, pool.v_ptrs, host.data_ptr(), P, HOST, s.cuda_stream)
+                    z.record(s)
+                    s.synchronize()
+                    order.append(f"{sname}/{name}/{what}/{rep}")
+                    if rep:
+                        best = min(best, a.elapsed_time(z))
+                peak = link["d2h"] if what == "pack" else link["h2d"]
+                t[what] = {"GBps": P / best / 1e6, "frac_of_memcpy": P / best / 1e6 / peak}
+            res[name] = t
+            plan.close(); rplan.close()
+        out[sname] = res
+        del pool, host
+        torch.cuda.empty_cache()
+    lk.lumen_kv_set_option("host_ctas", 0)
+    lk.lumen_kv_set_option("wide", 1)
+    best = out["32KiB_items"]["bulk_24_ctas"]
+    line = {"metric": "kv_pack_restore_payload_GBps", "value": best["pack"]["GBps"], "unit": "GB/s", "n_gpus": 1,
+            "steps": 2, "warmup": 1, "ms_per_step": (2 << 30) / best["pack"]["GBps"] / 1e6,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u16", "data": "synthetic",
+            "config": {"workload": ("hostlink: zero-copy pack of 2 GiB to pinned host and restore from it, Qwen3-32B "
+                                    "shape, 32 KiB items (page_size 16) and 2 KiB items (page_size 1), kernel and grid sweep"),
+                       "l2": "inputs larger than L2 (2 GiB per launch)"},
+            "variants": out, "launch_order": order,
+            "memcpy_peak_d2h_GBps": link["d2h"], "memcpy_peak_h2d_GBps": link["h2d"],
+            "roofline": {"bound": "host_link", "kernel": "lumen_kv_checkpoint_pack (kv_copy_bulk, 24 CTAs, zero-copy)",
+                         "achieved": best["pack"]["GBps"], "peak": link["d2h"], "unit": "GB/s",
+                         "frac": best["pack"]["frac_of_memcpy"], "traffic": None,
+                         "peak_source": "pinned cudaMemcpyAsync D2H, 1 GiB, best of 10, this run"},
+            "e2e": {"value": best["pack"]["GBps"], "unit": "GB/s", "h2d_bytes_per_step": 2 << 30,
+                    "d2h_bytes_per_step": 2 << 30},
+            "gpu_launches": len(order)}
+    print(json.dumps(line), flush=True)
+
+
+def run_dram(args):
+    """Is the HBM path at the DRAM's ceiling or at the kernel's?  Plain streaming kernels with the
+    library kernel's access shape (workloads/csrc/dramprobe.cu: read-only, write-only, contiguous
+    copy), torch's copy_ and a device-to-device cudaMemcpyAsync over 16 GiB buffers, next to the
+    pack and the restore of BASELINE.json configs[2]; all CUDA-event timed, 3 warm-up + 5 timed
+    launches each.  `of_pin_rate` = against dram__bytes.sum.peak_sustained x the memory clock that
+    ncu reports for this part (2,048 B/cycle x 3.996 GHz = 8,184 GB/s)."""
+    import torch
+    import paper_2606_17787_b200 as lk
+    from paper_2606_17787_b200.pool import KVPool
+    from workloads import MASTER_SEED
+    from workloads import device as wdev
+
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: there is no CPU path for --impl ours")
+    local = rank_env()[2]
+    torch.cuda.set_device(local)
+    wdev.build()
+    lk.lumen_kv_init()
+    peak, peak_src = measured_peaks()
+    PIN = 2048 * 3.996                                   # GB/s
+    s = torch.cuda.Stream()
+    sampler = ClockSampler(local, gpu_uuid(torch, local))
+    NB = 16 << 30
+    a_ = torch.empty(NB, dtype=torch.uint8, device="cuda")
+    b_ = torch.empty(NB, dtype=torch.uint8, device="cuda")
+    wdev.fill_plane(a_, MASTER_SEED, 0)
+    order = []
+
+    def timed(name, fn, traffic, reps=5):
+        with torch.cuda.stream(s):
+            for _ in range(3):
+                fn()
+            x, y = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize()
+            sampler.start()
+            x.record(s)
+            for _ in range(reps):
+                fn()
+            y.record(s)
+            sampler.poll()
+            s.synchronize()
+            sampler.stop()
+        ms = x.elapsed_time(y) / reps
+        order.extend([name] * (3 + reps))
+        g = traffic / ms / 1e6
+        return {"ms": ms, "traffic_GBps": g, "of_measured_copy_peak": g / peak, "of_pin_rate": g / PIN}
+
+    res = {
+        "probe_read_only": timed("probe_read", lambda: wdev.dram_probe("read", a_, b_, NB, s.cuda_stream), NB),
+        "probe_write_only": timed("probe_write", lambda: wdev.dram_probe("write", a_, b_, NB, s.cuda_stream), NB),
+        "probe_copy": timed("probe_copy", lambda: wdev.dram_probe("copy", a_, b_, NB, s.cuda_stream), 2 * NB),
+        "torch_copy_": timed("torch_copy", lambda: b_.copy_(a_), 2 * NB),
+    }
+    del a_, b_
+    torch.cuda.empty_cache()
+    w, label, _ = make_workload("cfg2", MASTER_SEED)
+    L, H, D, S, N = w.geom
+    pool = KVPool(L, H, D, S, N)
+    fill_pool(pool, MASTER_SEED, wdev)
+    dbuf = torch.empty(w.payload_bytes, dtype=torch.uint8, device="cuda")
+    path = HbmPath(torch, lk, pool, w, 0, lk.LUMEN_KV_KERNEL_AUTO, s, None)
+    res["lumen_kv_checkpoint_pack_cfg2"] = timed(
+        "pack", lambda: path.step(0, [dbuf], lk.LUMEN_KV_MEM_DEVICE, 0, None, "pack"), 2 * path.P)
+    res["lumen_kv_restore_unpack_cfg2"] = timed(
+        "unpack", lambda: path.step(0, [dbuf], lk.LUMEN_KV_MEM_DEVICE, 0, None, "unpack"), 2 * path.P)
+    head = res["lumen_kv_checkpoint_pack_cfg2"]
+    line = {"metric": "kv_pack_restore_payload_GBps", "value": head["traffic_GBps"] / 2, "unit": "GB/s", "n_gpus": 1,
+            "steps": 5, "warmup": 3, "ms_per_step": head["ms"], "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "u16", "data": "synthetic",
+            "config": {"workload": "dram: streaming read / write / copy probes (16 GiB) beside the pack and restore of "
+                                   + label, "l2": "inputs larger than L2 (16-32 GiB per launch)"},
+            "kernels": res, "launch_order": order, "pin_rate_GBps": PIN,
+            "roofline": {"bound": "hbm", "kernel": "lumen_kv_checkpoint_pack (kv_copy_warp32)",
+                         "achieved": head["traffic_GBps"], "peak": peak, "unit": "GB/s",
+                         "frac": head["traffic_GBps"] / peak, "traffic": None, "peak_source": peak_src},
+            "e2e": None, "gpu_launches": len(order), "clocks": sampler.summary()}
+    sampler.close()
+    print(json.dumps(line), flush=True)
+
+
 def main():
     args = parse_args()
     if args.impl == "reference":
@@ -1649,6 +1823,10 @@ def main():
         run_interference(args)
     elif args.workload == "overhead":
         run_overhead(args)
+    elif args.workload == "hostlink":
+        run_hostlink(args)
+    elif args.workload == "dram":
+        run_dram(args)
     else:
         run_ours(args)
 

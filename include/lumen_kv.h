@@ -563,6 +563,20 @@ LUMEN_KV_API void lumen_kv_trim(void);
  * done implicitly by the first launch on a device.  Errors: ECUDA.                     */
 LUMEN_KV_API int lumen_kv_init(void);
 
+/*
+ * Tuning knobs.  They exist to reproduce the A/B measurements of DESIGN.md; the defaults are
+ * the measured best and nothing needs them.  Each is also read once from the environment
+ * (LUMEN_KV_<NAME in capitals>) at the library's first use.  Process-wide; do not change them
+ * while another thread is inside pack/unpack.
+ *   "pdl"         1 (default) / 0 : programmatic dependent launch of the SIMT kernel
+ *   "wide"        1 (default) / 0 : 32-byte accesses where every address allows them, else 16-byte
+ *   "warp_unroll" 4 (default) / 8 : loads in flight per lane of the 16-byte kernel
+ *   "host_kernel" 2 (default, TMA bulk kernel) / 1 (SIMT kernel): what AUTO picks for a host buffer
+ *   "host_ctas"   0 (default: 24..96 by item size) / n : grid of the bulk kernel on a host buffer
+ * Errors: EINVAL (unknown name).
+ */
+LUMEN_KV_API int lumen_kv_set_option(const char* name, int value);
+
 LUMEN_KV_API const char* lumen_kv_strerror(int status);
 /* last cudaError_t seen by the calling thread inside the library (0 if none) */
 LUMEN_KV_API int lumen_kv_last_cuda_error(void);

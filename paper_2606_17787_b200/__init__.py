@@ -10,7 +10,7 @@ from .binding import (  # noqa: F401
     EXPORTS, LumenKVError, Plan, ReqArray, Stager, lumen_kv_chunk_info,
     lumen_kv_checkpoint_pack_staged, lumen_kv_restore_unpack_staged,
     lumen_kv_checkpoint_pack_staged_commit, lumen_kv_restore_unpack_staged_ready,
-    lumen_kv_checkpoint_pack_staged_async, lumen_kv_restore_unpack_staged_async, lumen_kv_init,
+    lumen_kv_checkpoint_pack_staged_async, lumen_kv_restore_unpack_staged_async, lumen_kv_init, lumen_kv_set_option,
     TAG_DTYPE, SEGMENT_DTYPE, Store, BackgroundCheckpointer, lumen_kv_choose_holder, lumen_kv_recover, lumen_kv_tags_num_pages, lumen_kv_page_tags, lumen_kv_page_tags_host, lumen_kv_longest_prefix, library_path, lumen_kv_checkpoint_pack, lumen_kv_geom,
     lumen_kv_plan_build, lumen_kv_plan_free, lumen_kv_req, lumen_kv_restore_unpack,
     lumen_kv_run_info, lumen_kv_req_layout, lumen_kv_strerror, lumen_kv_trim, lumen_kv_version, make_geom, plane_ptrs,

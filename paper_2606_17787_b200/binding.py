@@ -32,7 +32,7 @@ LUMEN_KV_MEM_DEVICE, LUMEN_KV_MEM_HOST_MAPPED = 0, 1
 EXPORTS = (
     "lumen_kv_plan_build", "lumen_kv_plan_build_layout", "lumen_kv_plan_bytes", "lumen_kv_plan_req_offset",
     "lumen_kv_plan_num_runs", "lumen_kv_plan_get_run", "lumen_kv_checkpoint_pack",
-    "lumen_kv_restore_unpack", "lumen_kv_plan_free", "lumen_kv_trim", "lumen_kv_init",
+    "lumen_kv_restore_unpack", "lumen_kv_plan_free", "lumen_kv_trim", "lumen_kv_init", "lumen_kv_set_option",
     "lumen_kv_checkpoint_pack_staged_async", "lumen_kv_restore_unpack_staged_async",
     "lumen_kv_stager_query", "lumen_kv_stager_wait", "lumen_kv_stager_sync",
     "lumen_kv_strerror", "lumen_kv_last_cuda_error", "lumen_kv_version",
@@ -150,6 +150,8 @@ def _lib() -> ctypes.CDLL:
     L.lumen_kv_stager_sync.argtypes = [vp, ctypes.c_uint64]
     L.lumen_kv_init.restype = ctypes.c_int
     L.lumen_kv_init.argtypes = []
+    L.lumen_kv_set_option.restype = ctypes.c_int
+    L.lumen_kv_set_option.argtypes = [ctypes.c_char_p, ctypes.c_int]
     L.lumen_kv_tags_num_pages.restype = i64
     L.lumen_kv_tags_num_pages.argtypes = [vp, i32, i32]
     L.lumen_kv_page_tags.restype = ctypes.c_int
@@ -518,6 +520,12 @@ def lumen_kv_restore_unpack_staged_async(plan: Plan, k_planes, v_planes, src_hos
                                          epoch: int = 0) -> int:
     return _staged_async("lumen_kv_restore_unpack_staged_async", plan, k_planes, v_planes, src_host,
                          src_bytes, stager, stream, flags_host, epoch)
+
+
+def lumen_kv_set_option(name: str, value: int) -> None:
+    rc = _lib().lumen_kv_set_option(name.encode(), int(value))
+    if rc:
+        raise LumenKVError(rc, "lumen_kv_set_option")
 
 
 def lumen_kv_init() -> None:

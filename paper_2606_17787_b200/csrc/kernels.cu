@@ -508,6 +508,18 @@ void read_env_once() {
     });
 }
 
+int set_option(const char* name, int value) {
+    if (!name) return -1;
+    read_env_once();                 // so that a later first launch does not overwrite the setting
+    if (!strcmp(name, "pdl")) g_pdl = value ? 1 : 0;
+    else if (!strcmp(name, "wide")) g_wide = value ? 1 : 0;
+    else if (!strcmp(name, "warp_unroll")) g_warp_unroll = (value == 8) ? 8 : 4;
+    else if (!strcmp(name, "host_kernel")) g_host_kernel = (value == kKernelWarp) ? kKernelWarp : kKernelBulk;
+    else if (!strcmp(name, "host_ctas")) g_host_ctas = value > 0 ? value : 0;
+    else return -1;
+    return 0;
+}
+
 cudaError_t device_state(DeviceState** out) {
     int dev = 0;
     cudaError_t e = cudaGetDevice(&dev);

@@ -44,6 +44,9 @@ cudaError_t launch_kv_copy(const CopyArgs& a);
 // shared-memory limit); launch_kv_copy does it by itself at the first launch on a device.
 cudaError_t init_current_device();
 
+// Tuning knobs (the LUMEN_KV_* environment variables, settable at run time): 0 or -1 (unknown name).
+int set_option(const char* name, int value);
+
 // Which kernel AUTO resolves to for these arguments (exposed for tests / bench notes).
 int resolve_kernel(const CopyArgs& a);
 

@@ -406,6 +406,10 @@ void lumen_kv_plan_free(lumen_kv_plan* plan) {
 
 void lumen_kv_trim(void) { lumen::arena().trim(); }
 
+int lumen_kv_set_option(const char* name, int value) {
+    return lumen::set_option(name, value) == 0 ? LUMEN_KV_OK : LUMEN_KV_EINVAL;
+}
+
 int lumen_kv_init(void) {
     const cudaError_t e = lumen::init_current_device();
     return e == cudaSuccess ? LUMEN_KV_OK : lumen::cuda_fail(e);

@@ -13,15 +13,39 @@ _SO = _HERE / "libkvfill.so"
 _lib = None
 
 
-def build(force: bool = False) -> Path:
-    if force or not _SO.exists() or _SO.stat().st_mtime < _SRC.stat().st_mtime:
+_PROBE_SRC = _HERE / "csrc" / "dramprobe.cu"
+_PROBE_SO = _HERE / "libdramprobe.so"
+_probe = None
+
+
+def _nvcc_shared(src: Path, so: Path, force: bool) -> None:
+    if force or not so.exists() or so.stat().st_mtime < src.stat().st_mtime:
         nvcc = os.environ.get("NVCC") or "/usr/local/cuda/bin/nvcc"
-        tmp = _SO.with_suffix(f".so.tmp{os.getpid()}")
+        tmp = so.with_suffix(f".so.tmp{os.getpid()}")
         subprocess.check_call([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3",
                                "-Xcompiler", "-fPIC,-fvisibility=hidden", "-shared", "-cudart", "static",
-                               "-o", str(tmp), str(_SRC)])
-        os.replace(tmp, _SO)
+                               "-o", str(tmp), str(src)])
+        os.replace(tmp, so)
+
+
+def build(force: bool = False) -> Path:
+    _nvcc_shared(_SRC, _SO, force)
+    _nvcc_shared(_PROBE_SRC, _PROBE_SO, force)
     return _SO
+
+
+def dram_probe(mode: str, src, dst, nbytes: int, stream: int = 0) -> None:
+    """Plain streaming read / write / copy over contiguous device buffers (csrc/dramprobe.cu)."""
+    global _probe
+    if _probe is None:
+        _probe = ctypes.CDLL(str(_PROBE_SO))
+        _probe.dramprobe_run.restype = ctypes.c_int
+        _probe.dramprobe_run.argtypes = [ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int64,
+                                         ctypes.c_void_p, ctypes.c_void_p]
+    rc = _probe.dramprobe_run({"read": 0, "write": 1, "copy": 2}[mode], src.data_ptr(), dst.data_ptr(),
+                              int(nbytes), None, stream)
+    if rc:
+        raise RuntimeError(f"dramprobe_run({mode}) failed ({rc})")
 
 
 def lib() -> ctypes.CDLL:
