@@ -133,7 +133,16 @@ typedef struct lumen_kv_plan lumen_kv_plan;  /* opaque; library owns its descrip
 #define LUMEN_KV_MEM_DEVICE      0  /* device pointer (HBM)                                   */
 #define LUMEN_KV_MEM_HOST_MAPPED 1  /* pinned host memory (cudaHostAlloc / cudaHostRegister);
                                        pass the HOST pointer, the kernel writes/reads it
-                                       directly over the host link                           */
+                                       directly over the host link (zero-copy).  One launch,
+                                       no staging memory; AUTO uses a few dozen single-warp
+                                       TMA CTAs so that the SMs stay free.  Every SM-issued
+                                       access crosses PCIe as a 128-byte TLP (one L2 line),
+                                       the copy engine uses 256-byte TLPs: this path tops out
+                                       at 92 % of what cudaMemcpyAsync reaches (measured 52.8
+                                       of 57.3 GB/s D2H, 51.5 of 55.6 H2D; counters in
+                                       profiles/r2_README.md) whatever kernel, grid or
+                                       operation size is used.  The staged calls below move
+                                       the same bytes with the copy engine (99 %).            */
 
 /*
  * lumen_kv_plan_build -- step a2: flatten the requests'

@@ -29,10 +29,10 @@ def test_oracle_eq1_hand_worked():
     n = 0
     for c in golden("holder"):
         got = po.choose_holder([frac(x) for x in c["q"]], c["held"], c["available"], c["serving"],
-                               c["footprint"], c["lam"], c["bw"])
+                               c["footprint"], frac(c["lam"]), c["bw"])
         assert got == c["expect"], c
         n += 1
-    assert n == 6
+    assert n == 9
     assert po.restore_pressure([26], 13, 26) == Fraction(3, 4)
     assert po.restore_pressure([], 13, 26) == Fraction(1, 2)
 
@@ -43,7 +43,7 @@ def test_oracle_recovery_hand_worked():
         assign, reuse, final = po.dispatch_and_rebalance(c["load"], c["alive"], [tuple(x) for x in c["interrupted"]])
         assert (assign, reuse, final) == (c["assign"], c["reuse"], c["final"]), c
         n += 1
-    assert n == 3
+    assert n == 5
 
 
 def random_recovery(rng):
@@ -92,7 +92,7 @@ def lk():
 def test_library_equals_oracle(lk):
     for c in golden("holder"):
         got = lk.lumen_kv_choose_holder([float(frac(x)) for x in c["q"]], c["held"], c["available"],
-                                        c["serving"], c["footprint"], c["lam"], c["bw"])
+                                        c["serving"], c["footprint"], float(frac(c["lam"])), c["bw"])
         assert got == (c["expect"] if c["expect"] is not None else -1), c
     rng = substream(42, "placement_lib")
     for _ in range(300):
