@@ -102,9 +102,10 @@ def iteration_ranges(w, delta: int, cycle: int):
 # neither take this process's GIL nor sit between the two event records of a timed region)
 # ------------------------------------------------------------------------------------
 _CLOCK_HELPER = r"""
-import signal, sys, time
+import os, signal, sys, time
 import pynvml as nv
 uuid, index, path = sys.argv[1], int(sys.argv[2]), sys.argv[3]
+parent = os.getppid()
 nv.nvmlInit()
 try:
     h = nv.nvmlDeviceGetHandleByUUID(uuid)
@@ -117,7 +118,7 @@ signal.signal(signal.SIGHUP, lambda *a: state.update(period=0.05))      # second
 signal.signal(signal.SIGUSR2, lambda *a: state.update(period=None))
 f = open(path, "w")
 f.write("max %d\n" % nv.nvmlDeviceGetMaxClockInfo(h, nv.NVML_CLOCK_SM)); f.flush()
-while not state["stop"]:
+while not state["stop"] and os.getppid() == parent:      # never outlive the bench process
     if state["period"] is None:
         time.sleep(0.001)
         continue
@@ -157,6 +158,8 @@ class ClockSampler:
         try:
             self.proc = subprocess.Popen([sys.executable, "-c", _CLOCK_HELPER, uuid, str(index), self.path],
                                          stdout=subprocess.DEVNULL, stderr=subprocess.DEVNULL)
+            import atexit
+            atexit.register(self.close)
         except Exception:
             self.proc = None
         try:
