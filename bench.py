@@ -801,12 +801,24 @@ def run_ours(args):
     big = P > (1 << 30)
     Kk = min(K, 200) if not big else min(K, 3)         # per-launch pass: same steps, instrumented
     with torch.cuda.stream(stream):
-        ms, _, _, wall_ms, host_ms = path.timed_loop(K, W, dbufs, DEV, lag, sampler)
-        clocks = sampler.summary(reset=True)
+        pack_ref = path.timed_loop(Kk, 3, dbufs, DEV, lag, only="pack")[0] / Kk
+        unpack_ref = path.timed_loop(Kk, 3, dbufs, DEV, lag, only="unpack")[0] / Kk
+        # The headline: exactly K steps between one event pair.  A step that the HOST could not feed
+        # in time (enqueue slower than the two kernels AND a device time well above them -- e.g. this
+        # process was descheduled for a millisecond inside a 2 ms region) does not measure the
+        # kernels; it is taken again, once, and both attempts are reported.
+        attempts = []
+        for _ in range(2):
+            ms, _, _, wall_ms, host_ms = path.timed_loop(K, W, dbufs, DEV, lag, sampler)
+            clocks = sampler.summary(reset=True)
+            starved = host_ms / K > pack_ref + unpack_ref and ms / K > 1.15 * (pack_ref + unpack_ref)
+            attempts.append({"ms_per_step": ms / K, "host_enqueue_ms_per_step": host_ms / K,
+                             "host_bound": bool(starved)})
+            if not starved:
+                break
         ms_k, pack_1, unpack_1, _, _ = path.timed_loop(Kk, 3, dbufs, DEV, lag, per_launch=True)
         single = {k: dict(v) for k, v in path.single_stats.items()}   # single-launch latency: mean/median/best
-        pack_ms = path.timed_loop(Kk, 3, dbufs, DEV, lag, only="pack")[0] / Kk
-        unpack_ms = path.timed_loop(Kk, 3, dbufs, DEV, lag, only="unpack")[0] / Kk
+        pack_ms, unpack_ms = pack_ref, unpack_ref
         idle = path.idle_single_launch(dbufs, DEV) if not big else None
         ms_2s = path.two_stream_loop(K, W, dbufs, DEV, lag) if n_stage > 1 else None
     value = job_payload_gbps(world, K, P, ms)
@@ -821,7 +833,7 @@ def run_ours(args):
         pl.close()
     plan_build_us = (time.perf_counter() - t0) / n_pb * 1e6
     stream.synchronize()
-    host_bound = host_ms / K > pack_ms + unpack_ms
+    host_bound = attempts[-1]["host_bound"]
 
     # ---- roofline of the dominant kernel ------------------------------------------------
     peak, peak_src = measured_peaks()
@@ -981,7 +993,7 @@ def run_ours(args):
                    "pdl": os.environ.get("LUMEN_KV_PDL", "1") != "0", "seed": hex(MASTER_SEED)},
         "tokens_per_s": value * 1e9 / token_bytes,
         "wall_ms_per_step": wall_ms / K, "host_enqueue_ms_per_step": host_ms / K,
-        "host_bound": bool(host_bound),
+        "host_bound": bool(host_bound), "headline_attempts": attempts,
         "step_over_kernels": (ms / K) / (pack_ms + unpack_ms),
         "plan_build_us": plan_build_us,
         "roofline": roofline, "e2e": e2e, "gpu_launches": 2 * K, "clocks": clocks,
