@@ -130,7 +130,12 @@ typedef struct lumen_kv_plan lumen_kv_plan;  /* opaque; library owns its descrip
 #define LUMEN_KV_KERNEL_BULK         0x200u /* TMA 1-D bulk copies through a shared-memory ring */
 
 /* where the checkpoint buffer lives */
-#define LUMEN_KV_MEM_DEVICE      0  /* device pointer (HBM)                                   */
+#define LUMEN_KV_MEM_DEVICE      0  /* device pointer into the CURRENT device's memory (HBM)  */
+#define LUMEN_KV_MEM_DEVICE_PEER 2  /* device pointer into ANOTHER GPU's memory (peer access
+                                       enabled by the caller): same kernels; the restore does
+                                       not ask L2 for its source ahead of the stream-order
+                                       wait, because only a device's own memory is cached
+                                       coherently in its L2                                   */
 #define LUMEN_KV_MEM_HOST_MAPPED 1  /* pinned host memory (cudaHostAlloc / cudaHostRegister);
                                        pass the HOST pointer, the kernel writes/reads it
                                        directly over the host link (zero-copy).  One launch,
@@ -582,6 +587,9 @@ LUMEN_KV_API int lumen_kv_init(void);
  *   "warp_unroll" 4 (default) / 8 : loads in flight per lane of the 16-byte kernel
  *   "host_kernel" 2 (default, TMA bulk kernel) / 1 (SIMT kernel): what AUTO picks for a host buffer
  *   "host_ctas"   0 (default: 24..96 by item size) / n : grid of the bulk kernel on a host buffer
+ *   "prefetch"    16 (default) / d >= 0 / -1 : the SIMT kernel asks L2 for the 4 KiB a warp d CTAs
+ *                 further on will copy (parameter-resident plans; larger plans announce their own
+ *                 4 KiB, whatever d) / no prefetch.  A hint: the bytes moved are the same.
  * Errors: EINVAL (unknown name).
  */
 LUMEN_KV_API int lumen_kv_set_option(const char* name, int value);

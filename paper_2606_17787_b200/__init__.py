@@ -17,5 +17,5 @@ from .binding import (  # noqa: F401
     LUMEN_KV_OK, LUMEN_KV_EINVAL, LUMEN_KV_ERANGE, LUMEN_KV_EOVERLAP, LUMEN_KV_ESIZE,
     LUMEN_KV_ENOMEM, LUMEN_KV_ECUDA, LUMEN_KV_ESINK, LUMEN_KV_VALIDATE_UNIQUE_DST, LUMEN_KV_MERGE_ADJACENT,
     LUMEN_KV_HOST_ONLY, LUMEN_KV_NO_INLINE, LUMEN_KV_KERNEL_AUTO, LUMEN_KV_KERNEL_WARP, LUMEN_KV_KERNEL_BULK,
-    LUMEN_KV_MEM_DEVICE, LUMEN_KV_MEM_HOST_MAPPED,
+    LUMEN_KV_MEM_DEVICE, LUMEN_KV_MEM_HOST_MAPPED, LUMEN_KV_MEM_DEVICE_PEER,
 )

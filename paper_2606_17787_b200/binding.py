@@ -27,7 +27,7 @@ LUMEN_KV_MERGE_ADJACENT = 0x2
 LUMEN_KV_HOST_ONLY = 0x4
 LUMEN_KV_NO_INLINE = 0x8
 LUMEN_KV_KERNEL_AUTO, LUMEN_KV_KERNEL_WARP, LUMEN_KV_KERNEL_BULK = 0x000, 0x100, 0x200
-LUMEN_KV_MEM_DEVICE, LUMEN_KV_MEM_HOST_MAPPED = 0, 1
+LUMEN_KV_MEM_DEVICE, LUMEN_KV_MEM_HOST_MAPPED, LUMEN_KV_MEM_DEVICE_PEER = 0, 1, 2
 
 EXPORTS = (
     "lumen_kv_plan_build", "lumen_kv_plan_build_layout", "lumen_kv_plan_bytes", "lumen_kv_plan_req_offset",

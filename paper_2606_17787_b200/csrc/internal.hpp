@@ -59,6 +59,6 @@ int gather_planes(const lumen_kv_plan* plan, const void* const* k_planes,
 // it may lie outside any allocation; only bytes of the chunk are ever addressed).
 int launch_part(const lumen_kv_plan* plan, const std::vector<const void*>& planes, uintptr_t buf,
                 bool buf_is_host, cudaStream_t stream, bool pack, int64_t ra, int64_t rb,
-                int32_t p0, int32_t p1);
+                int32_t p0, int32_t p1, bool buf_is_peer = false);
 
 }  // namespace lumen

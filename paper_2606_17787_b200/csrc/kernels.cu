@@ -59,6 +59,12 @@ __device__ __forceinline__ void pdl_launch_dependents() {
 }
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 
+// Hint: bring `bytes` (a multiple of 16) at `p` into L2.  L2 is the device's point of coherence,
+// so a line fetched early still shows every store that reaches L2 before the later load.
+__device__ __forceinline__ void l2_prefetch_bulk(const void* p, uint32_t bytes) {
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
+}
+
 // Where the descriptors live: in global memory (uploaded by plan_build) or, for small
 // plans, in the kernel parameters themselves (constant bank, no upload, no dependent
 // global loads before the first payload load).
@@ -181,7 +187,7 @@ template <int UNROLL, class Desc>
 __global__ void __launch_bounds__(kWarpsPerCta * 32)
 kv_copy_warp32(const __grid_constant__ PlaneTable planes, const __grid_constant__ Desc desc,
                int64_t n_runs, char* buf, uint32_t row_bytes, int32_t plane0, int sub_shift,
-               int pack) {
+               int pack, int32_t pf_dist) {
     pdl_launch_dependents();
     const int lane = threadIdx.x & 31;
     const int64_t task = static_cast<int64_t>(blockIdx.x) * kWarpsPerCta + (threadIdx.x >> 5);
@@ -191,11 +197,50 @@ kv_copy_warp32(const __grid_constant__ PlaneTable planes, const __grid_constant_
     if (!Desc::kInline) pdl_wait();
     const Item it = decode_item(desc, run, planes.p[blockIdx.y], plane0 + blockIdx.y, buf,
                                 row_bytes);
-    if (Desc::kInline) pdl_wait();
     const uint32_t nvec = it.bytes >> 5;
+    // L2 prefetch (pf_dist >= 0): one lane asks L2 for the 4 KiB source of the task that the warp
+    // pf_dist CTAs further on will copy (0: its own).  L2 is the device's point of coherence, so
+    // a line fetched early still shows every store that reaches L2 before the later load; that
+    // makes it legal in front of the wait, where the CTAs of the first wave -- resident while the
+    // previous grid's last wave drains -- would otherwise sit with nothing in flight.
+    const char* const src0 = (pack ? it.pool : it.buf) + static_cast<size_t>(sub) * (UNROLL * 1024);
+    const bool live = sub * (UNROLL * 32) < nvec;
+    auto prefetch_own = [&] {
+        const uint32_t left = it.bytes - sub * (UNROLL * 1024);
+        if (live) l2_prefetch_bulk(src0, left < UNROLL * 1024 ? left : UNROLL * 1024);
+    };
+    auto prefetch_ahead = [&] {
+        const uint64_t lin = static_cast<uint64_t>(blockIdx.y) * gridDim.x + blockIdx.x + pf_dist;
+        const uint32_t by = static_cast<uint32_t>(lin / gridDim.x);
+        const uint32_t bx = static_cast<uint32_t>(lin - static_cast<uint64_t>(by) * gridDim.x);
+        const int64_t task2 = static_cast<int64_t>(bx) * kWarpsPerCta + (threadIdx.x >> 5);
+        const int64_t run2 = task2 >> sub_shift;
+        if (by >= gridDim.y || run2 >= n_runs) return;
+        const uint32_t sub2 = static_cast<uint32_t>(task2 & ((int64_t{1} << sub_shift) - 1));
+        const Item it2 = decode_item(desc, run2, planes.p[by], plane0 + by, buf, row_bytes);
+        if (sub2 * (UNROLL * 1024) >= it2.bytes) return;
+        const uint32_t left = it2.bytes - sub2 * (UNROLL * 1024);
+        l2_prefetch_bulk((pack ? it2.pool : it2.buf) + static_cast<size_t>(sub2) * (UNROLL * 1024),
+                         left < UNROLL * 1024 ? left : UNROLL * 1024);
+    };
+    const bool leader = pf_dist >= 0 && lane == 0;
+    if (Desc::kInline) {
+        if (leader) {
+            if (static_cast<uint64_t>(blockIdx.y) * gridDim.x + blockIdx.x <
+                static_cast<uint32_t>(pf_dist) || pf_dist == 0)
+                prefetch_own();
+            if (pf_dist > 0) prefetch_ahead();
+        }
+        pdl_wait();
+    } else if (leader) {
+        // descriptors in global memory: decoding the task ahead would cost two more dependent
+        // loads (and, placed behind this warp's own loads, the registers of a fifth CTA per SM:
+        // measured, cfg 2 -3 %), so such plans only announce their own 4 KiB
+        prefetch_own();
+    }
+    if (!live) return;
     const uint32_t i = sub * (UNROLL * 32) + lane;
-    if (sub * (UNROLL * 32) >= nvec) return;
-    const char* src = (pack ? it.pool : it.buf) + (static_cast<size_t>(i) << 5);
+    const char* src = src0 + (static_cast<size_t>(lane) << 5);
     char* dst = (pack ? it.buf : it.pool) + (static_cast<size_t>(i) << 5);
     V8 v[UNROLL];
 #pragma unroll
@@ -405,10 +450,12 @@ struct WarpLaunch {
     int32_t plane0;
     int sub_shift;
     int pack;
+    int32_t pf_dist;   // L2 prefetch distance in CTAs (-1: off, 0: own task)
 };
 
 int g_pdl = 1;   // LUMEN_KV_PDL=0 launches without the programmatic attribute (A/B evidence)
 int g_wide = 1;   // LUMEN_KV_WIDE=0 keeps the 16-byte kernel even where 32-byte accesses are legal
+int g_prefetch = 16;   // LUMEN_KV_PREFETCH=d: L2 prefetch distance in CTAs (-1 off, 0 own task)
 constexpr int kWideUnroll = 4;
 
 template <class Desc>
@@ -423,7 +470,7 @@ cudaError_t launch_warp32(const PlaneTable& pt, const Desc& d, const WarpLaunch&
     cfg.attrs = attr;
     cfg.numAttrs = g_pdl ? 1 : 0;
     return cudaLaunchKernelEx(&cfg, kv_copy_warp32<kWideUnroll, Desc>, pt, d, w.n_runs, w.buf,
-                              w.row_bytes, w.plane0, w.sub_shift, w.pack);
+                              w.row_bytes, w.plane0, w.sub_shift, w.pack, w.pf_dist);
 }
 
 template <int UNROLL, class Desc>
@@ -502,6 +549,7 @@ void read_env_once() {
         if (const char* e = getenv("LUMEN_KV_WARP_UNROLL")) g_warp_unroll = (atoi(e) == 8) ? 8 : 4;
         if (const char* e = getenv("LUMEN_KV_PDL")) g_pdl = atoi(e) ? 1 : 0;
         if (const char* e = getenv("LUMEN_KV_WIDE")) g_wide = atoi(e) ? 1 : 0;
+        if (const char* e = getenv("LUMEN_KV_PREFETCH")) g_prefetch = atoi(e);
         if (const char* e = getenv("LUMEN_KV_HOST_KERNEL"))
             g_host_kernel = (e[0] == 'w') ? kKernelWarp : kKernelBulk;
         if (const char* e = getenv("LUMEN_KV_HOST_CTAS")) g_host_ctas = atoi(e);
@@ -513,6 +561,7 @@ int set_option(const char* name, int value) {
     read_env_once();                 // so that a later first launch does not overwrite the setting
     if (!strcmp(name, "pdl")) g_pdl = value ? 1 : 0;
     else if (!strcmp(name, "wide")) g_wide = value ? 1 : 0;
+    else if (!strcmp(name, "prefetch")) g_prefetch = value;
     else if (!strcmp(name, "warp_unroll")) g_warp_unroll = (value == 8) ? 8 : 4;
     else if (!strcmp(name, "host_kernel")) g_host_kernel = (value == kKernelWarp) ? kKernelWarp : kKernelBulk;
     else if (!strcmp(name, "host_ctas")) g_host_ctas = value > 0 ? value : 0;
@@ -588,6 +637,10 @@ cudaError_t launch_kv_copy(const CopyArgs& a) {
             w.plane0 = a.plane_base + plane0;
             w.sub_shift = sub_shift;
             w.pack = a.pack ? 1 : 0;
+            // only this device's own memory is cached coherently in its L2: a source in host
+            // memory or in a peer GPU's memory is never asked for ahead of the wait
+            const bool src_dev = a.pack || !(a.buf_is_host || a.buf_is_peer);
+            w.pf_dist = src_dev ? g_prefetch : -1;
             if (a.inline_desc) {
                 InlineDesc d;   // unused tail entries are never indexed (run < n_runs)
                 std::memcpy(d.runs, a.runs, static_cast<size_t>(a.n_runs) * sizeof(RunDesc));

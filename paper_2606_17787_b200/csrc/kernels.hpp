@@ -32,6 +32,7 @@ struct CopyArgs {
     int32_t plane_base = 0;          // absolute index of planes[0] (a launch over a plane sub-range)
     void* buf = nullptr;             // device-accessible checkpoint buffer
     bool buf_is_host = false;        // mapped pinned host memory
+    bool buf_is_peer = false;        // another GPU's memory (peer mapped): never prefetched early
     bool pack = true;                // true: planes -> buf, false: buf -> planes
     int kernel = kKernelAuto;
     cudaStream_t stream = nullptr;

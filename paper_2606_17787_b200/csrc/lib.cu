@@ -189,7 +189,7 @@ int gather_planes(const lumen_kv_plan* plan, const void* const* k_planes,
 
 int launch_part(const lumen_kv_plan* plan, const std::vector<const void*>& planes, uintptr_t buf,
                 bool buf_is_host, cudaStream_t stream, bool pack, int64_t ra, int64_t rb,
-                int32_t p0, int32_t p1) {
+                int32_t p0, int32_t p1, bool buf_is_peer) {
     if (rb <= ra || p1 <= p0) return LUMEN_KV_OK;
     CopyArgs a;
     a.inline_desc = plan->inline_desc;
@@ -205,6 +205,7 @@ int launch_part(const lumen_kv_plan* plan, const std::vector<const void*>& plane
     a.plane_base = p0;
     a.buf = reinterpret_cast<void*>(buf);
     a.buf_is_host = buf_is_host;
+    a.buf_is_peer = buf_is_peer;
     a.pack = pack;
     a.kernel = static_cast<int>((plan->flags & LUMEN_KV_KERNEL_MASK) >> LUMEN_KV_KERNEL_SHIFT);
     a.stream = stream;
@@ -246,7 +247,9 @@ int run_copy(const lumen_kv_plan* plan, const void* const* k_planes, const void*
              void* buf, int64_t buf_bytes, int kind, void* stream, bool pack) {
     if (!plan) return LUMEN_KV_EINVAL;
     if (plan->flags & LUMEN_KV_HOST_ONLY) return LUMEN_KV_EINVAL;
-    if (kind != LUMEN_KV_MEM_DEVICE && kind != LUMEN_KV_MEM_HOST_MAPPED) return LUMEN_KV_EINVAL;
+    if (kind != LUMEN_KV_MEM_DEVICE && kind != LUMEN_KV_MEM_HOST_MAPPED &&
+        kind != LUMEN_KV_MEM_DEVICE_PEER)
+        return LUMEN_KV_EINVAL;
     if (buf_bytes < plan->hp.total_bytes) return LUMEN_KV_ESIZE;
     if (plan->hp.total_bytes == 0) return LUMEN_KV_OK;  // A4: empty plan launches nothing
     if (!buf) return LUMEN_KV_EINVAL;
@@ -266,7 +269,8 @@ int run_copy(const lumen_kv_plan* plan, const void* const* k_planes, const void*
     if (reinterpret_cast<uintptr_t>(dev_buf) & 15) return LUMEN_KV_EINVAL;
     return launch_part(plan, planes, reinterpret_cast<uintptr_t>(dev_buf),
                        kind == LUMEN_KV_MEM_HOST_MAPPED, static_cast<cudaStream_t>(stream), pack, 0,
-                       plan->n_runs, 0, 2 * plan->hp.geom.num_layers);
+                       plan->n_runs, 0, 2 * plan->hp.geom.num_layers,
+                       kind == LUMEN_KV_MEM_DEVICE_PEER);
 }
 
 }  // namespace

@@ -741,3 +741,55 @@ def test_cuda_graph_capture(G, kernel):
         assert np.array_equal(G.plane_to_np(t), r)
     del g
     plan.close(); rplan.close()
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("kernel", ["warp", "warp_upload"])
+def test_l2_prefetch_is_only_a_hint(G, kernel):
+    """The SIMT kernel asks L2 for source bytes ahead of the stream-order wait (option
+    "prefetch": -1 off, 0 own task, d > 0 the task d CTAs further on).  Whatever the distance,
+    the bytes are the oracle's -- also when fill -> pack -> restore -> pack run back to back on
+    one stream with no host synchronisation in between, so that every kernel's early prefetch
+    meets the previous kernel's stores (the buffers are reused with new content every round:
+    a stale line would show)."""
+    import torch
+    lk = G.lk
+    w = cfg1_qwen14b(L=3, N=2048, n_reqs=24, grow_iters=2, median=200, hi=512, lo=20)
+    flags = G.KERNELS[kernel]
+    pool_a, pool_b = G.make_pool(w.geom, 7), G.make_pool(w.geom, 8)
+    ck_a, ck_b = G.Checkpointer(pool_a, flags), G.Checkpointer(pool_b, flags)
+    plan, rplan = ck_a.plan(w.reqs), ck_b.plan(w.restore_reqs, unique_dst=True)
+    whole, buf = G.alloc_buffer(plan.nbytes, "device")
+    whole2, buf2 = G.alloc_buffer(plan.nbytes, "device")
+    try:
+        for rnd, dist in enumerate([-1, 0, 1, 16, 37, 1000, 10 ** 6, 16, 16, 16]):
+            lk.lumen_kv_set_option("prefetch", dist)
+            seed = 100 + rnd
+            for i, t in enumerate(pool_a.planes()):
+                G.wdev.fill_plane(t, seed, i, torch.cuda.current_stream().cuda_stream)
+            ck_a.pack(plan, buf)
+            ck_b.unpack(rplan, buf)
+            ck_b.pack(rplan, buf2)
+            torch.cuda.synchronize()
+            K, V = G.host_planes(w.geom, seed)
+            B_ref = oracle.pack(w.geom, K, V, w.reqs)
+            assert np.array_equal(G.buf_to_np(buf, plan.nbytes), B_ref), dist
+            assert np.array_equal(G.buf_to_np(buf2, plan.nbytes), B_ref), dist
+            assert G.guards_intact(whole, plan.nbytes) and G.guards_intact(whole2, plan.nbytes)
+    finally:
+        lk.lumen_kv_set_option("prefetch", 16)
+    # a buffer declared as peer memory takes the same kernels (no early prefetch of it)
+    B = lk.binding
+    s = torch.cuda.current_stream().cuda_stream
+    buf.zero_()
+    B.lumen_kv_checkpoint_pack(plan, pool_a.k_ptrs, pool_a.v_ptrs, buf.data_ptr(), plan.nbytes,
+                               lk.LUMEN_KV_MEM_DEVICE_PEER, s)
+    B.lumen_kv_restore_unpack(rplan, pool_b.k_ptrs, pool_b.v_ptrs, buf.data_ptr(), plan.nbytes,
+                              lk.LUMEN_KV_MEM_DEVICE_PEER, s)
+    ck_b.pack(rplan, buf2)
+    torch.cuda.synchronize()
+    assert np.array_equal(G.buf_to_np(buf, plan.nbytes), B_ref)
+    assert np.array_equal(G.buf_to_np(buf2, plan.nbytes), B_ref)
+    with pytest.raises(lk.LumenKVError):
+        B.lumen_kv_checkpoint_pack(plan, pool_a.k_ptrs, pool_a.v_ptrs, buf.data_ptr(), plan.nbytes, 3, s)
+    plan.close(); rplan.close()
