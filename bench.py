@@ -369,7 +369,15 @@ def run_reference(args):
     line = {"impl": "reference", "metric": "kv_pack_restore_payload_GBps", "value": val, "unit": "GB/s",
             "n_gpus": args.gpus, "steps": steps, "warmup": args.warmup, "ms_per_step": dt / timed * 1e3,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u16",
-            "data": "synthetic", "config": {"workload": label, "timed_steps": timed},
+            "data": "synthetic",
+            # same keys as the CUDA arm's `config` (what is specific to an arm sits beside it)
+            "config": {"workload": label,
+                       "payload_bytes_per_direction_per_step": int(w.tokens) * 4 * w.geom[0] * w.geom[1] * w.geom[2],
+                       "tokens_per_step": int(w.tokens),
+                       "l2": "CPU arm: every step touches far more than the host caches hold "
+                             "(the step's sample is named in cpu_baseline.sample)",
+                       "seed": hex(MASTER_SEED)},
+            "timed_steps": timed,
             "cpu_baseline": {"value": val, "unit": "GB/s", "cores": 1, "kind": "oracle",
                              "sample": f"each step = {what}; plain single-thread C oracle"},
             "e2e": {"value": val, "unit": "GB/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -982,15 +990,18 @@ def run_ours(args):
         "n_gpus": world, "steps": K, "warmup": W, "ms_per_step": ms / K,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "u16", "data": "synthetic",
+        "runs_per_plan": runs_per_plan,
         "config": {"workload": label, "payload_bytes_per_direction_per_step": P,
-                   "tokens_per_step": w.tokens, "runs_per_plan": runs_per_plan,
+                   "tokens_per_step": w.tokens,
                    "l2": ("fits in L2 (latency config, no roofline claim)" if args.workload == "cfg0" else
                           f"inputs larger than L2: steps rotate over {n_stage} staging buffers of "
                           f"{P / 2**20:.0f} MiB and {len(ranges)} distinct delta sets; the restore reads "
                           f"the buffer packed {lag} steps earlier"),
-                   "kernel": args.kernel, "replicas": world,
-                   "descriptors": "uploaded" if args.upload_descriptors else "kernel parameters (plans <= 256 runs)",
-                   "pdl": os.environ.get("LUMEN_KV_PDL", "1") != "0", "seed": hex(MASTER_SEED)},
+                   "seed": hex(MASTER_SEED)},
+        "launch_config": {"kernel": args.kernel, "replicas": world,
+                          "descriptors": "uploaded" if args.upload_descriptors else "kernel parameters (plans <= 256 runs)",
+                          "pdl": os.environ.get("LUMEN_KV_PDL", "1") != "0",
+                          "l2_prefetch": int(os.environ.get("LUMEN_KV_PREFETCH", "16"))},
         "tokens_per_s": value * 1e9 / token_bytes,
         "wall_ms_per_step": wall_ms / K, "host_enqueue_ms_per_step": host_ms / K,
         "host_bound": bool(host_bound), "headline_attempts": attempts,
@@ -1853,6 +1864,8 @@ def run_dram(args):
         "probe_read_only": timed("probe_read", lambda: wdev.dram_probe("read", a_, b_, NB, s.cuda_stream), NB),
         "probe_write_only": timed("probe_write", lambda: wdev.dram_probe("write", a_, b_, NB, s.cuda_stream), NB),
         "probe_copy": timed("probe_copy", lambda: wdev.dram_probe("copy", a_, b_, NB, s.cuda_stream), 2 * NB),
+        "probe_copy_l2_prefetch_4k": timed("probe_copy_pf4k", lambda: wdev.dram_probe("copy_pf4k", a_, b_, NB, s.cuda_stream), 2 * NB),
+        "probe_copy_l2_prefetch_32k": timed("probe_copy_pf32k", lambda: wdev.dram_probe("copy_pf32k", a_, b_, NB, s.cuda_stream), 2 * NB),
         "torch_copy_": timed("torch_copy", lambda: b_.copy_(a_), 2 * NB),
     }
     del a_, b_

@@ -117,21 +117,54 @@ __device__ __forceinline__ Item decode_item(const Desc& desc, int64_t run,
 }
 
 // ---------------------------------------------------------------------------------
-// SIMT kernel: one warp per (run, plane, sub-chunk)
+// SIMT kernels: one warp per (run, plane, sub-chunk)
 //
-// A task is UNROLL*512 bytes of one item: every lane issues its UNROLL independent
-// 16-byte loads, then its UNROLL stores, and the warp retires -- no loop.  Items are
-// cut into 2^sub_shift sub-chunks so that a 64 x 16-token decode delta (about 8,000
-// items of 32 KiB) becomes tens of thousands of equal tasks: the grid has no tail wave,
-// and consecutive warps of a CTA stream consecutive sub-chunks of the same run.
+// A task is UNROLL * 32 lanes * VB bytes of one item (VB = bytes per access): every lane
+// issues its UNROLL independent loads, then its UNROLL stores, and the warp retires -- no
+// loop.  Items are cut into 2^sub_shift sub-chunks so that a 64 x 16-token decode delta
+// (about 8,000 items of 32 KiB) becomes tens of thousands of equal tasks: the grid has no
+// tail wave, and consecutive warps of a CTA stream consecutive sub-chunks of the same run.
+//   kv_copy_warp32 : VB = 32, the default whenever every address is a multiple of 32: sm_100
+//                    has 256-bit global loads / stores (LDG.E.256 / STG.E.256); 4 KiB per task,
+//                    half the CTAs and half the memory instructions per byte of the 16-byte
+//                    form: +1.7 % on cfg 1, +2 % on cfg 4.  An
+//                    L2::evict_first priority on both sides was measured too: no gain.
+//   kv_copy_warp   : VB = 16 (LDG/STG.E.128), rows / strides / buffers that are only 16-byte
+//                    aligned.
 // ---------------------------------------------------------------------------------
 constexpr int kWarpsPerCta = 8;
 
-template <int UNROLL, class Desc>
-__global__ void __launch_bounds__(kWarpsPerCta * 32)
-kv_copy_warp(const __grid_constant__ PlaneTable planes, const __grid_constant__ Desc desc,
-             int64_t n_runs, char* buf, uint32_t row_bytes, int32_t plane0, int sub_shift,
-             int pack) {
+template <int VB>
+struct Vec;
+template <>
+struct Vec<16> {
+    uint4 v;
+    __device__ __forceinline__ void load(const void* p) { v = ld_stream16(p); }
+    __device__ __forceinline__ void store(void* p) const { st_stream16(p, v); }
+};
+template <>
+struct Vec<32> {
+    uint32_t a[8];
+    __device__ __forceinline__ void load(const void* p) {
+        asm volatile("ld.global.L1::no_allocate.v8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                     : "=r"(a[0]), "=r"(a[1]), "=r"(a[2]), "=r"(a[3]), "=r"(a[4]), "=r"(a[5]),
+                       "=r"(a[6]), "=r"(a[7])
+                     : "l"(p)
+                     : "memory");
+    }
+    __device__ __forceinline__ void store(void* p) const {
+        asm volatile("st.global.L1::no_allocate.v8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"l"(p),
+                     "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(a[4]), "r"(a[5]), "r"(a[6]),
+                     "r"(a[7])
+                     : "memory");
+    }
+};
+
+template <int VB, int UNROLL, class Desc>
+__device__ __forceinline__ void warp_task(const PlaneTable& planes, const Desc& desc, int64_t n_runs,
+                                          char* buf, uint32_t row_bytes, int32_t plane0,
+                                          int sub_shift, int pack, int32_t pf_dist) {
+    constexpr uint32_t kTask = UNROLL * 32 * VB;          // bytes per warp
     pdl_launch_dependents();
     const int lane = threadIdx.x & 31;
     const int64_t task = static_cast<int64_t>(blockIdx.x) * kWarpsPerCta + (threadIdx.x >> 5);
@@ -144,70 +177,16 @@ kv_copy_warp(const __grid_constant__ PlaneTable planes, const __grid_constant__ 
     if (!Desc::kInline) pdl_wait();
     const Item it = decode_item(desc, run, planes.p[blockIdx.y], plane0 + blockIdx.y, buf,
                                 row_bytes);
-    if (Desc::kInline) pdl_wait();
-    const uint32_t nvec = it.bytes >> 4;
-    const uint32_t i = sub * (UNROLL * 32) + lane;
-    if (sub * (UNROLL * 32) >= nvec) return;           // this run is shorter than the longest
-    const char* src = (pack ? it.pool : it.buf) + (static_cast<size_t>(i) << 4);
-    char* dst = (pack ? it.buf : it.pool) + (static_cast<size_t>(i) << 4);
-
-    uint4 v[UNROLL];
-#pragma unroll
-    for (int u = 0; u < UNROLL; ++u)
-        if (i + u * 32 < nvec) v[u] = ld_stream16(src + u * 512);
-#pragma unroll
-    for (int u = 0; u < UNROLL; ++u)
-        if (i + u * 32 < nvec) st_stream16(dst + u * 512, v[u]);
-}
-
-// 32-byte variant, the default whenever every address is a multiple of 32: sm_100 has 256-bit
-// global loads / stores (LDG.E.256 / STG.E.256).  A task is UNROLL * 1 KiB = 4 KiB per warp, so
-// half the CTAs and half the memory instructions per byte: +1.7 % on cfg 1, +2 % on cfg 4
-// (DESIGN.md section 6.1).  An L2::evict_first priority on both sides was measured too: no gain.
-struct V8 {
-    uint32_t a[8];
-};
-__device__ __forceinline__ V8 ld_stream32(const void* p) {
-    V8 v;
-    asm volatile("ld.global.L1::no_allocate.v8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
-                 : "=r"(v.a[0]), "=r"(v.a[1]), "=r"(v.a[2]), "=r"(v.a[3]), "=r"(v.a[4]),
-                   "=r"(v.a[5]), "=r"(v.a[6]), "=r"(v.a[7])
-                 : "l"(p)
-                 : "memory");
-    return v;
-}
-__device__ __forceinline__ void st_stream32(void* p, const V8& v) {
-    asm volatile("st.global.L1::no_allocate.v8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"l"(p),
-                 "r"(v.a[0]), "r"(v.a[1]), "r"(v.a[2]), "r"(v.a[3]), "r"(v.a[4]), "r"(v.a[5]),
-                 "r"(v.a[6]), "r"(v.a[7])
-                 : "memory");
-}
-
-template <int UNROLL, class Desc>
-__global__ void __launch_bounds__(kWarpsPerCta * 32)
-kv_copy_warp32(const __grid_constant__ PlaneTable planes, const __grid_constant__ Desc desc,
-               int64_t n_runs, char* buf, uint32_t row_bytes, int32_t plane0, int sub_shift,
-               int pack, int32_t pf_dist) {
-    pdl_launch_dependents();
-    const int lane = threadIdx.x & 31;
-    const int64_t task = static_cast<int64_t>(blockIdx.x) * kWarpsPerCta + (threadIdx.x >> 5);
-    const int64_t run = task >> sub_shift;
-    if (run >= n_runs) return;
-    const uint32_t sub = static_cast<uint32_t>(task & ((int64_t{1} << sub_shift) - 1));
-    if (!Desc::kInline) pdl_wait();
-    const Item it = decode_item(desc, run, planes.p[blockIdx.y], plane0 + blockIdx.y, buf,
-                                row_bytes);
-    const uint32_t nvec = it.bytes >> 5;
-    // L2 prefetch (pf_dist >= 0): one lane asks L2 for the 4 KiB source of the task that the warp
+    // L2 prefetch (pf_dist >= 0): one lane asks L2 for the source of the task that the warp
     // pf_dist CTAs further on will copy (0: its own).  L2 is the device's point of coherence, so
     // a line fetched early still shows every store that reaches L2 before the later load; that
     // makes it legal in front of the wait, where the CTAs of the first wave -- resident while the
     // previous grid's last wave drains -- would otherwise sit with nothing in flight.
-    const char* const src0 = (pack ? it.pool : it.buf) + static_cast<size_t>(sub) * (UNROLL * 1024);
-    const bool live = sub * (UNROLL * 32) < nvec;
+    const bool live = sub * kTask < it.bytes;              // else: this run is shorter than the longest
+    const char* const src0 = (pack ? it.pool : it.buf) + static_cast<size_t>(sub) * kTask;
     auto prefetch_own = [&] {
-        const uint32_t left = it.bytes - sub * (UNROLL * 1024);
-        if (live) l2_prefetch_bulk(src0, left < UNROLL * 1024 ? left : UNROLL * 1024);
+        const uint32_t left = it.bytes - sub * kTask;
+        if (live) l2_prefetch_bulk(src0, left < kTask ? left : kTask);
     };
     auto prefetch_ahead = [&] {
         const uint64_t lin = static_cast<uint64_t>(blockIdx.y) * gridDim.x + blockIdx.x + pf_dist;
@@ -218,16 +197,17 @@ kv_copy_warp32(const __grid_constant__ PlaneTable planes, const __grid_constant_
         if (by >= gridDim.y || run2 >= n_runs) return;
         const uint32_t sub2 = static_cast<uint32_t>(task2 & ((int64_t{1} << sub_shift) - 1));
         const Item it2 = decode_item(desc, run2, planes.p[by], plane0 + by, buf, row_bytes);
-        if (sub2 * (UNROLL * 1024) >= it2.bytes) return;
-        const uint32_t left = it2.bytes - sub2 * (UNROLL * 1024);
-        l2_prefetch_bulk((pack ? it2.pool : it2.buf) + static_cast<size_t>(sub2) * (UNROLL * 1024),
-                         left < UNROLL * 1024 ? left : UNROLL * 1024);
+        if (sub2 * kTask >= it2.bytes) return;
+        const uint32_t left = it2.bytes - sub2 * kTask;
+        l2_prefetch_bulk((pack ? it2.pool : it2.buf) + static_cast<size_t>(sub2) * kTask,
+                         left < kTask ? left : kTask);
     };
+    // (one 32 KiB prefetch per CTA instead of 4 KiB per warp was measured as well: no difference)
     const bool leader = pf_dist >= 0 && lane == 0;
     if (Desc::kInline) {
         if (leader) {
-            if (static_cast<uint64_t>(blockIdx.y) * gridDim.x + blockIdx.x <
-                static_cast<uint32_t>(pf_dist) || pf_dist == 0)
+            if (pf_dist == 0 || static_cast<uint64_t>(blockIdx.y) * gridDim.x + blockIdx.x <
+                                    static_cast<uint32_t>(pf_dist))
                 prefetch_own();
             if (pf_dist > 0) prefetch_ahead();
         }
@@ -235,20 +215,37 @@ kv_copy_warp32(const __grid_constant__ PlaneTable planes, const __grid_constant_
     } else if (leader) {
         // descriptors in global memory: decoding the task ahead would cost two more dependent
         // loads (and, placed behind this warp's own loads, the registers of a fifth CTA per SM:
-        // measured, cfg 2 -3 %), so such plans only announce their own 4 KiB
+        // measured, cfg 2 -3 %), so such plans only announce their own task
         prefetch_own();
     }
     if (!live) return;
+    const uint32_t nvec = it.bytes / VB;
     const uint32_t i = sub * (UNROLL * 32) + lane;
-    const char* src = src0 + (static_cast<size_t>(lane) << 5);
-    char* dst = (pack ? it.buf : it.pool) + (static_cast<size_t>(i) << 5);
-    V8 v[UNROLL];
+    const char* src = src0 + static_cast<size_t>(lane) * VB;
+    char* dst = (pack ? it.buf : it.pool) + static_cast<size_t>(i) * VB;
+    Vec<VB> v[UNROLL];
 #pragma unroll
     for (int u = 0; u < UNROLL; ++u)
-        if (i + u * 32 < nvec) v[u] = ld_stream32(src + u * 1024);
+        if (i + u * 32 < nvec) v[u].load(src + u * (32 * VB));
 #pragma unroll
     for (int u = 0; u < UNROLL; ++u)
-        if (i + u * 32 < nvec) st_stream32(dst + u * 1024, v[u]);
+        if (i + u * 32 < nvec) v[u].store(dst + u * (32 * VB));
+}
+
+template <int UNROLL, class Desc>
+__global__ void __launch_bounds__(kWarpsPerCta * 32)
+kv_copy_warp(const __grid_constant__ PlaneTable planes, const __grid_constant__ Desc desc,
+             int64_t n_runs, char* buf, uint32_t row_bytes, int32_t plane0, int sub_shift,
+             int pack, int32_t pf_dist) {
+    warp_task<16, UNROLL>(planes, desc, n_runs, buf, row_bytes, plane0, sub_shift, pack, pf_dist);
+}
+
+template <int UNROLL, class Desc>
+__global__ void __launch_bounds__(kWarpsPerCta * 32)
+kv_copy_warp32(const __grid_constant__ PlaneTable planes, const __grid_constant__ Desc desc,
+               int64_t n_runs, char* buf, uint32_t row_bytes, int32_t plane0, int sub_shift,
+               int pack, int32_t pf_dist) {
+    warp_task<32, UNROLL>(planes, desc, n_runs, buf, row_bytes, plane0, sub_shift, pack, pf_dist);
 }
 
 // ---------------------------------------------------------------------------------
@@ -486,7 +483,7 @@ cudaError_t launch_warp(const PlaneTable& pt, const Desc& d, const WarpLaunch& w
     cfg.attrs = attr;
     cfg.numAttrs = g_pdl ? 1 : 0;
     return cudaLaunchKernelEx(&cfg, kv_copy_warp<UNROLL, Desc>, pt, d, w.n_runs, w.buf,
-                              w.row_bytes, w.plane0, w.sub_shift, w.pack);
+                              w.row_bytes, w.plane0, w.sub_shift, w.pack, w.pf_dist);
 }
 
 // CUDA loads a kernel lazily at its first launch, and that load can wait for kernels that are
@@ -640,7 +637,8 @@ cudaError_t launch_kv_copy(const CopyArgs& a) {
             // only this device's own memory is cached coherently in its L2: a source in host
             // memory or in a peer GPU's memory is never asked for ahead of the wait
             const bool src_dev = a.pack || !(a.buf_is_host || a.buf_is_peer);
-            w.pf_dist = src_dev ? g_prefetch : -1;
+            // the 16-byte kernel (2 KiB tasks, twice the CTAs) loses with it: cfg 1 3,169 -> 3,101 GB/s
+            w.pf_dist = (src_dev && wide) ? g_prefetch : -1;
             if (a.inline_desc) {
                 InlineDesc d;   // unused tail entries are never indexed (run < n_runs)
                 std::memcpy(d.runs, a.runs, static_cast<size_t>(a.n_runs) * sizeof(RunDesc));

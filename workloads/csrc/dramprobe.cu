@@ -33,12 +33,22 @@ constexpr int kWarps = 8;      // per CTA
 constexpr int kTask = 4096;    // bytes per warp task
 
 // mode 0: read, 1: write, 2: copy.  One warp per 4 KiB task, no loop (the library's shape).
+// pf_span > 0 (copy only): the task is announced to L2 first with one cp.async.bulk.prefetch.L2
+// of pf_span bytes -- 4096: every warp its own task, 32768: warp 0 the whole CTA's.
 template <int MODE>
 __global__ void __launch_bounds__(kWarps * 32)
-probe_kernel(const char* __restrict__ src, char* __restrict__ dst, int64_t n_tasks, uint32_t* sink) {
+probe_kernel(const char* __restrict__ src, char* __restrict__ dst, int64_t n_tasks, uint32_t* sink,
+             uint32_t pf_span) {
     const int lane = threadIdx.x & 31;
     const int64_t task = static_cast<int64_t>(blockIdx.x) * kWarps + (threadIdx.x >> 5);
     if (task >= n_tasks) return;
+    if (MODE == 2 && pf_span && lane == 0 && (pf_span <= kTask || (threadIdx.x >> 5) == 0)) {
+        const int64_t left = (n_tasks - task) * kTask;
+        const uint32_t n = left < pf_span ? static_cast<uint32_t>(left) : pf_span;
+        asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src + static_cast<size_t>(task) * kTask),
+                     "r"(n)
+                     : "memory");
+    }
     const size_t off = static_cast<size_t>(task) * kTask + static_cast<size_t>(lane) * 32;
     V8 v[4];
     if (MODE != 1) {
@@ -67,7 +77,8 @@ probe_kernel(const char* __restrict__ src, char* __restrict__ dst, int64_t n_tas
 
 extern "C" {
 
-// mode: 0 read src, 1 write dst, 2 copy src -> dst; nbytes % 4096 == 0; 32-byte aligned.
+// mode: 0 read src, 1 write dst, 2 copy src -> dst, 3 copy with a 4 KiB L2 prefetch per warp,
+// 4 copy with a 32 KiB L2 prefetch per CTA; nbytes % 4096 == 0; 32-byte aligned.
 __attribute__((visibility("default")))
 int dramprobe_run(int mode, const void* src, void* dst, int64_t nbytes, void* sink, void* stream) {
     if (nbytes <= 0 || nbytes % kTask) return -1;
@@ -79,9 +90,11 @@ int dramprobe_run(int mode, const void* src, void* dst, int64_t nbytes, void* si
     const char* a = static_cast<const char*>(src);
     char* b = static_cast<char*>(dst);
     uint32_t* k = static_cast<uint32_t*>(sink);
-    if (mode == 0) probe_kernel<0><<<static_cast<unsigned>(grid), kWarps * 32, 0, s>>>(a, b, n_tasks, k);
-    else if (mode == 1) probe_kernel<1><<<static_cast<unsigned>(grid), kWarps * 32, 0, s>>>(a, b, n_tasks, k);
-    else if (mode == 2) probe_kernel<2><<<static_cast<unsigned>(grid), kWarps * 32, 0, s>>>(a, b, n_tasks, k);
+    if (mode == 0) probe_kernel<0><<<static_cast<unsigned>(grid), kWarps * 32, 0, s>>>(a, b, n_tasks, k, 0u);
+    else if (mode == 1) probe_kernel<1><<<static_cast<unsigned>(grid), kWarps * 32, 0, s>>>(a, b, n_tasks, k, 0u);
+    else if (mode == 2) probe_kernel<2><<<static_cast<unsigned>(grid), kWarps * 32, 0, s>>>(a, b, n_tasks, k, 0u);
+    else if (mode == 3) probe_kernel<2><<<static_cast<unsigned>(grid), kWarps * 32, 0, s>>>(a, b, n_tasks, k, 4096u);
+    else if (mode == 4) probe_kernel<2><<<static_cast<unsigned>(grid), kWarps * 32, 0, s>>>(a, b, n_tasks, k, 32768u);
     else return -1;
     return cudaGetLastError() == cudaSuccess ? 0 : -2;
 }
