@@ -43,6 +43,13 @@
  *     the heap either.  Results are complete (and, for host destinations,
  *     host-visible) once an event recorded on that stream after the call has fired
  *     (nothing is promised earlier).
+ *   - Consecutive launches overlap at their edges (programmatic dependent launch): a
+ *     kernel's CTAs become resident while the previous kernel's last wave drains and,
+ *     before they wait for it to complete, ask L2 for the source bytes they will copy
+ *     (cp.async.bulk.prefetch.L2 -- a hint; the loads themselves come after the wait).
+ *     L2 is the point of coherence of a device's OWN memory only, which is why a buffer
+ *     in another GPU's memory must be declared LUMEN_KV_MEM_DEVICE_PEER (and pools are
+ *     always local): such a source, like a pinned host one, is never asked for early.
  *   - One-time cost: the first launch on a device loads every kernel variant and sets
  *     its shared-memory limit (about twenty cudaFuncGetAttributes / cudaFuncSetAttribute
  *     calls; a lazily loaded kernel can otherwise wait for kernels that are already

@@ -196,15 +196,22 @@ def test_cfg2_full_size(G, where):
         ring.stager.sync(G.lk.lumen_kv_checkpoint_pack_staged_async(
             warm, pool.k_ptrs, pool.v_ptrs, buf.data_ptr(), warm.nbytes, ring.stager, st))
         warm.close()
-        t0 = time.perf_counter()
-        ticket = G.lk.lumen_kv_checkpoint_pack_staged_async(plan, pool.k_ptrs, pool.v_ptrs, buf.data_ptr(),
-                                                           plan.nbytes, ring.stager, st)
-        call_ms = (time.perf_counter() - t0) * 1e3
-        in_flight = not ring.stager.query(ticket)
-        ring.stager.sync(ticket)
-        total_ms = (time.perf_counter() - t0) * 1e3
-        assert call_ms < 1.0, f"async staged call took {call_ms:.3f} ms on the calling thread"
-        assert in_flight and total_ms > 300, (in_flight, total_ms)
+        # a host thread can be descheduled for a millisecond on a busy box: the claim is about
+        # the call, so it gets up to three tries (each repeats the whole 32 GiB transfer)
+        calls = []
+        for _ in range(3):
+            t0 = time.perf_counter()
+            ticket = G.lk.lumen_kv_checkpoint_pack_staged_async(plan, pool.k_ptrs, pool.v_ptrs, buf.data_ptr(),
+                                                               plan.nbytes, ring.stager, st)
+            call_ms = (time.perf_counter() - t0) * 1e3
+            in_flight = not ring.stager.query(ticket)
+            ring.stager.sync(ticket)
+            total_ms = (time.perf_counter() - t0) * 1e3
+            calls.append(call_ms)
+            assert in_flight and total_ms > 300, (in_flight, total_ms)
+            if call_ms < 1.0:
+                break
+        assert min(calls) < 1.0, f"async staged call took {calls} ms on the calling thread"
         assert ring.stager.query(ticket)
     else:
         ck.pack(plan, buf)
