@@ -708,6 +708,8 @@ def large_config(torch, lk, name, seed, kflag, stream, sampler, peak, link, with
            "pack_ms": pack_ms, "unpack_ms": unpack_ms,
            "achieved_GBps": 2 * P / dom_ms / 1e6, "peak_GBps": peak, "frac": 2 * P / dom_ms / 1e6 / peak,
            "frac_formula": "2 * payload_bytes_per_direction / max(pack_ms, unpack_ms) / peak_GBps",
+           "frac_of_spec_8TBps": 2 * P / dom_ms / 1e6 / 8000.0,
+           "frac_of_pin_rate_8184GBps": 2 * P / dom_ms / 1e6 / 8184.0,
            "host_enqueue_ms_per_step": host_ms / 3,
            "timing": "3 warm-up + 3 timed steps between one event pair; pack_ms / unpack_ms = 3 launches of "
                      "that direction alone between one event pair; inputs larger than L2 (tens of GiB per launch)"}
@@ -855,6 +857,9 @@ def run_ours(args):
                 "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                 "traffic": traffic, "traffic_source": traffic_src,
                 "algorithmic_bytes_per_launch": 2 * P, "peak_source": peak_src,
+                # also against the data-sheet figure ("spec", 8 TB/s HBM3e) and against
+                # the pin rate ncu reports for this part (2,048 B/cycle x 3.996 GHz)
+                "frac_of_spec_8TBps": achieved / 8000.0, "frac_of_pin_rate_8184GBps": achieved / 8184.0,
                 "timing": (f"average launch duration = one CUDA-event pair around {Kk} back-to-back launches "
                            "of that direction alone (same plans and buffer rotation as the step), on the "
                            "launching stream, in this run; *_single_ms = one event pair per launch inside "
