@@ -24,7 +24,8 @@
  *
  * The result is exact (a permutation of 16-bit words); parity with the CUDA
  * path is bit-for-bit.  Pins: tests/test_oracle_pins.py (P1-P10 of SURVEY.md
- * section 8(c) C7).  No function here is "parity unpinned".
+ * section 8(c) C7) and tests/test_golden_pack.py (P11: the hand-worked example
+ * tests/golden/pack_tiny.txt).  No function here is "parity unpinned".
  *
  * lumen_oracle_pack_omp / lumen_oracle_unpack_omp are the same loop nest with
  * an OpenMP pragma over (request, layer) and a row memcpy innermost.  They
