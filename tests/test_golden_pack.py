@@ -16,7 +16,7 @@ GOLDEN = Path(__file__).resolve().parent / "golden" / "pack_tiny.txt"
 
 
 def load_golden():
-    g = {"req": [], "run": [], "row": {}, "restore_req": [], "placed": []}
+    g = {"req": [], "run": [], "row": {}, "restore_req": [], "placed": [], "layout": [], "at": []}
     for line in GOLDEN.read_text().splitlines():
         line = line.split("#")[0].strip()
         if not line:
@@ -27,8 +27,12 @@ def load_golden():
             g["geom"] = tuple(parts[0])
         elif key == "fill":
             g["fill"] = tuple(parts[0])
-        elif key == "restore_fill":
-            g["restore_fill"] = parts[0][0]
+        elif key in ("restore_fill", "layout_fill", "layout_extent_bytes"):
+            g[key] = parts[0][0]
+        elif key == "layout":
+            g["layout"].append((parts[1][0], parts[1][1]))          # (byte offset, plane stride tokens)
+        elif key == "at":
+            g["at"].append((parts[0][0], tuple(parts[1])))
         elif key in ("req", "restore_req"):
             g[key].append((np.asarray(parts[1], dtype=np.int32), parts[2][0], parts[2][1]))
         elif key == "run":
@@ -65,6 +69,15 @@ def golden_buffer(g):
             for j in range(te - tb):
                 out.extend(g["row"][(r, p, j)])
     return np.asarray(out, dtype=np.uint16)
+
+
+def golden_layout_buffer(g):
+    """The 25-row buffer of the explicit-layout example: hand-placed rows, the fill elsewhere."""
+    E = g["geom"][1] * g["geom"][2]
+    B = np.full(g["layout_extent_bytes"] // 2, g["layout_fill"], dtype=np.uint16)
+    for at, key in g["at"]:
+        B[at * E:(at + 1) * E] = g["row"][key]
+    return B
 
 
 def golden_restored_planes(g):
@@ -105,6 +118,25 @@ def test_oracle_pack_and_unpack_equal_the_hand_worked_example(impl):
         assert np.array_equal(V2[l], want[2 * l + 1])
 
 
+@pytest.mark.parametrize("impl", ["c", "numpy"])
+def test_oracle_layout_pack_and_unpack_equal_the_hand_worked_example(impl):
+    g = load_golden()
+    mod = oracle if impl == "c" else oracle_np
+    L, H, D, S, N = g["geom"]
+    K, V = source_planes(g)
+    lay = [(off // 2, stride) for off, stride in g["layout"]]      # the oracles take element offsets
+    B = np.full(g["layout_extent_bytes"] // 2, g["layout_fill"], dtype=np.uint16)
+    mod.pack_layout(g["geom"], K, V, g["req"], lay, B)
+    assert np.array_equal(B, golden_layout_buffer(g))
+    K2 = [np.full(N * S * H * D, g["restore_fill"], dtype=np.uint16) for _ in range(L)]
+    V2 = [np.full(N * S * H * D, g["restore_fill"], dtype=np.uint16) for _ in range(L)]
+    mod.unpack_layout(g["geom"], K2, V2, g["restore_req"], lay, golden_layout_buffer(g))
+    want = golden_restored_planes(g)
+    for l in range(L):
+        assert np.array_equal(K2[l], want[2 * l])
+        assert np.array_equal(V2[l], want[2 * l + 1])
+
+
 def test_plan_builder_produces_the_hand_worked_runs():
     from paper_2606_17787_b200 import build
     build.build()
@@ -119,6 +151,11 @@ def test_plan_builder_produces_the_hand_worked_runs():
         r = plan.run(i)
         got.append((r.req, r.src_slot, r.dst_token, r.count))
     assert got == g["run"]
+    plan.close()
+    plan = lk.lumen_kv_plan_build(lk.make_geom(L, H, D, S, N), g["req"], lk.LUMEN_KV_HOST_ONLY,
+                                  layouts=g["layout"])
+    assert plan.nbytes == g["layout_extent_bytes"]
+    assert [plan.req_offset(r) for r in range(3)] == [32, 288, 400]
     plan.close()
 
 
@@ -163,3 +200,35 @@ def test_cuda_path_equals_the_hand_worked_example(kernel, where):
     if ring:
         ring.close()
     G.release(whole)
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("kernel", ["warp", "warp_upload", "bulk"])
+def test_cuda_layout_path_equals_the_hand_worked_example(kernel):
+    import torch
+    from tests import gpu_util as G
+    G.build_all()
+    g = load_golden()
+    L, H, D, S, N = g["geom"]
+    K, V = source_planes(g)
+    pool_a, pool_b = G.KVPool(L, H, D, S, N), G.KVPool(L, H, D, S, N)
+    for t, a in zip(pool_a.planes(), [x for kv in zip(K, V) for x in kv]):
+        t.view(torch.int16).reshape(-1).copy_(torch.from_numpy(a.view(np.int16)))
+    for t in pool_b.planes():
+        t.view(torch.int16).fill_(g["restore_fill"])
+    flags = G.KERNELS[kernel]
+    ck_a, ck_b = G.Checkpointer(pool_a, flags), G.Checkpointer(pool_b, flags)
+    plan = ck_a.plan(g["req"], layouts=g["layout"])
+    rplan = ck_b.plan(g["restore_req"], unique_dst=True, layouts=g["layout"])
+    assert plan.nbytes == g["layout_extent_bytes"]
+    whole, buf = G.alloc_buffer(plan.nbytes, "device")
+    buf.view(torch.int16).fill_(g["layout_fill"])
+    ck_a.pack(plan, buf)
+    torch.cuda.synchronize()
+    assert np.array_equal(G.buf_to_np(buf, plan.nbytes), golden_layout_buffer(g))
+    assert G.guards_intact(whole, plan.nbytes)
+    ck_b.unpack(rplan, buf)
+    torch.cuda.synchronize()
+    for t, want in zip(pool_b.planes(), golden_restored_planes(g)):
+        assert np.array_equal(G.plane_to_np(t), want)
+    plan.close(); rplan.close()
