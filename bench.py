@@ -1871,6 +1871,8 @@ def run_dram(args):
         "probe_copy": timed("probe_copy", lambda: wdev.dram_probe("copy", a_, b_, NB, s.cuda_stream), 2 * NB),
         "probe_copy_l2_prefetch_4k": timed("probe_copy_pf4k", lambda: wdev.dram_probe("copy_pf4k", a_, b_, NB, s.cuda_stream), 2 * NB),
         "probe_copy_l2_prefetch_32k": timed("probe_copy_pf32k", lambda: wdev.dram_probe("copy_pf32k", a_, b_, NB, s.cuda_stream), 2 * NB),
+        "probe_copy_5_ctas_per_sm": timed("probe_copy_5cta", lambda: wdev.dram_probe("copy_5cta", a_, b_, NB, s.cuda_stream), 2 * NB),
+        "probe_copy_4_ctas_per_sm": timed("probe_copy_4cta", lambda: wdev.dram_probe("copy_4cta", a_, b_, NB, s.cuda_stream), 2 * NB),
         "torch_copy_": timed("torch_copy", lambda: b_.copy_(a_), 2 * NB),
     }
     del a_, b_
