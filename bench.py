@@ -49,17 +49,29 @@ def parse_args():
     ap.add_argument("--kernel", choices=["auto", "warp", "bulk"], default="auto")
     ap.add_argument("--upload-descriptors", action="store_true",
                     help="LUMEN_KV_NO_INLINE: upload small plans to device memory too (A/B evidence)")
+    ap.add_argument("--requests", type=int, default=0,
+                    help="cfg1 only: a decode batch of this many requests instead of configs[1]'s 64 (evidence "
+                         "for the descriptor size classes; the line says VARIANT)")
+    ap.add_argument("--median", type=int, default=0, help="cfg1 only, with --requests: lognormal median")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-large", action="store_true",
                     help="default run only: skip the large_configs block (cfg2 + cfg4 wave 0)")
     ap.add_argument("--e2e-steps", type=int, default=0, help="default: min(steps, 100)")
-    return ap.parse_args()
+    args = ap.parse_args()
+    if args.requests:
+        CFG1_VARIANT["n_reqs"] = args.requests
+        if args.median:
+            CFG1_VARIANT["median"] = args.median
+    return args
 
 
 # ------------------------------------------------------------------------------------
 # workload construction (structure only; see workloads/gen.py)
 # ------------------------------------------------------------------------------------
+CFG1_VARIANT = {}   # --requests / --median: a larger decode batch than configs[1] names (evidence only)
+
+
 def make_workload(name: str, seed: int, pages_cap=None):
     from workloads import cfg0_tiny, cfg1_qwen14b, cfg2_qwen32b, cfg4_longctx
     if name == "cfg0":
@@ -70,10 +82,14 @@ def make_workload(name: str, seed: int, pages_cap=None):
         delta = 0
     elif name == "cfg1":
         N = 60000 if pages_cap is None else min(60000, pages_cap)
-        w = cfg1_qwen14b(seed, N=N, grow_iters=CYCLE)
+        w = cfg1_qwen14b(seed, N=N, grow_iters=CYCLE, **CFG1_VARIANT)
         label = (f"BASELINE.json configs[1]: Qwen3-14B-shaped KV (40 layers, 8 kv_heads, head_dim 128, "
                  f"bf16, page_size 16, pool {N} pages), 64 requests lognormal(median 2k, sigma 1, "
                  f"clip 128..16k), 16-token delta per request per step")
+        if CFG1_VARIANT:
+            label = (f"VARIANT of configs[1] (not the BASELINE.json workload): {CFG1_VARIANT.get('n_reqs', 64)} "
+                     f"requests, lognormal median {CFG1_VARIANT.get('median', 2048)}, otherwise as configs[1]: "
+                     f"Qwen3-14B shape, pool {N} pages, 16-token delta per request per step")
         delta = 16
     elif name == "cfg2":
         w = cfg2_qwen32b(seed)
@@ -1004,7 +1020,7 @@ def run_ours(args):
                           f"the buffer packed {lag} steps earlier"),
                    "seed": hex(MASTER_SEED)},
         "launch_config": {"kernel": args.kernel, "replicas": world,
-                          "descriptors": "uploaded" if args.upload_descriptors else "kernel parameters (plans <= 256 runs)",
+                          "descriptors": "uploaded" if args.upload_descriptors else "kernel parameters (plans <= 1,024 runs and <= 512 requests; <= 256 / 128 in the small class)",
                           "pdl": os.environ.get("LUMEN_KV_PDL", "1") != "0",
                           "l2_prefetch": int(os.environ.get("LUMEN_KV_PREFETCH", "16"))},
         "tokens_per_s": value * 1e9 / token_bytes,

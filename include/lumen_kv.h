@@ -39,7 +39,8 @@
  *     synchronise the device or a stream and never allocate device or pinned memory;
  *     the only CUDA calls besides the launch are cudaGetDevice, for a host buffer one
  *     cudaHostGetDevicePointer (a table lookup), and for a plan with uploaded
- *     descriptors one cudaEventRecord.  After a thread's first call they do not touch
+ *     descriptors one cudaEventRecord (and, until the upload has been seen complete, one
+ *     cudaEventQuery / cudaStreamWaitEvent).  After a thread's first call they do not touch
  *     the heap either.  Results are complete (and, for host destinations,
  *     host-visible) once an event recorded on that stream after the call has fired
  *     (nothing is promised earlier).
@@ -125,10 +126,12 @@ typedef struct lumen_kv_plan lumen_kv_plan;  /* opaque; library owns its descrip
 #define LUMEN_KV_HOST_ONLY           0x4u /* build descriptors on the host only (no CUDA call);
                                              such a plan can be inspected but not executed   */
 #define LUMEN_KV_NO_INLINE           0x8u /* always upload the descriptors to device memory.
-                                             By default a plan of <= 256 runs and <= 128
-                                             requests (one decode step's deltas) is carried in
-                                             the kernel parameters: no upload, no device memory,
-                                             and plan_build makes no CUDA call for it          */
+                                             By default a plan of <= 1,024 runs and <= 512
+                                             requests (a decode step's deltas, also of a large
+                                             batch) is carried in the kernel parameters -- 6 KiB
+                                             up to 256 runs / 128 requests, 24 KiB above: no
+                                             upload, no device memory, and plan_build makes no
+                                             CUDA call for it                                  */
 /* kernel selection (default 0 = library heuristic); for benchmarking / evidence   */
 #define LUMEN_KV_KERNEL_SHIFT        8
 #define LUMEN_KV_KERNEL_MASK         0xF00u
@@ -160,10 +163,14 @@ typedef struct lumen_kv_plan lumen_kv_plan;  /* opaque; library owns its descrip
  * lumen_kv_plan_build -- step a2: flatten the requests'
  * ranges into token-run descriptors and upload them.
  *   geom, reqs : host pointers, read only during the call.  num_reqs >= 0.
- *   stream     : cudaStream_t on which the descriptor upload is enqueued; the plan
- *                may be used on that stream immediately, on other streams after the
- *                caller orders them behind it.  Ignored with LUMEN_KV_HOST_ONLY and for
- *                small plans that need no upload (see LUMEN_KV_NO_INLINE).
+ *   stream     : unused (kept in the signature; pass the stream the plan will run on or
+ *                NULL).  Plans that need an upload (more than 1,024 runs or 512 requests,
+ *                or LUMEN_KV_NO_INLINE) copy their descriptors on a stream of the
+ *                library's own, so that no copy sits between two kernels of the caller's
+ *                stream; pack / unpack order themselves behind that copy on whatever
+ *                stream they are given (one cudaStreamWaitEvent, none once the copy has
+ *                been seen complete; under stream capture the call waits for it on the
+ *                host instead).
  *   out        : receives the plan; release with lumen_kv_plan_free.
  * Zero-length ranges and num_reqs == 0 are legal (A4) and yield 0 bytes.
  * Errors: EINVAL, ERANGE, EOVERLAP (with VALIDATE_UNIQUE_DST), ENOMEM, ECUDA.

@@ -73,21 +73,27 @@ struct GlobalDesc {
     const ReqDesc* reqs;
     static constexpr bool kInline = false;
 };
-struct InlineDesc {
-    RunDesc runs[kInlineRuns];
-    ReqDesc reqs[kInlineReqs];
+template <int R, int Q>
+struct InlineDescT {
+    RunDesc runs[R];
+    ReqDesc reqs[Q];
     static constexpr bool kInline = true;
 };
+using InlineDesc = InlineDescT<kInlineRuns, kInlineReqs>;      // 6 KiB: one decode step's deltas
+using InlineDescL = InlineDescT<kInlineRunsL, kInlineReqsL>;   // 24 KiB: batches of a few hundred requests
+static_assert(sizeof(PlaneTable) + sizeof(InlineDescL) + 64 <= 32764, "kernel parameter space");
 __device__ __forceinline__ uint4 load_run(const GlobalDesc& d, int64_t run) {
     return __ldg(reinterpret_cast<const uint4*>(d.runs + run));
 }
 __device__ __forceinline__ longlong2 load_req(const GlobalDesc& d, uint32_t r) {
     return __ldg(reinterpret_cast<const longlong2*>(d.reqs + r));
 }
-__device__ __forceinline__ uint4 load_run(const InlineDesc& d, int64_t run) {
+template <int R, int Q>
+__device__ __forceinline__ uint4 load_run(const InlineDescT<R, Q>& d, int64_t run) {
     return *reinterpret_cast<const uint4*>(d.runs + run);
 }
-__device__ __forceinline__ longlong2 load_req(const InlineDesc& d, uint32_t r) {
+template <int R, int Q>
+__device__ __forceinline__ longlong2 load_req(const InlineDescT<R, Q>& d, uint32_t r) {
     return *reinterpret_cast<const longlong2*>(d.reqs + r);
 }
 
@@ -409,6 +415,12 @@ int g_warp_unroll = 4;   // LUMEN_KV_WARP_UNROLL=4|8 (tuning knob, read once; 4 
 
 int g_host_ctas = 0;   // grid of the bulk kernel when the buffer is host memory (0: default)
 
+template <class D>
+void fill_inline(D& d, const CopyArgs& a) {
+    std::memcpy(d.runs, a.runs, static_cast<size_t>(a.n_runs) * sizeof(RunDesc));
+    std::memcpy(d.reqs, a.reqs, static_cast<size_t>(a.n_reqs) * sizeof(ReqDesc));
+}
+
 template <int STAGES, class Desc>
 cudaError_t launch_bulk_desc(const PlaneTable& pt, const Desc& d, const CopyArgs& a, int32_t plane0,
                              int32_t np, const BulkCfg& c, int num_sms) {
@@ -429,10 +441,14 @@ cudaError_t launch_bulk_desc(const PlaneTable& pt, const Desc& d, const CopyArgs
 template <int STAGES>
 cudaError_t launch_bulk(const PlaneTable& pt, const CopyArgs& a, int32_t plane0, int32_t np,
                         const BulkCfg& c, int num_sms) {
+    if (a.inline_desc && a.n_runs <= kInlineRuns && a.n_reqs <= kInlineReqs) {
+        InlineDesc d;   // unused tail entries are never indexed (run < n_runs)
+        fill_inline(d, a);
+        return launch_bulk_desc<STAGES>(pt, d, a, plane0, np, c, num_sms);
+    }
     if (a.inline_desc) {
-        InlineDesc d;
-        std::memcpy(d.runs, a.runs, static_cast<size_t>(a.n_runs) * sizeof(RunDesc));
-        std::memcpy(d.reqs, a.reqs, static_cast<size_t>(a.n_reqs) * sizeof(ReqDesc));
+        InlineDescL d;
+        fill_inline(d, a);
         return launch_bulk_desc<STAGES>(pt, d, a, plane0, np, c, num_sms);
     }
     return launch_bulk_desc<STAGES>(pt, GlobalDesc{a.runs, a.reqs}, a, plane0, np, c, num_sms);
@@ -501,16 +517,20 @@ cudaError_t preload(K kernel, bool big_smem) {
 template <int STAGES>
 cudaError_t preload_bulk() {
     cudaError_t e = preload(kv_copy_bulk<STAGES, GlobalDesc>, true);
-    return e != cudaSuccess ? e : preload(kv_copy_bulk<STAGES, InlineDesc>, true);
+    if (e == cudaSuccess) e = preload(kv_copy_bulk<STAGES, InlineDesc>, true);
+    return e != cudaSuccess ? e : preload(kv_copy_bulk<STAGES, InlineDescL>, true);
 }
 
 cudaError_t preload_all() {
     cudaError_t e = preload(kv_copy_warp<4, GlobalDesc>, false);
     if (e == cudaSuccess) e = preload(kv_copy_warp<4, InlineDesc>, false);
+    if (e == cudaSuccess) e = preload(kv_copy_warp<4, InlineDescL>, false);
     if (e == cudaSuccess) e = preload(kv_copy_warp<8, GlobalDesc>, false);
     if (e == cudaSuccess) e = preload(kv_copy_warp<8, InlineDesc>, false);
+    if (e == cudaSuccess) e = preload(kv_copy_warp<8, InlineDescL>, false);
     if (e == cudaSuccess) e = preload(kv_copy_warp32<4, GlobalDesc>, false);
     if (e == cudaSuccess) e = preload(kv_copy_warp32<4, InlineDesc>, false);
+    if (e == cudaSuccess) e = preload(kv_copy_warp32<4, InlineDescL>, false);
     if (e == cudaSuccess) e = preload_bulk<3>();
     if (e == cudaSuccess) e = preload_bulk<4>();
     if (e == cudaSuccess) e = preload_bulk<6>();
@@ -639,10 +659,14 @@ cudaError_t launch_kv_copy(const CopyArgs& a) {
             const bool src_dev = a.pack || !(a.buf_is_host || a.buf_is_peer);
             // the 16-byte kernel (2 KiB tasks, twice the CTAs) loses with it: cfg 1 3,169 -> 3,101 GB/s
             w.pf_dist = (src_dev && wide) ? g_prefetch : -1;
-            if (a.inline_desc) {
+            if (a.inline_desc && a.n_runs <= kInlineRuns && a.n_reqs <= kInlineReqs) {
                 InlineDesc d;   // unused tail entries are never indexed (run < n_runs)
-                std::memcpy(d.runs, a.runs, static_cast<size_t>(a.n_runs) * sizeof(RunDesc));
-                std::memcpy(d.reqs, a.reqs, static_cast<size_t>(a.n_reqs) * sizeof(ReqDesc));
+                fill_inline(d, a);
+                e = wide ? launch_warp32(pt, d, w)
+                         : (g_warp_unroll == 4) ? launch_warp<4>(pt, d, w) : launch_warp<8>(pt, d, w);
+            } else if (a.inline_desc) {
+                InlineDescL d;
+                fill_inline(d, a);
                 e = wide ? launch_warp32(pt, d, w)
                          : (g_warp_unroll == 4) ? launch_warp<4>(pt, d, w) : launch_warp<8>(pt, d, w);
             } else {

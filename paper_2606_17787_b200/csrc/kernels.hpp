@@ -13,8 +13,13 @@ constexpr int kMaxPlanesPerLaunch = 256;  // plane pointers travel as kernel par
 // Small plans (one decode step: 64 requests x 1-2 runs) travel entirely in the kernel
 // parameters: no descriptor upload, no device blob, and a CTA starts its payload loads
 // without first waiting on two dependent descriptor loads from global memory.
+// Two size classes, so that the common decode step pays for 6 KiB of parameters and a batch of a
+// few hundred requests (whose upload would cost ~10 us per launch: a copy-engine hop between two
+// kernels) for 24 KiB; the parameter space of a kernel is 32,764 bytes.
 constexpr int kInlineRuns = 256;
 constexpr int kInlineReqs = 128;
+constexpr int kInlineRunsL = 1024;
+constexpr int kInlineReqsL = 512;
 
 enum KernelKind : int { kKernelAuto = 0, kKernelWarp = 1, kKernelBulk = 2 };
 

@@ -20,6 +20,16 @@ namespace lumen {
 
 thread_local int t_last_cuda_error = 0;
 
+int g_inline_max_runs = -1;   // -1: unset (LUMEN_KV_INLINE_MAX_RUNS, else kInlineRunsL)
+int inline_max_runs() {
+    if (g_inline_max_runs < 0) {
+        const char* e = std::getenv("LUMEN_KV_INLINE_MAX_RUNS");
+        const int v = e ? std::atoi(e) : kInlineRunsL;
+        g_inline_max_runs = v < 0 ? 0 : (v > kInlineRunsL ? kInlineRunsL : v);
+    }
+    return g_inline_max_runs;
+}
+
 int cuda_fail(cudaError_t e) {
     t_last_cuda_error = static_cast<int>(e);
     (void)cudaGetLastError();  // clear the sticky-free error state
@@ -35,6 +45,8 @@ struct Blob {
     int device = -1;        // the device `dev` and the events belong to
     bool host_only = false;
     bool captured = false;  // used under stream capture: a graph may replay it at any time
+    cudaEvent_t uploaded = nullptr;   // recorded behind the descriptor copy on the upload stream
+    bool upload_seen = false;         // that event has been seen complete: no wait is needed any more
     std::vector<std::pair<cudaStream_t, cudaEvent_t>> uses;  // last use per stream
 };
 
@@ -118,6 +130,7 @@ private:
     }
     static void destroy(Blob* b) {
         for (auto& u : b->uses) cudaEventDestroy(u.second);
+        if (b->uploaded) cudaEventDestroy(b->uploaded);
         if (b->host) cudaFreeHost(b->host);
         if (b->dev) cudaFree(b->dev);
         (void)cudaGetLastError();
@@ -133,11 +146,64 @@ Arena& arena() {
     return *a;
 }
 
+// Descriptor uploads run on a stream of the library's own (one per device), not on the caller's:
+// a copy-engine operation between two kernels of one stream costs ~10 us (it cannot start before
+// the first kernel has drained, and the second kernel starts cold behind it); on its own stream
+// the copy runs while the caller's stream is busy, and the kernel only waits for its event.
+constexpr int kMaxDev = 64;
+std::mutex g_upload_mu;
+cudaStream_t g_upload_stream[kMaxDev] = {};
+
+cudaError_t upload_stream(cudaStream_t* out) {
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= kMaxDev) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> g(g_upload_mu);
+    if (!g_upload_stream[dev]) {
+        e = cudaStreamCreateWithFlags(&g_upload_stream[dev], cudaStreamNonBlocking);
+        if (e != cudaSuccess) return e;
+    }
+    *out = g_upload_stream[dev];
+    return cudaSuccess;
+}
+
 }  // namespace
 }  // namespace lumen
 
 namespace lumen {
 namespace {
+
+// Orders `stream` behind the plan's descriptor upload (a no-op once the copy has been seen
+// complete, so that no event wait sits between two kernels of a decode loop).
+int await_upload(lumen_kv_plan* p, cudaStream_t stream) {
+    Blob* b = p->blob;
+    if (!b || b->upload_seen || !b->uploaded) return LUMEN_KV_OK;
+    cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+    if (cudaStreamIsCapturing(stream, &cs) != cudaSuccess) (void)cudaGetLastError();
+    if (cs != cudaStreamCaptureStatusNone) {
+        // An event of a stream outside the capture cannot become a graph dependency, and event
+        // queries are illegal under a global-mode capture: the few microseconds of the copy are
+        // waited for on the host, once, at capture time, with this thread in relaxed mode.
+        cudaStreamCaptureMode mode = cudaStreamCaptureModeRelaxed;
+        cudaError_t e = cudaThreadExchangeStreamCaptureMode(&mode);
+        if (e != cudaSuccess) return cuda_fail(e);
+        e = cudaEventSynchronize(b->uploaded);
+        (void)cudaThreadExchangeStreamCaptureMode(&mode);
+        if (e != cudaSuccess) return cuda_fail(e);
+        b->upload_seen = true;
+        return LUMEN_KV_OK;
+    }
+    cudaError_t e = cudaEventQuery(b->uploaded);
+    if (e == cudaSuccess) {
+        b->upload_seen = true;
+        return LUMEN_KV_OK;
+    }
+    (void)cudaGetLastError();
+    if (e != cudaErrorNotReady) return cuda_fail(e);
+    e = cudaStreamWaitEvent(stream, b->uploaded, 0);
+    return e == cudaSuccess ? LUMEN_KV_OK : cuda_fail(e);
+}
 
 // record "plan still in use on `stream`" so the arena does not recycle the blob early
 int note_use(lumen_kv_plan* p, cudaStream_t stream) {
@@ -209,6 +275,10 @@ int launch_part(const lumen_kv_plan* plan, const std::vector<const void*>& plane
     a.pack = pack;
     a.kernel = static_cast<int>((plan->flags & LUMEN_KV_KERNEL_MASK) >> LUMEN_KV_KERNEL_SHIFT);
     a.stream = stream;
+    if (!plan->inline_desc) {
+        const int rc = await_upload(const_cast<lumen_kv_plan*>(plan), stream);
+        if (rc != LUMEN_KV_OK) return rc;
+    }
     cudaError_t e = launch_kv_copy(a);
     if (e != cudaSuccess) return cuda_fail(e);
     if (plan->inline_desc) return LUMEN_KV_OK;   // nothing on the device to keep alive
@@ -316,7 +386,7 @@ int lumen_kv_plan_build_layout(const lumen_kv_geom* geom, const lumen_kv_req* re
 
     // Small plans (a decode step's deltas) need no device copy at all: the kernel receives
     // the descriptors in its parameters.
-    if (!(flags & (LUMEN_KV_HOST_ONLY | LUMEN_KV_NO_INLINE)) && p->n_runs <= kInlineRuns && num_reqs <= kInlineReqs) {
+    if (!(flags & (LUMEN_KV_HOST_ONLY | LUMEN_KV_NO_INLINE)) && p->n_runs <= inline_max_runs() && num_reqs <= kInlineReqsL) {
         p->inline_desc = true;
         p->h_runs = p->hp.runs.data();
         p->h_reqs = p->hp.reqs.data();
@@ -346,15 +416,21 @@ int lumen_kv_plan_build_layout(const lumen_kv_geom* geom, const lumen_kv_req* re
             char* d = static_cast<char*>(p->blob->dev);
             p->d_runs = reinterpret_cast<const RunDesc*>(d);
             p->d_reqs = reinterpret_cast<const ReqDesc*>(d + run_bytes);
-            cudaStream_t s = static_cast<cudaStream_t>(stream);
-            cudaError_t e = cudaMemcpyAsync(d, h, total, cudaMemcpyHostToDevice, s);
+            (void)stream;   // kept in the signature; the upload has a stream of its own (see above)
+            cudaStream_t s = nullptr;
+            cudaError_t e = upload_stream(&s);
+            Blob* b = p->blob;
+            if (e == cudaSuccess && !b->uploaded)
+                e = cudaEventCreateWithFlags(&b->uploaded, cudaEventDisableTiming);
+            // a recycled blob is idle (Arena::acquire): nothing enqueued still reads its device copy
+            if (e == cudaSuccess) e = cudaMemcpyAsync(d, h, total, cudaMemcpyHostToDevice, s);
+            if (e == cudaSuccess) e = cudaEventRecord(b->uploaded, s);
+            b->upload_seen = false;
             if (e != cudaSuccess) {
                 arena().release(p->blob);
                 delete p;
                 return cuda_fail(e);
             }
-            rc = note_use(p, s);
-            if (rc != LUMEN_KV_OK) { arena().release(p->blob); delete p; return rc; }
         }
     }
     // the vectors are no longer needed: descriptors live in the blob
@@ -411,6 +487,10 @@ void lumen_kv_plan_free(lumen_kv_plan* plan) {
 void lumen_kv_trim(void) { lumen::arena().trim(); }
 
 int lumen_kv_set_option(const char* name, int value) {
+    if (name && !std::strcmp(name, "inline_max_runs")) {   // A/B: which plans ride in the parameters
+        lumen::g_inline_max_runs = value < 0 ? 0 : (value > lumen::kInlineRunsL ? lumen::kInlineRunsL : value);
+        return LUMEN_KV_OK;
+    }
     return lumen::set_option(name, value) == 0 ? LUMEN_KV_OK : LUMEN_KV_EINVAL;
 }
 

@@ -9,7 +9,7 @@ from paper_2606_17787_b200.pool import KVPool, Checkpointer, StagingRing, pinned
 from workloads import device as wdev
 from workloads import fill_plane_np
 
-# "warp": plans of <= 256 runs travel in the kernel parameters; "warp_upload" forces the
+# "warp": plans of <= 1,024 runs / 512 requests travel in the kernel parameters; "warp_upload" forces the
 # descriptor upload to device memory for those too, so both descriptor paths are compared
 KERNELS = {"warp": lk.LUMEN_KV_KERNEL_WARP, "bulk": lk.LUMEN_KV_KERNEL_BULK,
            "auto": lk.LUMEN_KV_KERNEL_AUTO,
