@@ -793,3 +793,53 @@ def test_l2_prefetch_is_only_a_hint(G, kernel):
     with pytest.raises(lk.LumenKVError):
         B.lumen_kv_checkpoint_pack(plan, pool_a.k_ptrs, pool_a.v_ptrs, buf.data_ptr(), plan.nbytes, 3, s)
     plan.close(); rplan.close()
+
+
+@pytest.mark.parametrize("kernel", ["warp", "warp_upload", "bulk"])
+def test_descriptor_size_classes(G, kernel):
+    """Plans of 257 .. 1,024 runs / 129 .. 512 requests ride in the larger parameter block, plans
+    beyond that (and NO_INLINE ones) upload their descriptors on the library's own stream: the three
+    cases on the 32-byte kernel, the 16-byte kernel (48-byte rows) and the TMA kernel."""
+    lk = G.lk
+    shapes = [
+        dict(L=2, N=8192, n_reqs=300, grow_iters=1, median=60, hi=200, lo=20),            # requests > 128
+        dict(L=2, N=8192, n_reqs=100, grow_iters=1, median=120, hi=300, lo=40, delta=120),  # runs > 256
+        dict(L=2, H=1, D=24, N=8192, n_reqs=300, grow_iters=1, median=60, hi=200, lo=20),  # 16-byte kernel
+        dict(L=1, N=16384, n_reqs=600, grow_iters=1, median=40, hi=100, lo=20),           # > 512 requests: upload
+    ]
+    for i, kw in enumerate(shapes):
+        w = cfg1_qwen14b(**kw)
+        plan = lk.lumen_kv_plan_build(lk.make_geom(*w.geom), w.reqs, lk.LUMEN_KV_HOST_ONLY)
+        runs, reqs = plan.num_runs, len(w.reqs)
+        plan.close()
+        if i < 3:
+            assert 256 < runs <= 1024 or 128 < reqs <= 512, (runs, reqs)
+        else:
+            assert reqs > 512
+        run_case(G, w, kernel, "device" if i % 2 == 0 else "host", seed=40 + i)
+
+
+def test_upload_on_the_library_stream_orders_the_kernel(G):
+    """A plan with uploaded descriptors is used at once, on a stream that has just been created,
+    with no host synchronisation anywhere; descriptor blobs are recycled from plan to plan."""
+    import torch
+    lk = G.lk
+    w = cfg1_qwen14b(L=2, N=8192, n_reqs=32, grow_iters=40, median=200, hi=512, lo=20)
+    K, V = G.host_planes(w.geom, 11)
+    pool = G.make_pool(w.geom, 11)
+    ck = G.Checkpointer(pool, lk.LUMEN_KV_NO_INLINE)
+    torch.cuda.synchronize()
+    bufs, refs, cur, streams = [], [], w, []
+    for it in range(24):
+        s = torch.cuda.Stream()
+        streams.append(s)
+        plan = ck.plan(cur.reqs, stream=s)
+        buf = torch.empty(plan.nbytes, dtype=torch.uint8, device="cuda")
+        ck.pack(plan, buf, stream=s)
+        plan.close()
+        bufs.append(buf); refs.append(oracle.pack(cur.geom, K, V, cur.reqs))
+        cur = cur.advanced(16)
+    torch.cuda.synchronize()
+    for buf, ref in zip(bufs, refs):
+        assert np.array_equal(G.buf_to_np(buf, buf.numel()), ref)
+    lk.lumen_kv_trim()
