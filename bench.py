@@ -571,6 +571,15 @@ class HbmPath:
             pack_ms, unpack_ms = self.single_stats["pack"]["mean"], self.single_stats["unpack"]["mean"]
         return ms, pack_ms, unpack_ms, t_wall * 1e3, t_host * 1e3
 
+    def direction_ms(self, K, W, bufs, kind, lag_, sampler, only, passes=1):
+        """Average launch duration of one direction alone: K back-to-back launches between one event
+        pair.  With only 3 launches of 10-20 ms per pass (the 32 / 64 GiB configs) one stall between
+        two launches -- seen in about one run in four on this pool, 10-40 ms, not reproducible with
+        the same loop in isolation and not in the per-launch times -- would triple the figure, so
+        such a pass is taken `passes` times and the smallest is the kernel's; all are reported."""
+        got = [self.timed_loop(K, W, bufs, kind, lag_, sampler, only=only)[0] / K for _ in range(passes)]
+        return min(got), got
+
     def two_stream_loop(self, K, W, bufs, kind, lag_):
         """a8 on HBM buffers: the pack of step i on one stream, the restore of the buffer packed
         `lag_` steps earlier on a second one, ordered only by events on the buffers (a worker
@@ -712,9 +721,10 @@ def large_config(torch, lk, name, seed, kflag, stream, sampler, peak, link, with
         P = path.P
         with torch.cuda.stream(stream):
             ms, _, _, _, host_ms = path.timed_loop(3, 3, [dbuf], DEV, 0, sampler)
-            pack_ms = path.timed_loop(3, 3, [dbuf], DEV, 0, sampler, only="pack")[0] / 3
-            unpack_ms = path.timed_loop(3, 3, [dbuf], DEV, 0, sampler, only="unpack")[0] / 3
+            pack_ms, pack_passes = path.direction_ms(3, 3, [dbuf], DEV, 0, sampler, "pack", passes=2)
+            unpack_ms, unpack_passes = path.direction_ms(3, 3, [dbuf], DEV, 0, sampler, "unpack", passes=2)
         per_wave.append({"wave": wave, "ms_per_step": ms / 3, "pack_ms": pack_ms, "unpack_ms": unpack_ms,
+                         "pack_ms_passes": pack_passes, "unpack_ms_passes": unpack_passes,
                          "payload_GBps": 2 * P / (ms / 3) / 1e6})
         agg_bytes += 2 * P
         agg_ms += ms / 3
@@ -722,6 +732,7 @@ def large_config(torch, lk, name, seed, kflag, stream, sampler, peak, link, with
     out = {"payload_bytes_per_direction": P, "pool_pages": N, "page_size": S,
            "ms_per_step": ms / 3, "payload_GBps": 2 * P / (ms / 3) / 1e6,
            "pack_ms": pack_ms, "unpack_ms": unpack_ms,
+           "pack_ms_passes": pack_passes, "unpack_ms_passes": unpack_passes,
            "achieved_GBps": 2 * P / dom_ms / 1e6, "peak_GBps": peak, "frac": 2 * P / dom_ms / 1e6 / peak,
            "frac_formula": "2 * payload_bytes_per_direction / max(pack_ms, unpack_ms) / peak_GBps",
            "frac_of_spec_8TBps": 2 * P / dom_ms / 1e6 / 8000.0,
@@ -827,8 +838,9 @@ def run_ours(args):
     big = P > (1 << 30)
     Kk = min(K, 200) if not big else min(K, 3)         # per-launch pass: same steps, instrumented
     with torch.cuda.stream(stream):
-        pack_ref = path.timed_loop(Kk, 3, dbufs, DEV, lag, only="pack")[0] / Kk
-        unpack_ref = path.timed_loop(Kk, 3, dbufs, DEV, lag, only="unpack")[0] / Kk
+        # (tens-of-GiB configs: 3 launches per pass, the better of two passes -- see direction_ms)
+        pack_ref, pack_passes = path.direction_ms(Kk, 3, dbufs, DEV, lag, None, "pack", passes=2 if big else 1)
+        unpack_ref, unpack_passes = path.direction_ms(Kk, 3, dbufs, DEV, lag, None, "unpack", passes=2 if big else 1)
         # The headline: exactly K steps between one event pair.  A step that the HOST could not feed
         # in time (enqueue slower than the two kernels AND a device time well above them -- e.g. this
         # process was descheduled for a millisecond inside a 2 ms region) does not measure the
@@ -884,6 +896,7 @@ def run_ours(args):
                            "single_launch_after_idle_ms = one event pair per launch, queued behind a gate that opens after "
                            "12 ms in which the device runs one spinning warp (no memory traffic, no host latency inside)"),
                 "pack_ms": pack_ms, "unpack_ms": unpack_ms,
+                "pack_ms_passes": pack_passes, "unpack_ms_passes": unpack_passes,
                 "pack_single_ms": pack_1, "unpack_single_ms": unpack_1, "single_launch_ms": single,
                 "single_launch_after_idle_ms": idle,
                 "pack_traffic_GBps": 2 * P / pack_ms / 1e6, "unpack_traffic_GBps": 2 * P / unpack_ms / 1e6}
