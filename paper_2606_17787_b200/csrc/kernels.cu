@@ -10,13 +10,13 @@
 //   kv_copy_warp32 / kv_copy_warp : SIMT, the HBM <-> HBM path.  One warp per (run, plane,
 //                  sub-chunk), 32-byte (LDG/STG.E.256) or 16-byte accesses per lane, UNROLL
 //                  independent loads in flight per lane before the first store; descriptors
-//                  in global memory or in the kernel parameters; programmatic dependent launch.
+//                  in global memory or in the kernel parameters (two size classes);
+//                  programmatic dependent launch, with an L2 prefetch of the source
+//                  (cp.async.bulk.prefetch.L2, UBLKPF) ahead of the stream-order wait.
 //   kv_copy_bulk : TMA, the zero-copy host path (small grid).  Persistent single-warp CTAs;
-//                  one elected lane moves
-//                  whole items global -> shared ring -> global with 1-D
-//                  cp.async.bulk (UBLKCP), completion tracked by mbarriers (loads)
-//                  and bulk groups (stores).  The other lanes only prefetch and
-//                  decode descriptors.
+//                  one elected lane moves whole items global -> shared ring -> global with
+//                  1-D cp.async.bulk (UBLKCP), completion tracked by mbarriers (loads) and
+//                  bulk groups (stores).  The other lanes only decode descriptors.
 #include "kernels.hpp"
 
 #include <cstdlib>
