@@ -744,8 +744,9 @@ def test_cuda_graph_capture(G, kernel):
 
 
 @pytest.mark.gpu
+@pytest.mark.parametrize("shape", ["one_wave", "many_waves"])
 @pytest.mark.parametrize("kernel", ["warp", "warp_upload"])
-def test_l2_prefetch_is_only_a_hint(G, kernel):
+def test_l2_prefetch_is_only_a_hint(G, kernel, shape):
     """The SIMT kernel asks L2 for source bytes ahead of the stream-order wait (option
     "prefetch": -1 off, 0 own task, d > 0 the task d CTAs further on).  Whatever the distance,
     the bytes are the oracle's -- also when fill -> pack -> restore -> pack run back to back on
@@ -754,7 +755,10 @@ def test_l2_prefetch_is_only_a_hint(G, kernel):
     a stale line would show)."""
     import torch
     lk = G.lk
-    w = cfg1_qwen14b(L=3, N=2048, n_reqs=24, grow_iters=2, median=200, hi=512, lo=20)
+    # one_wave: 288 CTAs, all of them resident (and prefetching) while the previous kernel still
+    # runs; many_waves: 3,700 CTAs = 5 waves, the steady state behind the first wave as well
+    w = (cfg1_qwen14b(L=3, N=2048, n_reqs=24, grow_iters=2, median=200, hi=512, lo=20) if shape == "one_wave"
+         else cfg1_qwen14b(L=8, N=4096, n_reqs=120, grow_iters=2, median=150, hi=400, lo=20))
     flags = G.KERNELS[kernel]
     pool_a, pool_b = G.make_pool(w.geom, 7), G.make_pool(w.geom, 8)
     ck_a, ck_b = G.Checkpointer(pool_a, flags), G.Checkpointer(pool_b, flags)
