@@ -758,7 +758,7 @@ def test_l2_prefetch_is_only_a_hint(G, kernel, shape):
     # one_wave: 288 CTAs, all of them resident (and prefetching) while the previous kernel still
     # runs; many_waves: 3,700 CTAs = 5 waves, the steady state behind the first wave as well
     w = (cfg1_qwen14b(L=3, N=2048, n_reqs=24, grow_iters=2, median=200, hi=512, lo=20) if shape == "one_wave"
-         else cfg1_qwen14b(L=8, N=3072, n_reqs=120, grow_iters=2, median=150, hi=400, lo=20))
+         else cfg1_qwen14b(L=8, N=3200, n_reqs=120, grow_iters=2, median=150, hi=400, lo=20))
     flags = G.KERNELS[kernel]
     pool_a, pool_b = G.make_pool(w.geom, 7), G.make_pool(w.geom, 8)
     ck_a, ck_b = G.Checkpointer(pool_a, flags), G.Checkpointer(pool_b, flags)
