@@ -807,10 +807,10 @@ def test_descriptor_size_classes(G, kernel):
     cases on the 32-byte kernel, the 16-byte kernel (48-byte rows) and the TMA kernel."""
     lk = G.lk
     shapes = [
-        dict(L=2, N=8192, n_reqs=300, grow_iters=1, median=60, hi=200, lo=20),            # requests > 128
-        dict(L=2, N=8192, n_reqs=100, grow_iters=1, median=120, hi=300, lo=40, delta=120),  # runs > 256
-        dict(L=2, H=1, D=24, N=8192, n_reqs=300, grow_iters=1, median=60, hi=200, lo=20),  # 16-byte kernel
-        dict(L=1, N=16384, n_reqs=600, grow_iters=1, median=40, hi=100, lo=20),           # > 512 requests: upload
+        dict(L=2, N=4096, n_reqs=300, grow_iters=1, median=60, hi=200, lo=20),            # requests > 128
+        dict(L=2, N=4096, n_reqs=100, grow_iters=1, median=120, hi=300, lo=40, delta=120),  # runs > 256
+        dict(L=2, H=1, D=24, N=4096, n_reqs=300, grow_iters=1, median=60, hi=200, lo=20),  # 16-byte kernel
+        dict(L=1, N=6000, n_reqs=600, grow_iters=1, median=40, hi=100, lo=20),            # > 512 requests: upload
     ]
     for i, kw in enumerate(shapes):
         w = cfg1_qwen14b(**kw)
