@@ -12,9 +12,9 @@ runs would produce: only lengths and page scatter matter to the
 path, and the recipe for each BASELINE.json config is in DESIGN.md section 4.
 """
 from .gen import (MASTER_SEED, Workload, substream, cfg0_tiny, cfg1_qwen14b,
-                  cfg2_qwen32b, cfg3_burst, cfg4_longctx, random_tiny)
+                  cfg2_qwen32b, cfg3_burst, cfg4_longctx, random_mid, random_tiny)
 from .content import g_words, fill_plane_np
 
 __all__ = ["MASTER_SEED", "Workload", "substream", "cfg0_tiny", "cfg1_qwen14b",
-           "cfg2_qwen32b", "cfg3_burst", "cfg4_longctx", "random_tiny",
+           "cfg2_qwen32b", "cfg3_burst", "cfg4_longctx", "random_mid", "random_tiny",
            "g_words", "fill_plane_np"]

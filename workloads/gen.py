@@ -225,3 +225,30 @@ def random_tiny(rng: np.random.Generator, *, allow_shared=False) -> Workload:
         reqs.append((pa, tb, te))
         rreqs.append((pb, tb, te))
     return Workload("random_tiny", (L, H, D, S, N), reqs, rreqs, {"lens": lens})
+
+
+def random_mid(rng: np.random.Generator) -> Workload:
+    """Random geometry for differential fuzzing: up to 4 layers, rows of 16 B .. 2 KiB, page sizes
+    1 .. 64, up to 200 requests with ragged ranges (some empty), page tables scattered or -- in a
+    third of the cases -- physically consecutive (what MERGE_ADJACENT merges)."""
+    L = int(rng.integers(1, 5))
+    H = int(rng.integers(1, 9))
+    D = int(rng.choice([8, 16, 24, 32, 64, 128]))
+    while (H * D * 2) % 16:
+        D = int(rng.choice([8, 16, 24, 32, 64, 128]))
+    S = int(rng.choice([1, 2, 3, 7, 16, 32, 64]))
+    R = int(rng.integers(1, 200))
+    lens = [int(rng.integers(0, 6 * S + 40)) for _ in range(R)]
+    counts = [_pages(n, S) + int(rng.integers(0, 2)) for n in lens]
+    N = 2 * sum(counts) + int(rng.integers(1, 50))
+    perm_a, perm_b = rng.permutation(N), rng.permutation(N)
+    if rng.random() < 0.3:
+        perm_a, perm_b = np.arange(N), np.arange(N)[::-1].copy()
+    pts_a, pts_b = _chunks(perm_a, counts), _chunks(perm_b, counts)
+    reqs, rreqs = [], []
+    for pa, pb, n in zip(pts_a, pts_b, lens):
+        tb = int(rng.integers(0, n + 1))
+        te = int(rng.integers(tb, n + 1))
+        reqs.append((pa, tb, te))
+        rreqs.append((pb, tb, te))
+    return Workload("random_mid", (L, H, D, S, N), reqs, rreqs, {"lens": lens})
