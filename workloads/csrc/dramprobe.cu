@@ -92,12 +92,34 @@ probe_kernel(const char* __restrict__ src, char* __restrict__ dst, int64_t n_tas
     }
 }
 
+// Persistent form of the copy: gridDim.x CTAs stay resident and every warp walks the tasks with a
+// grid-wide stride (prefetching its next task into L2 when pf is set): what CTA launches cost.
+__global__ void __launch_bounds__(kWarps * 32)
+probe_copy_persistent(const char* __restrict__ src, char* __restrict__ dst, int64_t n_tasks, int pf) {
+    const int lane = threadIdx.x & 31;
+    const int64_t stride = static_cast<int64_t>(gridDim.x) * kWarps;
+    for (int64_t task = static_cast<int64_t>(blockIdx.x) * kWarps + (threadIdx.x >> 5); task < n_tasks;
+         task += stride) {
+        if (pf && lane == 0 && task + stride < n_tasks)
+            asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src + static_cast<size_t>(task + stride) * kTask),
+                         "r"(static_cast<uint32_t>(kTask))
+                         : "memory");
+        const size_t off = static_cast<size_t>(task) * kTask + static_cast<size_t>(lane) * 32;
+        V8 v[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) v[u] = ld32(src + off + u * 1024);
+#pragma unroll
+        for (int u = 0; u < 4; ++u) st32(dst + off + u * 1024, v[u]);
+    }
+}
+
 }  // namespace
 
 extern "C" {
 
 // mode: 0 read src, 1 write dst, 2 copy src -> dst, 3 copy with a 4 KiB L2 prefetch per warp,
-// 4 copy with a 32 KiB L2 prefetch per CTA, 5 / 6 copy at 5 / 4 CTAs per SM; nbytes % 4096 == 0;
+// 4 copy with a 32 KiB L2 prefetch per CTA, 5 / 6 copy at 5 / 4 CTAs per SM, 7 / 8 persistent copy
+// without / with prefetch; nbytes % 4096 == 0;
 // 32-byte aligned.
 __attribute__((visibility("default")))
 int dramprobe_run(int mode, const void* src, void* dst, int64_t nbytes, void* sink, void* stream) {
@@ -118,6 +140,15 @@ int dramprobe_run(int mode, const void* src, void* dst, int64_t nbytes, void* si
     // modes 5 / 6: the plain copy (2) at 5 / 4 CTAs per SM instead of 6 (extra live registers)
     else if (mode == 5) probe_kernel<2, 8><<<static_cast<unsigned>(grid), kWarps * 32, 0, s>>>(a, b, n_tasks, reinterpret_cast<uint32_t*>(b), 0u);
     else if (mode == 6) probe_kernel<2, 24><<<static_cast<unsigned>(grid), kWarps * 32, 0, s>>>(a, b, n_tasks, reinterpret_cast<uint32_t*>(b), 0u);
+    // modes 7 / 8: persistent copy, one resident wave of CTAs, without / with an L2 prefetch of the next task
+    else if (mode == 7 || mode == 8) {
+        int dev = 0, sms = 148;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        int per_sm = 4;   // exactly the CTAs that are resident at once
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, probe_copy_persistent, kWarps * 32, 0);
+        probe_copy_persistent<<<static_cast<unsigned>(sms * per_sm), kWarps * 32, 0, s>>>(a, b, n_tasks, mode == 8);
+    }
     else return -1;
     return cudaGetLastError() == cudaSuccess ? 0 : -2;
 }
