@@ -601,6 +601,7 @@ LUMEN_KV_API int lumen_kv_init(void);
  *   "warp_unroll" 4 (default) / 8 : loads in flight per lane of the 16-byte kernel
  *   "host_kernel" 2 (default, TMA bulk kernel) / 1 (SIMT kernel): what AUTO picks for a host buffer
  *   "host_ctas"   0 (default: 24..96 by item size) / n : grid of the bulk kernel on a host buffer
+ *   "inline_max_runs" 1024 (default) / n : plans of more than n runs upload their descriptors
  *   "prefetch"    16 (default) / d >= 0 / -1 : the SIMT kernel asks L2 for the 4 KiB a warp d CTAs
  *                 further on will copy (parameter-resident plans; larger plans announce their own
  *                 4 KiB, whatever d) / no prefetch.  A hint: the bytes moved are the same.
