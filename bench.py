@@ -1906,6 +1906,8 @@ def run_dram(args):
         "probe_copy_l2_prefetch_32k": timed("probe_copy_pf32k", lambda: wdev.dram_probe("copy_pf32k", a_, b_, NB, s.cuda_stream), 2 * NB),
         "probe_copy_5_ctas_per_sm": timed("probe_copy_5cta", lambda: wdev.dram_probe("copy_5cta", a_, b_, NB, s.cuda_stream), 2 * NB),
         "probe_copy_4_ctas_per_sm": timed("probe_copy_4cta", lambda: wdev.dram_probe("copy_4cta", a_, b_, NB, s.cuda_stream), 2 * NB),
+        "probe_copy_smem_carveout_7pct_dyn_4KiB": timed("probe_copy_carve_804", lambda: wdev.dram_probe(804, a_, b_, NB, s.cuda_stream), 2 * NB),
+        "probe_copy_smem_carveout_7pct_dyn_6KiB": timed("probe_copy_carve_806", lambda: wdev.dram_probe(806, a_, b_, NB, s.cuda_stream), 2 * NB),
         "probe_copy_persistent": timed("probe_copy_persistent", lambda: wdev.dram_probe("copy_persistent", a_, b_, NB, s.cuda_stream), 2 * NB),
         "probe_copy_persistent_l2_prefetch": timed("probe_copy_persistent_pf", lambda: wdev.dram_probe("copy_persistent_pf", a_, b_, NB, s.cuda_stream), 2 * NB),
         "torch_copy_": timed("torch_copy", lambda: b_.copy_(a_), 2 * NB),

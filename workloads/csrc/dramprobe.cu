@@ -149,6 +149,16 @@ int dramprobe_run(int mode, const void* src, void* dst, int64_t nbytes, void* si
         cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, probe_copy_persistent, kWarps * 32, 0);
         probe_copy_persistent<<<static_cast<unsigned>(sms * per_sm), kWarps * 32, 0, s>>>(a, b, n_tasks, mode == 8);
     }
+    // modes 100 + c*100 + d: the plain copy with a shared-memory carveout of c percent and d KiB of
+    // unused dynamic shared memory per CTA (occupancy limited through shared memory while L1 stays
+    // large); the resulting CTAs per SM are returned through *sink_host if given
+    else if (mode >= 100) {
+        const int carve = (mode - 100) / 100, dyn_kib = (mode - 100) % 100;
+        cudaFuncSetAttribute(probe_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
+        cudaFuncSetAttribute(probe_kernel<2>, cudaFuncAttributePreferredSharedMemoryCarveout, carve);
+        probe_kernel<2><<<static_cast<unsigned>(grid), kWarps * 32, dyn_kib * 1024, s>>>(a, b, n_tasks, k, 0u);
+        cudaFuncSetAttribute(probe_kernel<2>, cudaFuncAttributePreferredSharedMemoryCarveout, -1);
+    }
     else return -1;
     return cudaGetLastError() == cudaSuccess ? 0 : -2;
 }

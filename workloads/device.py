@@ -42,6 +42,11 @@ def dram_probe(mode: str, src, dst, nbytes: int, stream: int = 0) -> None:
         _probe.dramprobe_run.restype = ctypes.c_int
         _probe.dramprobe_run.argtypes = [ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int64,
                                          ctypes.c_void_p, ctypes.c_void_p]
+    if isinstance(mode, int):
+        rc = _probe.dramprobe_run(mode, src.data_ptr(), dst.data_ptr(), int(nbytes), None, stream)
+        if rc:
+            raise RuntimeError(f"dramprobe_run({mode}) failed ({rc})")
+        return
     rc = _probe.dramprobe_run({"read": 0, "write": 1, "copy": 2, "copy_pf4k": 3, "copy_pf32k": 4, "copy_5cta": 5, "copy_4cta": 6, "copy_persistent": 7, "copy_persistent_pf": 8}[mode], src.data_ptr(), dst.data_ptr(),
                               int(nbytes), None, stream)
     if rc:
