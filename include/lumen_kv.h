@@ -95,7 +95,9 @@ typedef enum {
     LUMEN_KV_ESIZE    = -4,  /* buffer smaller than lumen_kv_plan_bytes()                    */
     LUMEN_KV_ENOMEM   = -5,  /* host or device allocation of the descriptors failed          */
     LUMEN_KV_ECUDA    = -6,  /* CUDA runtime error; see lumen_kv_last_cuda_error()           */
-    LUMEN_KV_ESINK    = -7   /* background checkpointer: the sink rejected a delta           */
+    LUMEN_KV_ESINK    = -7,  /* background checkpointer: the sink rejected a delta           */
+    LUMEN_KV_ECAPACITY = -8  /* lumen_kv_copy_noalloc: the plan has more runs or requests than
+                                the library's built-in descriptor array holds                */
 } lumen_kv_status;
 
 /* Geometry of the caller's paged pool (host struct, read during plan_build only). */
@@ -124,7 +126,8 @@ typedef struct lumen_kv_plan lumen_kv_plan;  /* opaque; library owns its descrip
 #define LUMEN_KV_VALIDATE_UNIQUE_DST 0x1u /* reject plans that address a pool token slot twice  */
 #define LUMEN_KV_MERGE_ADJACENT      0x2u /* merge runs whose physical pages are adjacent     */
 #define LUMEN_KV_HOST_ONLY           0x4u /* build descriptors on the host only (no CUDA call);
-                                             such a plan can be inspected but not executed   */
+                                             such a plan can be inspected, and executed by
+                                             lumen_kv_copy_noalloc only                       */
 #define LUMEN_KV_NO_INLINE           0x8u /* always upload the descriptors to device memory.
                                              By default a plan of <= 1,024 runs and <= 512
                                              requests (a decode step's deltas, also of a large
@@ -236,6 +239,64 @@ LUMEN_KV_API int lumen_kv_checkpoint_pack(const lumen_kv_plan* plan,
 LUMEN_KV_API int lumen_kv_restore_unpack(const lumen_kv_plan* plan,
                             void* const* k_planes, void* const* v_planes,
                             const void* src, int64_t src_bytes, int src_kind, void* stream);
+
+/*
+ * lumen_kv_copy_noalloc -- pack (a3/a4) or restore (a7) for
+ * callers that must not allocate GPU memory.
+ *
+ * Who needs it.  A serving worker usually hands all free HBM to its KV pool at start-up, and
+ * that pool is fullest exactly when a restore is most urgent (a recovery burst):
+ * a cudaMalloc for a plan's descriptors may then fail, and cudaMalloc / cudaFree synchronise the
+ * whole device even when they succeed, which a decode loop cannot absorb.  Other callers run
+ * under a rule that all device memory comes from a pool of their own.  The regular calls need no
+ * device memory up to 1,024 runs / 512 requests; above that lumen_kv_plan_build allocates (and
+ * caches) device and pinned memory for the descriptors.  This call never does: it keeps the
+ * descriptors in an array that is part of the library's own image.
+ *
+ * Use.  Build the plan with LUMEN_KV_HOST_ONLY (host heap only, no CUDA call), then
+ *     lumen_kv_copy_noalloc(plan, LUMEN_KV_DIR_PACK or LUMEN_KV_DIR_RESTORE, k_planes, v_planes,
+ *                           buf, buf_bytes, buf_kind, stream);
+ * Arguments, buffer layout, alignment rules, buffer kinds and stream semantics are those of
+ * lumen_kv_checkpoint_pack / lumen_kv_restore_unpack, and so are the bytes that arrive.  Any plan
+ * is accepted (not only host-only ones); the plan may be freed as soon as the call returns.
+ *
+ * Limit.  At most LUMEN_KV_NOALLOC_MAX_RUNS runs and LUMEN_KV_NOALLOC_MAX_REQS requests per call
+ * (lumen_kv_plan_num_runs tells; a page-granular 32 GiB prefix restore of 16 requests is 8,192
+ * runs).  A larger plan is refused with LUMEN_KV_ECAPACITY before anything is enqueued: split
+ * the requests over several plans, or use the regular calls.  The array costs 1,088 KiB of
+ * device memory on every GPU that loads the library, held until the process exits.
+ *
+ * What it does.  It enqueues on `stream` one small kernel per 1,024 descriptors that writes them
+ * (they travel in its parameters) into the built-in array, then the copy kernel, one launch per
+ * 256 planes.  No cudaMalloc, cudaFree, cudaHostAlloc or other allocating call is made, on any
+ * call; nothing is synchronised.  The copy kernel is a plain form of the regular SIMT kernel
+ * (no overlap with the neighbouring launches, no L2 prefetch), so expect a few per cent less
+ * than the regular call.
+ *
+ * First call on a device.  It looks up the array's device address (cudaGetSymbolAddress) and
+ * loads three kernels; the CUDA runtime may load the library's module at that point.  Make
+ * that first call -- an empty plan will not do, it returns before the set-up; any 1-token plan
+ * does -- during start-up, with the device current, and before any stream capture is begun.
+ *
+ * Sharing.  Every call on a device uses the same array, and the array keeps what the last call
+ * wrote.  Nothing in it has to start at zero: a call overwrites the entries it will read and
+ * reads no others.  But two calls whose GPU work overlaps race on it -- the second call's
+ * descriptor writes can land while the first call's copy kernel still reads them, and the first
+ * call then moves the wrong bytes, silently.  Issue all calls for a device on ONE stream, or
+ * order them with events so that a call's work has completed before the next call's begins.
+ * (Calls from several host threads are serialised while they enqueue, so two threads that
+ * share a stream are safe; the regular calls never touch the array.)
+ *
+ * Errors: EINVAL (null, bad direction / kind, misaligned, unpinned host buffer), ECAPACITY,
+ * ESIZE (buf_bytes < lumen_kv_plan_bytes), ECUDA.
+ */
+#define LUMEN_KV_NOALLOC_MAX_RUNS 65536
+#define LUMEN_KV_NOALLOC_MAX_REQS 4096
+#define LUMEN_KV_DIR_PACK    0   /* planes -> buf */
+#define LUMEN_KV_DIR_RESTORE 1   /* buf -> planes */
+LUMEN_KV_API int lumen_kv_copy_noalloc(const lumen_kv_plan* plan, int direction,
+                             void* const* k_planes, void* const* v_planes,
+                             void* buf, int64_t buf_bytes, int buf_kind, void* stream);
 
 /*
  * Two-stage host path (steps a4 / a7 through the copy engines).

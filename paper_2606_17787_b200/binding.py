@@ -22,6 +22,9 @@ _SO = Path(__file__).resolve().parent / "liblumen_kv.so"
 # ---- constants mirrored from include/lumen_kv.h -----------------------------------
 LUMEN_KV_OK, LUMEN_KV_EINVAL, LUMEN_KV_ERANGE = 0, -1, -2
 LUMEN_KV_EOVERLAP, LUMEN_KV_ESIZE, LUMEN_KV_ENOMEM, LUMEN_KV_ECUDA, LUMEN_KV_ESINK = -3, -4, -5, -6, -7
+LUMEN_KV_ECAPACITY = -8
+LUMEN_KV_NOALLOC_MAX_RUNS, LUMEN_KV_NOALLOC_MAX_REQS = 65536, 4096
+LUMEN_KV_DIR_PACK, LUMEN_KV_DIR_RESTORE = 0, 1
 LUMEN_KV_VALIDATE_UNIQUE_DST = 0x1
 LUMEN_KV_MERGE_ADJACENT = 0x2
 LUMEN_KV_HOST_ONLY = 0x4
@@ -32,7 +35,7 @@ LUMEN_KV_MEM_DEVICE, LUMEN_KV_MEM_HOST_MAPPED, LUMEN_KV_MEM_DEVICE_PEER = 0, 1, 
 EXPORTS = (
     "lumen_kv_plan_build", "lumen_kv_plan_build_layout", "lumen_kv_plan_bytes", "lumen_kv_plan_req_offset",
     "lumen_kv_plan_num_runs", "lumen_kv_plan_get_run", "lumen_kv_checkpoint_pack",
-    "lumen_kv_restore_unpack", "lumen_kv_plan_free", "lumen_kv_trim", "lumen_kv_init", "lumen_kv_set_option",
+    "lumen_kv_restore_unpack", "lumen_kv_copy_noalloc", "lumen_kv_plan_free", "lumen_kv_trim", "lumen_kv_init", "lumen_kv_set_option",
     "lumen_kv_checkpoint_pack_staged_async", "lumen_kv_restore_unpack_staged_async",
     "lumen_kv_stager_query", "lumen_kv_stager_wait", "lumen_kv_stager_sync",
     "lumen_kv_strerror", "lumen_kv_last_cuda_error", "lumen_kv_version",
@@ -125,6 +128,9 @@ def _lib() -> ctypes.CDLL:
         f = getattr(L, name)
         f.restype = ctypes.c_int
         f.argtypes = [vp, ctypes.POINTER(vp), ctypes.POINTER(vp), vp, i64, ctypes.c_int, vp]
+    L.lumen_kv_copy_noalloc.restype = ctypes.c_int
+    L.lumen_kv_copy_noalloc.argtypes = [vp, ctypes.c_int, ctypes.POINTER(vp), ctypes.POINTER(vp), vp, i64,
+                                        ctypes.c_int, vp]
     L.lumen_kv_stager_create.restype = ctypes.c_int
     L.lumen_kv_stager_create.argtypes = [vp, i64, i32, ctypes.POINTER(vp)]
     L.lumen_kv_stager_destroy.restype = None
@@ -399,6 +405,22 @@ def lumen_kv_restore_unpack(plan: Plan, k_planes, v_planes, src: int, src_bytes:
                                         ctypes.c_void_p(int(stream)))
     if rc:
         raise LumenKVError(rc, "lumen_kv_restore_unpack")
+
+
+def lumen_kv_copy_noalloc(plan: Plan, direction: int, k_planes, v_planes, buf: int, buf_bytes: int,
+                          buf_kind: int = LUMEN_KV_MEM_DEVICE, stream: int = 0) -> None:
+    """Pack (LUMEN_KV_DIR_PACK) or restore (LUMEN_KV_DIR_RESTORE) without any GPU allocation, for a
+    worker whose HBM is all committed to its KV pool or whose decode loop cannot take the device-wide
+    stall of a cudaMalloc: the descriptors go into an array built into the library (at most
+    LUMEN_KV_NOALLOC_MAX_RUNS runs / LUMEN_KV_NOALLOC_MAX_REQS requests, else LUMEN_KV_ECAPACITY).
+    Build the plan with LUMEN_KV_HOST_ONLY; keep all such calls of a device on one stream (they share
+    the array).  Same bytes as lumen_kv_checkpoint_pack / lumen_kv_restore_unpack."""
+    L = plan.geom.num_layers
+    rc = _lib().lumen_kv_copy_noalloc(plan.handle, int(direction), _as_ptr_array(k_planes, L),
+                                      _as_ptr_array(v_planes, L), ctypes.c_void_p(int(buf)),
+                                      int(buf_bytes), int(buf_kind), ctypes.c_void_p(int(stream)))
+    if rc:
+        raise LumenKVError(rc, "lumen_kv_copy_noalloc")
 
 
 class Stager:

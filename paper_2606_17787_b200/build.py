@@ -16,7 +16,7 @@ PKG = Path(__file__).resolve().parent
 ROOT = PKG.parent
 CSRC = PKG / "csrc"
 SO = PKG / "liblumen_kv.so"
-SOURCES = [CSRC / "lib.cu", CSRC / "stager.cu", CSRC / "ckpt.cu", CSRC / "recover.cu", CSRC / "kernels.cu", CSRC / "tags.cu", CSRC / "plan.cpp", CSRC / "store.cpp", CSRC / "placement.cpp"]
+SOURCES = [CSRC / "lib.cu", CSRC / "stager.cu", CSRC / "ckpt.cu", CSRC / "recover.cu", CSRC / "kernels.cu", CSRC / "tags.cu", CSRC / "noalloc.cu", CSRC / "plan.cpp", CSRC / "store.cpp", CSRC / "placement.cpp"]
 HEADERS = [CSRC / "plan.hpp", CSRC / "kernels.hpp", CSRC / "internal.hpp", ROOT / "include" / "lumen_kv.h"]
 
 NVCC_FLAGS = [

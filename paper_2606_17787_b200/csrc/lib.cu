@@ -509,6 +509,8 @@ const char* lumen_kv_strerror(int status) {
         case LUMEN_KV_ENOMEM: return "out of memory (descriptors), or no room for the reservation in the store arena";
         case LUMEN_KV_ECUDA: return "CUDA runtime error (see lumen_kv_last_cuda_error)";
         case LUMEN_KV_ESINK: return "the checkpointer's sink rejected a delta";
+        case LUMEN_KV_ECAPACITY:
+            return "plan too large for lumen_kv_copy_noalloc (more than 65,536 runs or 4,096 requests)";
         default: return "unknown status";
     }
 }
