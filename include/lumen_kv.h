@@ -66,7 +66,9 @@
  *   - A plan is immutable and direction-agnostic: the same plan drives pack and
  *     unpack.  The caller owns pools, buffers, streams and page tables (page
  *     tables are copied at build time).  Plans may be used concurrently from
- *     different streams; one plan must not be used from two host threads at once.
+ *     different streams and from several host threads (the little state a plan keeps
+ *     about its descriptor upload and its last use per stream is locked; a plan handed
+ *     to an _async staged call is used by the stager's thread until its ticket is issued).
  *   - There is no CPU fallback: without a CUDA device pack and unpack fail with
  *     LUMEN_KV_ECUDA, and so does every plan_build that has descriptors to upload.
  */

@@ -48,6 +48,10 @@ struct Blob {
     cudaEvent_t uploaded = nullptr;   // recorded behind the descriptor copy on the upload stream
     bool upload_seen = false;         // that event has been seen complete: no wait is needed any more
     std::vector<std::pair<cudaStream_t, cudaEvent_t>> uses;  // last use per stream
+    // guards upload_seen, uses and captured: a plan handed to an _async staged call is launched
+    // from the stager's thread at a time the caller cannot observe, possibly while the caller
+    // uses the same plan in another call
+    std::mutex mu;
 };
 
 namespace {
@@ -178,7 +182,9 @@ namespace {
 // complete, so that no event wait sits between two kernels of a decode loop).
 int await_upload(lumen_kv_plan* p, cudaStream_t stream) {
     Blob* b = p->blob;
-    if (!b || b->upload_seen || !b->uploaded) return LUMEN_KV_OK;
+    if (!b) return LUMEN_KV_OK;
+    std::lock_guard<std::mutex> g(b->mu);
+    if (b->upload_seen || !b->uploaded) return LUMEN_KV_OK;
     cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
     if (cudaStreamIsCapturing(stream, &cs) != cudaSuccess) (void)cudaGetLastError();
     if (cs != cudaStreamCaptureStatusNone) {
@@ -213,6 +219,7 @@ int note_use(lumen_kv_plan* p, cudaStream_t stream) {
     // never recycled.
     cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
     if (cudaStreamIsCapturing(stream, &cs) != cudaSuccess) (void)cudaGetLastError();
+    std::lock_guard<std::mutex> g(b->mu);
     if (cs != cudaStreamCaptureStatusNone) {
         b->captured = true;
         return LUMEN_KV_OK;

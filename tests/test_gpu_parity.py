@@ -462,6 +462,61 @@ def test_staged_async_parity_and_ordering(G):
         G.release(whole)
 
 
+def test_uploaded_plan_used_from_several_threads_and_a_stager_at_once(G):
+    """One plan whose descriptors were uploaded (NO_INLINE) is used by four host threads, each
+    packing on a stream of its own, while a stager's thread issues an _async staged pack of the
+    same plan: the plan's bookkeeping (upload seen, last use per stream) is shared by all of
+    them.  Every buffer must equal the oracle's, round after round."""
+    import threading
+    import torch
+    lk = G.lk
+    w = cfg2_qwen32b(L=2, N=1200, n_reqs=5, prompt=1000)
+    seed = 77
+    K, V = G.host_planes(w.geom, seed)
+    B_ref = oracle.pack(w.geom, K, V, w.reqs)
+    pool = G.make_pool(w.geom, seed)
+    ring = G.StagingRing(1 << 20, 3)
+    host_whole, host_buf = G.alloc_buffer(w.payload_bytes, "host")
+    n_threads, rounds = 4, 6
+    bufs = [torch.zeros(w.payload_bytes, dtype=torch.uint8, device="cuda") for _ in range(n_threads)]
+    streams = [torch.cuda.Stream() for _ in range(n_threads)]
+    torch.cuda.synchronize()
+    for rnd in range(rounds):
+        plan = lk.lumen_kv_plan_build(pool.geom, w.reqs, lk.LUMEN_KV_KERNEL_WARP | lk.LUMEN_KV_NO_INLINE)
+        errors = []
+        start = threading.Barrier(n_threads + 1)
+
+        def worker(i):
+            try:
+                start.wait()
+                for _ in range(8):        # each call records a use of the plan on this thread's stream
+                    lk.lumen_kv_checkpoint_pack(plan, pool.k_ptrs, pool.v_ptrs, bufs[i].data_ptr(),
+                                                plan.nbytes, lk.LUMEN_KV_MEM_DEVICE, streams[i].cuda_stream)
+            except Exception as e:        # noqa: BLE001
+                errors.append(e)
+
+        threads = [threading.Thread(target=worker, args=(i,)) for i in range(n_threads)]
+        for t in threads:
+            t.start()
+        start.wait()
+        ticket = lk.lumen_kv_checkpoint_pack_staged_async(plan, pool.k_ptrs, pool.v_ptrs, host_buf.data_ptr(),
+                                                          plan.nbytes, ring.stager, 0)
+        for t in threads:
+            t.join()
+        plan.close()                      # freed while the stager may still be issuing from it
+        ring.stager.sync(ticket)
+        torch.cuda.synchronize()
+        assert not errors, errors
+        for i in range(n_threads):
+            assert np.array_equal(G.buf_to_np(bufs[i], w.payload_bytes), B_ref), f"round {rnd}, thread {i}"
+            bufs[i].zero_()
+        assert np.array_equal(G.buf_to_np(host_buf, w.payload_bytes), B_ref), f"round {rnd}, staged"
+        assert G.guards_intact(host_whole, w.payload_bytes)
+        host_buf.zero_()
+    ring.close()
+    G.release(host_whole)
+
+
 def test_staged_async_mixed_with_sync_errors_and_flags(G):
     import threading
     import torch
