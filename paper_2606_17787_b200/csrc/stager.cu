@@ -15,6 +15,10 @@
 #include "lumen_kv.h"
 #include "plan.hpp"
 
+namespace lumen {
+extern thread_local int t_last_cuda_error;   // lib.cu: what lumen_kv_last_cuda_error() returns
+}
+
 namespace {
 
 // One asynchronous call waiting for (or being issued by) the stager's thread.
@@ -34,6 +38,8 @@ struct TicketRec {
     uint64_t id = 0;
     cudaEvent_t done = nullptr;    // recorded behind the call's last operation once issued
     int status = LUMEN_KV_OK;
+    int cuda_error = 0;            // the cudaError_t behind a failed status (seen on the worker's thread)
+    int waiters = 0;               // stager_wait / stager_sync calls holding `done`: not pruned meanwhile
     bool issued = false;
 };
 
@@ -232,6 +238,7 @@ void worker_main(lumen_kv_stager* st) {
                 if (t.id == job.ticket) {
                     t.done = done;
                     t.status = rc;
+                    t.cuda_error = rc == LUMEN_KV_OK ? 0 : t_last_cuda_error;
                     t.issued = true;
                 }
         }
@@ -258,35 +265,51 @@ int run_staged_async(const lumen_kv_plan* plan, const void* const* k_planes,
         }
         plan_retain(plan);
     }
-    {
+    try {
         std::lock_guard<std::mutex> g(st->mu);
-        // completed tickets leave at the front (calls complete in submission order)
+        // completed tickets leave at the front (calls complete in submission order), unless a
+        // stager_wait / stager_sync on another thread still holds their event
         while (st->tickets.size() > 64 && st->tickets.front().issued &&
+               st->tickets.front().waiters == 0 &&
                (!st->tickets.front().done ||
                 cudaEventQuery(st->tickets.front().done) == cudaSuccess)) {
             if (st->tickets.front().done) cudaEventDestroy(st->tickets.front().done);
             st->tickets.pop_front();
         }
         (void)cudaGetLastError();
+        if (!empty && !st->worker_started) {
+            st->worker = std::thread(worker_main, st);   // may throw: nothing is queued yet
+            st->worker_started = true;
+        }
         TicketRec t;
-        t.id = job.ticket = st->next_ticket++;
+        t.id = st->next_ticket;
         t.issued = empty;          // an empty plan has nothing to issue: complete at once
         st->tickets.push_back(t);
-        *ticket = t.id;
         if (!empty) {
-            st->queue.push_back(std::move(job));
-            if (!st->worker_started) {
-                st->worker_started = true;
-                st->worker = std::thread(worker_main, st);
+            job.ticket = t.id;
+            try {
+                st->queue.push_back(std::move(job));
+            } catch (...) {
+                st->tickets.pop_back();
+                throw;
             }
         }
+        *ticket = st->next_ticket++;
+    } catch (...) {                // bad_alloc, system_error: nothing may cross the C boundary
+        if (!empty) {
+            cudaEventDestroy(job.begin);
+            plan_release(plan);
+        }
+        return LUMEN_KV_ENOMEM;
     }
     if (!empty) st->cv.notify_all();
     return LUMEN_KV_OK;
 }
 
 // Blocks until the ticket has been issued; *done receives its completion event (nullptr: nothing
-// to wait for).  Returns the call's status.
+// to wait for) and the ticket is pinned against pruning until unpin() -- another thread's _async
+// call would otherwise be free to destroy the event once it has completed.  Returns the call's
+// status; a failed call's cudaError_t is handed to the calling thread (lumen_kv_last_cuda_error).
 int wait_issued(lumen_kv_stager* st, uint64_t ticket, cudaEvent_t* done) {
     *done = nullptr;
     std::unique_lock<std::mutex> lk(st->mu);
@@ -297,11 +320,24 @@ int wait_issued(lumen_kv_stager* st, uint64_t ticket, cudaEvent_t* done) {
             if (t.id == ticket) rec = &t;
         if (!rec) return LUMEN_KV_OK;              // pruned: complete long ago
         if (rec->issued) {
-            *done = rec->done;
-            return rec->status;
+            if (rec->status != LUMEN_KV_OK) {
+                t_last_cuda_error = rec->cuda_error;
+                return rec->status;
+            }
+            if (rec->done) {
+                *done = rec->done;
+                ++rec->waiters;
+            }
+            return LUMEN_KV_OK;
         }
         st->cv.wait(lk);
     }
+}
+
+void unpin(lumen_kv_stager* st, uint64_t ticket) {
+    std::lock_guard<std::mutex> g(st->mu);
+    for (TicketRec& t : st->tickets)
+        if (t.id == ticket) --t.waiters;
 }
 
 }  // namespace
@@ -425,7 +461,10 @@ int lumen_kv_stager_query(lumen_kv_stager* st, uint64_t ticket) {
     for (const TicketRec& t : st->tickets)
         if (t.id == ticket) {
             if (!t.issued) return 0;
-            if (t.status != LUMEN_KV_OK) return t.status;
+            if (t.status != LUMEN_KV_OK) {
+                lumen::t_last_cuda_error = t.cuda_error;
+                return t.status;
+            }
             if (!t.done) return 1;
             const cudaError_t e = cudaEventQuery(t.done);
             if (e == cudaSuccess) return 1;
@@ -441,6 +480,7 @@ int lumen_kv_stager_wait(lumen_kv_stager* st, uint64_t ticket, void* stream) {
     const int rc = lumen::wait_issued(st, ticket, &done);
     if (rc != LUMEN_KV_OK || !done) return rc;
     const cudaError_t e = cudaStreamWaitEvent(static_cast<cudaStream_t>(stream), done, 0);
+    lumen::unpin(st, ticket);
     return e == cudaSuccess ? LUMEN_KV_OK : lumen::cuda_fail(e);
 }
 
@@ -450,6 +490,7 @@ int lumen_kv_stager_sync(lumen_kv_stager* st, uint64_t ticket) {
     const int rc = lumen::wait_issued(st, ticket, &done);
     if (rc != LUMEN_KV_OK || !done) return rc;
     const cudaError_t e = cudaEventSynchronize(done);
+    lumen::unpin(st, ticket);
     return e == cudaSuccess ? LUMEN_KV_OK : lumen::cuda_fail(e);
 }
 

@@ -517,6 +517,62 @@ def test_uploaded_plan_used_from_several_threads_and_a_stager_at_once(G):
     G.release(host_whole)
 
 
+def test_stager_wait_and_sync_race_ticket_pruning(G):
+    """a stager keeps 64 tickets and prunes completed ones when a new call is
+    submitted.  Threads that wait on / synchronise with old tickets while another thread keeps
+    submitting must never be handed a destroyed event: every wait and sync returns OK and the
+    last buffer equals the oracle's."""
+    import threading
+    import torch
+    lk = G.lk
+    w = cfg0_tiny()
+    K, V = G.host_planes(w.geom, 9)
+    B_ref = oracle.pack(w.geom, K, V, w.reqs)
+    pool = G.make_pool(w.geom, 9)
+    ring = G.StagingRing(4096, 2)
+    whole, buf = G.alloc_buffer(w.payload_bytes, "host")
+    plan = lk.lumen_kv_plan_build(pool.geom, w.reqs)
+    n_calls = 600
+    tickets, errors = [], []
+    done = threading.Event()
+
+    def waiter(k):
+        side = torch.cuda.Stream()
+        rng = np.random.default_rng(k)
+        try:
+            while True:
+                if not tickets:
+                    continue
+                t = tickets[int(rng.integers(max(0, len(tickets) - 80), len(tickets)))]
+                if rng.integers(2):
+                    ring.stager.wait(t, side.cuda_stream)
+                else:
+                    ring.stager.sync(t)
+                assert ring.stager.query(t) in (True, False)
+                if done.is_set():
+                    break
+            side.synchronize()
+        except Exception as e:            # noqa: BLE001
+            errors.append(e)
+
+    threads = [threading.Thread(target=waiter, args=(k,)) for k in range(3)]
+    for t in threads:
+        t.start()
+    for _ in range(n_calls):
+        tickets.append(lk.lumen_kv_checkpoint_pack_staged_async(plan, pool.k_ptrs, pool.v_ptrs, buf.data_ptr(),
+                                                                plan.nbytes, ring.stager, 0))
+    done.set()
+    for t in threads:
+        t.join()
+    ring.stager.sync(tickets[-1])
+    assert not errors, errors
+    assert tickets == list(range(tickets[0], tickets[0] + n_calls))
+    assert np.array_equal(G.buf_to_np(buf, w.payload_bytes), B_ref)
+    assert G.guards_intact(whole, w.payload_bytes)
+    plan.close(); ring.close()
+    G.release(whole)
+
+
 def test_staged_async_mixed_with_sync_errors_and_flags(G):
     import threading
     import torch
