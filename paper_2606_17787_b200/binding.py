@@ -732,11 +732,13 @@ class BackgroundCheckpointer:
     """Owner of a `lumen_kv_ckpt*` (the worker's background checkpointing thread).
     sink(request_id, t_begin, t_end, delta_ptr, delta_bytes, tags) is called on that thread
     (tags: a TAG_DTYPE array, empty unless notify() was given token IDs) and returns None / 0
-    when it took the delta, another int to reject it; or pass a Store."""
+    when it took the delta, another int to reject it (an exception rejects it too and is chained
+    to the error flush() raises); or pass a Store."""
 
     def __init__(self, geom: lumen_kv_geom, k_planes, v_planes, staging_ptr: int, slot_bytes: int,
                  n_slots: int, pinned_ptr: int, pinned_bytes: int, sink):
         L = geom.num_layers
+        self.sink_exception = None       # first exception a Python sink raised (re-raised by flush)
         if isinstance(sink, Store):      # native sink: deltas go straight into the store, no Python
             self._keep = sink
             self._cb = ctypes.cast(_lib().lumen_kv_store_sink, SINK_FN)
@@ -745,8 +747,16 @@ class BackgroundCheckpointer:
             def _call(_u, rid, tb, te, ptr, nb, tags, n_tags):
                 t = (np.ctypeslib.as_array((ctypes.c_uint8 * (16 * n_tags)).from_address(tags)).view(TAG_DTYPE).copy()
                      if n_tags else np.zeros(0, dtype=TAG_DTYPE))
-                rc = sink(int(rid), int(tb), int(te), int(ptr), int(nb), t)
-                return int(rc) if rc else 0          # None / 0: taken; anything else: rejected
+                # ctypes swallows an exception raised inside a callback and hands 0 to the C side,
+                # which would read "taken" and drop the delta silently: reject it instead, and keep
+                # the exception for flush()
+                try:
+                    rc = sink(int(rid), int(tb), int(te), int(ptr), int(nb), t)
+                    return int(rc) if rc else 0      # None / 0: taken; anything else: rejected
+                except BaseException as exc:         # noqa: BLE001
+                    if self.sink_exception is None:
+                        self.sink_exception = exc
+                    return -1
             self._cb = SINK_FN(_call)
             user = None
         out = ctypes.c_void_p()
@@ -790,7 +800,15 @@ class BackgroundCheckpointer:
                                                 ctypes.c_void_p(int(ready_event))), "lumen_kv_ckpt_notify")
 
     def flush(self) -> None:
-        self._check(_lib().lumen_kv_ckpt_flush(self._h), "lumen_kv_ckpt_flush")
+        """Raises LumenKVError(LUMEN_KV_ESINK) if a delta was rejected; if the rejection was an
+        exception raised by a Python sink, that exception is its __cause__ (once)."""
+        try:
+            self._check(_lib().lumen_kv_ckpt_flush(self._h), "lumen_kv_ckpt_flush")
+        except LumenKVError as e:
+            exc, self.sink_exception = self.sink_exception, None
+            if exc is not None:
+                raise e from exc
+            raise
 
     def progress(self, request_id: int) -> int:
         return self._check(_lib().lumen_kv_ckpt_progress(self._h, int(request_id)), "lumen_kv_ckpt_progress")

@@ -264,3 +264,55 @@ def test_sink_rejection_keeps_progress_and_surfaces(lk):
             assert np.array_equal(data, ref)
         assert at == bg.progress(rid)
     bg.close()
+
+
+@pytest.mark.gpu
+def test_raising_sink_rejects_the_delta(lk):
+    """ctypes turns an exception inside the sink callback into a return value of 0,
+    which the checkpointer would read as "taken".  The binding must hand back a rejection instead:
+    progress stays where it was, flush() raises ESINK with the sink's exception as its cause, and a
+    later notification delivers the same tokens again."""
+    import ctypes
+    import torch
+    from tests import gpu_util as G
+    G.build_all()
+    w = cfg1_qwen14b(L=2, N=512, n_reqs=2, grow_iters=4, median=60, hi=64, lo=50)
+    L, H, D, S, N = w.geom
+    tokb = 2 * L * H * D * 2
+    pool = G.make_pool(w.geom, 5)
+    K, V = G.host_planes(w.geom, 5)
+    ring_mem = torch.empty(3 << 20, dtype=torch.uint8, device="cuda")
+    pinned = G.pinned_buffer(256 * tokb)
+    got = {0: [], 1: []}
+    state = {"raise": True}
+
+    def sink(rid, tb, te, ptr, nb, tags):
+        if rid == 1 and state["raise"]:
+            raise RuntimeError("sink broke")
+        got[rid].append((tb, te, np.ctypeslib.as_array((ctypes.c_uint16 * (nb // 2)).from_address(ptr)).copy()))
+
+    bg = lk.BackgroundCheckpointer(pool.geom, pool.k_ptrs, pool.v_ptrs, ring_mem.data_ptr(), 1 << 20, 3,
+                                   pinned.data_ptr(), pinned.numel(), sink)
+    lens = [te for _, _, te in w.reqs]
+    bg.track(0, 0); bg.track(1, 0)
+    bg.notify([0, 1], [(pt, 0, n) for (pt, _, n) in w.reqs])
+    with pytest.raises(lk.LumenKVError) as e:
+        bg.flush()
+    assert e.value.status == lk.LUMEN_KV_ESINK
+    assert isinstance(e.value.__cause__, RuntimeError) and "sink broke" in str(e.value.__cause__)
+    assert bg.progress(0) == lens[0] and bg.progress(1) == 0 and got[1] == []
+    state["raise"] = False
+    bg.notify([1], [(w.reqs[1][0], 0, lens[1])])
+    try:
+        bg.flush()
+    except lk.LumenKVError as e2:                             # first_error is sticky by design
+        assert e2.status == lk.LUMEN_KV_ESINK and e2.__cause__ is None
+    assert bg.progress(1) == lens[1]
+    for rid in (0, 1):
+        at = 0
+        for tb, te, data in got[rid]:
+            assert tb == at
+            at = te
+            assert np.array_equal(data, oracle.pack(w.geom, K, V, [(w.reqs[rid][0], tb, te)]))
+        assert at == lens[rid]
+    bg.close()
