@@ -81,7 +81,10 @@
 extern "C" {
 #endif
 
-#define LUMEN_KV_VERSION 1
+/* 2: lumen_kv_sink_fn returns an int (0 = delta taken; version 1 sinks returned void),
+ *    LUMEN_KV_MEM_DEVICE means memory of the CURRENT device, LUMEN_KV_MEM_DEVICE_PEER,
+ *    lumen_kv_copy_noalloc, LUMEN_KV_ECAPACITY.  Compare lumen_kv_version() with the header's. */
+#define LUMEN_KV_VERSION 2
 
 #if defined(__GNUC__)
 #define LUMEN_KV_API __attribute__((visibility("default")))
@@ -145,12 +148,17 @@ typedef struct lumen_kv_plan lumen_kv_plan;  /* opaque; library owns its descrip
 #define LUMEN_KV_KERNEL_BULK         0x200u /* TMA 1-D bulk copies through a shared-memory ring */
 
 /* where the checkpoint buffer lives */
-#define LUMEN_KV_MEM_DEVICE      0  /* device pointer into the CURRENT device's memory (HBM)  */
+#define LUMEN_KV_MEM_DEVICE      0  /* device pointer into the CURRENT device's memory (HBM).
+                                       A pointer that cudaPointerGetAttributes places on
+                                       another device is handled as LUMEN_KV_MEM_DEVICE_PEER
+                                       (looked up when a thread first sees the buffer)         */
 #define LUMEN_KV_MEM_DEVICE_PEER 2  /* device pointer into ANOTHER GPU's memory (peer access
                                        enabled by the caller): same kernels; the restore does
                                        not ask L2 for its source ahead of the stream-order
                                        wait, because only a device's own memory is cached
-                                       coherently in its L2                                   */
+                                       coherently in its L2.  Tested on one GPU only (a local
+                                       buffer declared as peer): never run against real peer
+                                       memory                                                  */
 #define LUMEN_KV_MEM_HOST_MAPPED 1  /* pinned host memory (cudaHostAlloc / cudaHostRegister);
                                        pass the HOST pointer, the kernel writes/reads it
                                        directly over the host link (zero-copy).  One launch,

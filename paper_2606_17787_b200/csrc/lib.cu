@@ -113,18 +113,34 @@ public:
             free_[std::make_pair(b->device, b->cap)].push_back(b);
     }
 
+    // Every device that owns cached blobs is synchronised before its blobs are destroyed (a blob
+    // of another device than the current one may still have an upload or a kernel in flight).
     void trim() {
-        cudaDeviceSynchronize();
+        int cur = 0;
+        const bool have_cur = cudaGetDevice(&cur) == cudaSuccess;
         std::lock_guard<std::mutex> g(mu_);
+        std::map<int, std::vector<Blob*>> by_dev;
         for (auto& kv : free_)
-            for (Blob* b : kv.second) destroy(b);
+            for (Blob* b : kv.second) by_dev[b->device].push_back(b);
         free_.clear();
-        for (Blob* b : retired_) destroy(b);
+        for (Blob* b : retired_) by_dev[b->device].push_back(b);
         retired_.clear();
+        for (auto& kv : by_dev) {
+            if (cudaSetDevice(kv.first) == cudaSuccess) cudaDeviceSynchronize();
+            for (Blob* b : kv.second) destroy(b);
+        }
+        if (have_cur) cudaSetDevice(cur);
+        (void)cudaGetLastError();
     }
 
 private:
     static bool idle(Blob* b) {
+        // the descriptor upload reads the pinned staging: a plan built and freed unused must
+        // not have it rewritten under the copy
+        if (b->uploaded && cudaEventQuery(b->uploaded) != cudaSuccess) {
+            (void)cudaGetLastError();
+            return false;
+        }
         for (auto& u : b->uses)
             if (cudaEventQuery(u.second) != cudaSuccess) {
                 (void)cudaGetLastError();
@@ -320,6 +336,33 @@ int plan_chunks(const lumen_kv_plan* plan_, int64_t slot_bytes,
 
 namespace {
 
+// LUMEN_KV_MEM_DEVICE promises memory of the current device (its L2 may be asked for the bytes
+// early).  A caller that passes a peer GPU's buffer under that kind -- legal before the kinds were
+// told apart -- must not get stale data for it: the owner is looked up when a thread sees a
+// buffer for the first time (one pointer comparison per call afterwards), and a buffer of
+// another device is handled as LUMEN_KV_MEM_DEVICE_PEER.  A lookup that fails decides nothing.
+bool buffer_is_local(const void* buf) {
+    static thread_local const void* seen_buf = nullptr;
+    static thread_local int seen_dev = -1;
+    static thread_local bool seen_local = true;
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) {
+        (void)cudaGetLastError();
+        return true;
+    }
+    if (buf == seen_buf && dev == seen_dev) return seen_local;
+    cudaPointerAttributes at;
+    bool local = true;
+    if (cudaPointerGetAttributes(&at, buf) == cudaSuccess)
+        local = !(at.type == cudaMemoryTypeDevice && at.device != dev);
+    else
+        (void)cudaGetLastError();
+    seen_buf = buf;
+    seen_dev = dev;
+    seen_local = local;
+    return local;
+}
+
 int run_copy(const lumen_kv_plan* plan, const void* const* k_planes, const void* const* v_planes,
              void* buf, int64_t buf_bytes, int kind, void* stream, bool pack) {
     if (!plan) return LUMEN_KV_EINVAL;
@@ -344,6 +387,7 @@ int run_copy(const lumen_kv_plan* plan, const void* const* k_planes, const void*
         }
     }
     if (reinterpret_cast<uintptr_t>(dev_buf) & 15) return LUMEN_KV_EINVAL;
+    if (kind == LUMEN_KV_MEM_DEVICE && !buffer_is_local(dev_buf)) kind = LUMEN_KV_MEM_DEVICE_PEER;
     return launch_part(plan, planes, reinterpret_cast<uintptr_t>(dev_buf),
                        kind == LUMEN_KV_MEM_HOST_MAPPED, static_cast<cudaStream_t>(stream), pack, 0,
                        plan->n_runs, 0, 2 * plan->hp.geom.num_layers,
