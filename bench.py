@@ -365,6 +365,36 @@ def cpu_baseline(workload: str, seed: int, budget_s: float = 12.0):
     return out
 
 
+def l2_config(workload: str) -> str:
+    """`config.l2`, the same string in both arms (what is specific to an arm sits in `l2_note`)."""
+    return "fits in L2" if workload == "cfg0" else "inputs larger than L2"
+
+
+def flat_summary(line: dict) -> dict:
+    """The scalars a reader of the driver's record needs, as the LAST key of the line (the record
+    keeps the tail): large-config fractions, the staged host fractions, how often the headline
+    region was taken."""
+    out = {"headline_attempts_n": len(line.get("headline_attempts") or []),
+           "roofline_frac": (line.get("roofline") or {}).get("frac"),
+           "e2e_value": (line.get("e2e") or {}).get("value"),
+           "e2e_duplex_frac_of_duplex_memcpy_peak": (line.get("e2e") or {}).get("duplex_frac_of_duplex_memcpy_peak"),
+           "host_bound": line.get("host_bound")}
+    lc = line.get("large_configs") or {}
+    for key, tag in (("cfg2", "cfg2"), ("cfg4_wave0", "cfg4w0")):
+        c = lc.get(key) or {}
+        if c:
+            out[f"{tag}_hbm_frac"] = c.get("frac")
+            out[f"{tag}_pack_ms"] = c.get("pack_ms")
+            out[f"{tag}_unpack_ms"] = c.get("unpack_ms")
+            out[f"{tag}_ms_per_step"] = c.get("ms_per_step")
+            out[f"{tag}_host_enqueue_ms_per_step"] = c.get("host_enqueue_ms_per_step")
+        hs = c.get("host_staged") or {}
+        if "pack_frac_of_d2h_memcpy" in hs:
+            out[f"{tag}_staged_pack_frac"] = hs["pack_frac_of_d2h_memcpy"]
+            out[f"{tag}_staged_restore_frac"] = hs["restore_frac_of_h2d_memcpy"]
+    return out
+
+
 def run_reference(args):
     """--impl reference: the oracle, as it stands, on the host cores; rank 0 only."""
     if rank_env()[0] != 0:
@@ -390,9 +420,10 @@ def run_reference(args):
             "config": {"workload": label,
                        "payload_bytes_per_direction_per_step": int(w.tokens) * 4 * w.geom[0] * w.geom[1] * w.geom[2],
                        "tokens_per_step": int(w.tokens),
-                       "l2": "CPU arm: every step touches far more than the host caches hold "
-                             "(the step's sample is named in cpu_baseline.sample)",
+                       "l2": l2_config(args.workload),
                        "seed": hex(MASTER_SEED)},
+            "l2_note": "CPU arm: every step touches far more than the host caches hold "
+                       "(the step's sample is named in cpu_baseline.sample)",
             "timed_steps": timed,
             "cpu_baseline": {"value": val, "unit": "GB/s", "cores": 1, "kind": "oracle",
                              "sample": f"each step = {what}; plain single-thread C oracle"},
@@ -476,6 +507,28 @@ def memcpy_peaks(torch, nbytes=1 << 30):
             a.record(); dst.copy_(src, non_blocking=True); b.record(); torch.cuda.synchronize()
             best = min(best, a.elapsed_time(b))
         out[name] = nbytes / best / 1e6
+    # both directions at once: what two concurrent copies over the full-duplex link really reach
+    # (less than d2h + h2d: the two directions share the host's memory system)
+    h2 = torch.empty(nbytes, dtype=torch.uint8, pin_memory=True)
+    d2 = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+    sa, sb = torch.cuda.Stream(), torch.cuda.Stream()
+    best = float("inf")
+    for _ in range(10):
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        join = torch.cuda.Event()
+        torch.cuda.synchronize()
+        a.record(sa)
+        sb.wait_event(a)
+        with torch.cuda.stream(sa):
+            h.copy_(d, non_blocking=True)
+        with torch.cuda.stream(sb):
+            d2.copy_(h2, non_blocking=True)
+        join.record(sb)
+        sa.wait_event(join)
+        b.record(sa)
+        torch.cuda.synchronize()
+        best = min(best, a.elapsed_time(b))
+    out["duplex"] = 2 * nbytes / best / 1e6
     return out
 
 
@@ -1009,6 +1062,8 @@ def run_ours(args):
                                    "streams, ordered by events on the two host buffers (a8, full duplex)")
             e2e["duplex_frac_of_d2h_plus_h2d_peak"] = (e2e["staged_duplex_value"] / world /
                                                        (link["d2h"] + link["h2d"]))
+            e2e["memcpy_peak_duplex_GBps"] = link["duplex"]
+            e2e["duplex_frac_of_duplex_memcpy_peak"] = e2e["staged_duplex_value"] / world / link["duplex"]
         e2e["value"] = job_payload_gbps(world, Ke, P, ms_best)
         e2e["ms_per_step"] = ms_best / Ke
         probe = lk.lumen_kv_plan_build(geom, ra_p, lk.LUMEN_KV_HOST_ONLY)
@@ -1031,11 +1086,11 @@ def run_ours(args):
         "runs_per_plan": runs_per_plan,
         "config": {"workload": label, "payload_bytes_per_direction_per_step": P,
                    "tokens_per_step": w.tokens,
-                   "l2": ("fits in L2 (latency config, no roofline claim)" if args.workload == "cfg0" else
-                          f"inputs larger than L2: steps rotate over {n_stage} staging buffers of "
-                          f"{P / 2**20:.0f} MiB and {len(ranges)} distinct delta sets; the restore reads "
-                          f"the buffer packed {lag} steps earlier"),
+                   "l2": l2_config(args.workload),
                    "seed": hex(MASTER_SEED)},
+        "l2_note": ("cfg0 fits in L2 (latency config, no roofline claim)" if args.workload == "cfg0" else
+                    f"steps rotate over {n_stage} staging buffers of {P / 2**20:.0f} MiB and {len(ranges)} "
+                    f"distinct delta sets; the restore reads the buffer packed {lag} steps earlier"),
         "launch_config": {"kernel": args.kernel, "replicas": world,
                           "descriptors": "uploaded" if args.upload_descriptors else "kernel parameters (plans <= 1,024 runs and <= 512 requests; <= 256 / 128 in the small class)",
                           "pdl": os.environ.get("LUMEN_KV_PDL", "1") != "0",
@@ -1093,6 +1148,7 @@ def run_ours(args):
     if rank == 0:
         if world == 1 and not args.no_cpu_baseline:
             line["cpu_baseline"] = cpu_baseline(args.workload, MASTER_SEED)
+        line["summary"] = flat_summary(line)            # last on purpose
         print(json.dumps(line), flush=True)
     if dist is not None:
         dist.destroy_process_group()
