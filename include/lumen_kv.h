@@ -168,7 +168,7 @@ typedef struct lumen_kv_plan lumen_kv_plan;  /* opaque; library owns its descrip
                                        the copy engine uses 256-byte TLPs: this path tops out
                                        at 92 % of what cudaMemcpyAsync reaches (measured 52.8
                                        of 57.3 GB/s D2H, 51.5 of 55.6 H2D; counters in
-                                       profiles/r2_README.md) whatever kernel, grid or
+                                       profiles/README.md) whatever kernel, grid or
                                        operation size is used.  The staged calls below move
                                        the same bytes with the copy engine (99 %).            */
 
