@@ -492,7 +492,7 @@ def ncu_traffic(workload: str, kernel: str, direction: str):
         return None, None
     r = rows[-1]                                        # the newest capture is appended last
     return (int(r["dram_bytes_read"]) + int(r["dram_bytes_write"]),
-            f"profiles/{r['source']} (committed ncu --set full capture, not measured in this run)")
+            f"profiles/{r['source']} (committed ncu capture, {r.get('capture') or 'cold'}; not measured in this run)")
 
 
 def memcpy_peaks(torch, nbytes=1 << 30):
