@@ -329,6 +329,15 @@ LUMEN_KV_API int lumen_kv_copy_noalloc(const lumen_kv_plan* plan, int direction,
  * One stager serves one staged call at a time (calls on it are serialised by its events);
  * use one stager per direction to run pack and restore concurrently.
  *
+ * After an error.  A staged call that fails with ECUDA half-way (a launch or copy was refused)
+ * first waits for everything it did enqueue -- on `stream` and on the stager's copy stream --
+ * and then returns: the staging ring is consistent again and the stager can be used for the next
+ * call (a restore with ready flags still needs the flags of the chunks that were issued).  The
+ * host buffer (pack) or the plan's pool slots (restore) then hold a mixture of old and new
+ * bytes; nothing outside them is touched.  An asynchronous call reports the failure, with its
+ * cudaError_t, through lumen_kv_stager_query / _wait / _sync of its ticket; later tickets are
+ * still issued.
+ *
  * Stream semantics are those of the one-shot calls: the work is ordered after everything
  * enqueued on `stream` before the call, and work enqueued on `stream` after the call sees
  * the complete result (host buffer for pack, pool for restore).  host buffers: pinned
@@ -673,6 +682,8 @@ LUMEN_KV_API int lumen_kv_init(void);
  *   "host_kernel" 2 (default, TMA bulk kernel) / 1 (SIMT kernel): what AUTO picks for a host buffer
  *   "host_ctas"   0 (default: 24..96 by item size) / n : grid of the bulk kernel on a host buffer
  *   "inline_max_runs" 1024 (default) / n : plans of more than n runs upload their descriptors
+ *   "fail_after_chunks" -1 (default, off) / n >= 0 : TEST HOOK -- every staged call fails with ECUDA
+ *                 (cudaErrorUnknown) in front of its chunk n; used to test the error paths
  *   "prefetch"    16 (default) / d >= 0 / -1 : the SIMT kernel asks L2 for the 4 KiB a warp d CTAs
  *                 further on will copy (parameter-resident plans; larger plans announce their own
  *                 4 KiB, whatever d) / no prefetch.  A hint: the bytes moved are the same.

@@ -17,6 +17,8 @@ struct Blob;   // descriptor blob of the arena (lib.cu)
 
 // records the CUDA error for lumen_kv_last_cuda_error() and returns LUMEN_KV_ECUDA
 int cuda_fail(cudaError_t e);
+// failure injection for the staged paths (stager.cu)
+extern std::atomic<int> g_fail_after_chunks;
 }  // namespace lumen
 
 struct lumen_kv_plan {

@@ -542,6 +542,10 @@ int lumen_kv_set_option(const char* name, int value) {
         lumen::g_inline_max_runs = value < 0 ? 0 : (value > lumen::kInlineRunsL ? lumen::kInlineRunsL : value);
         return LUMEN_KV_OK;
     }
+    if (name && !std::strcmp(name, "fail_after_chunks")) {   // error-path tests of the staged calls
+        lumen::g_fail_after_chunks.store(value < 0 ? -1 : value);
+        return LUMEN_KV_OK;
+    }
     return lumen::set_option(name, value) == 0 ? LUMEN_KV_OK : LUMEN_KV_EINVAL;
 }
 

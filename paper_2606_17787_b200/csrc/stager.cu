@@ -17,6 +17,9 @@
 
 namespace lumen {
 extern thread_local int t_last_cuda_error;   // lib.cu: what lumen_kv_last_cuda_error() returns
+// lumen_kv_set_option("fail_after_chunks", n): every staged call fails with ECUDA in front of
+// its chunk n (0: before anything is enqueued); -1 (default): off.  For tests of the error paths.
+std::atomic<int> g_fail_after_chunks{-1};
 }
 
 namespace {
@@ -145,7 +148,7 @@ int prepare(const lumen_kv_plan* plan, const void* const* k_planes, const void* 
 
 // The per-chunk pipeline of one call, kernels on `stream`, transfers on the stager's copy
 // stream.  Called with st->issue_mu held.
-int issue(lumen_kv_stager* st, const Job& j, cudaStream_t stream) {
+int issue_chunks(lumen_kv_stager* st, const Job& j, cudaStream_t stream) {
     const lumen_kv_plan* plan = j.plan;
     const bool pack = j.pack;
     int64_t ci = 0;                     // chunk index = entry of lumen_kv_plan_get_chunks
@@ -154,7 +157,9 @@ int issue(lumen_kv_stager* st, const Job& j, cudaStream_t stream) {
         LUMEN_CUDA(cudaEventRecord(st->join, stream));
         LUMEN_CUDA(cudaStreamWaitEvent(st->copy, st->join, 0));
     }
+    const int fail_at = g_fail_after_chunks.load(std::memory_order_relaxed);
     for (const Chunk& c : *j.chunks) {
+        if (fail_at >= 0 && ci >= fail_at) return cuda_fail(cudaErrorUnknown);   // test hook
         const int slot = static_cast<int>(st->next++ % st->n_slots);
         char* sbase = st->base + int64_t{slot} * st->slot_bytes;
         // the address byte 0 of the checkpoint buffer would have if the chunk sat in this slot
@@ -189,6 +194,25 @@ int issue(lumen_kv_stager* st, const Job& j, cudaStream_t stream) {
         LUMEN_CUDA(cudaStreamWaitEvent(stream, st->join, 0));
     }
     return LUMEN_KV_OK;
+}
+
+// A call that fails half-way leaves slot events half-recorded: a kernel may have been launched
+// into a slot whose copy was never enqueued, and a later call -- possibly on another stream --
+// would find that slot "free" while the kernel still writes it.  So a failed call drains what it
+// did enqueue before it reports: once `stream` and the copy stream are idle every recorded slot
+// event is complete and any slot may be reused; the stager stays usable.  (A restore with ready
+// flags still needs the flags of the chunks it did issue.  Under stream capture nothing can be
+// drained; the capture is invalid after an error anyway.)  The error seen first is the one kept
+// for lumen_kv_last_cuda_error().
+int issue(lumen_kv_stager* st, const Job& j, cudaStream_t stream) {
+    const int rc = issue_chunks(st, j, stream);
+    if (rc == LUMEN_KV_OK) return rc;
+    const int first = t_last_cuda_error;
+    cudaStreamSynchronize(stream);
+    cudaStreamSynchronize(st->copy);
+    (void)cudaGetLastError();
+    t_last_cuda_error = first;
+    return rc;
 }
 
 int run_staged(const lumen_kv_plan* plan, const void* const* k_planes, const void* const* v_planes,

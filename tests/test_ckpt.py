@@ -316,3 +316,76 @@ def test_raising_sink_rejects_the_delta(lk):
             assert np.array_equal(data, oracle.pack(w.geom, K, V, [(w.reqs[rid][0], tb, te)]))
         assert at == lens[rid]
     bg.close()
+
+
+@pytest.mark.gpu
+def test_blocking_sink_and_failing_pack_do_not_hang_the_checkpointer(lk):
+    """(a) destroying a checkpointer whose sink is blocked for two
+    seconds waits for the sink and returns -- no deadlock; (b) a staged pack that fails inside the
+    background thread (failure injection) is reported by flush() as ECUDA, progress does not move,
+    and after the fault is gone a new notification delivers the tokens."""
+    import ctypes
+    import threading
+    import time
+    import torch
+    from tests import gpu_util as G
+    G.build_all()
+    w = cfg1_qwen14b(L=2, N=512, n_reqs=2, grow_iters=4, median=60, hi=64, lo=50)
+    L, H, D, S, N = w.geom
+    tokb = 2 * L * H * D * 2
+    pool = G.make_pool(w.geom, 5)
+    K, V = G.host_planes(w.geom, 5)
+    lens = [te for _, _, te in w.reqs]
+    ring_mem = torch.empty(3 << 20, dtype=torch.uint8, device="cuda")
+    pinned = G.pinned_buffer(256 * tokb)
+    entered = threading.Event()
+    got = []
+
+    def slow_sink(rid, tb, te, ptr, nb, tags):
+        entered.set()
+        time.sleep(2.0)
+        got.append((rid, tb, te))
+
+    bg = lk.BackgroundCheckpointer(pool.geom, pool.k_ptrs, pool.v_ptrs, ring_mem.data_ptr(), 1 << 20, 3,
+                                   pinned.data_ptr(), pinned.numel(), slow_sink)
+    bg.track(0, 0)
+    bg.notify([0], [(w.reqs[0][0], 0, lens[0])])
+    assert entered.wait(20.0)
+    t0 = time.perf_counter()
+    closer = threading.Thread(target=bg.close)
+    closer.start()
+    closer.join(30.0)
+    assert not closer.is_alive(), "lumen_kv_ckpt_destroy hangs behind a blocked sink"
+    assert time.perf_counter() - t0 < 25.0 and got and got[0][0] == 0
+
+    data = {0: [], 1: []}
+
+    def sink(rid, tb, te, ptr, nb, tags):
+        data[rid].append((tb, te, np.ctypeslib.as_array((ctypes.c_uint16 * (nb // 2)).from_address(ptr)).copy()))
+
+    bg = lk.BackgroundCheckpointer(pool.geom, pool.k_ptrs, pool.v_ptrs, ring_mem.data_ptr(), 1 << 20, 3,
+                                   pinned.data_ptr(), pinned.numel(), sink)
+    try:
+        bg.track(0, 0); bg.track(1, 0)
+        lk.lumen_kv_set_option("fail_after_chunks", 0)
+        bg.notify([0, 1], [(pt, 0, n) for (pt, _, n) in w.reqs])
+        with pytest.raises(lk.LumenKVError) as e:
+            bg.flush()
+        assert e.value.status == lk.LUMEN_KV_ECUDA
+        assert bg.progress(0) == 0 and bg.progress(1) == 0 and not data[0] and not data[1]
+    finally:
+        lk.lumen_kv_set_option("fail_after_chunks", -1)
+    bg.notify([0, 1], [(pt, 0, n) for (pt, _, n) in w.reqs])
+    try:
+        bg.flush()
+    except lk.LumenKVError as e2:                             # first_error is sticky by design
+        assert e2.status == lk.LUMEN_KV_ECUDA
+    for rid in (0, 1):
+        assert bg.progress(rid) == lens[rid]
+        at = 0
+        for tb, te, d in data[rid]:
+            assert tb == at
+            at = te
+            assert np.array_equal(d, oracle.pack(w.geom, K, V, [(w.reqs[rid][0], tb, te)]))
+        assert at == lens[rid]
+    bg.close()

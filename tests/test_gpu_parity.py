@@ -573,6 +573,78 @@ def test_stager_wait_and_sync_race_ticket_pruning(G):
     G.release(whole)
 
 
+def test_staged_calls_fail_cleanly_and_the_stager_stays_usable(G):
+    """Failure injection (lumen_kv_set_option("fail_after_chunks", n)): a staged call that fails
+    after n chunks reports ECUDA -- synchronously, or through query / wait / sync of its ticket,
+    with the cudaError_t on the asking thread -- and leaves its stager usable: the next calls on
+    the SAME stager, synchronous and asynchronous, on other streams, are bit-exact; so is a new
+    stager on the same ring memory."""
+    import torch
+    lk = G.lk
+    w = cfg2_qwen32b(L=2, N=1200, n_reqs=3, prompt=1000)      # 12 chunks of <= 1 MiB
+    seed = 41
+    K, V = G.host_planes(w.geom, seed)
+    B_ref = oracle.pack(w.geom, K, V, w.reqs)
+    K2, V2 = G.host_planes(w.geom, seed + 1)
+    oracle.unpack(w.geom, K2, V2, w.restore_reqs, B_ref)
+    pool_a = G.make_pool(w.geom, seed)
+    ring = G.StagingRing(1 << 20, 3)
+    whole, buf = G.alloc_buffer(w.payload_bytes, "host")
+    plan = lk.lumen_kv_plan_build(pool_a.geom, w.reqs)
+    rplan = lk.lumen_kv_plan_build(pool_a.geom, w.restore_reqs, lk.LUMEN_KV_VALIDATE_UNIQUE_DST)
+    assert len(plan.chunks(1 << 20)) > 5
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    try:
+        for n in (0, 1, 4):
+            buf.zero_()
+            lk.lumen_kv_set_option("fail_after_chunks", n)
+            with pytest.raises(lk.LumenKVError) as e:
+                lk.lumen_kv_checkpoint_pack_staged(plan, pool_a.k_ptrs, pool_a.v_ptrs, buf.data_ptr(), plan.nbytes,
+                                                   ring.stager, s1.cuda_stream)
+            assert e.value.status == lk.LUMEN_KV_ECUDA and e.value.cuda_error != 0
+            t_bad = lk.lumen_kv_checkpoint_pack_staged_async(plan, pool_a.k_ptrs, pool_a.v_ptrs, buf.data_ptr(),
+                                                             plan.nbytes, ring.stager, s2.cuda_stream)
+            for ask in (ring.stager.sync, lambda t: ring.stager.wait(t, s1.cuda_stream), ring.stager.query):
+                with pytest.raises(lk.LumenKVError) as e:
+                    ask(t_bad)
+                assert e.value.status == lk.LUMEN_KV_ECUDA and e.value.cuda_error != 0
+            lk.lumen_kv_set_option("fail_after_chunks", -1)
+            # the same stager, another stream: synchronous pack, then an asynchronous restore
+            lk.lumen_kv_checkpoint_pack_staged(plan, pool_a.k_ptrs, pool_a.v_ptrs, buf.data_ptr(), plan.nbytes,
+                                               ring.stager, s2.cuda_stream)
+            s2.synchronize()
+            assert np.array_equal(G.buf_to_np(buf, w.payload_bytes), B_ref), f"pack after failure at chunk {n}"
+            pool_b = G.make_pool(w.geom, seed + 1)
+            t_ok = lk.lumen_kv_restore_unpack_staged_async(rplan, pool_b.k_ptrs, pool_b.v_ptrs, buf.data_ptr(),
+                                                           rplan.nbytes, ring.stager, s1.cuda_stream)
+            assert t_ok == t_bad + 1
+            ring.stager.sync(t_ok)
+            assert ring.stager.query(t_ok)
+            for t, ref in zip(pool_b.planes(), [x for kv in zip(K2, V2) for x in kv]):
+                assert np.array_equal(G.plane_to_np(t), ref), f"restore after failure at chunk {n}"
+            with pytest.raises(lk.LumenKVError):                  # the failed ticket stays failed
+                ring.stager.query(t_bad)
+        # a failing restore, then a second stager on the same ring memory
+        lk.lumen_kv_set_option("fail_after_chunks", 2)
+        pool_c = G.make_pool(w.geom, seed + 1)
+        with pytest.raises(lk.LumenKVError):
+            lk.lumen_kv_restore_unpack_staged(rplan, pool_c.k_ptrs, pool_c.v_ptrs, buf.data_ptr(), rplan.nbytes,
+                                              ring.stager, s1.cuda_stream)
+        lk.lumen_kv_set_option("fail_after_chunks", -1)
+        second = lk.Stager(ring.mem.data_ptr(), 1 << 20, 3)
+        lk.lumen_kv_restore_unpack_staged(rplan, pool_c.k_ptrs, pool_c.v_ptrs, buf.data_ptr(), rplan.nbytes,
+                                          second, s2.cuda_stream)
+        s2.synchronize()
+        for t, ref in zip(pool_c.planes(), [x for kv in zip(K2, V2) for x in kv]):
+            assert np.array_equal(G.plane_to_np(t), ref)
+        second.close()
+    finally:
+        lk.lumen_kv_set_option("fail_after_chunks", -1)
+    assert G.guards_intact(whole, w.payload_bytes)
+    plan.close(); rplan.close(); ring.close()
+    G.release(whole)
+
+
 def test_staged_async_mixed_with_sync_errors_and_flags(G):
     import threading
     import torch
