@@ -540,6 +540,22 @@ LUMEN_KV_API int lumen_kv_store_sink(void* store, uint64_t request_id, int64_t t
                                       int64_t t_end, const void* delta, int64_t delta_bytes,
                                       const lumen_kv_tag* tags, int32_t n_tags);
 LUMEN_KV_API int64_t lumen_kv_store_sink_errors(const lumen_kv_store* store);
+/*
+ * Reserve-then-commit into the store (for lumen_kv_ckpt_set_direct; user = the lumen_kv_store*).
+ * acquire claims [t_begin, t_end) at the tail of the request's reservation and returns the
+ * position inside the arena where its delta belongs (layout of lumen_kv_store_append:
+ * [plane][token][head][dim]), or NULL if the request is unknown, the range does not continue
+ * what is stored plus what is already claimed, the reservation is too small, or a copying
+ * append is in progress.  Claims of one request stack up in order.  The writer fills the bytes,
+ * then calls lumen_kv_store_append / lumen_kv_store_sink with delta == that position: nothing
+ * is copied, and the delta and its tags become visible to lookups only then.
+ * abort voids every outstanding claim of the request; what they covered stays invisible.
+ * lumen_kv_store_arena returns the arena the store was created on.
+ */
+LUMEN_KV_API void* lumen_kv_store_acquire(void* store, uint64_t request_id, int64_t t_begin,
+                                          int64_t t_end, int64_t delta_bytes);
+LUMEN_KV_API void lumen_kv_store_abort(void* store, uint64_t request_id);
+LUMEN_KV_API void* lumen_kv_store_arena(const lumen_kv_store* store, int64_t* arena_bytes);
 LUMEN_KV_API int64_t lumen_kv_store_segments(const lumen_kv_store* store, uint64_t request_id,
                                              int64_t prefix_tokens, lumen_kv_segment* out,
                                              int64_t cap);
@@ -587,6 +603,28 @@ LUMEN_KV_API int lumen_kv_ckpt_create(const lumen_kv_geom* geom, const void* con
                                       int64_t pinned_bytes, lumen_kv_sink_fn sink, void* user,
                                       lumen_kv_ckpt** out);
 LUMEN_KV_API void lumen_kv_ckpt_destroy(lumen_kv_ckpt* ckpt);          /* flushes, joins the thread */
+/*
+ * Reserve-then-commit delivery: the copy engine writes each delta straight to its final place.
+ * By default a delta crosses host memory twice -- copy engine -> the checkpointer's pinned
+ * halves, then the sink copies it to wherever it keeps checkpoints (for the store: 0.65-0.75 of
+ * the D2H peak end to end).  With set_direct, the checkpointer asks `acquire(user, id, t_begin,
+ * t_end, delta_bytes)` for the delta's destination before it packs a batch; if every delta of
+ * the batch gets one (a pointer inside the PINNED region [region, region + region_bytes),
+ * a multiple of one plane row from its base), the batch is packed to those positions and the
+ * sink is then called with delta == that pointer, as the commit.  A claim that will not be
+ * committed (rejected, failed or voided delta) is returned through `abort(user, id)` once no
+ * copy can still be writing it.  Batches whose average delta is below min_avg_delta_bytes, or
+ * for which any acquire returns NULL, go the default way.  acquire == NULL switches it off.
+ * Both callbacks run on the checkpointer's thread.  For a lumen_kv_store: region =
+ * lumen_kv_store_arena, acquire = lumen_kv_store_acquire, abort = lumen_kv_store_abort.
+ * Errors: EINVAL (null, misaligned, region not pinned).
+ */
+typedef void* (*lumen_kv_acquire_fn)(void* user, uint64_t request_id, int64_t t_begin,
+                                      int64_t t_end, int64_t delta_bytes);
+typedef void (*lumen_kv_abort_fn)(void* user, uint64_t request_id);
+LUMEN_KV_API int lumen_kv_ckpt_set_direct(lumen_kv_ckpt* ckpt, void* region, int64_t region_bytes,
+                                          lumen_kv_acquire_fn acquire, lumen_kv_abort_fn abort,
+                                          int64_t min_avg_delta_bytes);
 LUMEN_KV_API int lumen_kv_ckpt_track(lumen_kv_ckpt* ckpt, uint64_t request_id, int64_t t_prev);
 LUMEN_KV_API int lumen_kv_ckpt_untrack(lumen_kv_ckpt* ckpt, uint64_t request_id);
 /* reqs[i].page_table / page_table_len: request ids[i]'s current table; reqs[i].t_end = t_cur;

@@ -47,6 +47,7 @@ EXPORTS = (
     "lumen_kv_store_reserved", "lumen_kv_store_reserve", "lumen_kv_store_release",
     "lumen_kv_store_append", "lumen_kv_store_tokens", "lumen_kv_store_lookup",
     "lumen_kv_store_segments", "lumen_kv_store_sink", "lumen_kv_store_sink_errors",
+    "lumen_kv_store_acquire", "lumen_kv_store_abort", "lumen_kv_store_arena", "lumen_kv_ckpt_set_direct",
     "lumen_kv_store_restore",
     "lumen_kv_choose_holder", "lumen_kv_recover",
     "lumen_kv_ckpt_create", "lumen_kv_ckpt_destroy", "lumen_kv_ckpt_track", "lumen_kv_ckpt_untrack",
@@ -199,6 +200,14 @@ def _lib() -> ctypes.CDLL:
     L.lumen_kv_ckpt_create.argtypes = [ctypes.POINTER(lumen_kv_geom), ctypes.POINTER(vp),
                                        ctypes.POINTER(vp), vp, i64, i32, vp, i64, SINK_FN, vp,
                                        ctypes.POINTER(vp)]
+    L.lumen_kv_store_acquire.restype = vp
+    L.lumen_kv_store_acquire.argtypes = [vp, u64, i64, i64, i64]
+    L.lumen_kv_store_abort.restype = None
+    L.lumen_kv_store_abort.argtypes = [vp, u64]
+    L.lumen_kv_store_arena.restype = vp
+    L.lumen_kv_store_arena.argtypes = [vp, ctypes.POINTER(i64)]
+    L.lumen_kv_ckpt_set_direct.restype = ctypes.c_int
+    L.lumen_kv_ckpt_set_direct.argtypes = [vp, vp, i64, vp, vp, i64]
     L.lumen_kv_ckpt_destroy.restype = None
     L.lumen_kv_ckpt_destroy.argtypes = [vp]
     L.lumen_kv_ckpt_track.restype = ctypes.c_int
@@ -668,6 +677,15 @@ class Store:
             raise LumenKVError(rc, "lumen_kv_store_restore")
         return int(out.value)
 
+    def acquire(self, request_id: int, t_begin: int, t_end: int) -> int:
+        """Claim [t_begin, t_end) at the request's tail; returns the arena address (0: refused)."""
+        p = _lib().lumen_kv_store_acquire(self._h, int(request_id), int(t_begin), int(t_end),
+                                          (int(t_end) - int(t_begin)) * self.token_bytes)
+        return int(p or 0)
+
+    def abort(self, request_id: int) -> None:
+        _lib().lumen_kv_store_abort(self._h, int(request_id))
+
     @property
     def sink_errors(self) -> int:
         return self._check(_lib().lumen_kv_store_sink_errors(self._h), "lumen_kv_store_sink_errors")
@@ -736,8 +754,12 @@ class BackgroundCheckpointer:
     to the error flush() raises); or pass a Store."""
 
     def __init__(self, geom: lumen_kv_geom, k_planes, v_planes, staging_ptr: int, slot_bytes: int,
-                 n_slots: int, pinned_ptr: int, pinned_bytes: int, sink):
+                 n_slots: int, pinned_ptr: int, pinned_bytes: int, sink, direct_min_bytes=1 << 20):
+        """direct_min_bytes (Store sinks only): batches whose average delta is at least this large are
+        copied straight into the store's arena (lumen_kv_ckpt_set_direct) when the arena is pinned;
+        None switches that off.  `self.direct` tells whether it is on."""
         L = geom.num_layers
+        self.direct = False
         self.sink_exception = None       # first exception a Python sink raised (re-raised by flush)
         if isinstance(sink, Store):      # native sink: deltas go straight into the store, no Python
             self._keep = sink
@@ -767,6 +789,16 @@ class BackgroundCheckpointer:
         if rc:
             raise LumenKVError(rc, "lumen_kv_ckpt_create")
         self._h = out
+        if isinstance(sink, Store) and direct_min_bytes is not None:
+            nb = ctypes.c_int64(0)
+            arena = _lib().lumen_kv_store_arena(sink._h, ctypes.byref(nb))
+            rc = _lib().lumen_kv_ckpt_set_direct(self._h, ctypes.c_void_p(arena), nb.value,
+                                                 ctypes.cast(_lib().lumen_kv_store_acquire, ctypes.c_void_p),
+                                                 ctypes.cast(_lib().lumen_kv_store_abort, ctypes.c_void_p),
+                                                 int(direct_min_bytes))
+            if rc not in (LUMEN_KV_OK, LUMEN_KV_EINVAL):     # EINVAL: the arena is not pinned memory
+                raise LumenKVError(rc, "lumen_kv_ckpt_set_direct")
+            self.direct = rc == LUMEN_KV_OK
 
     def _check(self, rc, where):
         if rc < 0:

@@ -65,6 +65,12 @@ struct Batch {
     uint64_t epoch = 0;
     int half = 0;
     int rc = LUMEN_KV_OK;
+    // direct batches: the copy engine writes every job's delta to dst[i], a position the sink's
+    // owner handed out (lumen_kv_ckpt_set_direct); off[i] = dst[i] - region base
+    bool direct = false;
+    std::vector<char*> dst;
+    std::vector<int64_t> off;
+    std::vector<char> open_claim;   // acquired and neither committed (sink) nor aborted yet
 };
 
 }  // namespace
@@ -79,6 +85,11 @@ struct lumen_kv_ckpt {
     int device = 0;
     lumen_kv_stager* stager = nullptr;
     cudaStream_t stream = nullptr;
+    // reserve-then-commit delivery (lumen_kv_ckpt_set_direct); read by the thread under mu
+    char* direct_base = nullptr;
+    int64_t direct_bytes = 0, direct_min = 0;
+    lumen_kv_acquire_fn acquire = nullptr;
+    lumen_kv_abort_fn abort_claim = nullptr;
     uint64_t* flags[2] = {nullptr, nullptr};   // pinned, one word per chunk, per buffer half
     int64_t flags_cap[2] = {0, 0};
     uint64_t epoch = 0;
@@ -123,6 +134,57 @@ bool wait_flag(lumen_kv_ckpt* c, const Batch& b, int64_t idx) {
     }
 }
 
+// Gives back every claim of the batch that has not been committed.
+void release_claims(lumen_kv_ckpt* c, Batch& b) {
+    for (size_t i = 0; i < b.open_claim.size(); ++i)
+        if (b.open_claim[i]) {
+            c->abort_claim(c->user, b.jobs[i].id);
+            b.open_claim[i] = 0;
+        }
+}
+
+// Reserve-then-commit: if the sink's owner hands out a final position for every delta of the
+// batch, the batch is packed straight to those positions (an explicit-layout plan whose buffer
+// is the owner's region) and the sink call that follows is the commit -- PAPER.md:147's "visible
+// only upon complete reception" is then the commit, not the copy.  Small deltas keep the classic
+// path (one chunk and one copy per batch instead of one per request).
+void try_direct(lumen_kv_ckpt* c, Batch& b, const std::vector<lumen_kv_req>& reqs) {
+    b.direct = false;
+    lumen_kv_acquire_fn acquire;
+    int64_t min_avg;
+    {
+        std::lock_guard<std::mutex> g(c->mu);
+        acquire = c->acquire;
+        min_avg = c->direct_min;
+    }
+    const size_t n = b.jobs.size();
+    if (!acquire || n == 0) return;
+    int64_t total = 0;
+    for (const lumen_kv_req& q : reqs) total += (q.t_end - q.t_begin) * c->token_bytes;
+    if (total < min_avg * static_cast<int64_t>(n)) return;
+    for (const lumen_kv_req& q : reqs)
+        if (q.t_end == q.t_begin) return;
+    b.dst.assign(n, nullptr);
+    b.off.assign(n, 0);
+    b.open_claim.assign(n, 0);
+    const int64_t row = c->token_bytes / (2 * c->geom.num_layers);
+    for (size_t i = 0; i < n; ++i) {
+        const Job& j = b.jobs[i];
+        const int64_t bytes = (j.te - j.tb) * c->token_bytes;
+        char* p = static_cast<char*>(acquire(c->user, j.id, j.tb, j.te, bytes));
+        const int64_t off = p ? p - c->direct_base : -1;
+        if (!p || off < 0 || off % row != 0 || off + bytes > c->direct_bytes) {
+            if (p) c->abort_claim(c->user, j.id);
+            release_claims(c, b);                   // all or nothing: the batch goes the classic way
+            return;
+        }
+        b.dst[i] = p;
+        b.off[i] = off;
+        b.open_claim[i] = 1;
+    }
+    b.direct = true;
+}
+
 // Stage 1: build the plan of the batch and enqueue its pack into one half of the pinned buffer.
 void submit(lumen_kv_ckpt* c, Batch& b) {
     const int32_t n = static_cast<int32_t>(b.jobs.size());
@@ -134,7 +196,17 @@ void submit(lumen_kv_ckpt* c, Batch& b) {
         reqs[i].t_begin = b.jobs[i].tb;
         reqs[i].t_end = b.jobs[i].te;
     }
-    b.rc = lumen_kv_plan_build(&c->geom, reqs.data(), n, 0, c->stream, &b.plan);
+    try_direct(c, b, reqs);
+    if (b.direct) {
+        std::vector<lumen_kv_req_layout> lays(static_cast<size_t>(n));
+        for (int32_t i = 0; i < n; ++i) {
+            lays[i].buf_offset = b.off[i];
+            lays[i].plane_stride_tokens = b.jobs[i].te - b.jobs[i].tb;
+        }
+        b.rc = lumen_kv_plan_build_layout(&c->geom, reqs.data(), lays.data(), n, 0, c->stream, &b.plan);
+    } else {
+        b.rc = lumen_kv_plan_build(&c->geom, reqs.data(), n, 0, c->stream, &b.plan);
+    }
     if (b.rc != LUMEN_KV_OK) return;
     const int64_t n_chunks = lumen_kv_plan_num_chunks(b.plan, c->slot_bytes);
     if (n_chunks < 0) {
@@ -169,9 +241,14 @@ void submit(lumen_kv_ckpt* c, Batch& b) {
             last = j.ev;
         }
     b.epoch = ++c->epoch;
-    b.rc = lumen_kv_checkpoint_pack_staged_commit(b.plan, c->k.data(), c->v.data(),
-                                                  c->pinned + b.half * half_bytes, half_bytes,
-                                                  c->stager, c->stream, c->flags[b.half], b.epoch);
+    if (b.direct)   // the checkpoint buffer IS the sink owner's region: no pinned half in between
+        b.rc = lumen_kv_checkpoint_pack_staged_commit(b.plan, c->k.data(), c->v.data(), c->direct_base,
+                                                      c->direct_bytes, c->stager, c->stream,
+                                                      c->flags[b.half], b.epoch);
+    else
+        b.rc = lumen_kv_checkpoint_pack_staged_commit(b.plan, c->k.data(), c->v.data(),
+                                                      c->pinned + b.half * half_bytes, half_bytes,
+                                                      c->stager, c->stream, c->flags[b.half], b.epoch);
 }
 
 // Stage 2: hand every request's delta to the sink as soon as the chunks that hold it have
@@ -203,7 +280,23 @@ void deliver(lumen_kv_ckpt* c, Batch& b) {
             if (it == c->reqs.end() || it->second.gen != j.gen) continue;   // void: see fail_request
         }
         bool taken = true;
-        if (end > off) {
+        if (b.direct) {
+            // the block of request i is [off_i, off_i + bytes); chunks commit in index order, so
+            // the last chunk that intersects the block completes it
+            const int64_t lo = b.off[i], hi = lo + (j.te - j.tb) * c->token_bytes;
+            int64_t last = -1;
+            for (int64_t k = 0; k < n_chunks; ++k)
+                if (b.chunks[static_cast<size_t>(k)].byte_begin < hi &&
+                    b.chunks[static_cast<size_t>(k)].byte_end > lo)
+                    last = k;
+            if (last < 0 || !wait_flag(c, b, last)) {
+                b.rc = LUMEN_KV_ECUDA;
+                break;
+            }
+            taken = c->sink(c->user, j.id, j.tb, j.te, b.dst[i], hi - lo, j.tags.data(),
+                            static_cast<int32_t>(j.tags.size())) == 0;
+            if (taken) b.open_claim[i] = 0;                 // committed
+        } else if (end > off) {
             while (ci < n_chunks && b.chunks[static_cast<size_t>(ci)].byte_end < end) ++ci;
             if (ci >= n_chunks || !wait_flag(c, b, ci)) {   // the chunk that completes request i
                 b.rc = LUMEN_KV_ECUDA;
@@ -222,7 +315,14 @@ void deliver(lumen_kv_ckpt* c, Batch& b) {
             sink_rc = LUMEN_KV_ESINK;
         }
     }
-    if (b.rc != LUMEN_KV_OK) cudaStreamSynchronize(c->stream);
+    if (b.rc != LUMEN_KV_OK || b.direct) {
+        // a direct batch may hold claims that were not committed (void jobs, a rejection, a
+        // failure): the copy engine must have left their bytes before the owner gets them back
+        bool open = b.rc != LUMEN_KV_OK;
+        for (char oc : b.open_claim) open = open || oc;
+        if (open) cudaStreamSynchronize(c->stream);
+    }
+    if (b.direct) release_claims(c, b);
     if (b.plan) lumen_kv_plan_free(b.plan);
     b.plan = nullptr;
     std::lock_guard<std::mutex> g(c->mu);
@@ -376,6 +476,32 @@ int lumen_kv_ckpt_create(const lumen_kv_geom* geom, const void* const* k_planes,
     c->busy = true;
     c->thread = std::thread(run, c);
     *out = c;
+    return LUMEN_KV_OK;
+}
+
+int lumen_kv_ckpt_set_direct(lumen_kv_ckpt* c, void* region, int64_t region_bytes,
+                             lumen_kv_acquire_fn acquire, lumen_kv_abort_fn abort_fn,
+                             int64_t min_avg_delta_bytes) {
+    if (!c) return LUMEN_KV_EINVAL;
+    if (!acquire) {                                 // switch it off
+        std::lock_guard<std::mutex> g(c->mu);
+        c->acquire = nullptr;
+        return LUMEN_KV_OK;
+    }
+    if (!abort_fn || !region || region_bytes < 16 || min_avg_delta_bytes < 0 ||
+        (reinterpret_cast<uintptr_t>(region) & 15))
+        return LUMEN_KV_EINVAL;
+    void* alias = nullptr;                          // the copy engine writes there: must be pinned
+    if (cudaHostGetDevicePointer(&alias, region, 0) != cudaSuccess) {
+        (void)cudaGetLastError();
+        return LUMEN_KV_EINVAL;
+    }
+    std::lock_guard<std::mutex> g(c->mu);
+    c->direct_base = static_cast<char*>(region);
+    c->direct_bytes = region_bytes;
+    c->direct_min = min_avg_delta_bytes;
+    c->abort_claim = abort_fn;
+    c->acquire = acquire;
     return LUMEN_KV_OK;
 }
 

@@ -25,7 +25,8 @@ struct Entry {
     int64_t region_bytes = 0;
     int64_t max_tokens = 0;
     int64_t tokens = 0;         // tokens completely received
-    int64_t receiving = 0;      // tokens of an append in progress (not yet visible)
+    int64_t receiving = 0;      // tokens of appends in progress / claimed (not yet visible)
+    int claims = 0;             // outstanding lumen_kv_store_acquire claims (filled in place, in order)
     std::vector<Delta> deltas;
     std::vector<lumen_kv_tag> tags;
 };
@@ -220,27 +221,71 @@ int lumen_kv_store_append(lumen_kv_store* s, uint64_t id, int64_t t_begin, int64
     for (int32_t i = 0; i < n_tags; ++i)
         if (tags[i].end_pos <= t_begin || tags[i].end_pos > t_end) return LUMEN_KV_EINVAL;
     char* dst;
+    bool in_place = false;
     {
         std::lock_guard<std::mutex> g(s->mu);
         auto it = s->reqs.find(id);
         if (it == s->reqs.end()) return LUMEN_KV_EINVAL;
         Entry& e = it->second;
-        if (e.receiving || t_begin != e.tokens || t_end > e.max_tokens) return LUMEN_KV_EINVAL;
-        if (n == 0) return LUMEN_KV_OK;
-        e.receiving = n;                                   // claims the region's tail
+        if (t_begin != e.tokens || t_end > e.max_tokens) return LUMEN_KV_EINVAL;
         dst = s->arena + e.region_off + e.tokens * s->token_bytes;
+        if (e.claims > 0) {
+            // commit of the oldest claim (lumen_kv_store_acquire): the bytes are already in place
+            if (n == 0 || delta != dst || n > e.receiving) return LUMEN_KV_EINVAL;
+            in_place = true;
+        } else {
+            if (e.receiving) return LUMEN_KV_EINVAL;
+            if (n == 0) return LUMEN_KV_OK;
+            e.receiving = n;                               // claims the region's tail
+        }
     }
-    s->pool->copy(dst, static_cast<const char*>(delta), delta_bytes);
+    if (!in_place) s->pool->copy(dst, static_cast<const char*>(delta), delta_bytes);
     {
         // publication: the delta and its tags become visible together, after the last byte
         std::lock_guard<std::mutex> g(s->mu);
-        Entry& e = s->reqs.find(id)->second;
+        auto it = s->reqs.find(id);
+        if (it == s->reqs.end()) return LUMEN_KV_EINVAL;
+        Entry& e = it->second;
+        if (in_place && (e.claims == 0 || t_begin != e.tokens)) return LUMEN_KV_EINVAL;   // aborted meanwhile
         e.deltas.push_back(Delta{t_begin, t_end, static_cast<int64_t>(dst - s->arena)});
         e.tags.insert(e.tags.end(), tags, tags + n_tags);
         e.tokens = t_end;
-        e.receiving = 0;
+        e.receiving -= n;
+        if (in_place) --e.claims;
     }
     return LUMEN_KV_OK;
+}
+
+void* lumen_kv_store_acquire(void* store, uint64_t id, int64_t t_begin, int64_t t_end,
+                             int64_t delta_bytes) {
+    lumen_kv_store* s = static_cast<lumen_kv_store*>(store);
+    if (!s || t_begin < 0 || t_end <= t_begin) return nullptr;
+    const int64_t n = t_end - t_begin;
+    if (delta_bytes != n * s->token_bytes) return nullptr;
+    std::lock_guard<std::mutex> g(s->mu);
+    auto it = s->reqs.find(id);
+    if (it == s->reqs.end()) return nullptr;
+    Entry& e = it->second;
+    if (e.receiving != 0 && e.claims == 0) return nullptr;      // a copying append is in progress
+    if (t_begin != e.tokens + e.receiving || t_end > e.max_tokens) return nullptr;
+    e.receiving += n;
+    ++e.claims;
+    return s->arena + e.region_off + t_begin * s->token_bytes;
+}
+
+void lumen_kv_store_abort(void* store, uint64_t id) {
+    lumen_kv_store* s = static_cast<lumen_kv_store*>(store);
+    if (!s) return;
+    std::lock_guard<std::mutex> g(s->mu);
+    auto it = s->reqs.find(id);
+    if (it == s->reqs.end() || it->second.claims == 0) return;
+    it->second.receiving = 0;                                   // every outstanding claim is void
+    it->second.claims = 0;
+}
+
+void* lumen_kv_store_arena(const lumen_kv_store* s, int64_t* bytes) {
+    if (bytes) *bytes = s ? s->arena_bytes : 0;
+    return s ? s->arena : nullptr;
 }
 
 int64_t lumen_kv_store_tokens(const lumen_kv_store* s, uint64_t id) {

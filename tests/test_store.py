@@ -3,6 +3,7 @@ arithmetic, append-only deltas, visibility, tags and segments -- on the CPU agai
 Python model and the oracle; then the whole chain on the GPU: incremental packs -> store ->
 failure -> tag lookup -> restore of the longest checkpointed prefix straight out of the arena,
 equal to the oracle's restore of that prefix."""
+import ctypes
 import threading
 
 import numpy as np
@@ -272,3 +273,179 @@ def test_concurrent_appends_and_churn(lk):
         st.release(r)
     assert st.available == arena.size
     st.reserve(9999, arena.size // tokb)                          # coalesced back into one hole
+
+
+def test_acquire_commit_abort_and_racing_lookup(lk):
+    """Reserve-then-commit (lumen_kv_store_acquire): a writer gets the final position of a delta,
+    fills it in place and commits with an append whose source IS that position.  Until the commit
+    neither tokens(), lookup() nor segments() show the claim -- also while another thread keeps
+    looking (visible only upon complete reception); claims stack in order; abort
+    voids them; the stored bytes equal oracle.pack of each delta."""
+    w = cfg0_tiny(full_prefix=True)
+    L, H, D, S, N = w.geom
+    tokb = 2 * L * H * D * 2
+    from workloads import fill_plane_np
+    E = H * D
+    K = [fill_plane_np(3, 2 * l, N * S * E) for l in range(L)]
+    V = [fill_plane_np(3, 2 * l + 1, N * S * E) for l in range(L)]
+    pt, _, n_tok = w.reqs[1]                                     # 100 tokens
+    toks = substream(7, "acq").integers(0, 5000, size=n_tok).astype(np.int32)
+    keep, arena = _arena(2 * n_tok * tokb)
+    st = lk.Store(arena.ctypes.data, arena.size, tokb, S)
+    st.reserve(5, n_tok); st.reserve(6, n_tok)
+    regen = lk.lumen_kv_page_tags_host(toks, 0, 0, n_tok, S)
+    stop = threading.Event()
+    seen, bad = [], []
+
+    def looker():
+        last = 0
+        while not stop.is_set():
+            t, p = st.tokens(5), st.lookup(5, regen)
+            if t < last or p > t or p % S not in (0, t % S) and p != t:
+                bad.append((t, p))
+            last = t
+            seen.append(t)
+
+    th = threading.Thread(target=looker, daemon=True)
+    th.start()
+    try:
+        _acquire_commit_abort_body(lk, st, w, K, V, pt, tokb, S, regen, arena, stop, th, seen, bad)
+    finally:
+        stop.set()
+        th.join(10)
+
+
+def _acquire_commit_abort_body(lk, st, w, K, V, pt, tokb, S, regen, arena, stop, th, seen, bad):
+    cuts = [0, 37, 64, 100]
+    # two stacked claims, filled and committed in order
+    p0 = st.acquire(5, 0, 37)
+    p1 = st.acquire(5, 37, 64)
+    assert p0 and p1 == p0 + 37 * tokb
+    assert st.acquire(5, 37, 64) == 0 and st.acquire(5, 70, 80) == 0     # must continue the claims
+    assert st.acquire(5, 64, 101) == 0                                    # beyond the reservation
+    assert st.tokens(5) == 0 and st.lookup(5, regen) == 0
+    with pytest.raises(lk.LumenKVError):                                  # a copying append cannot jump the claims
+        st.append(5, 0, 37, np.zeros(37 * tokb, dtype=np.uint8).ctypes.data, 37 * tokb, regen[:0])
+    for (a, b), dst in (((0, 37), p0), ((37, 64), p1)):
+        delta = oracle.pack(w.geom, K, V, [(pt, a, b)])
+        view = np.ctypeslib.as_array((ctypes.c_uint16 * delta.size).from_address(dst))
+        view[:] = delta                                                   # "the copy engine"
+        assert st.tokens(5) == a                                          # filled, not committed
+        tags = regen[(regen["end_pos"] > a) & (regen["end_pos"] <= b)]
+        st.append(5, a, b, dst, delta.size * 2, tags)                     # the commit: no copy
+        assert st.tokens(5) == b
+    assert st.lookup(5, regen) == 64
+    # a claim that is aborted leaves no trace; the next claim takes the same place
+    p2 = st.acquire(5, 64, 100)
+    assert p2 == p0 + 64 * tokb
+    st.abort(5)
+    assert st.tokens(5) == 64 and st.acquire(5, 64, 100) == p2
+    with pytest.raises(lk.LumenKVError):                                  # commit with a foreign pointer
+        st.append(5, 64, 100, p2 + 2, 36 * tokb, regen[:0])
+    delta = oracle.pack(w.geom, K, V, [(pt, 64, 100)])
+    np.ctypeslib.as_array((ctypes.c_uint16 * delta.size).from_address(p2))[:] = delta
+    st.append(5, 64, 100, p2, delta.size * 2, regen[(regen["end_pos"] > 64)])
+    stop.set(); th.join()
+    assert not bad and st.tokens(5) == 100 and st.lookup(5, regen) == 100
+    assert set(seen) <= set(cuts)                                         # only committed states were ever seen
+    segs = st.segments(5, 100)
+    assert [(int(s["t_begin"]), int(s["t_end"])) for s in segs] == [(0, 37), (37, 64), (64, 100)]
+    base = arena.ctypes.data
+    for s in segs:
+        a, b = int(s["t_begin"]), int(s["t_end"])
+        off = int(s["buf_offset"])
+        got = arena[off: off + (b - a) * tokb].view(np.uint16)
+        assert np.array_equal(got, oracle.pack(w.geom, K, V, [(pt, a, b)]))
+    # the classic copying append still works on another request, and refuses to run under a claim
+    assert st.acquire(6, 0, 10)
+    with pytest.raises(lk.LumenKVError):
+        st.release(6)                                                     # claimed: not releasable
+    st.abort(6)
+    d = oracle.pack(w.geom, K, V, [(pt, 0, 10)])
+    st.append(6, 0, 10, d.ctypes.data, d.size * 2, regen[:0])
+    assert st.tokens(6) == 10
+    st.release(6); st.release(5)
+    assert st.reserved == 0 and base == arena.ctypes.data
+
+
+@pytest.mark.gpu
+def test_gpu_background_checkpointer_writes_straight_into_the_store(lk):
+    """lumen_kv_ckpt_set_direct: with a pinned arena the background checkpointer packs every
+    delta to the position the store hands out (no second host copy) and commits it with the sink
+    call.  Prefill in several pieces (stacked claims), decode deltas, a request whose reservation
+    runs out (acquire refuses -> that batch goes the copying way and the store rejects it): the
+    store's content equals oracle.pack of every delta, tags and progress are those of the copying
+    path, and restore out of the store reproduces the oracle's pool."""
+    import torch
+    from tests import gpu_util as G
+    G.build_all()
+    w = cfg1_qwen14b(L=2, N=1024, n_reqs=5, grow_iters=8, median=150, hi=300, lo=60)
+    L, H, D, S, N = w.geom
+    tokb = 2 * L * H * D * 2
+    lens = [te for _, _, te in w.reqs]
+    steps, delta_tok = 6, 3
+    rng = substream(8, "direct")
+    hist = [rng.integers(0, 32000, size=n + steps * delta_tok).astype(np.int32) for n in lens]
+    K, V = G.host_planes(w.geom, 31)
+    results = {}
+    for mode in ("direct", "copy"):
+        pool = G.make_pool(w.geom, 31)
+        arena_t = G.pinned_buffer(sum(n + steps * delta_tok for n in lens) * tokb)
+        arena_t.zero_()
+        st = lk.Store(arena_t.data_ptr(), arena_t.numel(), tokb, S, copy_threads=2)
+        for rid, n in enumerate(lens):
+            st.reserve(rid, n + steps * delta_tok - (4 if rid == 4 else 0))     # request 4 runs out of room
+        ring_mem = torch.empty(3 << 20, dtype=torch.uint8, device="cuda")
+        pinned = G.pinned_buffer(2 * 100 * tokb)                 # halves of 100 tokens: prefill comes in pieces
+        bg = lk.BackgroundCheckpointer(pool.geom, pool.k_ptrs, pool.v_ptrs, ring_mem.data_ptr(), 1 << 20, 3,
+                                       pinned.data_ptr(), pinned.numel(), st,
+                                       direct_min_bytes=0 if mode == "direct" else None)
+        assert bg.direct == (mode == "direct")
+        for rid in range(len(lens)):
+            bg.track(rid, 0)
+        bg.notify(list(range(len(lens))), [(pt, 0, n) for (pt, _, n) in w.reqs], token_ids=hist)
+        for step in range(1, steps + 1):
+            bg.notify(list(range(len(lens))), [(pt, 0, n + step * delta_tok) for (pt, _, n) in w.reqs],
+                      token_ids=hist)
+            if step == 3:
+                bg.flush()
+        try:
+            bg.flush()
+            raised = None
+        except lk.LumenKVError as e:
+            raised = e.status
+        assert raised == lk.LUMEN_KV_ESINK                       # request 4's last delta did not fit
+        final = [n + steps * delta_tok for n in lens]
+        for rid in range(4):
+            assert bg.progress(rid) == final[rid] == st.tokens(rid)
+        assert st.tokens(4) == bg.progress(4) < final[4]
+        state = []
+        for rid in range(len(lens)):
+            segs = st.segments(rid, st.tokens(rid))
+            at = 0
+            for s in segs:
+                a, b, off = int(s["t_begin"]), int(s["t_end"]), int(s["buf_offset"])
+                assert a == at
+                at = b
+                got = arena_t[off: off + (b - a) * tokb].numpy().view(np.uint16)
+                assert np.array_equal(got, oracle.pack(w.geom, K, V, [(w.reqs[rid][0], a, b)])), (mode, rid, a, b)
+            assert at == st.tokens(rid)
+            regen = lk.lumen_kv_page_tags_host(hist[rid], 0, 0, st.tokens(rid), S)
+            state.append((st.tokens(rid), st.lookup(rid, regen)))
+        results[mode] = state
+        # recovery out of the store into fresh pages == the oracle's restore of the same prefix
+        pool_b = G.make_pool(w.geom, 32)
+        K2, V2 = G.host_planes(w.geom, 32)
+        ringr = G.StagingRing(1 << 20, 3)
+        for rid, (pt_new, _, _) in enumerate(w.restore_reqs):
+            n = st.tokens(rid)
+            got = st.restore(rid, hist[rid][:n], pool_b.geom, pt_new, pool_b.k_ptrs, pool_b.v_ptrs, ringr.stager)
+            assert got == state[rid][1]
+            if got:
+                oracle.unpack(w.geom, K2, V2, [(pt_new, 0, got)],
+                              oracle.pack(w.geom, K, V, [(w.reqs[rid][0], 0, got)]))
+        torch.cuda.synchronize()
+        for t, ref in zip(pool_b.planes(), [x for kv in zip(K2, V2) for x in kv]):
+            assert np.array_equal(G.plane_to_np(t), ref), mode
+        ringr.close(); bg.close(); st.close()
+    assert results["direct"] == results["copy"]
